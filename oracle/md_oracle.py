@@ -1,0 +1,223 @@
+"""ctypes front end of the CPU oracle (oracle/md_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+`--impl reference` legs -- never by the product package.  Shares nothing with
+paper_2003_14061_b200/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "md_oracle.c")
+_LIB = os.path.join(_HERE, "libmd_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 build of the oracle (fp contraction off: every a*b+c rounds twice unless written fma())."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-std=c11", "-O2", "-march=native", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+               "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+class _Energy(C.Structure):
+    _fields_ = [("ke", C.c_double), ("pe_pair", C.c_double), ("pe_bond", C.c_double), ("virial", C.c_double),
+                ("px", C.c_double), ("py", C.c_double), ("pz", C.c_double), ("vmax", C.c_double),
+                ("step", C.c_int64), ("n_rebuilds", C.c_int64),
+                ("max_neighbors", C.c_int32), ("max_cell_occupancy", C.c_int32),
+                ("mean_neighbors", C.c_double)]
+
+
+@dataclass
+class Energies:
+    ke: float
+    pe_pair: float
+    pe_bond: float
+    virial: float
+    px: float
+    py: float
+    pz: float
+    vmax: float
+    step: int
+    n_rebuilds: int
+    max_neighbors: int
+    max_cell_occupancy: int
+    mean_neighbors: float
+
+    @property
+    def pe(self) -> float:
+        return self.pe_pair + self.pe_bond
+
+    @property
+    def total(self) -> float:
+        return self.ke + self.pe
+
+
+_lib = None
+_dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_ip = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+_lp = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_create.restype = C.c_void_p
+        L.orc_create.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_force_brute_search.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_state.argtypes = [C.c_void_p, _dp, C.c_void_p]
+        L.orc_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
+        L.orc_set_bonds.restype = C.c_int
+        L.orc_rebuild_neighbors.argtypes = [C.c_void_p]
+        L.orc_step.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_step.restype = C.c_int
+        L.orc_energies.argtypes = [C.c_void_p, C.POINTER(_Energy)]
+        for name in ("orc_get_positions", "orc_get_velocities", "orc_get_forces", "orc_set_velocities"):
+            getattr(L, name).argtypes = [C.c_void_p, _dp]
+        L.orc_get_atom_energies.argtypes = [C.c_void_p, _dp, _dp]
+        L.orc_neighbor_total.argtypes = [C.c_void_p]
+        L.orc_neighbor_total.restype = C.c_int64
+        L.orc_get_neighbors.argtypes = [C.c_void_p, _ip, _ip]
+        L.orc_brute_forces.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
+        L.orc_brute_forces_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp, _dp, _dp, _dp]
+        L.orc_brute_neighbors_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp,
+                                                 C.c_int32, _ip, _ip]
+        L.orc_brute_neighbors_sample.restype = C.c_int32
+        L.orc_set_threads.argtypes = [C.c_int]
+        L.orc_get_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def set_threads(n: int) -> None:
+    lib().orc_set_threads(int(n))
+
+
+def get_threads() -> int:
+    return int(lib().orc_get_threads())
+
+
+def _c(a, dtype=np.float64):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def brute_forces(r, box, r_cut):
+    """All-pairs minimum-image truncated LJ: (f[N,3], u[N], w[N]); u, w double counted per atom."""
+    r = _c(r)
+    n = r.shape[0]
+    f, u, w = np.empty((n, 3)), np.empty(n), np.empty(n)
+    lib().orc_brute_forces(n, float(box), r, float(r_cut), f, u, w)
+    return f, u, w
+
+
+def brute_forces_sample(r, box, r_cut, idx):
+    r, idx = _c(r), _c(idx, np.int64)
+    ns = idx.shape[0]
+    f, u, w = np.empty((ns, 3)), np.empty(ns), np.empty(ns)
+    lib().orc_brute_forces_sample(r.shape[0], float(box), r, float(r_cut), ns, idx, f, u, w)
+    return f, u, w
+
+
+def brute_neighbors_sample(r, box, r_n, idx, cap=256):
+    """Neighbor sets by definition for the atoms in idx: list of sorted int arrays."""
+    r, idx = _c(r), _c(idx, np.int64)
+    ns = idx.shape[0]
+    counts = np.empty(ns, np.int32)
+    out = np.empty((ns, cap), np.int32)
+    mx = lib().orc_brute_neighbors_sample(r.shape[0], float(box), r, float(r_n), ns, idx, cap, counts, out)
+    if mx > cap:
+        return brute_neighbors_sample(r, box, r_n, idx, cap=int(mx))
+    return [out[k, :counts[k]].copy() for k in range(ns)]
+
+
+class OracleMD:
+    """Plain CPU MD of the same model (see md_oracle.c header for the passages followed)."""
+
+    def __init__(self, n_atoms, box, r_cut, r_shell, dt, brute_search=False):
+        self._L = lib()
+        self.n = int(n_atoms)
+        self.box, self.r_cut, self.r_shell, self.dt = float(box), float(r_cut), float(r_shell), float(dt)
+        self._h = self._L.orc_create(self.n, self.box, self.r_cut, self.r_shell, self.dt)
+        if not self._h:
+            raise ValueError("orc_create failed")
+        if brute_search:
+            self._L.orc_force_brute_search(self._h, 1)
+
+    def close(self):
+        if self._h:
+            self._L.orc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, r, v=None):
+        r = _c(r)
+        assert r.shape == (self.n, 3)
+        vp = None
+        if v is not None:
+            v = _c(v)
+            vp = v.ctypes.data_as(C.c_void_p)
+        self._L.orc_set_state(self._h, r, vp)
+
+    def set_velocities(self, v):
+        self._L.orc_set_velocities(self._h, _c(v))
+
+    def set_bonds(self, bonds, k, r0):
+        b = _c(bonds, np.int32).reshape(-1, 2)
+        return self._L.orc_set_bonds(self._h, b.shape[0], b, float(k), float(r0))
+
+    def rebuild_neighbors(self):
+        self._L.orc_rebuild_neighbors(self._h)
+
+    def step(self, n=1):
+        return self._L.orc_step(self._h, int(n))
+
+    def energies(self) -> Energies:
+        e = _Energy()
+        self._L.orc_energies(self._h, C.byref(e))
+        return Energies(**{k: getattr(e, k) for k, _ in _Energy._fields_})
+
+    def _get(self, name):
+        out = np.empty((self.n, 3))
+        getattr(self._L, name)(self._h, out)
+        return out
+
+    def positions(self):
+        return self._get("orc_get_positions")
+
+    def velocities(self):
+        return self._get("orc_get_velocities")
+
+    def forces(self):
+        return self._get("orc_get_forces")
+
+    def atom_energies(self):
+        u, w = np.empty(self.n), np.empty(self.n)
+        self._L.orc_get_atom_energies(self._h, u, w)
+        return u, w
+
+    def neighbors(self):
+        """(counts[N], flat list in CSR order)."""
+        tot = self._L.orc_neighbor_total(self._h)
+        counts = np.empty(self.n, np.int32)
+        flat = np.empty(max(tot, 1), np.int32)
+        self._L.orc_get_neighbors(self._h, counts, flat)
+        return counts, flat[:tot]
+
+    def neighbor_sets(self):
+        counts, flat = self.neighbors()
+        off = np.concatenate([[0], np.cumsum(counts, dtype=np.int64)])
+        return [np.sort(flat[off[i]:off[i + 1]]) for i in range(self.n)]

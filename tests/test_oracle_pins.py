@@ -1,0 +1,362 @@
+"""Pins for the CPU oracle (oracle/md_oracle.c): every check here is against something other than
+the oracle itself -- numpy all-pairs sums written from the textbook potential, finite differences of
+that energy, closed forms on the lattices, values printed in the paper, conservation laws, symmetries.
+Pin numbers P1..P12 follow SURVEY.md section 8(c)."""
+import math
+
+import numpy as np
+import pytest
+
+from md_workloads import get_config, make_state, scaled_config, gaussian_velocities, sc_lattice
+from md_workloads.configs import MDConfig, R_WCA
+from oracle.md_oracle import OracleMD, brute_forces, brute_forces_sample, brute_neighbors_sample
+
+
+# ---- independent numpy definitions (textbook forms, different algebra from the C code) ----------
+def np_pair_tables(r, box, r_cut):
+    """All-pairs minimum image by rounding; u(r) = 4(r^-12 - r^-6) - u(r_c); |f| = 24(2 r^-13 - r^-7)."""
+    d = r[:, None, :] - r[None, :, :]
+    d -= box * np.round(d / box)
+    dist = np.sqrt((d * d).sum(-1))
+    np.fill_diagonal(dist, np.inf)
+    inside = dist < r_cut
+    uc = 4.0 * (r_cut ** -12 - r_cut ** -6)
+    u = np.where(inside, 4.0 * (dist ** -12 - dist ** -6) - uc, 0.0)
+    fmag = np.where(inside, 24.0 * (2.0 * dist ** -13 - dist ** -7), 0.0)
+    f = (fmag / dist)[:, :, None] * d
+    return dist, u, f.sum(1), (fmag * np.where(inside, dist, 0.0)).sum(1)
+
+
+def np_total_energy(r, box, r_cut):
+    return 0.5 * np_pair_tables(r, box, r_cut)[1].sum()
+
+
+def fluid_state(n_side=8, rho=0.8, amp=0.18, seed=3):
+    n = n_side ** 3
+    box = (n / rho) ** (1 / 3)
+    rng = np.random.default_rng(seed)
+    r = sc_lattice(n, box) + rng.uniform(-amp, amp, (n, 3))
+    return np.mod(r, box), box
+
+
+def oracle_for(r, box, r_cut, r_shell=0.4, dt=0.005, v=None, brute=False):
+    o = OracleMD(r.shape[0], box, r_cut, r_shell, dt, brute_search=brute)
+    o.set_state(r, v)
+    return o
+
+
+def rel_err(f, ref):
+    """SURVEY 8(c) A11 norm: per-atom inf-norm error over max(|f_ref|_inf, f_rms)."""
+    frms = math.sqrt(float((ref * ref).sum()) / ref.shape[0])
+    den = np.maximum(np.abs(ref).max(1), frms if frms > 0 else 1.0)
+    return float((np.abs(f - ref).max(1) / den).max())
+
+
+# ---- P1: listed forces/energies == all-pairs definition -----------------------------------------
+@pytest.mark.parametrize("r_cut,rho", [(R_WCA, 0.8), (2.5, 0.8442), (2.5, 0.38)])
+def test_p1_forces_match_numpy_all_pairs(r_cut, rho):
+    r, box = fluid_state(8, rho, 0.2 if rho > 0.5 else 0.4)
+    o = oracle_for(r, box, r_cut, 0.3)
+    _, u_np, f_np, w_np = np_pair_tables(r, box, r_cut)
+    assert rel_err(o.forces(), f_np) < 1e-12
+    u, w = o.atom_energies()
+    assert np.allclose(u, u_np.sum(1), rtol=1e-12, atol=1e-12)
+    assert np.allclose(w, w_np, rtol=1e-12, atol=1e-11)
+    e = o.energies()
+    assert e.pe_pair == pytest.approx(0.5 * u_np.sum(), rel=1e-12)
+    assert e.virial == pytest.approx(0.5 * w_np.sum(), rel=1e-12)
+    # the C brute-force routine is the same definition: it must agree too (used at larger N below)
+    fb, ub, wb = brute_forces(r, box, r_cut)
+    assert rel_err(fb, f_np) < 1e-12 and np.allclose(ub, u_np.sum(1), rtol=1e-12, atol=1e-12)
+
+
+def test_p1_force_is_minus_gradient_of_numpy_energy():
+    r, box = fluid_state(6, 0.8, 0.2, seed=5)
+    o = oracle_for(r, box, R_WCA)
+    f = o.forces()
+    h = 1e-5
+    for i, k in [(0, 0), (17, 1), (101, 2), (215, 0)]:
+        rp, rm = r.copy(), r.copy()
+        rp[i, k] += h
+        rm[i, k] -= h
+        g = (np_total_energy(rp, box, R_WCA) - np_total_energy(rm, box, R_WCA)) / (2 * h)
+        assert f[i, k] == pytest.approx(-g, rel=1e-6, abs=1e-6)
+
+
+def test_p1_cell_search_equals_brute_search_and_definition():
+    for r_cut, rho, amp in [(R_WCA, 0.8, 0.25), (2.5, 0.8442, 0.2)]:
+        r, box = fluid_state(12, rho, amp, seed=9)            # N = 1728, several cells per edge
+        a = oracle_for(r, box, r_cut, 0.3).neighbor_sets()
+        b = oracle_for(r, box, r_cut, 0.3, brute=True).neighbor_sets()
+        assert all(np.array_equal(x, y) for x, y in zip(a, b))
+        # and the definition evaluated in numpy (distance by rounding) on a sample of atoms
+        dist = np_pair_tables(r, box, r_cut)[0]
+        for i in range(0, r.shape[0], 97):
+            assert np.array_equal(a[i], np.nonzero(dist[i] < r_cut + 0.3)[0])
+        idx = np.arange(0, r.shape[0], 53)
+        s = brute_neighbors_sample(r, box, r_cut + 0.3, idx)
+        assert all(np.array_equal(s[k], a[i]) for k, i in enumerate(idx))
+
+
+def test_p1_config1_after_melting_matches_brute_force():
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 2)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    o.step(300)
+    fb, ub, wb = brute_forces(o.positions(), box, cfg.r_cut)
+    assert rel_err(o.forces(), fb) < 1e-13
+    assert o.energies().pe_pair == pytest.approx(0.5 * ub.sum(), rel=1e-13)
+    idx = np.array([0, 5, 4095])
+    fs, _, _ = brute_forces_sample(o.positions(), box, cfg.r_cut, idx)
+    assert np.array_equal(fs, fb[idx])
+
+
+# ---- P2 / P3: Newton 3 and momentum -------------------------------------------------------------
+def test_p2_p3_zero_net_force_and_momentum():
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 1)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    vrms = math.sqrt(3 * cfg.temperature)
+    for _ in range(3):
+        o.step(100)
+        f = o.forces()
+        assert np.abs(f.sum(0)).max() <= 1e-12 * np.abs(f).max(1).sum()
+        e = o.energies()
+        assert max(abs(e.px), abs(e.py), abs(e.pz)) <= 1e-12 * math.sqrt(cfg.n_atoms) * vrms * 10
+
+
+# ---- P4 (A17): energy conservation over 1000 steps of config 1 ----------------------------------
+def test_p4_energy_drift_config1():
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 1)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    e0 = o.energies().total
+    es = []
+    for _ in range(20):
+        o.step(50)
+        es.append(o.energies().total)
+    es = np.array(es)
+    n = cfg.n_atoms
+    assert np.abs(es - e0).max() / n <= 2e-3          # DESIGN.md R17 bound (parity unpinned by the paper)
+    slope = np.polyfit(np.arange(1, 21) * 50.0, es / n, 1)[0]
+    assert abs(slope) * 1000 <= 2e-3
+
+
+# ---- P5: closed forms on the initial lattices ---------------------------------------------------
+def lj_shift(rc):
+    return 4.0 * (rc ** -12 - rc ** -6)
+
+
+def test_p5_sc_lattice_closed_forms(golden):
+    g = golden("lattice_closed_forms.txt")
+    rho = 0.8
+    assert 3 * (4 * (rho ** 4 - rho ** 2) + 1) == pytest.approx(g["sc_pe_per_atom"], rel=1e-12)
+    assert 3 * 48 * (rho ** 4 - rho ** 2 / 2) == pytest.approx(g["sc_virial_per_atom"], rel=1e-12)
+    for dr, key in [(0.3, "sc_neighbors_dr03"), (0.4, "sc_neighbors_dr04"), (0.5, "sc_neighbors_dr05")]:
+        cfg = scaled_config("wca_4k", 4096, r_shell=dr)
+        r, v, _, box = make_state(cfg, 1)
+        o = oracle_for(r, box, cfg.r_cut, dr, cfg.dt, v)
+        e = o.energies()
+        counts, _ = o.neighbors()
+        assert counts.min() == counts.max() == int(g[key])
+        assert e.pe_pair / cfg.n_atoms == pytest.approx(g["sc_pe_per_atom"], rel=1e-12)
+        assert e.virial / cfg.n_atoms == pytest.approx(g["sc_virial_per_atom"], rel=1e-12)
+        assert e.ke == pytest.approx(1.5 * (cfg.n_atoms - 1) * cfg.temperature, rel=1e-13)
+        f = o.forces()
+        assert np.abs(f).max() <= 1e-12 * 24.0 * 6          # every f_i = 0 by symmetry
+
+
+def test_p5_fcc_lattice_closed_forms(golden):
+    g = golden("lattice_closed_forms.txt")
+    rho, rc = 0.8442, 2.5
+    a = (4 / rho) ** (1 / 3)
+    shells = [(1, 12), (2, 6), (3, 24), (4, 12), (5, 24), (6, 8)]
+    uc = lj_shift(rc)
+    assert uc == pytest.approx(g["lj25_energy_shift"], rel=1e-10)
+    pe = vir = 0.0
+    nn = nin = 0
+    for k, mult in shells:
+        d = a * math.sqrt(k / 2)
+        if d < rc + 0.3:
+            nn += mult
+        if d < rc:
+            nin += mult
+            pe += 0.5 * mult * (4 * (d ** -12 - d ** -6) - uc)
+            vir += 0.5 * mult * 24 * (2 * d ** -12 - d ** -6)
+    assert (nn, nin) == (int(g["fcc_neighbors"]), int(g["fcc_pairs_in_cutoff"]))
+    assert pe == pytest.approx(g["fcc_pe_per_atom"], rel=1e-12)
+    assert vir == pytest.approx(g["fcc_virial_per_atom"], rel=1e-12)
+    cfg = scaled_config("lj_1m", 4 * 8 ** 3)
+    r, v, _, box = make_state(cfg, 1)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    e = o.energies()
+    counts, _ = o.neighbors()
+    assert counts.min() == counts.max() == 78
+    assert e.pe_pair / cfg.n_atoms == pytest.approx(g["fcc_pe_per_atom"], rel=1e-12)
+    assert e.virial / cfg.n_atoms == pytest.approx(g["fcc_virial_per_atom"], rel=1e-11)
+    assert np.abs(o.forces()).max() <= 1e-11
+    assert e.ke == pytest.approx(1.5 * (cfg.n_atoms - 1) * cfg.temperature, rel=1e-13)
+
+
+# ---- P6: the pair kernel on two atoms, inside the box and across a periodic face ----------------
+@pytest.mark.parametrize("rc", [R_WCA, 2.5])
+def test_p6_two_atom_values(rc):
+    box = 12.0
+    uc = lj_shift(rc)
+    filler = np.array([[6.0, 6.0, 6.0]])            # third atom far from both (keeps N > 2 generic)
+    for sep, f_expect, u_expect in [
+        (1.0, 24.0, 0.0 - uc),
+        (rc * (1 - 1e-9), 24 * (2 * rc ** -13 - rc ** -7), 0.0),
+        (rc * (1 + 1e-12), 0.0, 0.0),
+        (rc + 0.2, 0.0, 0.0),
+    ]:
+        for x0 in (3.0, box - 0.4 * sep):           # second placement straddles the periodic face
+            for axis in range(3):
+                r = np.full((2, 3), 1.5)
+                r[0, axis] = x0
+                r[1, axis] = (x0 + sep) % box
+                r = np.vstack([r, filler])
+                o = oracle_for(r, box, rc, 0.3)
+                f = o.forces()
+                e = o.energies()
+                # repulsive (f_expect > 0) pushes atom 0 towards -axis, atom 1 towards +axis
+                assert f[0, axis] == pytest.approx(-f_expect, rel=1e-7, abs=1e-7)
+                assert f[1, axis] == pytest.approx(+f_expect, rel=1e-7, abs=1e-7)
+                assert np.abs(f[0] + f[1]).max() <= 1e-13 * max(1.0, abs(f_expect))
+                assert e.pe_pair == pytest.approx(u_expect, rel=1e-7, abs=2e-7)
+                if sep >= rc:
+                    assert np.all(f == 0.0) and e.pe_pair == 0.0 and e.virial == 0.0
+                else:
+                    assert e.virial == pytest.approx(f_expect * sep, rel=1e-7, abs=1e-6)
+
+
+# ---- P7: FENE -------------------------------------------------------------------------------------
+def test_p7_fene_bond(golden):
+    g = golden("lattice_closed_forms.txt")
+    k, r0, box = 30.0, 1.5, 12.0
+    # textbook: U = -1/2 k R0^2 ln(1 - r^2/R0^2); with WCA on the bonded pair the net force vanishes at r*
+    f_net = lambda x: 24 * (2 * x ** -13 - x ** -7) - k * x / (1 - x * x / (r0 * r0))
+    lo, hi = 0.9, 1.0
+    for _ in range(80):
+        mid = 0.5 * (lo + hi)
+        lo, hi = (mid, hi) if f_net(mid) > 0 else (lo, mid)
+    rstar = 0.5 * (lo + hi)
+    assert rstar == pytest.approx(g["fene_wca_bond_minimum"], abs=1e-6)
+    ustar = -0.5 * k * r0 * r0 * math.log(1 - rstar ** 2 / r0 ** 2)
+    assert ustar == pytest.approx(g["fene_energy_at_minimum"], abs=1e-5)
+
+    def two(sep):
+        r = np.array([[box - 0.3, 2.0, 2.0], [(box - 0.3 + sep) % box, 2.0, 2.0], [6.0, 6.0, 6.0]])
+        o = oracle_for(r, box, R_WCA, 0.4)
+        rc = o.set_bonds(np.array([[0, 1]], np.int32), k, r0)
+        return o, rc
+    o, rc = two(rstar)
+    assert rc == 0 and np.abs(o.forces()).max() < 1e-9
+    e = o.energies()
+    assert e.pe_bond == pytest.approx(ustar, rel=1e-12)
+    assert e.pe_pair == pytest.approx(4 * (rstar ** -12 - rstar ** -6) + 1, rel=1e-9)
+    o, rc = two(1.2)
+    fene = -k * 1.2 / (1 - 1.44 / 2.25)
+    assert o.forces()[1, 0] == pytest.approx(fene, rel=1e-12)      # attractive: pulls atom 1 back (-x)
+    assert o.forces()[0, 0] == pytest.approx(-fene, rel=1e-12)
+    assert o.energies().virial == pytest.approx(fene * 1.2, rel=1e-12)
+    assert two(1.5)[1] == -3 and two(1.6)[1] == -3                # r >= R0 is an error
+
+
+# ---- P8: time reversal ----------------------------------------------------------------------------
+def test_p8_reversibility():
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 4)
+    r = np.mod(r + np.random.default_rng(0).uniform(-0.05, 0.05, r.shape), box)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    o.step(100)
+    o.set_velocities(-o.velocities())
+    o.step(100)
+    d = o.positions() - r
+    d -= box * np.round(d / box)
+    assert np.abs(d).max() < 1e-9
+    assert np.abs(o.velocities() + v).max() < 1e-8
+
+
+# ---- P10: second-order integrator: energy error scales as dt^2 ------------------------------------
+def test_p10_dt_squared_scaling():
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(scaled_config("wca_4k", 1000), 1)
+    o0 = oracle_for(r, box, cfg.r_cut, cfg.r_shell, 0.004, v)
+    o0.step(400)                                       # melt first, then restart from this state
+    r1, v1 = o0.positions(), o0.velocities()
+    fl = []
+    for dt in (0.004, 0.002, 0.001):       # dt = 0.008 is past the asymptotic regime (secular drift)
+        o = oracle_for(r1, box, cfg.r_cut, cfg.r_shell, dt, v1)
+        e0 = o.energies().total
+        errs = []
+        for _ in range(int(round(1.6 / dt / 10))):
+            o.step(10)
+            errs.append(o.energies().total - e0)
+        fl.append(np.std(errs))
+    assert 3.2 < fl[0] / fl[1] < 4.8 and 3.2 < fl[1] / fl[2] < 4.8      # 4 +- 20 %
+
+
+# ---- P11: symmetries -------------------------------------------------------------------------------
+def test_p11_translation_and_permutation():
+    r, box = fluid_state(10, 0.8, 0.2, seed=11)
+    rc, dr = R_WCA, 0.4
+    base = oracle_for(r, box, rc, dr)
+    f0, s0 = base.forces(), base.neighbor_sets()
+    shift = np.array([0.37 * box, 0.91 * box, 0.123])
+    t = oracle_for(np.mod(r + shift, box), box, rc, dr)
+    assert rel_err(t.forces(), f0) < 1e-12
+    st = t.neighbor_sets()
+    assert sum(not np.array_equal(a, b) for a, b in zip(s0, st)) <= 1   # a pair at r_n +- 1e-15 may flip
+    perm = np.random.default_rng(1).permutation(r.shape[0])
+    p = oracle_for(r[perm], box, rc, dr)
+    assert rel_err(p.forces(), f0[perm]) < 1e-12
+    inv = np.empty_like(perm)
+    inv[perm] = np.arange(perm.size)
+    sp = p.neighbor_sets()
+    for new, old in enumerate(perm):
+        assert np.array_equal(np.sort(inv[s0[old]]), sp[new])
+
+
+# ---- P12: neighbor-set invariants and list validity during a run ----------------------------------
+def test_p12_list_invariants_and_validity():
+    cfg = scaled_config("wca_4k", 1728)
+    r, v, _, box = make_state(cfg, 3)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    for it in range(40):
+        o.step(25)
+        pos = o.positions()
+        sets = o.neighbor_sets()
+        if it % 10 == 0:
+            pairs = {(i, int(j)) for i, s in enumerate(sets) for j in s}
+            assert all((j, i) in pairs for (i, j) in pairs)            # symmetric relation
+            assert all(i != j for (i, j) in pairs)                     # no self
+            assert sum(len(s) for s in sets) == len(pairs)             # no duplicates
+        # validity: every pair closer than r_c is in the current list
+        inr = brute_neighbors_sample(pos, box, cfg.r_cut, np.arange(cfg.n_atoms))
+        assert all(np.isin(a, s).all() for a, s in zip(inr, sets))
+    assert o.energies().n_rebuilds > 50
+
+
+# ---- P9: the list statistics the paper prints (statistical pin) -----------------------------------
+@pytest.mark.parametrize("col,n_side", [(0, 32), (1, 30)])
+def test_p9_paper_list_statistics(golden, col, n_side):
+    g = golden("paper_list_statistics.txt")
+    n = n_side ** 3
+    cfg = MDConfig("paper", n, "sc", g["density"][col], g["temperature"][col], g["r_cut"][col],
+                   g["shell"][col], g["dt"][col], 0)
+    r, v, _, box = make_state(cfg, 1)
+    o = oracle_for(r, box, cfg.r_cut, cfg.r_shell, cfg.dt, v)
+    o.step(300)
+    e1 = o.energies()
+    o.step(300)
+    e2 = o.energies()
+    assert e2.mean_neighbors == pytest.approx(g["mean_neighbors"][col], rel=0.10)
+    # max cell occupancy ("layers") grows slowly with N: allow -25 % for our smaller box
+    assert 0.75 * g["layers"][col] <= e2.max_cell_occupancy <= 1.1 * g["layers"][col]
+    # refresh interval: rule = accumulate dt*vmax until delta/2.  vmax ~ sqrt(T ln N): scale our
+    # measurement to the paper's N and nominal T before comparing with the printed 10.2 / 9.8.
+    interval = 300.0 / (e2.n_rebuilds - e1.n_rebuilds)
+    t_meas = e2.ke / (1.5 * (n - 1))
+    scaled = interval * math.sqrt(t_meas / g["temperature"][col]) * math.sqrt(math.log(n) / math.log(g["largest_n"][col]))
+    assert scaled == pytest.approx(g["refresh_interval"][col], rel=0.12)
