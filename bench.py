@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- atom-timesteps/s (fp64) of the MD hot path on B200, per the driver contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config wca_2m] ...
+
+A "step" is one MD time step of the whole hot path (integrate, device-side rebuild decision, cell binning +
+reorder + neighbor matrix when triggered, forces) over all N atoms of the workload.  Default workload:
+BASELINE.json configs[2] at the mid-point shell (WCA fluid, N = 2,097,152 on a 128^3 lattice, rho 0.8, T 1.0,
+dt 0.005, shell 0.4), the size BASELINE.json's metric is quoted on.  Multi-GPU (--gpus N under torchrun) runs N
+independent replicas with different seeds ("replicas only"): no data-path collective.
+
+Prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/) instead, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from md_workloads import get_config, make_state, scaled_config  # noqa: E402
+
+METRIC = "atom-timesteps/sec (fp64)"
+UNIT = "atom-steps/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def load_ncu_traffic(kernel_key):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu summary (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "roofline_traffic.txt")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        for line in fh:
+            line = line.split("#", 1)[0].strip()
+            if line.startswith(kernel_key + " "):
+                return float(line.split()[1])
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(cfg, seed, budget_s, steps=None, n_atoms=None):
+    """Time the oracle as it stands on a bounded sample: returns (atom-steps/s, sample text, threads, steps, N)."""
+    from oracle.md_oracle import OracleMD, get_threads
+    scfg = cfg if not n_atoms or n_atoms == cfg.n_atoms else scaled_config(cfg.name, n_atoms)
+    r, v, bonds, box = make_state(scfg, seed)
+    o = OracleMD(scfg.n_atoms, box, scfg.r_cut, scfg.r_shell, scfg.dt)
+    o.set_state(r, v)
+    if bonds is not None:
+        o.set_bonds(bonds, scfg.fene_k, scfg.fene_r0)
+    t0 = time.perf_counter()
+    o.step(2)
+    per = (time.perf_counter() - t0) / 2
+    if steps is None:
+        steps = int(max(2, min(200, budget_s / max(per, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    rate = scfg.n_atoms * steps / dt
+    sample = (f"{steps} steps of {scfg.name} (N={scfg.n_atoms}) from the t=0 lattice state after 2 untimed steps, "
+              f"rebuilds included, {dt:.1f} s")
+    return rate, sample, get_threads(), steps, scfg.n_atoms
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores; K steps, each over a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle.md_oracle import OracleMD, get_threads
+    # calibrate on a small system, then pick the largest lattice that keeps (K + W) steps within ~150 s
+    small = scaled_config(cfg.name, 32 ** 3) if cfg.lattice == "sc" else scaled_config(cfg.name, 4 * 16 ** 3) \
+        if cfg.lattice == "fcc" else scaled_config(cfg.name, 64 * cfg.chain_len * 8)
+    rate0, _, _, _, _ = oracle_rate(small, 1, 2.0)
+    want = rate0 * 150.0 / max(1, args.steps + args.warmup)
+    if cfg.lattice == "sc":
+        side = int(min(round(cfg.n_atoms ** (1 / 3)), max(16, int(want ** (1 / 3)))))
+        n = side ** 3
+    elif cfg.lattice == "fcc":
+        side = int(min(round((cfg.n_atoms / 4) ** (1 / 3)), max(8, int((want / 4) ** (1 / 3)))))
+        n = 4 * side ** 3
+    else:
+        n = int(min(cfg.n_atoms, max(64 * cfg.chain_len, (int(want) // (64 * cfg.chain_len)) * 64 * cfg.chain_len)))
+    scfg = cfg if n == cfg.n_atoms else scaled_config(cfg.name, n)
+    r, v, bonds, box = make_state(scfg, 1)
+    o = OracleMD(scfg.n_atoms, box, scfg.r_cut, scfg.r_shell, scfg.dt)
+    o.set_state(r, v)
+    if bonds is not None:
+        o.set_bonds(bonds, scfg.fene_k, scfg.fene_r0)
+    o.step(args.warmup)
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    dt = time.perf_counter() - t0
+    value = scfg.n_atoms * args.steps / dt
+    sample = f"each step = one oracle time step over N={scfg.n_atoms} atoms of {cfg.name}'s state point ({scfg.lattice} lattice start)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_atoms": cfg.n_atoms, "sample_n_atoms": scfg.n_atoms},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": get_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="wca_2m")
+    ap.add_argument("--variant", default="full", choices=["full", "newton3"])
+    ap.add_argument("--mode", default="fused", choices=["fused", "split"])
+    ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    cfg = get_config(args.config)
+
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import paper_2003_14061_b200 as md
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the MD path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    seed = 1 + rank
+    r0, v0, bonds, box = make_state(cfg, seed)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=args.variant,
+                    step_mode=args.mode if args.variant == "full" else "split", block_size=args.block)
+    g.set_state(r0, v0)
+    if bonds is not None:
+        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    info = g.info()
+    n = cfg.n_atoms
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps --------------------------
+    g.step(args.warmup)
+    e_start = g.energies()
+    launches0 = g.info()["kernel_launches"]
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall0 = time.perf_counter()
+    ev0.record()
+    g.step(args.steps)
+    ev1.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = g.info()["kernel_launches"] - launches0
+    e_end = g.energies()
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * n * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel-class device timers over a second pass of K steps (Table 2 of the paper; roofline) ----
+    g.set_profiling(True)
+    g.reset_timers()
+    g.step(args.steps)
+    timers = g.timers()
+    g.set_profiling(False)
+    e_prof = g.energies()
+    rebuilds_prof = e_prof.n_rebuilds - e_end.n_rebuilds
+    mbar = 0.5 * (e_end.mean_neighbors + e_prof.mean_neighbors)
+    peak, peak_src = load_peaks()
+    if args.mode == "fused" and args.variant == "full":
+        kname, tk = "k_force<fused step>", timers["fused_step"]
+        bytes_per_atom = 28.0 * mbar + 100.0     # W 4m + m_i 4 + r_i 24 + gathers 24m + v r/w 48 + r' write 24
+    else:
+        kname, tk = "k_force", timers["force"]
+        bytes_per_atom = 28.0 * mbar + 52.0      # SURVEY 8(d) B_ns: W 4m + m_i 4 + r_i 24 + gathers 24m + f write 24
+        if args.variant == "newton3":
+            tk = dict(tk, launches=tk["launches"] // 2)
+    dur_ms = tk["ms"] / max(1, tk["launches"])
+    achieved = bytes_per_atom * n / (dur_ms * 1e-3) / 1e9
+    floor_bytes = 4.0 * mbar + 100.0
+    traffic = load_ncu_traffic(f"{args.config}:{kname}")
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_atom": bytes_per_atom, "mean_neighbors": mbar, "avg_launch_ms": dur_ms,
+                "accounting": "north_star B_ns (every gather charged 24 B)",
+                "frac_compulsory": floor_bytes * n / (dur_ms * 1e-3) / 1e9 / peak,
+                "compulsory_bytes_per_atom": floor_bytes}
+    nebr = timers["nebr"]
+    breakdown = {k: round(v["ms"] / args.steps, 6) for k, v in timers.items()}
+    nebr_info = {"rebuilds": int(rebuilds_prof), "ms_per_rebuild": nebr["ms"] / max(1, rebuilds_prof),
+                 "steps_per_rebuild": args.steps / max(1, rebuilds_prof)}
+
+    # ---- end to end through the C ABI with HOST buffers: H2D state, one step, D2H positions + energies ------
+    e2e = None
+    if not args.no_e2e:
+        rh, vh = g.positions(), g.velocities()
+        out = np.empty_like(rh)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            g.set_state(rh, vh)          # host -> device (pinned staging inside the library), rebuild, forces
+            g.step(1)
+            g.positions(out)             # device -> host
+            vh = g.velocities()
+            en = g.energies()
+            rh = out
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
+               "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
+               "what": "md_set_state(host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        rate, sample, cores, _, _ = oracle_rate(cfg, 1, args.cpu_seconds)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_atoms": n, "lattice": cfg.lattice, "density": cfg.density,
+                   "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
+                   "force_variant": args.variant, "step_mode": args.mode, "block_size": info["block_size"],
+                   "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
+                   "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "l2": "working set per step (positions 2x64 MB, velocities 48 MB, W rows ~100 MB) exceeds the 126 MB L2; no flush"},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "wall_s": t_wall, "rebuilds_in_timed_region": int(e_end.n_rebuilds - e_start.n_rebuilds),
+        "energy_per_atom": {"start": e_start.total / n, "end": e_end.total / n},
+        "temperature_end": e_end.ke / (1.5 * (n - 1)),
+        "ms_per_step_by_kernel_class": breakdown, "neighbor_build": nebr_info,
+        "device": info["device_name"],
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

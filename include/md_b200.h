@@ -1,0 +1,175 @@
+/*
+ * md_b200.h -- C ABI of the B200 (sm_100a) short-range molecular-dynamics hot path.
+ *
+ * The library implements, in hand-written CUDA, the per-time-step path of
+ * D. C. Rapaport, "GPU molecular dynamics: Algorithms and performance" (arXiv 2003.14061):
+ *   cell assignment and occupancy counting          (steps N1-N2)
+ *   cell ordering of the atoms by prefix scan        (N3-N4 and the reorder of sec. 2.4(4))
+ *   neighbor-matrix construction W[m][i]             (N5; layout PAPER.md:68)
+ *   pair forces over W without / with Newton's 3rd   (F1)
+ *   leapfrog integration with periodic wrap          (Table 2 "integration")
+ *   energy / virial / momentum / max-velocity sums   (F2 and the reductions of PAPER.md:58, 64-66)
+ *   displacement-triggered rebuild of W
+ *   optional FENE bond lists for polymer chains
+ * The paper prints no equations; the model (truncated, energy-shifted Lennard-Jones; two-half-kick
+ * leapfrog; rebuild when the accumulated dt*max|v| exceeds r_shell/2) is fixed in DESIGN.md, "Readings".
+ *
+ * Conventions
+ *   - Reduced units (sigma = epsilon = m = 1).  Cubic periodic box [0, L)^3.  All arithmetic is fp64.
+ *   - Every array argument is a HOST pointer owned by the caller unless its name ends in `_device`.
+ *     Layout of per-atom vectors at the boundary: xyz[3*i + k], i = ORIGINAL atom id (the device keeps
+ *     atoms in cell order and re-sorts them at every rebuild; that is invisible here).
+ *   - No C++ exceptions cross the boundary.  Functions returning int give MD_OK (0) or a negative
+ *     md_status; md_last_error() returns a thread-local description of the last failure.
+ *   - The library runs on the CUDA stream given in md_params.stream (0 = a stream it creates) and
+ *     allocates device memory through the hooks given to md_set_allocator (default cudaMalloc/cudaFree).
+ *   - There is no CPU fallback: without a CUDA device every call that needs one fails with MD_ERR_CUDA.
+ */
+#ifndef MD_B200_H
+#define MD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define MD_API __attribute__((visibility("default")))
+#else
+#define MD_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct md_system md_system;
+
+typedef enum md_status {
+    MD_OK = 0,
+    MD_ERR_INVALID = -1,        /* bad argument or call order */
+    MD_ERR_NEBR_OVERFLOW = -2,  /* some atom has more than Mmax neighbors (never truncated silently) */
+    MD_ERR_BOND_BROKEN = -3,    /* a FENE bond reached r >= R0 */
+    MD_ERR_NONFINITE = -4,      /* NaN/Inf in the state */
+    MD_ERR_CUDA = -5,           /* CUDA runtime error (text in md_last_error) */
+    MD_ERR_UNSUPPORTED = -6,    /* e.g. fewer than 3 cells per edge, more than 2 bonds per atom */
+    MD_ERR_NOMEM = -7
+} md_status;
+
+enum { MD_LATTICE_AUTO = 0, MD_LATTICE_SC = 1, MD_LATTICE_FCC = 2, MD_LATTICE_NONE = 3 };
+/* force_variant: the trade-off of PAPER.md:68 */
+enum { MD_FORCE_FULL_LIST = 0,      /* A: one thread per atom, every pair twice, no Newton-3, no atomics */
+       MD_FORCE_NEWTON3_ATOMICS = 1 /* B: half list, f_j updated with fp64 atomics */ };
+/* step_mode: how one time step is mapped to kernels */
+enum { MD_STEP_FUSED = 0,           /* force + kick + drift in one kernel (leapfrog form), variant A only */
+       MD_STEP_SPLIT = 1            /* the paper's structure: integrate / force / integrate as separate kernels */ };
+
+/* Parameters of md_create_ex.  Fill with md_params_default() first.  The library copies it. */
+typedef struct md_params {
+    int64_t  n_atoms;
+    double   box;            /* L; if <= 0 it is (n_atoms/density)^(1/3) */
+    double   density;        /* used when box <= 0; if both are given they must agree to 1e-12 relative */
+    double   r_cut;          /* r_c: pair cutoff (2^(1/6) gives the soft-sphere / WCA system) */
+    double   r_shell;        /* delta: neighbor shell thickness */
+    double   dt;
+    uint64_t seed;           /* seed of the counter-based velocity generator */
+    double   temperature;    /* initial velocities: Gaussian, zero net momentum, sum v^2 = 3(N-1)T */
+    int32_t  lattice;        /* MD_LATTICE_*; NONE: call md_set_state before stepping */
+    int32_t  force_variant;  /* MD_FORCE_* */
+    int32_t  step_mode;      /* MD_STEP_* (NEWTON3 forces imply SPLIT) */
+    int32_t  max_neighbors;  /* Mmax, rows of W; 0 = auto: multiple of 16 >= 1.35*(4/3)pi r_n^3 rho + 12 */
+    int32_t  block_size;     /* threads per block of the per-atom kernels; 0 = default */
+    int32_t  device;         /* CUDA device ordinal; -1 = current */
+    void    *stream;         /* cudaStream_t to run on; NULL = the library creates its own */
+    uint32_t flags;          /* MD_FLAG_* */
+} md_params;
+
+enum { MD_FLAG_NO_GRAPH = 1u  /* launch kernels one by one instead of replaying a captured CUDA graph */ };
+
+/* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */
+typedef struct md_energy {
+    double  ke;                 /* 1/2 sum |v|^2 */
+    double  pe_pair;            /* 1/2 sum_i u_i  (u_i counts each pair twice: "actually 2U") */
+    double  pe_bond;            /* FENE energy */
+    double  virial;             /* sum over pairs of f_ij . r_ij (pair + bond) */
+    double  px, py, pz;         /* total momentum */
+    double  vmax;               /* max |v| */
+    int64_t step;               /* steps taken since creation / md_set_state */
+    int64_t n_rebuilds;         /* neighbor-matrix rebuilds since then (initial build not counted) */
+    int32_t max_neighbors;      /* max_i m_i of the current matrix */
+    int32_t max_cell_occupancy; /* max_c k_c of the last binning (the paper's layer count N_l) */
+    double  mean_neighbors;     /* mean m_i of the current matrix, FULL-list convention for both variants */
+} md_energy;
+
+typedef struct md_info {
+    int64_t n_atoms, n_pad;     /* n_pad: row pitch of W (atoms rounded up to 128) */
+    double  box, r_neighbor, cell_width;
+    int32_t cells_per_edge, max_neighbors, block_size, force_variant, step_mode, n_bonds_per_atom_max;
+    int64_t device_bytes;       /* device memory held by this system */
+    int64_t kernel_launches;    /* kernels launched by this system since creation */
+    char    device_name[64];
+} md_info;
+
+/* Kernel classes of md_get_timers, after Table 2 of the paper. */
+enum { MD_T_INTEGRATE = 0, MD_T_CELLS = 1, MD_T_REORDER = 2, MD_T_NEBR = 3, MD_T_FORCE = 4, MD_T_ENERGY = 5,
+       MD_T_FUSED_STEP = 6, MD_T_COUNT = 8 };
+
+MD_API void md_params_default(md_params *p);
+
+/* PAPER.md:107 states the problem as: N atoms on a cubic grid, density, cutoff, shell, time step, random
+ * velocities.  Lattice: SC when N is a perfect cube, else FCC when N/4 is; T = 1; variant A, fused steps.
+ * Returns NULL on failure.  On return the neighbor matrix, forces and energies at t = 0 are valid. */
+MD_API md_system *md_create(int64_t n_atoms, double box, double density, double r_cut, double r_shell, double dt,
+                     uint64_t seed);
+MD_API md_system *md_create_ex(const md_params *p);
+MD_API void md_destroy(md_system *s);
+
+/* Optional bond list for the chain workload: n_bonds pairs ij[2*b], ij[2*b+1] of ORIGINAL
+ * atom ids, FENE force -k r / (1 - r^2/R0^2) on top of the pair force (which also acts on bonded pairs).
+ * At most 2 bonds per atom (linear chains).  Only before the first md_step after create / md_set_state.
+ * Forces and energies are re-evaluated. */
+MD_API int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, double R0);
+
+/* Advance n time steps.  Asynchronous on the stream except for one status read at the end.
+ * After an error other than MD_ERR_INVALID the state is undefined; only md_destroy is valid. */
+MD_API int md_step(md_system *s, int64_t n);
+
+/* Energy / virial / momentum / max-velocity reductions of the current state.  Synchronises. */
+MD_API int md_energies(md_system *s, md_energy *out);
+
+/* xyz: host, 3*N doubles, original-id order.  Positions are wrapped into [0, L).  Synchronise. */
+MD_API int md_get_positions(md_system *s, double *xyz);
+MD_API int md_get_velocities(md_system *s, double *xyz);
+MD_API int md_get_forces(md_system *s, double *xyz);
+
+/* Replace positions and velocities (host, 3*N each, original-id order; vxyz may be NULL = keep).
+ * Positions must lie in [0, L].  Re-bins, rebuilds W, re-evaluates forces, resets step and rebuild
+ * counters and the displacement accumulator; bonds are kept. */
+MD_API int md_set_state(md_system *s, const double *xyz, const double *vxyz);
+
+/* Test hooks.  md_rebuild_neighbors forces a rebuild now.  md_get_neighbors returns the matrix by ORIGINAL
+ * ids: counts[N]; list[N * max_neighbors] with row i = neighbors of atom i (unordered, -1 padded); for the
+ * Newton-3 variant the half list is symmetrised so both variants return the full relation.
+ * list may be NULL (counts only). */
+MD_API int md_rebuild_neighbors(md_system *s);
+MD_API int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_neighbors_out);
+
+MD_API int md_get_info(md_system *s, md_info *out);
+
+/* Per-kernel-class device timers (CUDA events on the library's stream around every launch while enabled).
+ * ms[MD_T_COUNT], launches[MD_T_COUNT] accumulate since the last md_reset_timers.  Synchronises. */
+MD_API int md_set_profiling(md_system *s, int enabled);
+MD_API int md_get_timers(md_system *s, double *ms, int64_t *launches);
+MD_API int md_reset_timers(md_system *s);
+
+/* Device-memory hooks (process-wide; set before md_create*).  alloc(bytes, stream, user) returns a device
+ * pointer or NULL; free_(ptr, user).  The Python binding routes these to torch's caching allocator. */
+typedef void *(*md_alloc_fn)(size_t bytes, void *stream, void *user);
+typedef void (*md_free_fn)(void *ptr, void *user);
+MD_API void md_set_allocator(md_alloc_fn alloc, md_free_fn free_, void *user);
+
+MD_API const char *md_last_error(void);
+MD_API const char *md_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_B200_H */

@@ -1,0 +1,10 @@
+"""B200-native (sm_100a) short-range molecular dynamics hot path of arXiv 2003.14061 (Rapaport).
+
+The product is the C-ABI library `libmd_b200.so` (include/md_b200.h, sources in csrc/); this package is its
+thin Python binding.  Build with `python -m paper_2003_14061_b200.build`.
+"""
+from .binding import (Energies, MDError, MDSystem, load_library, use_torch_allocator, EXPORTS, LIB_PATH,
+                      TIMER_NAMES)
+
+__all__ = ["Energies", "MDError", "MDSystem", "load_library", "use_torch_allocator", "EXPORTS", "LIB_PATH",
+           "TIMER_NAMES"]

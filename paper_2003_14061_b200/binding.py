@@ -1,0 +1,269 @@
+"""Thin ctypes binding of libmd_b200.so (include/md_b200.h): argument marshalling only.
+
+Every step of the MD path runs in the CUDA kernels of the library.  PyTorch supplies device memory
+(its caching allocator, through md_set_allocator) and the stream.  There is no CPU fallback: if the
+library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libmd_b200.so")
+
+MD_OK, MD_ERR_INVALID, MD_ERR_NEBR_OVERFLOW, MD_ERR_BOND_BROKEN = 0, -1, -2, -3
+MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM = -4, -5, -6, -7
+LATTICE = {"auto": 0, "sc": 1, "fcc": 2, "none": 3}
+FORCE_VARIANT = {"full": 0, "newton3": 1}
+STEP_MODE = {"fused": 0, "split": 1}
+TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "reserved")
+
+EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_step", "md_energies",
+           "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",
+           "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
+           "md_set_allocator", "md_last_error", "md_version")
+
+
+class MDError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"md_b200 error {code}: {msg}")
+        self.code = code
+
+
+class _Params(C.Structure):
+    _fields_ = [("n_atoms", C.c_int64), ("box", C.c_double), ("density", C.c_double), ("r_cut", C.c_double),
+                ("r_shell", C.c_double), ("dt", C.c_double), ("seed", C.c_uint64), ("temperature", C.c_double),
+                ("lattice", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
+                ("max_neighbors", C.c_int32), ("block_size", C.c_int32), ("device", C.c_int32),
+                ("stream", C.c_void_p), ("flags", C.c_uint32)]
+
+
+class _Energy(C.Structure):
+    _fields_ = [("ke", C.c_double), ("pe_pair", C.c_double), ("pe_bond", C.c_double), ("virial", C.c_double),
+                ("px", C.c_double), ("py", C.c_double), ("pz", C.c_double), ("vmax", C.c_double),
+                ("step", C.c_int64), ("n_rebuilds", C.c_int64),
+                ("max_neighbors", C.c_int32), ("max_cell_occupancy", C.c_int32), ("mean_neighbors", C.c_double)]
+
+
+class _Info(C.Structure):
+    _fields_ = [("n_atoms", C.c_int64), ("n_pad", C.c_int64), ("box", C.c_double), ("r_neighbor", C.c_double),
+                ("cell_width", C.c_double), ("cells_per_edge", C.c_int32), ("max_neighbors", C.c_int32),
+                ("block_size", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
+                ("n_bonds_per_atom_max", C.c_int32), ("device_bytes", C.c_int64), ("kernel_launches", C.c_int64),
+                ("device_name", C.c_char * 64)]
+
+
+@dataclass
+class Energies:
+    ke: float
+    pe_pair: float
+    pe_bond: float
+    virial: float
+    px: float
+    py: float
+    pz: float
+    vmax: float
+    step: int
+    n_rebuilds: int
+    max_neighbors: int
+    max_cell_occupancy: int
+    mean_neighbors: float
+
+    @property
+    def pe(self) -> float:
+        return self.pe_pair + self.pe_bond
+
+    @property
+    def total(self) -> float:
+        return self.ke + self.pe
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+_dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_ip = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+
+_lib = None
+_keep = []          # callback objects must outlive the library's use of them
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen the C-ABI library and declare signatures.  Needs no GPU."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise MDError(MD_ERR_CUDA, f"{path} not built: run `python -m paper_2003_14061_b200.build` "
+                                   "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    L.md_params_default.argtypes = [C.POINTER(_Params)]
+    L.md_create.restype = C.c_void_p
+    L.md_create.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_uint64]
+    L.md_create_ex.restype = C.c_void_p
+    L.md_create_ex.argtypes = [C.POINTER(_Params)]
+    L.md_destroy.argtypes = [C.c_void_p]
+    L.md_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
+    L.md_step.argtypes = [C.c_void_p, C.c_int64]
+    L.md_energies.argtypes = [C.c_void_p, C.POINTER(_Energy)]
+    for n in ("md_get_positions", "md_get_velocities", "md_get_forces"):
+        getattr(L, n).argtypes = [C.c_void_p, _dp]
+    L.md_set_state.argtypes = [C.c_void_p, _dp, C.c_void_p]
+    L.md_rebuild_neighbors.argtypes = [C.c_void_p]
+    L.md_get_neighbors.argtypes = [C.c_void_p, _ip, C.c_void_p, C.POINTER(C.c_int32)]
+    L.md_get_info.argtypes = [C.c_void_p, C.POINTER(_Info)]
+    L.md_set_profiling.argtypes = [C.c_void_p, C.c_int]
+    L.md_get_timers.argtypes = [C.c_void_p, _dp, np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")]
+    L.md_reset_timers.argtypes = [C.c_void_p]
+    L.md_set_allocator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.md_last_error.restype = C.c_char_p
+    L.md_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def use_torch_allocator():
+    """Route the library's device allocations to torch's caching allocator."""
+    import torch
+    L = load_library()
+
+    def _alloc(nbytes, stream, _user):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+        except Exception:
+            return None
+
+    def _free(ptr, _user):
+        try:
+            torch.cuda.caching_allocator_delete(int(ptr))
+        except Exception:
+            pass
+
+    a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
+    _keep.extend([a, f])
+    L.md_set_allocator(C.cast(a, C.c_void_p), C.cast(f, C.c_void_p), None)
+
+
+def _err(L):
+    return (L.md_last_error() or b"").decode()
+
+
+class MDSystem:
+    """One MD system on one GPU (the handle of md_create_ex)."""
+
+    def __init__(self, n_atoms, r_cut, r_shell, dt, box=0.0, density=0.0, seed=1, temperature=1.0, lattice="auto",
+                 force_variant="full", step_mode="fused", max_neighbors=0, block_size=0, device=-1,
+                 torch_memory=True, flags=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise MDError(MD_ERR_CUDA, "no CUDA device: the MD path has no CPU fallback")
+        L = load_library()
+        if torch_memory and not _keep:
+            use_torch_allocator()
+        p = _Params()
+        L.md_params_default(C.byref(p))
+        p.n_atoms, p.box, p.density, p.r_cut, p.r_shell, p.dt = int(n_atoms), box, density, r_cut, r_shell, dt
+        p.seed, p.temperature = int(seed), temperature
+        p.lattice, p.force_variant, p.step_mode = LATTICE[lattice], FORCE_VARIANT[force_variant], STEP_MODE[step_mode]
+        p.max_neighbors, p.block_size, p.device, p.flags = max_neighbors, block_size, device, flags
+        p.stream = torch.cuda.current_stream().cuda_stream or None
+        self._L = L
+        self._h = L.md_create_ex(C.byref(p))
+        if not self._h:
+            raise MDError(MD_ERR_INVALID, _err(L))
+        self.n = int(n_atoms)
+
+    @classmethod
+    def from_config(cls, cfg, **kw):
+        lattice = kw.pop("lattice", cfg.lattice if cfg.lattice in ("sc", "fcc") else "none")
+        return cls(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, density=cfg.density, temperature=cfg.temperature,
+                   lattice=lattice, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.md_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != MD_OK:
+            raise MDError(rc, _err(self._L))
+
+    def set_state(self, r, v=None):
+        r = np.ascontiguousarray(r, np.float64)
+        vp = None
+        if v is not None:
+            v = np.ascontiguousarray(v, np.float64)
+            vp = v.ctypes.data_as(C.c_void_p)
+        self._ck(self._L.md_set_state(self._h, r, vp))
+
+    def set_bonds(self, bonds, k, r0):
+        b = np.ascontiguousarray(bonds, np.int32).reshape(-1, 2)
+        self._ck(self._L.md_set_bonds(self._h, b.shape[0], b, float(k), float(r0)))
+
+    def step(self, n=1):
+        self._ck(self._L.md_step(self._h, int(n)))
+
+    def rebuild_neighbors(self):
+        self._ck(self._L.md_rebuild_neighbors(self._h))
+
+    def energies(self) -> Energies:
+        e = _Energy()
+        self._ck(self._L.md_energies(self._h, C.byref(e)))
+        return Energies(**{k: getattr(e, k) for k, _ in _Energy._fields_})
+
+    def _get(self, name, out=None):
+        if out is None:
+            out = np.empty((self.n, 3))
+        self._ck(getattr(self._L, name)(self._h, out))
+        return out
+
+    def positions(self, out=None):
+        return self._get("md_get_positions", out)
+
+    def velocities(self, out=None):
+        return self._get("md_get_velocities", out)
+
+    def forces(self, out=None):
+        return self._get("md_get_forces", out)
+
+    def neighbors(self, with_list=True):
+        """(counts[N], list[N, Mmax] of original ids, -1 padded)."""
+        info = self.info()
+        counts = np.empty(self.n, np.int32)
+        lst = np.empty((self.n, info["max_neighbors"]), np.int32) if with_list else None
+        mm = C.c_int32(0)
+        self._ck(self._L.md_get_neighbors(self._h, counts, lst.ctypes.data_as(C.c_void_p) if with_list else None,
+                                          C.byref(mm)))
+        return counts, lst
+
+    def neighbor_sets(self):
+        counts, lst = self.neighbors()
+        return [np.sort(lst[i, :counts[i]]) for i in range(self.n)]
+
+    def info(self) -> dict:
+        i = _Info()
+        self._ck(self._L.md_get_info(self._h, C.byref(i)))
+        d = {k: getattr(i, k) for k, _ in _Info._fields_}
+        d["device_name"] = d["device_name"].decode()
+        return d
+
+    def set_profiling(self, on: bool):
+        self._ck(self._L.md_set_profiling(self._h, int(bool(on))))
+
+    def reset_timers(self):
+        self._ck(self._L.md_reset_timers(self._h))
+
+    def timers(self) -> dict:
+        ms = np.zeros(8)
+        n = np.zeros(8, np.int64)
+        self._ck(self._L.md_get_timers(self._h, ms, n))
+        return {name: {"ms": float(ms[k]), "launches": int(n[k])} for k, name in enumerate(TIMER_NAMES) if name != "reserved"}

@@ -1,0 +1,589 @@
+// C-ABI layer of the MD hot path: argument checks, device memory, the time-step driver.  All arithmetic
+// of the method runs in the kernels of md_kernels.cu; the host loop below only enqueues them (PAPER.md:79:
+// "Essentially all computation is done on the GPU").  See include/md_b200.h for the contract of each call.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "md_init.h"
+#include "md_types.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+md_alloc_fn g_alloc = nullptr;
+md_free_fn g_free = nullptr;
+void *g_alloc_user = nullptr;
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            set_error("%s failed at %s:%d: %s", #call, __FILE__, __LINE__, cudaGetErrorString(e__)); \
+            return MD_ERR_CUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+struct EvPair {
+    cudaEvent_t a, b;
+    int cls;
+};
+
+}  // namespace
+
+struct md_system {
+    md_params prm;
+    MdDev P;
+    MdLaunch lc;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    int device = 0;
+    char device_name[64] = "";
+    std::vector<void *> allocs;
+    int64_t bytes = 0;
+    DevCtrl *h_ctrl = nullptr;     // pinned
+    double *h_stage = nullptr;     // pinned staging, 6 N doubles
+    int64_t step = 0;
+    int64_t launches = 0;
+    bool has_state = false;
+    bool stepped = false;
+    int n_bonds_max = 0;
+    double r_n = 0, cell_w = 0;
+    // profiling
+    bool profiling = false;
+    std::vector<EvPair> pending, pool;
+    double t_ms[MD_T_COUNT] = {0};
+    int64_t t_n[MD_T_COUNT] = {0};
+};
+
+namespace {
+
+void *dev_alloc(md_system *s, size_t bytes)
+{
+    void *p = nullptr;
+    bytes = (bytes + 255) & ~(size_t)255;
+    if (g_alloc) p = g_alloc(bytes, (void *)s->stream, g_alloc_user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+    if (!p) return nullptr;
+    s->allocs.push_back(p);
+    s->bytes += (int64_t)bytes;
+    cudaMemsetAsync(p, 0, bytes, s->stream);
+    return p;
+}
+
+void dev_free_all(md_system *s)
+{
+    for (void *p : s->allocs) {
+        if (g_free) g_free(p, g_alloc_user);
+        else cudaFree(p);
+    }
+    s->allocs.clear();
+}
+
+// RAII bracket: CUDA events around one launch wrapper while profiling is on
+struct Timed {
+    md_system *s;
+    EvPair ev;
+    bool on;
+    Timed(md_system *s_, int cls, int n_launch) : s(s_), on(s_->profiling)
+    {
+        s->launches += n_launch;
+        s->t_n[cls] += n_launch;
+        if (!on) return;
+        if (!s->pool.empty()) { ev = s->pool.back(); s->pool.pop_back(); }
+        else { cudaEventCreate(&ev.a); cudaEventCreate(&ev.b); }
+        ev.cls = cls;
+        cudaEventRecord(ev.a, s->stream);
+    }
+    ~Timed()
+    {
+        if (!on) return;
+        cudaEventRecord(ev.b, s->stream);
+        s->pending.push_back(ev);
+    }
+};
+
+void resolve_timers(md_system *s)
+{
+    for (EvPair &e : s->pending) {
+        cudaEventSynchronize(e.b);
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.a, e.b) == cudaSuccess) s->t_ms[e.cls] += (double)ms;
+        s->pool.push_back(e);
+    }
+    s->pending.clear();
+}
+
+int fetch_ctrl(md_system *s)
+{
+    CK(cudaMemcpyAsync(s->h_ctrl, s->P.ctrl, sizeof(DevCtrl), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaGetLastError());
+    return MD_OK;
+}
+
+int check_device_status(md_system *s)
+{
+    int rc = fetch_ctrl(s);
+    if (rc) return rc;
+    const int err = s->h_ctrl->err;
+    if (err) {
+        switch (err) {
+        case MD_ERR_NEBR_OVERFLOW:
+            set_error("neighbor matrix overflow: some atom has more than Mmax = %d neighbors", s->P.Mmax);
+            break;
+        case MD_ERR_BOND_BROKEN: set_error("FENE bond stretched to r >= R0"); break;
+        case MD_ERR_NONFINITE: set_error("non-finite position or velocity"); break;
+        default: set_error("device error %d", err);
+        }
+    }
+    return err;
+}
+
+// cells + reorder + neighbor matrix.  Always enqueued; the kernels return at once unless the device-side
+// decision (decide() in md_kernels.cu) asked for a rebuild.
+void enqueue_rebuild(md_system *s)
+{
+    { Timed t(s, MD_T_CELLS, mdk_launches_of(LK_CELLS)); mdk_cells(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_REORDER, s->P.has_bonds ? 2 : 1); mdk_reorder(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_NEBR, 1); mdk_build(s->P, s->lc, s->stream); }
+}
+
+void enqueue_forces_only(md_system *s)
+{
+    if (s->P.half_list) { Timed t(s, MD_T_FORCE, 2); mdk_force_newton3(s->P, s->lc, s->stream); }
+    else { Timed t(s, MD_T_FORCE, 1); mdk_force(s->P, s->lc, 0, s->stream); }
+}
+
+// state already in scratch (xyz | vxyz, original order): load, bin, build W, evaluate forces
+int install_state(md_system *s)
+{
+    s->launches += 2;
+    mdk_load_state(s->P, s->stream);
+    mdk_force_rebuild(s->P, s->stream);
+    enqueue_rebuild(s);
+    enqueue_forces_only(s);
+    s->step = 0;
+    s->stepped = false;
+    s->has_state = true;
+    int rc = check_device_status(s);
+    if (rc) return rc;
+    // the initial build is not counted as a rebuild
+    s->h_ctrl->n_rebuilds = 0;
+    CK(cudaMemsetAsync(&s->P.ctrl->n_rebuilds, 0, sizeof(int), s->stream));
+    return MD_OK;
+}
+
+int upload_state(md_system *s, const double *xyz, const double *vxyz)
+{
+    const size_t n3 = 3 * (size_t)s->P.N;
+    if (!vxyz) {   // keep velocities: bring them to original order in the second half of scratch first
+        if (!s->has_state) { set_error("md_set_state: no velocities to keep"); return MD_ERR_INVALID; }
+        s->launches += 1;
+        mdk_export(s->P, 1, n3, s->stream);
+    }
+    memcpy(s->h_stage, xyz, n3 * sizeof(double));
+    CK(cudaMemcpyAsync(s->P.scratch, s->h_stage, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    if (vxyz) {
+        memcpy(s->h_stage + n3, vxyz, n3 * sizeof(double));
+        CK(cudaMemcpyAsync(s->P.scratch + n3, s->h_stage + n3, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    }
+    return install_state(s);
+}
+
+int download(md_system *s, int what, double *out)
+{
+    if (!s || !out) { set_error("null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("no state loaded"); return MD_ERR_INVALID; }
+    const size_t n3 = 3 * (size_t)s->P.N;
+    s->launches += 1;
+    mdk_export(s->P, what, 0, s->stream);
+    CK(cudaMemcpyAsync(s->h_stage, s->P.scratch, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaGetLastError());
+    memcpy(out, s->h_stage, n3 * sizeof(double));
+    return MD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *md_last_error(void) { return g_err; }
+const char *md_version(void) { return "md_b200 0.1 (sm_100a)"; }
+
+void md_set_allocator(md_alloc_fn alloc, md_free_fn free_, void *user)
+{
+    g_alloc = alloc;
+    g_free = free_;
+    g_alloc_user = user;
+}
+
+void md_params_default(md_params *p)
+{
+    if (!p) return;
+    memset(p, 0, sizeof(*p));
+    p->temperature = 1.0;
+    p->lattice = MD_LATTICE_AUTO;
+    p->force_variant = MD_FORCE_FULL_LIST;
+    p->step_mode = MD_STEP_FUSED;
+    p->device = -1;
+}
+
+void md_destroy(md_system *s)
+{
+    if (!s) return;
+    if (s->stream) cudaStreamSynchronize(s->stream);
+    for (EvPair &e : s->pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (EvPair &e : s->pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    dev_free_all(s);
+    if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
+    if (s->h_stage) cudaFreeHost(s->h_stage);
+    if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
+    delete s;
+}
+
+md_system *md_create_ex(const md_params *pp)
+{
+    if (!pp) { set_error("md_create_ex: null params"); return nullptr; }
+    md_params p = *pp;
+    if (p.n_atoms <= 0 || p.n_atoms >= (1ll << 29)) { set_error("n_atoms must be in [1, 2^29)"); return nullptr; }
+    if (!(p.r_cut > 0) || !(p.r_shell >= 0) || !(p.dt > 0) || !(p.temperature >= 0)) {
+        set_error("r_cut, dt must be > 0; r_shell, temperature >= 0");
+        return nullptr;
+    }
+    if (p.box > 0) {
+        if (p.density > 0) {
+            const double d = (double)p.n_atoms / (p.box * p.box * p.box);
+            if (fabs(d - p.density) > 1e-12 * p.density) { set_error("box and density disagree"); return nullptr; }
+        }
+    } else if (p.density > 0) {
+        p.box = cbrt((double)p.n_atoms / p.density);
+    } else {
+        set_error("give box or density");
+        return nullptr;
+    }
+    p.density = (double)p.n_atoms / (p.box * p.box * p.box);
+    if (p.force_variant != MD_FORCE_FULL_LIST && p.force_variant != MD_FORCE_NEWTON3_ATOMICS) { set_error("bad force_variant"); return nullptr; }
+    if (p.force_variant == MD_FORCE_NEWTON3_ATOMICS) p.step_mode = MD_STEP_SPLIT;
+    if (p.step_mode != MD_STEP_FUSED && p.step_mode != MD_STEP_SPLIT) { set_error("bad step_mode"); return nullptr; }
+    if (p.block_size == 0) p.block_size = 128;
+    if (p.block_size != 64 && p.block_size != 128 && p.block_size != 256 && p.block_size != 512) {
+        set_error("block_size must be 64, 128, 256 or 512");
+        return nullptr;
+    }
+    const double rn = p.r_cut + p.r_shell;
+    int nc = (int)floor(p.box / rn);
+    if (nc >= 1 && p.box / nc - rn < 1e-9 * rn) nc -= 1;     // keep the cell strictly wider than r_n
+    if (nc < 3) { set_error("box too small: %d cells per edge (need >= 3)", nc); return nullptr; }
+    if ((int64_t)nc * nc * nc > (1ll << 30)) { set_error("too many cells"); return nullptr; }
+    if (p.max_neighbors <= 0) {
+        const double ideal = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
+        p.max_neighbors = 16 * (int)ceil((1.35 * ideal + 12.0) / 16.0);
+    }
+    if (p.lattice == MD_LATTICE_AUTO) {
+        p.lattice = md_init_pick_lattice(p.n_atoms);
+        if (!p.lattice) { set_error("n_atoms fits neither a simple-cubic nor an FCC lattice"); return nullptr; }
+    }
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_error("no CUDA device: this library has no CPU fallback");
+        cudaGetLastError();
+        return nullptr;
+    }
+    md_system *s = new md_system();
+    s->prm = p;
+    auto fail = [&](const char *what) -> md_system * {
+        if (what) set_error("%s: %s", what, cudaGetErrorString(cudaGetLastError()));
+        md_destroy(s);
+        return nullptr;
+    };
+    if (p.device >= 0 && cudaSetDevice(p.device) != cudaSuccess) return fail("cudaSetDevice");
+    if (cudaGetDevice(&s->device) != cudaSuccess) return fail("cudaGetDevice");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return fail("cudaGetDeviceProperties");
+    snprintf(s->device_name, sizeof(s->device_name), "%s", prop.name);
+    if (prop.major < 10) { set_error("device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); md_destroy(s); return nullptr; }
+    if (p.stream) s->stream = (cudaStream_t)p.stream;
+    else {
+        if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) return fail("cudaStreamCreate");
+        s->own_stream = true;
+    }
+
+    MdDev &P = s->P;
+    memset(&P, 0, sizeof(P));
+    P.N = (int)p.n_atoms;
+    P.N_pad = (P.N + 127) & ~127;
+    P.Mmax = p.max_neighbors;
+    P.nc = nc;
+    P.NC = nc * nc * nc;
+    P.half_list = p.force_variant == MD_FORCE_NEWTON3_ATOMICS;
+    P.scan_blocks = (P.NC + 2047) / 2048;
+    P.L = p.box; P.half_L = 0.5 * p.box; P.inv_w = (double)nc / p.box;
+    P.rc2 = p.r_cut * p.r_cut;
+    P.rn2 = rn * rn;
+    { const double sc = 1.0 / P.rc2, sc3 = sc * sc * sc; P.uc = 4.0 * sc3 * (sc3 - 1.0); }
+    P.dt = p.dt; P.hdt = 0.5 * p.dt; P.thresh = 0.5 * p.r_shell;
+    s->r_n = rn; s->cell_w = p.box / nc;
+    s->lc.block = p.block_size;
+    s->lc.grid_atoms = (P.N + p.block_size - 1) / p.block_size;
+
+    const size_t np = (size_t)P.N_pad;
+    bool ok = true;
+    auto A = [&](size_t bytes) { void *q = dev_alloc(s, bytes); if (!q) ok = false; return q; };
+    for (int k = 0; k < 2; k++) {
+        P.pos[k] = (pos_t *)A(np * sizeof(pos_t));
+        P.vel[k] = (double *)A(3 * np * sizeof(double));
+        P.id[k] = (int *)A(np * sizeof(int));
+    }
+    P.frc = (double *)A(3 * np * sizeof(double));
+    P.cell_of = (int *)A(np * sizeof(int));
+    P.slot = (int *)A(np * sizeof(int));
+    P.perm = (int *)A(np * sizeof(int));
+    P.nnb = (int *)A(np * sizeof(int));
+    P.cell_count = (int *)A(((size_t)P.NC + 1) * sizeof(int));
+    P.cell_start = (int *)A(((size_t)P.NC + 1) * sizeof(int));
+    P.block_sums = (int *)A(((size_t)P.scan_blocks + 1) * sizeof(int));
+    P.W = (int *)A((size_t)P.Mmax * np * sizeof(int));
+    P.partials = (double *)A((size_t)RED_N * ((P.N + 255) / 256) * sizeof(double));
+    P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
+    P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
+    if (!ok) { set_error("device allocation failed (%.1f MB so far)", s->bytes / 1048576.0); md_destroy(s); return nullptr; }
+    if (cudaMallocHost((void **)&s->h_ctrl, sizeof(DevCtrl)) != cudaSuccess) return fail("cudaMallocHost");
+    if (cudaMallocHost((void **)&s->h_stage, 6 * (size_t)P.N * sizeof(double)) != cudaSuccess) return fail("cudaMallocHost");
+    memset(s->h_ctrl, 0, sizeof(DevCtrl));
+
+    if (p.lattice != MD_LATTICE_NONE) {
+        std::vector<double> xyz(3 * (size_t)P.N), v(3 * (size_t)P.N);
+        if (!md_init_lattice(p.lattice, p.n_atoms, p.box, xyz.data())) {
+            set_error("n_atoms = %lld does not fit lattice %d", (long long)p.n_atoms, p.lattice);
+            md_destroy(s);
+            return nullptr;
+        }
+        md_init_velocities(p.n_atoms, p.temperature, p.seed, v.data());
+        if (upload_state(s, xyz.data(), v.data()) != MD_OK) { md_destroy(s); return nullptr; }
+    } else if (cudaStreamSynchronize(s->stream) != cudaSuccess) {
+        return fail("cudaStreamSynchronize");
+    }
+    return s;
+}
+
+md_system *md_create(int64_t n_atoms, double box, double density, double r_cut, double r_shell, double dt, uint64_t seed)
+{
+    md_params p;
+    md_params_default(&p);
+    p.n_atoms = n_atoms; p.box = box; p.density = density; p.r_cut = r_cut; p.r_shell = r_shell; p.dt = dt; p.seed = seed;
+    return md_create_ex(&p);
+}
+
+int md_set_state(md_system *s, const double *xyz, const double *vxyz)
+{
+    if (!s || !xyz) { set_error("md_set_state: null argument"); return MD_ERR_INVALID; }
+    const double L = s->P.L;
+    for (size_t i = 0; i < 3 * (size_t)s->P.N; i++)
+        if (!(xyz[i] >= 0.0 && xyz[i] <= L)) { set_error("md_set_state: coordinate %zu = %g outside [0, L]", i, xyz[i]); return MD_ERR_INVALID; }
+    return upload_state(s, xyz, vxyz);
+}
+
+int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, double R0)
+{
+    if (!s || (n_bonds > 0 && !ij) || n_bonds < 0 || !(R0 > 0)) { set_error("md_set_bonds: bad argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("md_set_bonds: load a state first"); return MD_ERR_INVALID; }
+    if (s->stepped) { set_error("md_set_bonds: only before the first md_step"); return MD_ERR_INVALID; }
+    MdDev &P = s->P;
+    const size_t n = (size_t)P.N;
+    std::vector<int> tab(2 * n, -1);
+    int mx = 0;
+    for (int64_t b = 0; b < n_bonds; b++) {
+        const int i = ij[2 * b], j = ij[2 * b + 1];
+        if (i < 0 || j < 0 || i >= P.N || j >= P.N || i == j) { set_error("md_set_bonds: bad pair (%d, %d)", i, j); return MD_ERR_INVALID; }
+        for (int side = 0; side < 2; side++) {
+            const int a = side ? j : i, c = side ? i : j;
+            if (tab[a] < 0) tab[a] = c;
+            else if (tab[n + a] < 0) tab[n + a] = c;
+            else { set_error("md_set_bonds: atom %d has more than 2 bonds", a); return MD_ERR_UNSUPPORTED; }
+            mx = std::max(mx, tab[n + a] >= 0 ? 2 : 1);
+        }
+    }
+    if (!P.bond_orig) {
+        P.bond_orig = (int *)dev_alloc(s, 2 * n * sizeof(int));
+        P.bond_dev = (int *)dev_alloc(s, 2 * (size_t)P.N_pad * sizeof(int));
+        P.inv = (int *)dev_alloc(s, n * sizeof(int));
+        if (!P.bond_orig || !P.bond_dev || !P.inv) { set_error("device allocation failed"); return MD_ERR_NOMEM; }
+    }
+    CK(cudaMemcpyAsync(P.bond_orig, tab.data(), 2 * n * sizeof(int), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    P.has_bonds = n_bonds > 0;
+    P.fene_k = k;
+    P.fene_R02 = R0 * R0;
+    s->n_bonds_max = mx;
+    // a rebuild fills inv / bond_dev for the current order, then forces are re-evaluated
+    s->launches += 1;
+    mdk_force_rebuild(P, s->stream);
+    enqueue_rebuild(s);
+    enqueue_forces_only(s);
+    int rc = check_device_status(s);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(&P.ctrl->n_rebuilds, 0, sizeof(int), s->stream));
+    return MD_OK;
+}
+
+int md_rebuild_neighbors(md_system *s)
+{
+    if (!s || !s->has_state) { set_error("md_rebuild_neighbors: no state"); return MD_ERR_INVALID; }
+    s->launches += 1;
+    mdk_force_rebuild(s->P, s->stream);
+    enqueue_rebuild(s);
+    enqueue_forces_only(s);
+    return check_device_status(s);
+}
+
+int md_step(md_system *s, int64_t n)
+{
+    if (!s || n < 0) { set_error("md_step: bad argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("md_step: no state loaded (lattice NONE needs md_set_state)"); return MD_ERR_INVALID; }
+    if (n == 0) return MD_OK;
+    s->stepped = true;
+    const MdDev &P = s->P;
+    cudaStream_t st = s->stream;
+    if (s->prm.step_mode == MD_STEP_FUSED) {
+        // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
+        { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+        enqueue_rebuild(s);
+        for (int64_t k = 1; k < n; k++) {
+            { Timed t(s, MD_T_FUSED_STEP, 1); mdk_force(P, s->lc, 1, st); }
+            enqueue_rebuild(s);
+        }
+        { Timed t(s, MD_T_FORCE, 1); mdk_force(P, s->lc, 2, st); }
+    } else {
+        for (int64_t k = 0; k < n; k++) {
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+            enqueue_rebuild(s);
+            enqueue_forces_only(s);
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick(P, s->lc, st); }
+        }
+    }
+    s->step += n;
+    return check_device_status(s);
+}
+
+int md_energies(md_system *s, md_energy *out)
+{
+    if (!s || !out) { set_error("md_energies: null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("md_energies: no state"); return MD_ERR_INVALID; }
+    { Timed t(s, MD_T_ENERGY, 1); mdk_energy(s->P, s->lc, s->stream); }
+    int rc = check_device_status(s);
+    if (rc) return rc;
+    const DevCtrl &c = *s->h_ctrl;
+    out->ke = c.red[RED_KE];
+    out->pe_pair = c.red[RED_PE];
+    out->pe_bond = c.red[RED_PEB];
+    out->virial = c.red[RED_VIR];
+    out->px = c.red[RED_PX]; out->py = c.red[RED_PY]; out->pz = c.red[RED_PZ];
+    out->vmax = sqrt(c.red[RED_VMAX2]);
+    out->step = s->step;
+    out->n_rebuilds = c.n_rebuilds;
+    out->max_neighbors = c.max_nnb;
+    out->max_cell_occupancy = c.max_occ;
+    out->mean_neighbors = (double)c.nnb_total * (s->P.half_list ? 2.0 : 1.0) / (double)s->P.N;
+    if (!std::isfinite(out->ke + out->pe_pair + out->pe_bond)) { set_error("non-finite energy"); return MD_ERR_NONFINITE; }
+    return MD_OK;
+}
+
+int md_get_positions(md_system *s, double *xyz) { return download(s, 0, xyz); }
+int md_get_velocities(md_system *s, double *xyz) { return download(s, 1, xyz); }
+int md_get_forces(md_system *s, double *xyz) { return download(s, 2, xyz); }
+
+int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_neighbors_out)
+{
+    if (!s || !counts) { set_error("md_get_neighbors: null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("md_get_neighbors: no state"); return MD_ERR_INVALID; }
+    int rc = fetch_ctrl(s);
+    if (rc) return rc;
+    const MdDev &P = s->P;
+    const int N = P.N, M = P.Mmax;
+    const size_t np = (size_t)P.N_pad;
+    const int rows = std::min(M, std::max(1, s->h_ctrl->max_nnb));
+    std::vector<int> nnb(N), id(N), W((size_t)rows * np);
+    CK(cudaMemcpy(nnb.data(), P.nnb, N * sizeof(int), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(id.data(), P.id[s->h_ctrl->v_dst], N * sizeof(int), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(W.data(), P.W, (size_t)rows * np * sizeof(int), cudaMemcpyDeviceToHost));
+    if (max_neighbors_out) *max_neighbors_out = M;
+    std::vector<int> cnt(N, 0);
+    bool overflow = false;
+    auto add = [&](int a, int b) {
+        if (cnt[a] < M) { if (list) list[(size_t)a * M + cnt[a]] = b; }
+        else overflow = true;
+        cnt[a]++;
+    };
+    for (int p = 0; p < N; p++)
+        for (int m = 0; m < nnb[p]; m++) {
+            const int i = id[p], j = id[W[(size_t)m * np + p]];
+            add(i, j);
+            if (P.half_list) add(j, i);
+        }
+    for (int i = 0; i < N; i++) {
+        counts[i] = cnt[i];
+        if (list) for (int m = std::min(cnt[i], M); m < M; m++) list[(size_t)i * M + m] = -1;
+    }
+    if (overflow) { set_error("md_get_neighbors: symmetrised list exceeds Mmax"); return MD_ERR_NEBR_OVERFLOW; }
+    return MD_OK;
+}
+
+int md_get_info(md_system *s, md_info *out)
+{
+    if (!s || !out) { set_error("md_get_info: null argument"); return MD_ERR_INVALID; }
+    memset(out, 0, sizeof(*out));
+    out->n_atoms = s->P.N; out->n_pad = s->P.N_pad;
+    out->box = s->P.L; out->r_neighbor = s->r_n; out->cell_width = s->cell_w;
+    out->cells_per_edge = s->P.nc; out->max_neighbors = s->P.Mmax; out->block_size = s->lc.block;
+    out->force_variant = s->prm.force_variant; out->step_mode = s->prm.step_mode;
+    out->n_bonds_per_atom_max = s->n_bonds_max;
+    out->device_bytes = s->bytes;
+    out->kernel_launches = s->launches;
+    snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);
+    return MD_OK;
+}
+
+int md_set_profiling(md_system *s, int enabled)
+{
+    if (!s) { set_error("null system"); return MD_ERR_INVALID; }
+    s->profiling = enabled != 0;
+    return MD_OK;
+}
+
+int md_get_timers(md_system *s, double *ms, int64_t *launches)
+{
+    if (!s) { set_error("null system"); return MD_ERR_INVALID; }
+    CK(cudaStreamSynchronize(s->stream));
+    resolve_timers(s);
+    for (int k = 0; k < MD_T_COUNT; k++) {
+        if (ms) ms[k] = s->t_ms[k];
+        if (launches) launches[k] = s->t_n[k];
+    }
+    return MD_OK;
+}
+
+int md_reset_timers(md_system *s)
+{
+    if (!s) { set_error("null system"); return MD_ERR_INVALID; }
+    CK(cudaStreamSynchronize(s->stream));
+    resolve_timers(s);
+    for (int k = 0; k < MD_T_COUNT; k++) { s->t_ms[k] = 0; s->t_n[k] = 0; }
+    return MD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,754 @@
+// CUDA kernels (sm_100a) of the short-range MD hot path.  One thread per atom replaces every atom loop
+// of the serial program.  Steps are named after the paper's list:
+//   N1/N2  k_bin            cell assignment c_i and in-cell slot l_i by atomic occupancy counting
+//   N3/N4  k_scan_*         prefix scan of the occupancies k_c (the GPU alternative the paper describes in
+//                           sec. 2.4(4)) -> CSR cell_start; replaces the dense cell x layer matrix H
+//          k_place/k_reorder  cell-order sort of the atoms at EVERY rebuild (paper: every 100 steps)
+//   N5     k_build          neighbor matrix W[m][i], row m contiguous over atoms
+//   F1     k_force          pair forces over W, no Newton-3 (variant A) / k_force_n3 half list + atomics (variant B)
+//   F2     k_energy         block reductions finished by the last block
+//          k_kick_drift / k_kick   leapfrog integration with periodic wrap
+// The model arithmetic follows DESIGN.md "Readings" (R1..R8).  No code is shared with oracle/.
+#include "md_types.h"
+
+#define FULL_MASK 0xffffffffu
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double minimg(double d, double L, double half)
+{
+    return d > half ? d - L : (d < -half ? d + L : d);
+}
+
+__device__ __forceinline__ double wrap1(double x, double L)
+{
+    if (x >= L) x -= L;
+    else if (x < 0.0) { x += L; if (x >= L) x = 0.0; }
+    return x;
+}
+
+// squared minimum-image distance, fixed IEEE operation order (R5): the accept/reject decisions
+// r^2 < r_n^2 and r^2 < r_c^2 are taken on bit-identical values on every implementation.
+__device__ __forceinline__ double dist2(const pos_t &a, const pos_t &b, double L, double half, double &dx, double &dy,
+                                        double &dz)
+{
+    dx = minimg(a.x - b.x, L, half);
+    dy = minimg(a.y - b.y, L, half);
+    dz = minimg(a.z - b.z, L, half);
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+}
+
+__device__ __forceinline__ pos_t ld_pos(const pos_t *p)
+{
+    // 32-byte record -> two 128-bit read-only loads (one sector)
+    const double2 *q = reinterpret_cast<const double2 *>(p);
+    double2 a = __ldg(q), b = __ldg(q + 1);
+    pos_t r;
+    r.x = a.x; r.y = a.y; r.z = b.x; r.w = b.y;
+    return r;
+}
+
+__device__ __forceinline__ void st_pos(pos_t *p, double x, double y, double z)
+{
+    double2 *q = reinterpret_cast<double2 *>(p);
+    q[0] = make_double2(x, y);
+    q[1] = make_double2(z, 0.0);
+}
+
+__device__ __forceinline__ int cell_coord(double x, double inv_w, int nc)
+{
+    int q = (int)floor(x * inv_w);
+    q = q < 0 ? 0 : q;
+    return q >= nc ? nc - 1 : q;
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(FULL_MASK, v, o));
+    return v;
+}
+__device__ __forceinline__ int warp_sum_i(int v)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+    return v;
+}
+__device__ __forceinline__ int warp_max_i(int v)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = max(v, __shfl_xor_sync(FULL_MASK, v, o));
+    return v;
+}
+
+// block-wide max of a non-negative double; result valid in thread 0.  sm: >= 32 doubles.
+__device__ __forceinline__ double block_max(double v, double *sm)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    v = warp_max(v);
+    if (lane == 0) sm[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        v = lane < nw ? sm[lane] : 0.0;
+        v = warp_max(v);
+    }
+    return v;
+}
+
+// The rebuild decision (R8), taken by ONE thread of the last block of the kernel
+// that drifted the positions.  It also fixes which buffers the rebuild kernels read and write, so the host
+// never needs to know whether a rebuild happened.
+__device__ void decide(const MdDev &P, bool pos_pingpong)
+{
+    volatile DevCtrl *c = P.ctrl;
+    const double vmax2 = __longlong_as_double((long long)c->vmax2_bits);
+    c->vmax2_bits = 0ull;
+    double acc = c->disp_acc + P.dt * sqrt(vmax2);
+    const int need = acc > P.thresh;
+    if (need) {
+        acc = 0.0;
+        c->n_rebuilds += 1;
+        c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+    }
+    c->disp_acc = acc;
+    c->need_rebuild = need;
+    const int ps = pos_pingpong ? (c->p_dst ^ 1) : c->p_dst;
+    c->p_src = ps;
+    c->p_dst = need ? (ps ^ 1) : ps;
+    const int vs = c->v_dst;
+    c->v_src = vs;
+    c->v_dst = need ? (vs ^ 1) : vs;
+}
+
+// thread 0 of each block: publish the block's max v^2, then take a ticket; the last block decides.
+__device__ __forceinline__ void publish_vmax_and_decide(const MdDev &P, double bmax2, bool pos_pingpong)
+{
+    DevCtrl *c = P.ctrl;
+    atomicMax(&c->vmax2_bits, (unsigned long long)__double_as_longlong(bmax2));
+    __threadfence();
+    const unsigned t = atomicInc(&c->ticket[TK_INTEGRATE], gridDim.x - 1);
+    if (t == gridDim.x - 1) {
+        __threadfence();
+        decide(P, pos_pingpong);
+    }
+}
+
+__device__ __forceinline__ void set_err(const MdDev &P, int code) { atomicCAS(&P.ctrl->err, 0, code); }
+
+// ------------------------------------------------------------------------------------------------
+// control / staging kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_force_rebuild(const __grid_constant__ MdDev P)
+{
+    DevCtrl *c = P.ctrl;
+    c->need_rebuild = 1;
+    c->p_src = c->p_dst; c->p_dst ^= 1;
+    c->v_src = c->v_dst; c->v_dst ^= 1;
+    c->disp_acc = 0.0;
+    c->vmax2_bits = 0ull;
+    c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+}
+
+// scratch = [xyz (3N) | vxyz (3N)] in original-id order -> device arrays in identity order
+__global__ void k_load_state(const __grid_constant__ MdDev P)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const int pc = P.ctrl->p_dst, vc = P.ctrl->v_dst;
+    const double *s = P.scratch + 3 * (size_t)i;
+    double x = wrap1(s[0], P.L), y = wrap1(s[1], P.L), z = wrap1(s[2], P.L);
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) set_err(P, MD_ERR_NONFINITE);
+    st_pos(P.pos[pc] + i, x, y, z);
+    const double *v = P.scratch + 3 * (size_t)P.N + 3 * (size_t)i;
+    double *vel = P.vel[vc];
+    vel[i] = v[0]; vel[P.N_pad + i] = v[1]; vel[2 * (size_t)P.N_pad + i] = v[2];
+    P.id[vc][i] = i;
+}
+
+// device order -> scratch in original-id order.  what: 0 positions, 1 velocities, 2 forces
+__global__ void k_export(const __grid_constant__ MdDev P, int what, size_t offset)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const int pc = P.ctrl->p_dst, vc = P.ctrl->v_dst;
+    const int id = P.id[vc][i];
+    double *o = P.scratch + offset + 3 * (size_t)id;
+    if (what == 0) {
+        pos_t r = P.pos[pc][i];
+        o[0] = r.x; o[1] = r.y; o[2] = r.z;
+    } else {
+        const double *a = what == 1 ? P.vel[vc] : P.frc;
+        o[0] = a[i]; o[1] = a[P.N_pad + i]; o[2] = a[2 * (size_t)P.N_pad + i];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// integration (split mode): first half kick + drift + wrap + max velocity + rebuild decision
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDev P)
+{
+    __shared__ double sm[32];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
+    double v2 = 0.0;
+    if (i < P.N) {
+        pos_t *pp = P.pos[pc] + i;
+        double *vx = P.vel[vc] + i, *vy = vx + P.N_pad, *vz = vy + P.N_pad;
+        const double *fx = P.frc + i, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
+        pos_t r = *pp;
+        const double ax = *vx + P.hdt * *fx, ay = *vy + P.hdt * *fy, az = *vz + P.hdt * *fz;
+        *vx = ax; *vy = ay; *vz = az;
+        const double x = wrap1(r.x + P.dt * ax, P.L), y = wrap1(r.y + P.dt * ay, P.L), z = wrap1(r.z + P.dt * az, P.L);
+        st_pos(pp, x, y, z);
+        v2 = ax * ax + ay * ay + az * az;
+        if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
+    }
+    const double bm = block_max(v2, sm);
+    if (threadIdx.x == 0) publish_vmax_and_decide(P, bm, false);
+}
+
+// second half kick
+__global__ void __launch_bounds__(256) k_kick(const __grid_constant__ MdDev P)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const int vc = __ldcg(&P.ctrl->v_dst);
+    double *v = P.vel[vc] + i;
+    const double *f = P.frc + i;
+#pragma unroll
+    for (int k = 0; k < 3; k++) v[(size_t)k * P.N_pad] += P.hdt * f[(size_t)k * P.N_pad];
+}
+
+// ------------------------------------------------------------------------------------------------
+// cells: N1/N2 binning with atomic occupancy counters, N3/N4 as a prefix scan
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const pos_t r = P.pos[__ldcg(&P.ctrl->p_src)][i];
+    const int cx = cell_coord(r.x, P.inv_w, P.nc), cy = cell_coord(r.y, P.inv_w, P.nc), cz = cell_coord(r.z, P.inv_w, P.nc);
+    const int c = cx + P.nc * (cy + P.nc * cz);
+    P.cell_of[i] = c;
+    P.slot[i] = atomicAdd(&P.cell_count[c], 1);      // l_i; "incrementing k_c requires an atomic operation" (N2)
+}
+
+constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    __shared__ int ssum[SCAN_T / 32], smax[SCAN_T / 32];
+    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_V;
+    int sum = 0, mx = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_V; k++) {
+        const int idx = base + k;
+        const int c = idx < P.NC ? P.cell_count[idx] : 0;
+        sum += c;
+        mx = max(mx, c);
+    }
+    sum = warp_sum_i(sum);
+    mx = warp_max_i(mx);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { ssum[wid] = sum; smax[wid] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int s = 0, m = 0;
+        for (int w = 0; w < SCAN_T / 32; w++) { s += ssum[w]; m = max(m, smax[w]); }
+        P.block_sums[blockIdx.x] = s;
+        atomicMax(&P.ctrl->max_occ, m);              // N3: the paper's layer count N_l = max_c k_c
+    }
+}
+
+// exclusive scan of the per-tile sums, one block
+__global__ void __launch_bounds__(1024) k_scan_top(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    __shared__ int wsum[32];
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int start = 0; start < P.scan_blocks; start += 1024) {
+        const int idx = start + threadIdx.x;
+        const int v = idx < P.scan_blocks ? P.block_sums[idx] : 0;
+        int inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(FULL_MASK, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) wsum[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            int w = wsum[lane], winc = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(FULL_MASK, winc, o);
+                if (lane >= o) winc += t;
+            }
+            wsum[lane] = winc - w;                   // exclusive prefix of warp totals
+        }
+        __syncthreads();
+        const int carry = carry_s;
+        const int excl = carry + wsum[wid] + inc - v;
+        if (idx < P.scan_blocks) P.block_sums[idx] = excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = excl + v;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    __shared__ int wsum[SCAN_T / 32];
+    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_V;
+    int c[SCAN_V], sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_V; k++) {
+        const int idx = base + k;
+        c[k] = idx < P.NC ? P.cell_count[idx] : 0;
+        sum += c[k];
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(FULL_MASK, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    int woff = 0;
+    for (int w = 0; w < wid; w++) woff += wsum[w];
+    int run = P.block_sums[blockIdx.x] + woff + inc - sum;
+#pragma unroll
+    for (int k = 0; k < SCAN_V; k++) {
+        const int idx = base + k;
+        if (idx < P.NC) {
+            P.cell_start[idx] = run;
+            P.cell_count[idx] = 0;                   // ready for the next binning
+            run += c[k];
+            if (idx == P.NC - 1) P.cell_start[P.NC] = run;
+        }
+    }
+}
+
+// N4 in CSR form: the atom's place in the cell-ordered sequence s
+__global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
+}
+
+// Cell-order gather of r, v and the permanent serial numbers.  The atomics of N2 leave the
+// order inside a cell indeterminate; ranking the cell's members by their previous slot makes
+// the order -- and with it every floating-point sum downstream -- reproducible run to run.
+__global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P.N) return;
+    const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
+    const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
+    const int a = P.perm[p];
+    const int c = P.cell_of[a];
+    const int s = P.cell_start[c], e = P.cell_start[c + 1];
+    int rank = 0;
+    for (int q = s; q < e; q++) rank += (P.perm[q] < a);
+    const int n = s + rank;
+    const pos_t r = P.pos[ps][a];
+    st_pos(P.pos[pd] + n, r.x, r.y, r.z);
+    const double *vi = P.vel[vs] + a;
+    double *vo = P.vel[vd] + n;
+#pragma unroll
+    for (int k = 0; k < 3; k++) vo[(size_t)k * P.N_pad] = vi[(size_t)k * P.N_pad];
+    const int id = P.id[vs][a];
+    P.id[vd][n] = id;
+    if (P.has_bonds) P.inv[id] = n;
+}
+
+__global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= P.N) return;
+    const int id = P.id[__ldcg(&P.ctrl->v_dst)][n];
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        const int partner = P.bond_orig[(size_t)k * P.N + id];
+        P.bond_dev[(size_t)k * P.N_pad + n] = partner >= 0 ? P.inv[partner] : -1;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// N5: neighbor matrix.  With the atoms in cell order (x fastest) the 27-cell stencil of an atom is 9
+// contiguous runs of the atom array (one per (dy,dz), 3 cells long, split only at the periodic x wrap).
+// ------------------------------------------------------------------------------------------------
+template <bool HALF>
+__device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, int b, int e,
+                                         int &m)
+{
+    for (int j = b; j < e; j++) {
+        if (HALF ? (j <= i) : (j == i)) continue;
+        const pos_t rj = ld_pos(pos + j);
+        double dx, dy, dz;
+        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+        if (r2 < P.rn2) {
+            if (m < P.Mmax) P.W[(size_t)m * P.N_pad + i] = j;
+            m++;
+        }
+    }
+}
+
+template <bool HALF>
+__global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    __shared__ int smx[4];
+    __shared__ int ssum[4];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    int m = 0;
+    if (i < P.N) {
+        const pos_t ri = pos[i];
+        const int nc = P.nc;
+        const int cx = cell_coord(ri.x, P.inv_w, nc), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
+        const int x0 = cx - 1, x1 = cx + 1;
+        const int xa = x0 < 0 ? 0 : x0, xb = x1 >= nc ? nc - 1 : x1;
+        for (int dz = -1; dz <= 1; dz++) {
+            int z = cz + dz;
+            z = z < 0 ? z + nc : (z >= nc ? z - nc : z);
+            for (int dy = -1; dy <= 1; dy++) {
+                int y = cy + dy;
+                y = y < 0 ? y + nc : (y >= nc ? y - nc : y);
+                const int row = nc * (y + nc * z);
+                scan_run<HALF>(P, pos, ri, i, P.cell_start[row + xa], P.cell_start[row + xb + 1], m);
+                if (x0 < 0) scan_run<HALF>(P, pos, ri, i, P.cell_start[row + nc - 1], P.cell_start[row + nc], m);
+                if (x1 >= nc) scan_run<HALF>(P, pos, ri, i, P.cell_start[row], P.cell_start[row + 1], m);
+            }
+        }
+        P.nnb[i] = m < P.Mmax ? m : P.Mmax;
+        if (m > P.Mmax) set_err(P, MD_ERR_NEBR_OVERFLOW);
+    }
+    // statistics of the matrix (md_energy.max_neighbors / mean_neighbors)
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int wm = warp_max_i(m), ws = warp_sum_i(m);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int mx = 0, sm = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        atomicMax(&P.ctrl->max_nnb, mx);
+        atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// F1: pair forces.  Thread i walks column i of W; row m is contiguous over i, so the 32 threads of a
+// warp read 128 consecutive bytes of W per row; the partner positions are gathers.
+// ------------------------------------------------------------------------------------------------
+struct PairAcc {
+    double fx, fy, fz;
+};
+
+__device__ __forceinline__ void pair_force(const MdDev &P, const pos_t &ri, const pos_t &rj, PairAcc &a)
+{
+    double dx, dy, dz;
+    const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+    if (r2 < P.rc2) {
+        const double s = 1.0 / r2, s3 = s * s * s;
+        const double fc = 48.0 * s3 * (s3 - 0.5) * s;
+        a.fx += fc * dx; a.fy += fc * dy; a.fz += fc * dz;
+    }
+}
+
+template <bool CHECK>
+__device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
+{
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        const int j = P.bond_dev[(size_t)k * P.N_pad + i];
+        if (j < 0) continue;
+        const pos_t rj = ld_pos(pos + j);
+        double dx, dy, dz;
+        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+        if (!(r2 < P.fene_R02)) { if (CHECK) set_err(P, MD_ERR_BOND_BROKEN); continue; }
+        const double fc = -P.fene_k / (1.0 - r2 / P.fene_R02);
+        a.fx += fc * dx; a.fy += fc * dy; a.fz += fc * dz;
+    }
+}
+
+// MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = wrap(r + dt v) into the other position
+// buffer, max |v|, rebuild decision.  MODE 2: store f and apply the closing half kick v += dt/2 f.
+template <int MODE, bool BONDS, int BLOCK>
+__global__ void __launch_bounds__(BLOCK) k_force(const __grid_constant__ MdDev P)
+{
+    __shared__ double sm[32];
+    const int i = blockIdx.x * BLOCK + threadIdx.x;
+    const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
+    const pos_t *__restrict__ pos = P.pos[pc];
+    double v2 = 0.0;
+    if (i < P.N) {
+        const pos_t ri = ld_pos(pos + i);
+        const int m = P.nnb[i];
+        const int *__restrict__ w = P.W + i;
+        PairAcc a = {0.0, 0.0, 0.0};
+#pragma unroll 4
+        for (int k = 0; k < m; k++) {
+            const int j = __ldcs(w + (size_t)k * P.N_pad);
+            const pos_t rj = ld_pos(pos + j);
+            pair_force(P, ri, rj, a);
+        }
+        if (BONDS) bond_force<true>(P, pos, ri, i, a);
+        if (MODE == 0 || MODE == 2) {
+            double *f = P.frc + i;
+            f[0] = a.fx; f[P.N_pad] = a.fy; f[2 * (size_t)P.N_pad] = a.fz;
+        }
+        if (MODE == 2) {
+            double *v = P.vel[vc] + i;
+            v[0] += P.hdt * a.fx; v[P.N_pad] += P.hdt * a.fy; v[2 * (size_t)P.N_pad] += P.hdt * a.fz;
+        }
+        if (MODE == 1) {
+            double *v = P.vel[vc] + i;
+            const double vx = v[0] + P.dt * a.fx, vy = v[P.N_pad] + P.dt * a.fy, vz = v[2 * (size_t)P.N_pad] + P.dt * a.fz;
+            v[0] = vx; v[P.N_pad] = vy; v[2 * (size_t)P.N_pad] = vz;
+            const double x = wrap1(ri.x + P.dt * vx, P.L), y = wrap1(ri.y + P.dt * vy, P.L), z = wrap1(ri.z + P.dt * vz, P.L);
+            st_pos(P.pos[pc ^ 1] + i, x, y, z);
+            v2 = vx * vx + vy * vy + vz * vz;
+            if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
+        }
+    }
+    if (MODE == 1) {
+        const double bm = block_max(v2, sm);
+        if (threadIdx.x == 0) publish_vmax_and_decide(P, bm, true);
+    }
+}
+
+// Variant B: each pair once; f_i in registers, f_j by fp64 atomics.  f must be zero on entry.
+template <bool BONDS>
+__global__ void __launch_bounds__(256) k_force_n3(const __grid_constant__ MdDev P)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    const pos_t ri = ld_pos(pos + i);
+    const int m = P.nnb[i];
+    const int *__restrict__ w = P.W + i;
+    double *fx = P.frc, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
+    PairAcc a = {0.0, 0.0, 0.0};
+    for (int k = 0; k < m; k++) {
+        const int j = __ldcs(w + (size_t)k * P.N_pad);
+        const pos_t rj = ld_pos(pos + j);
+        double dx, dy, dz;
+        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+        if (r2 < P.rc2) {
+            const double s = 1.0 / r2, s3 = s * s * s;
+            const double fc = 48.0 * s3 * (s3 - 0.5) * s;
+            const double gx = fc * dx, gy = fc * dy, gz = fc * dz;
+            a.fx += gx; a.fy += gy; a.fz += gz;
+            atomicAdd(fx + j, -gx); atomicAdd(fy + j, -gy); atomicAdd(fz + j, -gz);
+        }
+    }
+    if (BONDS) bond_force<true>(P, pos, ri, i, a);
+    atomicAdd(fx + i, a.fx); atomicAdd(fy + i, a.fy); atomicAdd(fz + i, a.fz);
+}
+
+__global__ void __launch_bounds__(256) k_zero_forces(const __grid_constant__ MdDev P)
+{
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i < 3 * (size_t)P.N_pad) P.frc[i] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// F2 and the other global sums: warp shuffles -> shared memory -> one partial per block
+// -> the last block (atomic ticket + memory fence) finishes in a fixed order, so results are reproducible.
+// ------------------------------------------------------------------------------------------------
+template <bool BONDS>
+__global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P, int max_grid)
+{
+    __shared__ double sm[RED_N][8];
+    __shared__ bool last;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
+    const pos_t *__restrict__ pos = P.pos[pc];
+    double q[RED_N];
+#pragma unroll
+    for (int k = 0; k < RED_N; k++) q[k] = 0.0;
+    if (i < P.N) {
+        const pos_t ri = ld_pos(pos + i);
+        const int m = P.nnb[i];
+        const int *__restrict__ w = P.W + i;
+        double u = 0.0, vir = 0.0;
+        for (int k = 0; k < m; k++) {
+            const int j = __ldcs(w + (size_t)k * P.N_pad);
+            const pos_t rj = ld_pos(pos + j);
+            double dx, dy, dz;
+            const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+            if (r2 < P.rc2) {
+                const double s = 1.0 / r2, s3 = s * s * s;
+                u += 4.0 * s3 * (s3 - 1.0) - P.uc;
+                vir += 48.0 * s3 * (s3 - 0.5);         // fc * r^2
+            }
+        }
+        const double pair_scale = P.half_list ? 1.0 : 0.5;   // full list: u_i counts every pair twice
+        q[RED_PE] = pair_scale * u;
+        q[RED_VIR] = pair_scale * vir;
+        if (BONDS) {
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+                const int j = P.bond_dev[(size_t)k * P.N_pad + i];
+                if (j < 0) continue;
+                const pos_t rj = ld_pos(pos + j);
+                double dx, dy, dz;
+                const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+                if (!(r2 < P.fene_R02)) { set_err(P, MD_ERR_BOND_BROKEN); continue; }
+                const double x = 1.0 - r2 / P.fene_R02;
+                q[RED_PEB] += 0.5 * (-0.5 * P.fene_k * P.fene_R02 * log(x));
+                q[RED_VIR] += 0.5 * (-P.fene_k / x) * r2;
+            }
+        }
+        const double *v = P.vel[vc] + i;
+        const double vx = v[0], vy = v[P.N_pad], vz = v[2 * (size_t)P.N_pad];
+        const double v2 = vx * vx + vy * vy + vz * vz;
+        q[RED_KE] = 0.5 * v2;
+        q[RED_PX] = vx; q[RED_PY] = vy; q[RED_PZ] = vz;
+        q[RED_VMAX2] = v2;
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < RED_N; k++) {
+        const double r = k == RED_VMAX2 ? warp_max(q[k]) : warp_sum(q[k]);
+        if (lane == 0) sm[k][wid] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < RED_N) {
+        const int k = threadIdx.x;
+        double r = sm[k][0];
+        for (int w = 1; w < (int)(blockDim.x >> 5); w++) r = k == RED_VMAX2 ? fmax(r, sm[k][w]) : r + sm[k][w];
+        P.partials[(size_t)k * max_grid + blockIdx.x] = r;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicInc(&P.ctrl->ticket[TK_ENERGY], gridDim.x - 1);
+        last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    // the last block sums the partials of all blocks (itself included), fixed order
+    for (int k = 0; k < RED_N; k++) {
+        double r = 0.0;
+        const volatile double *p = P.partials + (size_t)k * max_grid;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) r = k == RED_VMAX2 ? fmax(r, p[b]) : r + p[b];
+        r = k == RED_VMAX2 ? warp_max(r) : warp_sum(r);
+        __syncthreads();
+        if (lane == 0) sm[0][wid] = r;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = sm[0][0];
+            for (int w = 1; w < (int)(blockDim.x >> 5); w++) t = k == RED_VMAX2 ? fmax(t, sm[0][w]) : t + sm[0][w];
+            P.ctrl->red[k] = t;
+        }
+    }
+}
+
+inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// launch wrappers
+// ------------------------------------------------------------------------------------------------
+void mdk_force_rebuild(const MdDev &P, cudaStream_t st) { k_force_rebuild<<<1, 1, 0, st>>>(P); }
+
+void mdk_load_state(const MdDev &P, cudaStream_t st) { k_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+
+void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st) { k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset); }
+
+void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+
+void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+
+void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    k_bin<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    k_scan_reduce<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
+    k_scan_top<<<1, 1024, 0, st>>>(P);
+    k_scan_apply<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
+    k_place<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+}
+
+void mdk_reorder(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    k_reorder<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    if (P.has_bonds) k_bonds_remap<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+}
+
+void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    if (P.half_list) k_build<true><<<cdiv(P.N, 128), 128, 0, st>>>(P);
+    else k_build<false><<<cdiv(P.N, 128), 128, 0, st>>>(P);
+}
+
+template <int MODE, bool BONDS>
+static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
+{
+    switch (block) {
+    case 64: k_force<MODE, BONDS, 64><<<cdiv(P.N, 64), 64, 0, st>>>(P); break;
+    case 256: k_force<MODE, BONDS, 256><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
+    case 512: k_force<MODE, BONDS, 512><<<cdiv(P.N, 512), 512, 0, st>>>(P); break;
+    default: k_force<MODE, BONDS, 128><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
+    }
+}
+
+void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
+{
+    if (P.has_bonds) {
+        if (mode == 0) launch_force_block<0, true>(P, lc.block, st);
+        else if (mode == 1) launch_force_block<1, true>(P, lc.block, st);
+        else launch_force_block<2, true>(P, lc.block, st);
+    } else {
+        if (mode == 0) launch_force_block<0, false>(P, lc.block, st);
+        else if (mode == 1) launch_force_block<1, false>(P, lc.block, st);
+        else launch_force_block<2, false>(P, lc.block, st);
+    }
+}
+
+void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    k_zero_forces<<<cdiv(3LL * P.N_pad, 256), 256, 0, st>>>(P);
+    if (P.has_bonds) k_force_n3<true><<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    else k_force_n3<false><<<cdiv(P.N, 256), 256, 0, st>>>(P);
+}
+
+void mdk_energy(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    const int grid = cdiv(P.N, 256);
+    if (P.has_bonds) k_energy<true><<<grid, 256, 0, st>>>(P, grid);
+    else k_energy<false><<<grid, 256, 0, st>>>(P, grid);
+}
+
+int mdk_launches_of(int which)
+{
+    switch (which) {
+    case LK_CELLS: return 5;
+    case LK_FORCE_N3: return 2;
+    default: return 1;
+    }
+}

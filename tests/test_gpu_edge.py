@@ -1,0 +1,106 @@
+"""GPU edge cases and error behaviour of the C ABI."""
+import numpy as np
+import pytest
+
+from md_workloads import get_config, make_state, scaled_config
+from md_workloads.configs import R_WCA
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def md():
+    import paper_2003_14061_b200 as m
+    m.load_library()
+    return m
+
+
+def test_invalid_arguments(md):
+    with pytest.raises(md.MDError):
+        md.MDSystem(0, R_WCA, 0.4, 0.005, density=0.8)
+    with pytest.raises(md.MDError):
+        md.MDSystem(4096, R_WCA, 0.4, 0.005)                          # neither box nor density
+    with pytest.raises(md.MDError):
+        md.MDSystem(4096, R_WCA, 0.4, 0.005, density=0.8, box=10.0)   # inconsistent
+    with pytest.raises(md.MDError):
+        md.MDSystem(27, R_WCA, 0.4, 0.005, density=0.8)               # box < 3 cells
+    with pytest.raises(md.MDError):
+        md.MDSystem(4097, R_WCA, 0.4, 0.005, density=0.8)             # fits no lattice
+    g = md.MDSystem(4096, R_WCA, 0.4, 0.005, density=0.8, lattice="none")
+    with pytest.raises(md.MDError):
+        g.step(1)                                                     # no state yet
+    r, v, _, box = make_state(get_config("wca_4k"), 1)
+    bad = r.copy()
+    bad[5, 1] = box * 1.5
+    with pytest.raises(md.MDError):
+        g.set_state(bad, v)
+    g.set_state(r, v)
+    g.step(0)
+    assert g.energies().step == 0
+
+
+def test_neighbor_overflow_is_reported(md):
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 1, jitter_amp=0.12)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", max_neighbors=4)
+    with pytest.raises(md.MDError) as ei:
+        g.set_state(r, v)
+    assert ei.value.code == -2
+
+
+def test_zero_shell_rebuilds_every_step(md):
+    cfg = scaled_config("wca_4k", 4096, r_shell=0.0)
+    r, v, _, box = make_state(cfg, 1, jitter_amp=0.1)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, 0.0, cfg.dt, box=box, lattice="none")
+    g.set_state(r, v)
+    from oracle.md_oracle import OracleMD
+    o = OracleMD(cfg.n_atoms, box, cfg.r_cut, 0.0, cfg.dt)
+    o.set_state(r, v)
+    g.step(20)
+    o.step(20)
+    e, eo = g.energies(), o.energies()
+    assert e.n_rebuilds == eo.n_rebuilds == 20
+    assert e.total == pytest.approx(eo.total, rel=1e-9)
+
+
+def test_broken_bond_is_reported(md):
+    cfg = scaled_config("chains_1m", 4096, chain_len=16)
+    r, v, bonds, box = make_state(cfg, 1)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g.set_state(r, v)
+    far = np.array([[0, 2048]], np.int32)                              # beads of different chains, far apart
+    with pytest.raises(md.MDError) as ei:
+        g.set_bonds(far, cfg.fene_k, cfg.fene_r0)
+    assert ei.value.code == -3
+    g2 = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g2.set_state(r, v)
+    with pytest.raises(md.MDError) as ei:
+        g2.set_bonds(np.array([[0, 1], [0, 2], [0, 3]], np.int32), 30.0, 1.5)
+    assert ei.value.code == -6
+
+
+def test_info_and_timers(md):
+    cfg = get_config("wca_4k")
+    g = md.MDSystem.from_config(cfg, seed=1)
+    i = g.info()
+    assert i["n_atoms"] == 4096 and i["n_pad"] == 4096 and i["cells_per_edge"] == 11 and i["max_neighbors"] == 32
+    assert "B200" in i["device_name"] or i["device_name"]
+    g.set_profiling(True)
+    g.reset_timers()
+    k0 = g.info()["kernel_launches"]
+    g.step(50)
+    t = g.timers()
+    assert t["fused_step"]["launches"] == 49 and t["fused_step"]["ms"] > 0
+    assert t["nebr"]["launches"] == 50
+    assert g.info()["kernel_launches"] - k0 == sum(x["launches"] for x in t.values())
+
+
+def test_set_state_keeps_velocities_when_none(md):
+    cfg = get_config("wca_4k")
+    g = md.MDSystem.from_config(cfg, seed=3)
+    g.step(30)
+    v = g.velocities()
+    r = g.positions()
+    g.set_state(r)                                                     # velocities kept, order reset
+    assert np.array_equal(g.velocities(), v)
+    assert np.array_equal(g.positions(), r)

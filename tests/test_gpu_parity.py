@@ -1,0 +1,174 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+Tolerances are BASELINE.json north_star's: neighbor sets exact, forces 1e-10, positions 1e-9 and energies 1e-9
+after 10 steps."""
+import numpy as np
+import pytest
+
+from md_workloads import get_config, make_state, scaled_config
+from oracle.md_oracle import OracleMD, brute_forces_sample, brute_neighbors_sample
+from parity_util import ENERGY_RTOL, FORCE_RTOL, POS_ATOL, force_rel_err, pos_err, sets_equal
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def md():
+    import paper_2003_14061_b200 as m
+    m.load_library()
+    return m
+
+
+def small_cases():
+    return {
+        "wca_4k": (get_config("wca_4k"), {}),
+        "wca_ragged_1000": (scaled_config("wca_4k", 1000), {}),                     # N not a multiple of 32/128
+        "wca_dr03_13824": (scaled_config("wca_2m_dr03", 24 ** 3), {}),
+        "wca_dr05_13824": (scaled_config("wca_2m_dr05", 24 ** 3), {}),
+        "lj_6912": (scaled_config("lj_1m", 4 * 12 ** 3), {}),
+        "chains_4096": (scaled_config("chains_1m", 4096, chain_len=16), {}),
+    }
+
+
+def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw):
+    """GPU system and oracle loaded with the SAME state (from md_workloads or evolved by the oracle)."""
+    jit = 0.0 if state == "lattice" else (0.12 if cfg.lattice != "chains" else 0.0)
+    r, v, bonds, box = make_state(cfg, seed, jitter_amp=jit)
+    o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(r, v)
+    if bonds is not None:
+        assert o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0) == 0
+    if state == "thermal":
+        assert o.step(200) == 0
+        r, v = o.positions(), o.velocities()
+        o.set_state(r, v)
+        if bonds is not None:
+            o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
+                    step_mode=mode, **kw)
+    g.set_state(r, v)
+    if bonds is not None:
+        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    return g, o, box
+
+
+@pytest.mark.parametrize("case", list(small_cases()))
+@pytest.mark.parametrize("variant", ["full", "newton3"])
+@pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
+def test_neighbor_sets_and_forces(md, case, variant, state):
+    cfg, _ = small_cases()[case]
+    if state == "lattice" and cfg.lattice == "chains":
+        pytest.skip("chain start has no separate lattice state")
+    for seed in (1, 2, 3) if state != "thermal" else (1,):
+        g, o, box = make_pair(md, cfg, seed, variant=variant, mode="split", state=state)
+        counts, lst = g.neighbors()
+        nbad, first = sets_equal(counts, lst, o)
+        assert nbad == 0, f"neighbor sets differ for {nbad} atoms (first: atom {first})"
+        fo = o.forces()
+        fg = g.forces()
+        if state == "lattice" and cfg.lattice in ("sc", "fcc"):
+            # every f_i = 0 analytically: only an absolute test makes sense;
+            # a single pair force is < 24 and at most 78 pairs contribute
+            assert np.abs(fg).max() <= 1e-12 * 24.0 * 78 and np.abs(fo).max() <= 1e-12 * 24.0 * 78
+        else:
+            assert force_rel_err(fg, fo) <= FORCE_RTOL
+        eg, eo = g.energies(), o.energies()
+        assert eg.pe_pair == pytest.approx(eo.pe_pair, rel=ENERGY_RTOL, abs=1e-9)
+        assert eg.pe_bond == pytest.approx(eo.pe_bond, rel=ENERGY_RTOL, abs=1e-9)
+        assert eg.virial == pytest.approx(eo.virial, rel=ENERGY_RTOL, abs=1e-7)
+        assert eg.ke == pytest.approx(eo.ke, rel=1e-12)
+        if variant == "full":                                    # variant B stores (and reports) the half matrix
+            assert eg.max_neighbors == eo.max_neighbors
+        assert eg.mean_neighbors == pytest.approx(eo.mean_neighbors, rel=1e-12)
+        g.close()
+
+
+@pytest.mark.parametrize("case", list(small_cases()))
+@pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("newton3", "split")])
+def test_ten_steps(md, case, variant, mode):
+    cfg, _ = small_cases()[case]
+    for seed in (1, 2, 3):
+        g, o, box = make_pair(md, cfg, seed, variant=variant, mode=mode, state="jitter")
+        g.step(10)
+        assert o.step(10) == 0
+        assert pos_err(g.positions(), o.positions(), box) <= POS_ATOL
+        assert np.abs(g.velocities() - o.velocities()).max() <= 1e-8
+        eg, eo = g.energies(), o.energies()
+        assert eg.ke == pytest.approx(eo.ke, rel=ENERGY_RTOL)
+        assert eg.pe == pytest.approx(eo.pe, rel=ENERGY_RTOL)
+        assert eg.step == eo.step == 10
+        n = cfg.n_atoms
+        for pg, po in ((eg.px, eo.px), (eg.py, eo.py), (eg.pz, eo.pz)):
+            assert abs(pg - po) <= 1e-9 * np.sqrt(n)
+        assert force_rel_err(g.forces(), o.forces()) <= 1e-8     # after 10 steps positions differ by ~1e-13
+        g.close()
+
+
+def test_steps_one_at_a_time_equal_one_call(md):
+    """md_step(1) x 10 (closing/opening half kicks each call) and md_step(10) (fused leapfrog) agree."""
+    cfg = get_config("wca_4k")
+    g1, o, box = make_pair(md, cfg, 1, mode="fused")
+    g2, _, _ = make_pair(md, cfg, 1, mode="fused")
+    for _ in range(10):
+        g1.step(1)
+    g2.step(10)
+    assert pos_err(g1.positions(), g2.positions(), box) <= 1e-12
+    assert np.abs(g1.velocities() - g2.velocities()).max() <= 1e-12
+
+
+def test_thermalised_run_with_rebuilds(md):
+    """200 steps from the lattice (about 20 rebuilds): the list must stay valid, so energies track the oracle's
+    to chaos-limited accuracy and the conserved quantities hold."""
+    cfg = get_config("wca_4k")
+    g, o, box = make_pair(md, cfg, 1, mode="fused", state="lattice")
+    e0 = g.energies()
+    g.step(200)
+    o.step(200)
+    eg, eo = g.energies(), o.energies()
+    assert eg.n_rebuilds > 10 and abs(eg.n_rebuilds - eo.n_rebuilds) <= 1
+    assert abs(eg.total - e0.total) / cfg.n_atoms < 2e-3
+    assert eg.total == pytest.approx(eo.total, rel=1e-7)
+    assert max(abs(eg.px), abs(eg.py), abs(eg.pz)) < 1e-9
+    # forces on the GPU's own final state against the all-pairs definition (list validity)
+    pos = g.positions()
+    idx = np.arange(0, cfg.n_atoms, 7)
+    fb, _, _ = brute_forces_sample(pos, box, cfg.r_cut, idx)
+    assert force_rel_err(g.forces()[idx], fb) <= FORCE_RTOL
+
+
+def test_md_create_initial_state_matches_generator(md):
+    for name in ("wca_4k", "lj_6912"):
+        cfg = small_cases()[name][0]
+        r, v, _, box = make_state(cfg, 5)
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, density=cfg.density, seed=5,
+                        temperature=cfg.temperature)
+        assert np.abs(g.positions() - r).max() < 1e-12
+        assert np.abs(g.velocities() - v).max() < 1e-12
+        e = g.energies()
+        assert e.ke == pytest.approx(1.5 * (cfg.n_atoms - 1) * cfg.temperature, rel=1e-12)
+        g.close()
+
+
+def test_runs_are_bitwise_reproducible(md):
+    cfg = get_config("wca_4k")
+    out = []
+    for _ in range(2):
+        g, _, _ = make_pair(md, cfg, 2, mode="fused")
+        g.step(120)
+        out.append((g.positions(), g.velocities(), g.forces()))
+        g.close()
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+def test_medium_system_full_comparison(md):
+    """configs[1] size (N = 262,144): spans ~2000 blocks; the oracle's cell search handles it in seconds."""
+    cfg = get_config("wca_262k")
+    g, o, box = make_pair(md, cfg, 1, mode="fused")
+    counts, lst = g.neighbors()
+    assert sets_equal(counts, lst, o)[0] == 0
+    assert force_rel_err(g.forces(), o.forces()) <= FORCE_RTOL
+    g.step(10)
+    o.step(10)
+    assert pos_err(g.positions(), o.positions(), box) <= POS_ATOL
+    eg, eo = g.energies(), o.energies()
+    assert eg.ke == pytest.approx(eo.ke, rel=ENERGY_RTOL) and eg.pe == pytest.approx(eo.pe, rel=ENERGY_RTOL)
