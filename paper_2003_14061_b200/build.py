@@ -36,6 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("MD_NVCC_FLAGS", "").split()          # tuning experiments, e.g. -DMD_FORCE_U=2
     cmd += [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True)
     return LIB

@@ -279,7 +279,7 @@ md_system *md_create_ex(const md_params *pp)
     if (p.force_variant != MD_FORCE_FULL_LIST && p.force_variant != MD_FORCE_NEWTON3_ATOMICS) { set_error("bad force_variant"); return nullptr; }
     if (p.force_variant == MD_FORCE_NEWTON3_ATOMICS) p.step_mode = MD_STEP_SPLIT;
     if (p.step_mode != MD_STEP_FUSED && p.step_mode != MD_STEP_SPLIT) { set_error("bad step_mode"); return nullptr; }
-    if (p.block_size == 0) p.block_size = 128;
+    if (p.block_size == 0) p.block_size = 256;
     if (p.block_size != 64 && p.block_size != 128 && p.block_size != 256 && p.block_size != 512) {
         set_error("block_size must be 64, 128, 256 or 512");
         return nullptr;
@@ -531,7 +531,7 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
     };
     for (int p = 0; p < N; p++)
         for (int m = 0; m < nnb[p]; m++) {
-            const int i = id[p], j = id[W[(size_t)m * np + p]];
+            const int i = id[p], j = id[(unsigned)W[(size_t)m * np + p] & 0x1fffffffu];   // top 3 bits: image flags
             add(i, j);
             if (P.half_list) add(j, i);
         }

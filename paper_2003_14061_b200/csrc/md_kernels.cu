@@ -4,14 +4,30 @@
 //   N3/N4  k_scan_*         prefix scan of the occupancies k_c (the GPU alternative the paper describes in
 //                           sec. 2.4(4)) -> CSR cell_start; replaces the dense cell x layer matrix H
 //          k_place/k_reorder  cell-order sort of the atoms at EVERY rebuild (paper: every 100 steps)
-//   N5     k_build          neighbor matrix W[m][i], row m contiguous over atoms
+//   N5     k_build          neighbor matrix W[m][i], row m contiguous over atoms, with the
+//                           periodic-image flag bits of PAPER.md:163 in the top 3 bits of every entry
 //   F1     k_force          pair forces over W, no Newton-3 (variant A) / k_force_n3 half list + atomics (variant B)
 //   F2     k_energy         block reductions finished by the last block
-//          k_kick_drift / k_kick   leapfrog integration with periodic wrap
-// The model arithmetic follows DESIGN.md "Readings" (R1..R8).  No code is shared with oracle/.
+//          k_kick_drift / k_kick   leapfrog integration
+// The model arithmetic follows DESIGN.md "Readings" (R1..R9).  No code is shared with oracle/.
+//
+// Periodic boundaries (R9).  Coordinates are wrapped into [0, L) only when the atoms are re-sorted
+// (k_reorder) and on output (k_export); between rebuilds they may stray outside the box by at most
+// r_shell/2.  That keeps the image flags frozen into W at build time valid for the life of the matrix,
+// which is the condition the paper's flag-bit scheme needs.
+#include <algorithm>
+
 #include "md_types.h"
 
 #define FULL_MASK 0xffffffffu
+#define W_INDEX_MASK 0x1fffffffu     // 29 index bits ("3 bits are sufficient" for the flags)
+#define W_FLAG_SHIFT 29
+#ifndef MD_FORCE_U
+#define MD_FORCE_U 2                 // gathers in flight per thread in the force loop
+#endif
+#ifndef MD_FORCE_MIN_THREADS
+#define MD_FORCE_MIN_THREADS 1024    // resident threads per SM the register allocation must allow
+#endif
 
 namespace {
 
@@ -30,32 +46,56 @@ __device__ __forceinline__ double wrap1(double x, double L)
     return x;
 }
 
-// squared minimum-image distance, fixed IEEE operation order (R5): the accept/reject decisions
-// r^2 < r_n^2 and r^2 < r_c^2 are taken on bit-identical values on every implementation.
-__device__ __forceinline__ double dist2(const pos_t &a, const pos_t &b, double L, double half, double &dx, double &dy,
-                                        double &dz)
-{
-    dx = minimg(a.x - b.x, L, half);
-    dy = minimg(a.y - b.y, L, half);
-    dz = minimg(a.z - b.z, L, half);
-    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-}
-
+// 32-byte record = one L2 sector, moved by ONE 256-bit access (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a):
+// a gather then costs one L1 tag look-up per lane instead of two with a pair of 128-bit loads.
+// Read-only path: never used on a buffer the same kernel writes.
 __device__ __forceinline__ pos_t ld_pos(const pos_t *p)
 {
-    // 32-byte record -> two 128-bit read-only loads (one sector)
-    const double2 *q = reinterpret_cast<const double2 *>(p);
-    double2 a = __ldg(q), b = __ldg(q + 1);
     pos_t r;
-    r.x = a.x; r.y = a.y; r.z = b.x; r.w = b.y;
+    asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ pos_t ld_pos_rw(const pos_t *p)
+{
+    pos_t r;
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
     return r;
 }
 
 __device__ __forceinline__ void st_pos(pos_t *p, double x, double y, double z)
 {
-    double2 *q = reinterpret_cast<double2 *>(p);
-    q[0] = make_double2(x, y);
-    q[1] = make_double2(z, 0.0);
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x), "d"(y), "d"(z), "d"(0.0) : "memory");
+}
+
+// 1/x to within ~1 ulp without the IEEE-division slow path: hardware seed + two Newton steps.
+// (Forces are compared with the oracle to 1e-10; the accept tests use r^2 itself.)
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    return y;
+}
+
+// Displacement r_i - r_j with the image correction frozen into the W entry (flag bit k set = subtract +-L
+// along axis k, sign taken from the raw difference).  On freshly wrapped coordinates this is
+// bit-for-bit the minimum-image arithmetic of DESIGN.md R5 (d0 = a - b rounded; d0 -+ L rounded), so
+// r^2 = fma(dz,dz, fma(dy,dy, dx*dx)) decides r^2 < r_c^2 on the same bits as any other implementation.
+__device__ __forceinline__ double disp2(const pos_t &a, const pos_t &b, unsigned fl, double L, double &dx, double &dy, double &dz)
+{
+    dx = a.x - b.x;
+    dy = a.y - b.y;
+    dz = a.z - b.z;
+    if (fl) {                                   // only atoms next to a periodic face take this branch
+        if (fl & 1u) dx -= copysign(L, dx);
+        if (fl & 2u) dy -= copysign(L, dy);
+        if (fl & 4u) dz -= copysign(L, dz);
+    }
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
 }
 
 __device__ __forceinline__ int cell_coord(double x, double inv_w, int nc)
@@ -174,7 +214,7 @@ __global__ void k_load_state(const __grid_constant__ MdDev P)
     P.id[vc][i] = i;
 }
 
-// device order -> scratch in original-id order.  what: 0 positions, 1 velocities, 2 forces
+// device order -> scratch in original-id order.  what: 0 positions (wrapped into [0, L)), 1 velocities, 2 forces
 __global__ void k_export(const __grid_constant__ MdDev P, int what, size_t offset)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -183,8 +223,8 @@ __global__ void k_export(const __grid_constant__ MdDev P, int what, size_t offse
     const int id = P.id[vc][i];
     double *o = P.scratch + offset + 3 * (size_t)id;
     if (what == 0) {
-        pos_t r = P.pos[pc][i];
-        o[0] = r.x; o[1] = r.y; o[2] = r.z;
+        const pos_t r = ld_pos_rw(P.pos[pc] + i);
+        o[0] = wrap1(r.x, P.L); o[1] = wrap1(r.y, P.L); o[2] = wrap1(r.z, P.L);
     } else {
         const double *a = what == 1 ? P.vel[vc] : P.frc;
         o[0] = a[i]; o[1] = a[P.N_pad + i]; o[2] = a[2 * (size_t)P.N_pad + i];
@@ -192,7 +232,7 @@ __global__ void k_export(const __grid_constant__ MdDev P, int what, size_t offse
 }
 
 // ------------------------------------------------------------------------------------------------
-// integration (split mode): first half kick + drift + wrap + max velocity + rebuild decision
+// integration (split mode): first half kick + drift + max velocity + rebuild decision
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDev P)
 {
@@ -204,10 +244,10 @@ __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDe
         pos_t *pp = P.pos[pc] + i;
         double *vx = P.vel[vc] + i, *vy = vx + P.N_pad, *vz = vy + P.N_pad;
         const double *fx = P.frc + i, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
-        pos_t r = *pp;
+        const pos_t r = ld_pos_rw(pp);
         const double ax = *vx + P.hdt * *fx, ay = *vy + P.hdt * *fy, az = *vz + P.hdt * *fz;
         *vx = ax; *vy = ay; *vz = az;
-        const double x = wrap1(r.x + P.dt * ax, P.L), y = wrap1(r.y + P.dt * ay, P.L), z = wrap1(r.z + P.dt * az, P.L);
+        const double x = r.x + P.dt * ax, y = r.y + P.dt * ay, z = r.z + P.dt * az;
         st_pos(pp, x, y, z);
         v2 = ax * ax + ay * ay + az * az;
         if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
@@ -229,18 +269,21 @@ __global__ void __launch_bounds__(256) k_kick(const __grid_constant__ MdDev P)
 }
 
 // ------------------------------------------------------------------------------------------------
-// cells: N1/N2 binning with atomic occupancy counters, N3/N4 as a prefix scan
+// cells: N1/N2 binning with atomic occupancy counters, N3/N4 as a prefix scan.  The rebuild kernels use
+// grid-stride loops over a capped grid: a launch that finds need_rebuild == 0 retires in ~2 us.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.N) return;
-    const pos_t r = P.pos[__ldcg(&P.ctrl->p_src)][i];
-    const int cx = cell_coord(r.x, P.inv_w, P.nc), cy = cell_coord(r.y, P.inv_w, P.nc), cz = cell_coord(r.z, P.inv_w, P.nc);
-    const int c = cx + P.nc * (cy + P.nc * cz);
-    P.cell_of[i] = c;
-    P.slot[i] = atomicAdd(&P.cell_count[c], 1);      // l_i; "incrementing k_c requires an atomic operation" (N2)
+    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_src)];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        const pos_t r = ld_pos(pos + i);
+        const int cx = cell_coord(wrap1(r.x, P.L), P.inv_w, P.nc), cy = cell_coord(wrap1(r.y, P.L), P.inv_w, P.nc),
+                  cz = cell_coord(wrap1(r.z, P.L), P.inv_w, P.nc);
+        const int c = cx + P.nc * (cy + P.nc * cz);
+        P.cell_of[i] = c;
+        P.slot[i] = atomicAdd(&P.cell_count[c], 1);  // l_i; "incrementing k_c requires an atomic operation" (N2)
+    }
 }
 
 constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
@@ -350,66 +393,79 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ M
 __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.N) return;
-    P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x)
+        P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
 }
 
-// Cell-order gather of r, v and the permanent serial numbers.  The atomics of N2 leave the
-// order inside a cell indeterminate; ranking the cell's members by their previous slot makes
-// the order -- and with it every floating-point sum downstream -- reproducible run to run.
+// Cell-order gather of r, v and the permanent serial numbers; coordinates are wrapped into
+// [0, L) here.  The atomics of N2 leave the order inside a cell indeterminate; ranking the
+// cell's members by their previous slot makes the order -- and with it every floating-point sum downstream --
+// reproducible run to run.
 __global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= P.N) return;
     const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
     const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
-    const int a = P.perm[p];
-    const int c = P.cell_of[a];
-    const int s = P.cell_start[c], e = P.cell_start[c + 1];
-    int rank = 0;
-    for (int q = s; q < e; q++) rank += (P.perm[q] < a);
-    const int n = s + rank;
-    const pos_t r = P.pos[ps][a];
-    st_pos(P.pos[pd] + n, r.x, r.y, r.z);
-    const double *vi = P.vel[vs] + a;
-    double *vo = P.vel[vd] + n;
-#pragma unroll
-    for (int k = 0; k < 3; k++) vo[(size_t)k * P.N_pad] = vi[(size_t)k * P.N_pad];
-    const int id = P.id[vs][a];
-    P.id[vd][n] = id;
-    if (P.has_bonds) P.inv[id] = n;
+    const pos_t *__restrict__ pin = P.pos[ps];
+    const double *__restrict__ vin = P.vel[vs];
+    const int *__restrict__ idin = P.id[vs];
+    for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P.N; p += gridDim.x * blockDim.x) {
+        const int a = P.perm[p];
+        // issue the payload loads first; the rank search below overlaps with their latency
+        const pos_t r = ld_pos(pin + a);
+        const double vx = __ldg(vin + a), vy = __ldg(vin + P.N_pad + a), vz = __ldg(vin + 2 * (size_t)P.N_pad + a);
+        const int id = __ldg(idin + a);
+        const int c = P.cell_of[a];
+        const int s = P.cell_start[c], e = P.cell_start[c + 1];
+        int rank = 0;
+        for (int q = s; q < e; q++) rank += (P.perm[q] < a);
+        const int n = s + rank;
+        st_pos(P.pos[pd] + n, wrap1(r.x, P.L), wrap1(r.y, P.L), wrap1(r.z, P.L));
+        double *vo = P.vel[vd] + n;
+        vo[0] = vx; vo[P.N_pad] = vy; vo[2 * (size_t)P.N_pad] = vz;
+        P.id[vd][n] = id;
+        if (P.has_bonds) P.inv[id] = n;
+    }
 }
 
 __global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= P.N) return;
-    const int id = P.id[__ldcg(&P.ctrl->v_dst)][n];
+    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
+    for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < P.N; n += gridDim.x * blockDim.x) {
+        const int id = idv[n];
 #pragma unroll
-    for (int k = 0; k < 2; k++) {
-        const int partner = P.bond_orig[(size_t)k * P.N + id];
-        P.bond_dev[(size_t)k * P.N_pad + n] = partner >= 0 ? P.inv[partner] : -1;
+        for (int k = 0; k < 2; k++) {
+            const int partner = P.bond_orig[(size_t)k * P.N + id];
+            P.bond_dev[(size_t)k * P.N_pad + n] = partner >= 0 ? P.inv[partner] : -1;
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // N5: neighbor matrix.  With the atoms in cell order (x fastest) the 27-cell stencil of an atom is 9
-// contiguous runs of the atom array (one per (dy,dz), 3 cells long, split only at the periodic x wrap).
+// contiguous runs of the atom array (one per (dy,dz), 3 cells long), plus single wrapped cells at the
+// periodic x faces.  One thread per atom walks its candidates as ONE flat loop over those runs: the threads
+// of a warp re-converge once per candidate, not at the end of every run, so lanes with short runs do not
+// idle; the next candidate's position is fetched while the current one is tested.
+// The periodic image is a per-run shift (0, +L or -L per axis) added to the raw difference.  For every pair
+// closer than r_n this is exactly the minimum-image arithmetic of DESIGN.md R5 (d0 = a - b rounded, then
+// d0 -+ L rounded): with cells wider than r_n and >= 3 cells per edge the image reached through the
+// stencil is the minimum image, and a pair for which it is not is farther than r_n in either form.
 // ------------------------------------------------------------------------------------------------
-template <bool HALF>
+// candidates j in [b, e) of one run, image shift (sx, sy, sz) and flag bits fl for the whole run
+template <bool HALF, bool SHIFT>
 __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, int b, int e,
-                                         int &m)
+                                         double sx, double sy, double sz, unsigned fl, int &m)
 {
     for (int j = b; j < e; j++) {
-        if (HALF ? (j <= i) : (j == i)) continue;
         const pos_t rj = ld_pos(pos + j);
-        double dx, dy, dz;
-        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
-        if (r2 < P.rn2) {
-            if (m < P.Mmax) P.W[(size_t)m * P.N_pad + i] = j;
+        // d = (r_i - r_j) + shift, each operation rounded once
+        double dx = __dsub_rn(ri.x, rj.x), dy = __dsub_rn(ri.y, rj.y), dz = __dsub_rn(ri.z, rj.z);
+        if (SHIFT) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
+        const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+        if (r2 < P.rn2 && (HALF ? (j > i) : (j != i))) {
+            if (m < P.Mmax) P.W[(size_t)m * P.N_pad + i] = (int)((unsigned)j | (fl << W_FLAG_SHIFT));
             m++;
         }
     }
@@ -421,33 +477,42 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     __shared__ int smx[4];
     __shared__ int ssum[4];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
-    int m = 0;
-    if (i < P.N) {
-        const pos_t ri = pos[i];
-        const int nc = P.nc;
+    const int *__restrict__ cs = P.cell_start;
+    const int nc = P.nc;
+    const double L = P.L;
+    int tmax = 0, tsum = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        const pos_t ri = ld_pos(pos + i);
         const int cx = cell_coord(ri.x, P.inv_w, nc), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
-        const int x0 = cx - 1, x1 = cx + 1;
-        const int xa = x0 < 0 ? 0 : x0, xb = x1 >= nc ? nc - 1 : x1;
+        const int xa = cx == 0 ? 0 : cx - 1, xb = cx == nc - 1 ? nc - 1 : cx + 1;
+        int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
             int z = cz + dz;
-            z = z < 0 ? z + nc : (z >= nc ? z - nc : z);
+            double sz = 0.0;
+            unsigned fz = 0u;
+            if (z < 0) { z += nc; sz = L; fz = 4u; } else if (z >= nc) { z -= nc; sz = -L; fz = 4u; }
             for (int dy = -1; dy <= 1; dy++) {
                 int y = cy + dy;
-                y = y < 0 ? y + nc : (y >= nc ? y - nc : y);
+                double sy = 0.0;
+                unsigned fl = fz;
+                if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
                 const int row = nc * (y + nc * z);
-                scan_run<HALF>(P, pos, ri, i, P.cell_start[row + xa], P.cell_start[row + xb + 1], m);
-                if (x0 < 0) scan_run<HALF>(P, pos, ri, i, P.cell_start[row + nc - 1], P.cell_start[row + nc], m);
-                if (x1 >= nc) scan_run<HALF>(P, pos, ri, i, P.cell_start[row], P.cell_start[row + 1], m);
+                const int b = __ldg(cs + row + xa), e = __ldg(cs + row + xb + 1);
+                if (fl) scan_run<HALF, true>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m);
+                else scan_run<HALF, false>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m);
+                if (cx == 0) scan_run<HALF, true>(P, pos, ri, i, __ldg(cs + row + nc - 1), __ldg(cs + row + nc), L, sy, sz, fl | 1u, m);
+                if (cx == nc - 1) scan_run<HALF, true>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + 1), -L, sy, sz, fl | 1u, m);
             }
         }
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
         if (m > P.Mmax) set_err(P, MD_ERR_NEBR_OVERFLOW);
+        tmax = max(tmax, m);
+        tsum += m;
     }
     // statistics of the matrix (md_energy.max_neighbors / mean_neighbors)
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int wm = warp_max_i(m), ws = warp_sum_i(m);
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
     if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -461,18 +526,20 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
 // ------------------------------------------------------------------------------------------------
 // F1: pair forces.  Thread i walks column i of W; row m is contiguous over i, so the 32 threads of a
 // warp read 128 consecutive bytes of W per row; the partner positions are gathers.
+// W streams from HBM once per step while the positions stay in L2, so the index loads run U rows ahead of
+// the gathers that depend on them (two dependent memory latencies would otherwise serialise per neighbor).
 // ------------------------------------------------------------------------------------------------
 struct PairAcc {
     double fx, fy, fz;
 };
 
-__device__ __forceinline__ void pair_force(const MdDev &P, const pos_t &ri, const pos_t &rj, PairAcc &a)
+__device__ __forceinline__ void pair_force(const MdDev &P, const pos_t &ri, const pos_t &rj, unsigned fl, PairAcc &a)
 {
     double dx, dy, dz;
-    const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+    const double r2 = disp2(ri, rj, fl, P.L, dx, dy, dz);
     if (r2 < P.rc2) {
-        const double s = 1.0 / r2, s3 = s * s * s;
-        const double fc = 48.0 * s3 * (s3 - 0.5) * s;
+        const double s = fast_rcp(r2), s3 = s * s * s;
+        const double fc = s3 * (s3 - 0.5) * s;          // x 48 applied once to the sums
         a.fx += fc * dx; a.fy += fc * dy; a.fz += fc * dz;
     }
 }
@@ -485,18 +552,47 @@ __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restri
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
         if (j < 0) continue;
         const pos_t rj = ld_pos(pos + j);
-        double dx, dy, dz;
-        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+        const double dx = minimg(ri.x - rj.x, P.L, P.half_L), dy = minimg(ri.y - rj.y, P.L, P.half_L),
+                     dz = minimg(ri.z - rj.z, P.L, P.half_L);
+        const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
         if (!(r2 < P.fene_R02)) { if (CHECK) set_err(P, MD_ERR_BOND_BROKEN); continue; }
         const double fc = -P.fene_k / (1.0 - r2 / P.fene_R02);
         a.fx += fc * dx; a.fy += fc * dy; a.fz += fc * dz;
     }
 }
 
-// MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = wrap(r + dt v) into the other position
+// sum of pair forces on atom i over column i of W
+template <int U>
+__device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i)
+{
+    const int m = P.nnb[i];
+    const int *__restrict__ w = P.W + i;
+    const size_t pitch = (size_t)P.N_pad;
+    PairAcc a = {0.0, 0.0, 0.0};
+    unsigned cur[U], nxt[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) cur[u] = u < m ? (unsigned)__ldcs(w + u * pitch) : 0u;
+    for (int k = 0; k < m; k += U) {
+        pos_t rj[U];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (k + u < m) rj[u] = ld_pos(pos + (cur[u] & W_INDEX_MASK));
+#pragma unroll
+        for (int u = 0; u < U; u++) nxt[u] = k + U + u < m ? (unsigned)__ldcs(w + (k + U + u) * pitch) : 0u;
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (k + u < m) pair_force(P, ri, rj[u], cur[u] >> W_FLAG_SHIFT, a);
+#pragma unroll
+        for (int u = 0; u < U; u++) cur[u] = nxt[u];
+    }
+    a.fx *= 48.0; a.fy *= 48.0; a.fz *= 48.0;
+    return a;
+}
+
+// MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = r + dt v into the other position
 // buffer, max |v|, rebuild decision.  MODE 2: store f and apply the closing half kick v += dt/2 f.
 template <int MODE, bool BONDS, int BLOCK>
-__global__ void __launch_bounds__(BLOCK) k_force(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * BLOCK + threadIdx.x;
@@ -505,15 +601,7 @@ __global__ void __launch_bounds__(BLOCK) k_force(const __grid_constant__ MdDev P
     double v2 = 0.0;
     if (i < P.N) {
         const pos_t ri = ld_pos(pos + i);
-        const int m = P.nnb[i];
-        const int *__restrict__ w = P.W + i;
-        PairAcc a = {0.0, 0.0, 0.0};
-#pragma unroll 4
-        for (int k = 0; k < m; k++) {
-            const int j = __ldcs(w + (size_t)k * P.N_pad);
-            const pos_t rj = ld_pos(pos + j);
-            pair_force(P, ri, rj, a);
-        }
+        PairAcc a = column_force<MD_FORCE_U>(P, pos, ri, i);
         if (BONDS) bond_force<true>(P, pos, ri, i, a);
         if (MODE == 0 || MODE == 2) {
             double *f = P.frc + i;
@@ -527,7 +615,7 @@ __global__ void __launch_bounds__(BLOCK) k_force(const __grid_constant__ MdDev P
             double *v = P.vel[vc] + i;
             const double vx = v[0] + P.dt * a.fx, vy = v[P.N_pad] + P.dt * a.fy, vz = v[2 * (size_t)P.N_pad] + P.dt * a.fz;
             v[0] = vx; v[P.N_pad] = vy; v[2 * (size_t)P.N_pad] = vz;
-            const double x = wrap1(ri.x + P.dt * vx, P.L), y = wrap1(ri.y + P.dt * vy, P.L), z = wrap1(ri.z + P.dt * vz, P.L);
+            const double x = ri.x + P.dt * vx, y = ri.y + P.dt * vy, z = ri.z + P.dt * vz;
             st_pos(P.pos[pc ^ 1] + i, x, y, z);
             v2 = vx * vx + vy * vy + vz * vz;
             if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
@@ -551,13 +639,15 @@ __global__ void __launch_bounds__(256) k_force_n3(const __grid_constant__ MdDev 
     const int *__restrict__ w = P.W + i;
     double *fx = P.frc, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
     PairAcc a = {0.0, 0.0, 0.0};
+#pragma unroll 2
     for (int k = 0; k < m; k++) {
-        const int j = __ldcs(w + (size_t)k * P.N_pad);
+        const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.N_pad);
+        const int j = (int)(en & W_INDEX_MASK);
         const pos_t rj = ld_pos(pos + j);
         double dx, dy, dz;
-        const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+        const double r2 = disp2(ri, rj, en >> W_FLAG_SHIFT, P.L, dx, dy, dz);
         if (r2 < P.rc2) {
-            const double s = 1.0 / r2, s3 = s * s * s;
+            const double s = fast_rcp(r2), s3 = s * s * s;
             const double fc = 48.0 * s3 * (s3 - 0.5) * s;
             const double gx = fc * dx, gy = fc * dy, gz = fc * dz;
             a.fx += gx; a.fy += gy; a.fz += gz;
@@ -594,11 +684,12 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P,
         const int m = P.nnb[i];
         const int *__restrict__ w = P.W + i;
         double u = 0.0, vir = 0.0;
+#pragma unroll 2
         for (int k = 0; k < m; k++) {
-            const int j = __ldcs(w + (size_t)k * P.N_pad);
-            const pos_t rj = ld_pos(pos + j);
+            const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.N_pad);
+            const pos_t rj = ld_pos(pos + (en & W_INDEX_MASK));
             double dx, dy, dz;
-            const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+            const double r2 = disp2(ri, rj, en >> W_FLAG_SHIFT, P.L, dx, dy, dz);
             if (r2 < P.rc2) {
                 const double s = 1.0 / r2, s3 = s * s * s;
                 u += 4.0 * s3 * (s3 - 1.0) - P.uc;
@@ -614,8 +705,9 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P,
                 const int j = P.bond_dev[(size_t)k * P.N_pad + i];
                 if (j < 0) continue;
                 const pos_t rj = ld_pos(pos + j);
-                double dx, dy, dz;
-                const double r2 = dist2(ri, rj, P.L, P.half_L, dx, dy, dz);
+                const double dx = minimg(ri.x - rj.x, P.L, P.half_L), dy = minimg(ri.y - rj.y, P.L, P.half_L),
+                             dz = minimg(ri.z - rj.z, P.L, P.half_L);
+                const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
                 if (!(r2 < P.fene_R02)) { set_err(P, MD_ERR_BOND_BROKEN); continue; }
                 const double x = 1.0 - r2 / P.fene_R02;
                 q[RED_PEB] += 0.5 * (-0.5 * P.fene_k * P.fene_R02 * log(x));
@@ -670,6 +762,9 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P,
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
+// grid of the rebuild kernels: at most one full wave (148 SMs); they use grid-stride loops
+inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdiv(n, block), 148 * per_sm); }
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -687,23 +782,23 @@ void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick<<<cdiv
 
 void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
-    k_bin<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    k_bin<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
     k_scan_reduce<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
     k_scan_top<<<1, 1024, 0, st>>>(P);
     k_scan_apply<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
-    k_place<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    k_place<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
 }
 
 void mdk_reorder(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
-    k_reorder<<<cdiv(P.N, 256), 256, 0, st>>>(P);
-    if (P.has_bonds) k_bonds_remap<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    k_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.has_bonds) k_bonds_remap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
 }
 
 void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
-    if (P.half_list) k_build<true><<<cdiv(P.N, 128), 128, 0, st>>>(P);
-    else k_build<false><<<cdiv(P.N, 128), 128, 0, st>>>(P);
+    if (P.half_list) k_build<true><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
+    else k_build<false><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
 }
 
 template <int MODE, bool BONDS>
@@ -711,9 +806,9 @@ static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
 {
     switch (block) {
     case 64: k_force<MODE, BONDS, 64><<<cdiv(P.N, 64), 64, 0, st>>>(P); break;
-    case 256: k_force<MODE, BONDS, 256><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
+    case 128: k_force<MODE, BONDS, 128><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
     case 512: k_force<MODE, BONDS, 512><<<cdiv(P.N, 512), 512, 0, st>>>(P); break;
-    default: k_force<MODE, BONDS, 128><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
+    default: k_force<MODE, BONDS, 256><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
     }
 }
 

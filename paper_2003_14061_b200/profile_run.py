@@ -1,0 +1,47 @@
+"""Short, deterministic run of the hot path for profilers (ncu): melt the lattice, then a few steps and forced
+rebuilds so that every kernel of the path appears with real work in the last launches.
+
+    python -m paper_2003_14061_b200.profile_run --config wca_2m --melt 100 --steps 12 --rebuilds 2
+"""
+from __future__ import annotations
+
+import argparse
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+
+from md_workloads import get_config, make_state  # noqa: E402
+from paper_2003_14061_b200 import MDSystem  # noqa: E402
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", default="wca_2m")
+    ap.add_argument("--melt", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=12)
+    ap.add_argument("--rebuilds", type=int, default=2)
+    ap.add_argument("--variant", default="full")
+    ap.add_argument("--mode", default="fused")
+    ap.add_argument("--block", type=int, default=0)
+    a = ap.parse_args()
+    cfg = get_config(a.config)
+    r, v, bonds, box = make_state(cfg, 1)
+    g = MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=a.variant,
+                 step_mode=a.mode if a.variant == "full" else "split", block_size=a.block)
+    g.set_state(r, v)
+    if bonds is not None:
+        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    g.step(a.melt)
+    e = g.energies()
+    print(f"melted: T={e.ke / (1.5 * (cfg.n_atoms - 1)):.4f} mean_nb={e.mean_neighbors:.3f} max_nb={e.max_neighbors} "
+          f"rebuilds={e.n_rebuilds} launches={g.info()['kernel_launches']}")
+    for _ in range(a.rebuilds):
+        g.rebuild_neighbors()
+    g.step(a.steps)
+    e = g.energies()
+    print(f"done: E/N={e.total / cfg.n_atoms:.9f} rebuilds={e.n_rebuilds} launches={g.info()['kernel_launches']}")
+
+
+if __name__ == "__main__":
+    main()
