@@ -51,7 +51,9 @@ typedef enum md_status {
     MD_ERR_NONFINITE = -4,      /* NaN/Inf in the state */
     MD_ERR_CUDA = -5,           /* CUDA runtime error (text in md_last_error) */
     MD_ERR_UNSUPPORTED = -6,    /* e.g. fewer than 3 cells per edge, more than 2 bonds per atom */
-    MD_ERR_NOMEM = -7
+    MD_ERR_NOMEM = -7,
+    MD_ERR_TILE_OVERFLOW = -8   /* tiled W: a block's cell neighbourhood holds more atoms than its shared-memory
+                                   tile (strongly inhomogeneous density); re-create with MD_FLAG_GLOBAL_W */
 } md_status;
 
 enum { MD_LATTICE_AUTO = 0, MD_LATTICE_SC = 1, MD_LATTICE_FCC = 2, MD_LATTICE_NONE = 3 };
@@ -82,7 +84,13 @@ typedef struct md_params {
     uint32_t flags;          /* MD_FLAG_* */
 } md_params;
 
-enum { MD_FLAG_NO_GRAPH = 1u  /* launch kernels one by one instead of replaying a captured CUDA graph */ };
+enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying a captured CUDA graph */
+       MD_FLAG_GLOBAL_W = 2u  /* W holds 29-bit global atom indices and partner positions are gathered through
+                                 L1/L2 (the paper's literal layout).  Default for variant A is the
+                                 tiled layout: every thread block stages the cell neighbourhood of its atoms in
+                                 shared memory and W holds 16-bit indices into that tile.
+                                 Variant B (Newton-3) always uses the global layout. */ };
+enum { MD_W_GLOBAL = 0, MD_W_TILED = 1 };
 
 /* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */
 typedef struct md_energy {
@@ -106,6 +114,12 @@ typedef struct md_info {
     int64_t device_bytes;       /* device memory held by this system */
     int64_t kernel_launches;    /* kernels launched by this system since creation */
     char    device_name[64];
+    int32_t w_layout;           /* MD_W_GLOBAL / MD_W_TILED */
+    int32_t tile_cells[3];      /* tiled: cells per thread block along x, y, z */
+    int32_t tile_capacity;      /* tiled: atoms the shared-memory tile can hold */
+    int32_t tile_threads;       /* tiled: threads per block of the build / force kernels */
+    int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node */
+    int32_t reserved_[1];
 } md_info;
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */

@@ -16,7 +16,8 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libmd_b200.so")
 
 MD_OK, MD_ERR_INVALID, MD_ERR_NEBR_OVERFLOW, MD_ERR_BOND_BROKEN = 0, -1, -2, -3
-MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM = -4, -5, -6, -7
+MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM, MD_ERR_TILE_OVERFLOW = -4, -5, -6, -7, -8
+FLAG_NO_GRAPH, FLAG_GLOBAL_W = 1, 2
 LATTICE = {"auto": 0, "sc": 1, "fcc": 2, "none": 3}
 FORCE_VARIANT = {"full": 0, "newton3": 1}
 STEP_MODE = {"fused": 0, "split": 1}
@@ -54,7 +55,9 @@ class _Info(C.Structure):
                 ("cell_width", C.c_double), ("cells_per_edge", C.c_int32), ("max_neighbors", C.c_int32),
                 ("block_size", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
                 ("n_bonds_per_atom_max", C.c_int32), ("device_bytes", C.c_int64), ("kernel_launches", C.c_int64),
-                ("device_name", C.c_char * 64)]
+                ("device_name", C.c_char * 64), ("w_layout", C.c_int32), ("tile_cells", C.c_int32 * 3),
+                ("tile_capacity", C.c_int32), ("tile_threads", C.c_int32), ("use_graph", C.c_int32),
+                ("reserved_", C.c_int32 * 1)]
 
 
 @dataclass
@@ -254,6 +257,8 @@ class MDSystem:
         self._ck(self._L.md_get_info(self._h, C.byref(i)))
         d = {k: getattr(i, k) for k, _ in _Info._fields_}
         d["device_name"] = d["device_name"].decode()
+        d["tile_cells"] = list(d["tile_cells"])
+        d.pop("reserved_", None)
         return d
 
     def set_profiling(self, on: bool):

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -146,6 +147,9 @@ int check_device_status(md_system *s)
             break;
         case MD_ERR_BOND_BROKEN: set_error("FENE bond stretched to r >= R0"); break;
         case MD_ERR_NONFINITE: set_error("non-finite position or velocity"); break;
+        case MD_ERR_TILE_OVERFLOW:
+            set_error("tiled W: a block's cell neighbourhood holds more than %d atoms; re-create with MD_FLAG_GLOBAL_W", s->P.tg.cap);
+            break;
         default: set_error("device error %d", err);
         }
     }
@@ -158,13 +162,19 @@ void enqueue_rebuild(md_system *s)
 {
     { Timed t(s, MD_T_CELLS, mdk_launches_of(LK_CELLS)); mdk_cells(s->P, s->lc, s->stream); }
     { Timed t(s, MD_T_REORDER, s->P.has_bonds ? 2 : 1); mdk_reorder(s->P, s->lc, s->stream); }
-    { Timed t(s, MD_T_NEBR, 1); mdk_build(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_NEBR, 1); if (s->P.tiled) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
+}
+
+void enqueue_force(md_system *s, int mode)
+{
+    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream);
+    else mdk_force(s->P, s->lc, mode, s->stream);
 }
 
 void enqueue_forces_only(md_system *s)
 {
     if (s->P.half_list) { Timed t(s, MD_T_FORCE, 2); mdk_force_newton3(s->P, s->lc, s->stream); }
-    else { Timed t(s, MD_T_FORCE, 1); mdk_force(s->P, s->lc, 0, s->stream); }
+    else { Timed t(s, MD_T_FORCE, 1); enqueue_force(s, 0); }
 }
 
 // state already in scratch (xyz | vxyz, original order): load, bin, build W, evaluate forces
@@ -215,6 +225,45 @@ int download(md_system *s, int what, double *out)
     CK(cudaGetLastError());
     memcpy(out, s->h_stage, n3 * sizeof(double));
     return MD_OK;
+}
+
+int env_int(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    return v && *v ? atoi(v) : dflt;
+}
+
+// Box of cells per thread block, block size and tile capacity of the tiled W layout (md_types.h: TileGeom).
+// Defaults aim at ~0.8 own atoms per thread and a 2 x 2 cross-section in y, z (halo factor ~4.5 for the WCA
+// configs); MD_TILE_S / _R / _RZ / _THREADS / _CAP override them for tuning runs.
+bool choose_tile(MdDev &P, size_t smem_optin)
+{
+    TileGeom &G = P.tg;
+    const int nc = P.nc;
+    const double per_cell = (double)P.N / P.NC;
+    G.R = std::min(std::max(env_int("MD_TILE_R", 2), 1), 3);
+    G.RZ = std::min(std::max(env_int("MD_TILE_RZ", 2), 1), 3);
+    G.threads = env_int("MD_TILE_THREADS", per_cell > 8.0 ? 512 : 256);
+    if (G.threads != 128 && G.threads != 256 && G.threads != 512) { set_error("MD_TILE_THREADS must be 128, 256 or 512"); return false; }
+    int S = env_int("MD_TILE_S", 0);
+    if (S <= 0) S = (int)lround(0.8 * G.threads / (G.R * G.RZ * per_cell));
+    S = std::min(std::max(S, 1), nc);
+    G.nsx = (nc + S - 1) / S;
+    G.S = (nc + G.nsx - 1) / G.nsx;                 // balance the boxes along x
+    G.nsx = (nc + G.S - 1) / G.S;
+    G.nsy = (nc + G.R - 1) / G.R;
+    G.nsz = (nc + G.RZ - 1) / G.RZ;
+    const double mean = (double)(G.S + 2) * (G.R + 2) * (G.RZ + 2) * per_cell;
+    int cap = env_int("MD_TILE_CAP", 0);
+    if (cap <= 0) cap = (int)(1.35 * mean + 6.0 * sqrt(mean) + 32.0);
+    cap = (cap + 31) & ~31;
+    if (cap > 8192) cap = 8192;
+    G.cap = cap;
+    if (mean > 0.8 * cap) { set_error("tiled W: %.0f atoms per tile exceed the 13-bit tile index; use MD_FLAG_GLOBAL_W or smaller MD_TILE_S", mean); return false; }
+    if (mdk_tile_smem(G, true) > smem_optin) { set_error("tiled W: tile of %d atoms does not fit shared memory", cap); return false; }
+    P.tiled = 1;
+    if (mdk_tile_configure(P) != 0) { set_error("tiled W: cudaFuncSetAttribute failed: %s", cudaGetErrorString(cudaGetLastError())); return false; }
+    return true;
 }
 
 }  // namespace
@@ -315,7 +364,7 @@ md_system *md_create_ex(const md_params *pp)
     if (cudaGetDevice(&s->device) != cudaSuccess) return fail("cudaGetDevice");
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return fail("cudaGetDeviceProperties");
-    snprintf(s->device_name, sizeof(s->device_name), "%s", prop.name);
+    snprintf(s->device_name, sizeof(s->device_name), "%.63s", prop.name);
     if (prop.major < 10) { set_error("device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); md_destroy(s); return nullptr; }
     if (p.stream) s->stream = (cudaStream_t)p.stream;
     else {
@@ -341,6 +390,12 @@ md_system *md_create_ex(const md_params *pp)
     s->lc.block = p.block_size;
     s->lc.grid_atoms = (P.N + p.block_size - 1) / p.block_size;
 
+    P.tiled = 0;
+    if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
+        if (!choose_tile(P, prop.sharedMemPerBlockOptin)) { md_destroy(s); return nullptr; }
+    }
+    P.max_grid = std::max((P.N + 255) / 256, P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
+
     const size_t np = (size_t)P.N_pad;
     bool ok = true;
     auto A = [&](size_t bytes) { void *q = dev_alloc(s, bytes); if (!q) ok = false; return q; };
@@ -357,8 +412,9 @@ md_system *md_create_ex(const md_params *pp)
     P.cell_count = (int *)A(((size_t)P.NC + 1) * sizeof(int));
     P.cell_start = (int *)A(((size_t)P.NC + 1) * sizeof(int));
     P.block_sums = (int *)A(((size_t)P.scan_blocks + 1) * sizeof(int));
-    P.W = (int *)A((size_t)P.Mmax * np * sizeof(int));
-    P.partials = (double *)A((size_t)RED_N * ((P.N + 255) / 256) * sizeof(double));
+    P.W = (int *)A((size_t)(P.tiled ? P.Mmax / 2 : P.Mmax) * np * sizeof(int));
+    P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
+    if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
     if (!ok) { set_error("device allocation failed (%.1f MB so far)", s->bytes / 1048576.0); md_destroy(s); return nullptr; }
@@ -464,10 +520,10 @@ int md_step(md_system *s, int64_t n)
         { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
         enqueue_rebuild(s);
         for (int64_t k = 1; k < n; k++) {
-            { Timed t(s, MD_T_FUSED_STEP, 1); mdk_force(P, s->lc, 1, st); }
+            { Timed t(s, MD_T_FUSED_STEP, 1); enqueue_force(s, 1); }
             enqueue_rebuild(s);
         }
-        { Timed t(s, MD_T_FORCE, 1); mdk_force(P, s->lc, 2, st); }
+        { Timed t(s, MD_T_FORCE, 1); enqueue_force(s, 2); }
     } else {
         for (int64_t k = 0; k < n; k++) {
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
@@ -484,7 +540,7 @@ int md_energies(md_system *s, md_energy *out)
 {
     if (!s || !out) { set_error("md_energies: null argument"); return MD_ERR_INVALID; }
     if (!s->has_state) { set_error("md_energies: no state"); return MD_ERR_INVALID; }
-    { Timed t(s, MD_T_ENERGY, 1); mdk_energy(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_ENERGY, 1); if (s->P.tiled) mdk_tile_energy(s->P, s->stream); else mdk_energy(s->P, s->lc, s->stream); }
     int rc = check_device_status(s);
     if (rc) return rc;
     const DevCtrl &c = *s->h_ctrl;
@@ -516,7 +572,8 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
     const MdDev &P = s->P;
     const int N = P.N, M = P.Mmax;
     const size_t np = (size_t)P.N_pad;
-    const int rows = std::min(M, std::max(1, s->h_ctrl->max_nnb));
+    const int nrows = std::min(M, std::max(1, s->h_ctrl->max_nnb));
+    const int rows = P.tiled ? (nrows + 1) / 2 : nrows;      // tiled: two 16-bit entries per 32-bit word
     std::vector<int> nnb(N), id(N), W((size_t)rows * np);
     CK(cudaMemcpy(nnb.data(), P.nnb, N * sizeof(int), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(id.data(), P.id[s->h_ctrl->v_dst], N * sizeof(int), cudaMemcpyDeviceToHost));
@@ -529,12 +586,42 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
         else overflow = true;
         cnt[a]++;
     };
-    for (int p = 0; p < N; p++)
-        for (int m = 0; m < nnb[p]; m++) {
-            const int i = id[p], j = id[(unsigned)W[(size_t)m * np + p] & 0x1fffffffu];   // top 3 bits: image flags
-            add(i, j);
-            if (P.half_list) add(j, i);
+    if (P.tiled) {
+        // rebuild every block's tile layout from cell_start exactly as the kernels do (md_tile.cu: tile_setup)
+        std::vector<int> cs((size_t)P.NC + 1), map;
+        CK(cudaMemcpy(cs.data(), P.cell_start, cs.size() * sizeof(int), cudaMemcpyDeviceToHost));
+        const int nblocks = P.tg.nsx * P.tg.nsy * P.tg.nsz;
+        for (int b = 0; b < nblocks; b++) {
+            const TileBox B = tile_box(P.tg, P.nc, b);
+            map.clear();
+            std::vector<std::pair<int, int>> own;            // (global start, length) of the box's own rows
+            for (int q = 0; q < B.nq; q++) {
+                int rowc, ysh, zsh, xa, xc;
+                tile_row(B, P.nc, q, rowc, ysh, zsh, xa, xc);
+                const int g[3] = {cs[rowc + xa], cs[rowc + B.x0], cs[rowc + xc]};
+                const int n[3] = {cs[rowc + xa + 1] - g[0], cs[rowc + B.x0 + B.sxc] - g[1], cs[rowc + xc + 1] - g[2]};
+                for (int k = 0; k < 3; k++) for (int u = 0; u < n[k]; u++) map.push_back(g[k] + u);
+                const int qy = q % B.nyq, qz = q / B.nyq;
+                if (qy >= 1 && qy <= B.ny && qz >= 1 && qz <= B.nz) own.push_back({g[1], n[1]});
+            }
+            for (auto &r : own)
+                for (int pidx = r.first; pidx < r.first + r.second; pidx++)
+                    for (int m = 0; m < nnb[pidx]; m++) {
+                        const unsigned w2 = (unsigned)W[(size_t)(m >> 1) * np + pidx];
+                        const unsigned e = (m & 1) ? (w2 >> 16) : (w2 & 0xffffu);
+                        const unsigned l = e & T_INDEX_MASK;
+                        if (l >= map.size()) { set_error("md_get_neighbors: corrupt tile index"); return MD_ERR_INVALID; }
+                        add(id[pidx], id[map[l]]);
+                    }
         }
+    } else {
+        for (int p = 0; p < N; p++)
+            for (int m = 0; m < nnb[p]; m++) {
+                const int i = id[p], j = id[(unsigned)W[(size_t)m * np + p] & 0x1fffffffu];   // top 3 bits: image flags
+                add(i, j);
+                if (P.half_list) add(j, i);
+            }
+    }
     for (int i = 0; i < N; i++) {
         counts[i] = cnt[i];
         if (list) for (int m = std::min(cnt[i], M); m < M; m++) list[(size_t)i * M + m] = -1;
@@ -552,6 +639,11 @@ int md_get_info(md_system *s, md_info *out)
     out->cells_per_edge = s->P.nc; out->max_neighbors = s->P.Mmax; out->block_size = s->lc.block;
     out->force_variant = s->prm.force_variant; out->step_mode = s->prm.step_mode;
     out->n_bonds_per_atom_max = s->n_bonds_max;
+    out->w_layout = s->P.tiled ? MD_W_TILED : MD_W_GLOBAL;
+    if (s->P.tiled) {
+        out->tile_cells[0] = s->P.tg.S; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
+        out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
+    }
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

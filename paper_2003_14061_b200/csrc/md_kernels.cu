@@ -17,172 +17,9 @@
 // which is the condition the paper's flag-bit scheme needs.
 #include <algorithm>
 
-#include "md_types.h"
-
-#define FULL_MASK 0xffffffffu
-#define W_INDEX_MASK 0x1fffffffu     // 29 index bits ("3 bits are sufficient" for the flags)
-#define W_FLAG_SHIFT 29
-#ifndef MD_FORCE_U
-#define MD_FORCE_U 2                 // gathers in flight per thread in the force loop
-#endif
-#ifndef MD_FORCE_MIN_THREADS
-#define MD_FORCE_MIN_THREADS 1024    // resident threads per SM the register allocation must allow
-#endif
+#include "md_device.cuh"
 
 namespace {
-
-// ------------------------------------------------------------------------------------------------
-// small device helpers
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double minimg(double d, double L, double half)
-{
-    return d > half ? d - L : (d < -half ? d + L : d);
-}
-
-__device__ __forceinline__ double wrap1(double x, double L)
-{
-    if (x >= L) x -= L;
-    else if (x < 0.0) { x += L; if (x >= L) x = 0.0; }
-    return x;
-}
-
-// 32-byte record = one L2 sector, moved by ONE 256-bit access (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a):
-// a gather then costs one L1 tag look-up per lane instead of two with a pair of 128-bit loads.
-// Read-only path: never used on a buffer the same kernel writes.
-__device__ __forceinline__ pos_t ld_pos(const pos_t *p)
-{
-    pos_t r;
-    asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
-    return r;
-}
-
-__device__ __forceinline__ pos_t ld_pos_rw(const pos_t *p)
-{
-    pos_t r;
-    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
-    return r;
-}
-
-__device__ __forceinline__ void st_pos(pos_t *p, double x, double y, double z)
-{
-    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x), "d"(y), "d"(z), "d"(0.0) : "memory");
-}
-
-// 1/x to within ~1 ulp without the IEEE-division slow path: hardware seed + two Newton steps.
-// (Forces are compared with the oracle to 1e-10; the accept tests use r^2 itself.)
-__device__ __forceinline__ double fast_rcp(double x)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    return y;
-}
-
-// Displacement r_i - r_j with the image correction frozen into the W entry (flag bit k set = subtract +-L
-// along axis k, sign taken from the raw difference).  On freshly wrapped coordinates this is
-// bit-for-bit the minimum-image arithmetic of DESIGN.md R5 (d0 = a - b rounded; d0 -+ L rounded), so
-// r^2 = fma(dz,dz, fma(dy,dy, dx*dx)) decides r^2 < r_c^2 on the same bits as any other implementation.
-__device__ __forceinline__ double disp2(const pos_t &a, const pos_t &b, unsigned fl, double L, double &dx, double &dy, double &dz)
-{
-    dx = a.x - b.x;
-    dy = a.y - b.y;
-    dz = a.z - b.z;
-    if (fl) {                                   // only atoms next to a periodic face take this branch
-        if (fl & 1u) dx -= copysign(L, dx);
-        if (fl & 2u) dy -= copysign(L, dy);
-        if (fl & 4u) dz -= copysign(L, dz);
-    }
-    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-}
-
-__device__ __forceinline__ int cell_coord(double x, double inv_w, int nc)
-{
-    int q = (int)floor(x * inv_w);
-    q = q < 0 ? 0 : q;
-    return q >= nc ? nc - 1 : q;
-}
-
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
-    return v;
-}
-__device__ __forceinline__ double warp_max(double v)
-{
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(FULL_MASK, v, o));
-    return v;
-}
-__device__ __forceinline__ int warp_sum_i(int v)
-{
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
-    return v;
-}
-__device__ __forceinline__ int warp_max_i(int v)
-{
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v = max(v, __shfl_xor_sync(FULL_MASK, v, o));
-    return v;
-}
-
-// block-wide max of a non-negative double; result valid in thread 0.  sm: >= 32 doubles.
-__device__ __forceinline__ double block_max(double v, double *sm)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    v = warp_max(v);
-    if (lane == 0) sm[wid] = v;
-    __syncthreads();
-    if (wid == 0) {
-        v = lane < nw ? sm[lane] : 0.0;
-        v = warp_max(v);
-    }
-    return v;
-}
-
-// The rebuild decision (R8), taken by ONE thread of the last block of the kernel
-// that drifted the positions.  It also fixes which buffers the rebuild kernels read and write, so the host
-// never needs to know whether a rebuild happened.
-__device__ void decide(const MdDev &P, bool pos_pingpong)
-{
-    volatile DevCtrl *c = P.ctrl;
-    const double vmax2 = __longlong_as_double((long long)c->vmax2_bits);
-    c->vmax2_bits = 0ull;
-    double acc = c->disp_acc + P.dt * sqrt(vmax2);
-    const int need = acc > P.thresh;
-    if (need) {
-        acc = 0.0;
-        c->n_rebuilds += 1;
-        c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
-    }
-    c->disp_acc = acc;
-    c->need_rebuild = need;
-    const int ps = pos_pingpong ? (c->p_dst ^ 1) : c->p_dst;
-    c->p_src = ps;
-    c->p_dst = need ? (ps ^ 1) : ps;
-    const int vs = c->v_dst;
-    c->v_src = vs;
-    c->v_dst = need ? (vs ^ 1) : vs;
-}
-
-// thread 0 of each block: publish the block's max v^2, then take a ticket; the last block decides.
-__device__ __forceinline__ void publish_vmax_and_decide(const MdDev &P, double bmax2, bool pos_pingpong)
-{
-    DevCtrl *c = P.ctrl;
-    atomicMax(&c->vmax2_bits, (unsigned long long)__double_as_longlong(bmax2));
-    __threadfence();
-    const unsigned t = atomicInc(&c->ticket[TK_INTEGRATE], gridDim.x - 1);
-    if (t == gridDim.x - 1) {
-        __threadfence();
-        decide(P, pos_pingpong);
-    }
-}
-
-__device__ __forceinline__ void set_err(const MdDev &P, int code) { atomicCAS(&P.ctrl->err, 0, code); }
 
 // ------------------------------------------------------------------------------------------------
 // control / staging kernels
@@ -669,10 +506,9 @@ __global__ void __launch_bounds__(256) k_zero_forces(const __grid_constant__ MdD
 // -> the last block (atomic ticket + memory fence) finishes in a fixed order, so results are reproducible.
 // ------------------------------------------------------------------------------------------------
 template <bool BONDS>
-__global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P, int max_grid)
+__global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
 {
-    __shared__ double sm[RED_N][8];
-    __shared__ bool last;
+    __shared__ RedSmem S;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pos = P.pos[pc];
@@ -721,43 +557,7 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P,
         q[RED_PX] = vx; q[RED_PY] = vy; q[RED_PZ] = vz;
         q[RED_VMAX2] = v2;
     }
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int k = 0; k < RED_N; k++) {
-        const double r = k == RED_VMAX2 ? warp_max(q[k]) : warp_sum(q[k]);
-        if (lane == 0) sm[k][wid] = r;
-    }
-    __syncthreads();
-    if (threadIdx.x < RED_N) {
-        const int k = threadIdx.x;
-        double r = sm[k][0];
-        for (int w = 1; w < (int)(blockDim.x >> 5); w++) r = k == RED_VMAX2 ? fmax(r, sm[k][w]) : r + sm[k][w];
-        P.partials[(size_t)k * max_grid + blockIdx.x] = r;
-    }
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned t = atomicInc(&P.ctrl->ticket[TK_ENERGY], gridDim.x - 1);
-        last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    // the last block sums the partials of all blocks (itself included), fixed order
-    for (int k = 0; k < RED_N; k++) {
-        double r = 0.0;
-        const volatile double *p = P.partials + (size_t)k * max_grid;
-        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) r = k == RED_VMAX2 ? fmax(r, p[b]) : r + p[b];
-        r = k == RED_VMAX2 ? warp_max(r) : warp_sum(r);
-        __syncthreads();
-        if (lane == 0) sm[0][wid] = r;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t = sm[0][0];
-            for (int w = 1; w < (int)(blockDim.x >> 5); w++) t = k == RED_VMAX2 ? fmax(t, sm[0][w]) : t + sm[0][w];
-            P.ctrl->red[k] = t;
-        }
-    }
+    reduce_finish(P, q, S);
 }
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
@@ -835,8 +635,8 @@ void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)
 void mdk_energy(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     const int grid = cdiv(P.N, 256);
-    if (P.has_bonds) k_energy<true><<<grid, 256, 0, st>>>(P, grid);
-    else k_energy<false><<<grid, 256, 0, st>>>(P, grid);
+    if (P.has_bonds) k_energy<true><<<grid, 256, 0, st>>>(P);
+    else k_energy<false><<<grid, 256, 0, st>>>(P);
 }
 
 int mdk_launches_of(int which)

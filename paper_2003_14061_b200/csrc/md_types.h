@@ -37,11 +37,77 @@ struct DevCtrl {
 
 enum { TK_INTEGRATE = 0, TK_ENERGY = 1, TK_FORCE = 2 };
 
+// Shared-memory tile decomposition of the W layout MD_W_TILED.  The cells are cut into
+// boxes of S x R x RZ cells (x fastest).  One thread block owns the atoms of one box -- R*RZ contiguous index
+// ranges, because atoms are kept in cell order -- and stages the positions of the box plus one halo cell on
+// every side (the 27-cell neighbourhoods of all its atoms) in shared memory: (R+2)(RZ+2) "tile
+// rows", each the contiguous atoms of S+2 cells along x.  W then holds 16-bit entries: 13 bits of index
+// into that tile + the 3 periodic-image flag bits of PAPER.md:163.
+struct TileGeom {
+    int S, R, RZ;            // cells per box along x, y, z
+    int nsx, nsy, nsz;       // boxes per axis
+    int cap;                 // tile capacity in atoms (<= 8192: 13 index bits)
+    int threads;             // block size of the tile kernels
+};
+
+struct TileBox {
+    int x0, sxc, y0, ny, z0, nz;   // first cell and number of cells of the box along each axis
+    int nyq, nq;                   // tile rows per z plane (ny + 2) and in total
+};
+
+__host__ __device__ inline TileBox tile_box(const TileGeom &G, int nc, int b)
+{
+    TileBox B;
+    const int bx = b % G.nsx, by = (b / G.nsx) % G.nsy, bz = b / (G.nsx * G.nsy);
+    B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
+    B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
+    B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
+    B.nyq = B.ny + 2;
+    B.nq = B.nyq * (B.nz + 2);
+    return B;
+}
+
+// Tile row q of a box: the row of cells (y0-1 + q % nyq, z0-1 + q / nyq), wrapped periodically.
+// rowc = linear index of its x = 0 cell; ysh, zsh in {-1, 0, +1}: image shift of the row in units of L
+// (added to r_i - r_j); xa, xc = x index of the halo cells before / after the box (wrapped at the faces).
+__host__ __device__ inline void tile_row(const TileBox &B, int nc, int q, int &rowc, int &ysh, int &zsh, int &xa, int &xc)
+{
+    int y = B.y0 - 1 + q % B.nyq, z = B.z0 - 1 + q / B.nyq;
+    ysh = 0; zsh = 0;
+    if (y < 0) { y += nc; ysh = 1; } else if (y >= nc) { y -= nc; ysh = -1; }
+    if (z < 0) { z += nc; zsh = 1; } else if (z >= nc) { z -= nc; zsh = -1; }
+    rowc = nc * (y + nc * z);
+    xa = B.x0 == 0 ? nc - 1 : B.x0 - 1;
+    xc = B.x0 + B.sxc == nc ? 0 : B.x0 + B.sxc;
+}
+
+constexpr int TILE_Q_MAX = 25;      // (R + 2)(RZ + 2) with R, RZ <= 3
+constexpr int TILE_OWN_MAX = 9;     // R * RZ
+
+// Tile descriptor of one box: written to global memory by the build kernel (the layout only changes when
+// cell_start does, i.e. at a rebuild), read back with one coalesced load by every force / energy kernel.
+struct TileDesc {
+    int n_own, T, nq, pad;                              // atoms owned by the box, atoms in the tile, tile rows
+    int own_base[TILE_OWN_MAX];                         // global index of the first own atom of own row k
+    int own_loc[TILE_OWN_MAX];                          // its index in the tile
+    int own_pre[TILE_OWN_MAX + 1];                      // exclusive prefix of the own-row lengths
+    struct Row {
+        int g[3], n[3];                                 // the (up to) 3 contiguous pieces of the row: start, length
+        int off;                                        // tile index of the row's first atom
+    } row[TILE_Q_MAX];
+};
+constexpr int TILE_DESC_INTS = (int)(sizeof(TileDesc) / sizeof(int));
+constexpr int TILE_DESC_HEAD = 4 + 2 * TILE_OWN_MAX + TILE_OWN_MAX + 1;     // ints before row[]
+#define T_INDEX_MASK 0x1fffu
+#define T_FLAG_SHIFT 13
+
 // The unvarying parameter block.  The paper copies it to constant memory; here it is a
 // __grid_constant__ kernel argument, which lives in the same constant bank without a separate copy.
 struct MdDev {
     int N, N_pad, Mmax, nc, NC;
     int has_bonds, half_list, scan_blocks;
+    int tiled, max_grid;                // W layout (1 = MD_W_TILED); row pitch of `partials`
+    TileGeom tg;
     double L, half_L, inv_w;            // inv_w = nc / L
     double rc2, rn2, uc;
     double dt, hdt, thresh;             // thresh = r_shell / 2
@@ -51,7 +117,9 @@ struct MdDev {
     double *frc;                        // SoA, same pitch
     int *id[2];                         // device slot -> original atom id
     int *cell_of, *slot, *cell_count, *cell_start, *perm, *block_sums;
+    int *tile_desc;                     // tiled layout: TileDesc per box
     int *W, *nnb;                       // neighbor matrix W[m * N_pad + i], counts m_i
+                                        // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
@@ -76,6 +144,12 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    // 0 pos, 1 vel, 2 frc -> scratch + offset
+// tiled layout (md_tile.cu)
+int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
+size_t mdk_tile_smem(const TileGeom &G, bool with_cells);
+void mdk_tile_build(const MdDev &P, cudaStream_t st);
+void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st);
+void mdk_tile_energy(const MdDev &P, cudaStream_t st);
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,
        LK_ENERGY, LK_EXPORT };

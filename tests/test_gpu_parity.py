@@ -43,6 +43,8 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
         o.set_state(r, v)
         if bonds is not None:
             o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    if variant == "full-globalw":          # variant A on the paper's literal W layout (global indices, L1/L2 gathers)
+        variant, kw = "full", dict(kw, flags=md.FLAG_GLOBAL_W)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
                     step_mode=mode, **kw)
     g.set_state(r, v)
@@ -52,7 +54,7 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
 
 
 @pytest.mark.parametrize("case", list(small_cases()))
-@pytest.mark.parametrize("variant", ["full", "newton3"])
+@pytest.mark.parametrize("variant", ["full", "full-globalw", "newton3"])
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
 def test_neighbor_sets_and_forces(md, case, variant, state):
     cfg, _ = small_cases()[case]
@@ -76,14 +78,15 @@ def test_neighbor_sets_and_forces(md, case, variant, state):
         assert eg.pe_bond == pytest.approx(eo.pe_bond, rel=ENERGY_RTOL, abs=1e-9)
         assert eg.virial == pytest.approx(eo.virial, rel=ENERGY_RTOL, abs=1e-7)
         assert eg.ke == pytest.approx(eo.ke, rel=1e-12)
-        if variant == "full":                                    # variant B stores (and reports) the half matrix
+        if variant != "newton3":                                 # variant B stores (and reports) the half matrix
             assert eg.max_neighbors == eo.max_neighbors
         assert eg.mean_neighbors == pytest.approx(eo.mean_neighbors, rel=1e-12)
         g.close()
 
 
 @pytest.mark.parametrize("case", list(small_cases()))
-@pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("newton3", "split")])
+@pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("full-globalw", "fused"),
+                                          ("full-globalw", "split"), ("newton3", "split")])
 def test_ten_steps(md, case, variant, mode):
     cfg, _ = small_cases()[case]
     for seed in (1, 2, 3):
@@ -172,3 +175,40 @@ def test_medium_system_full_comparison(md):
     assert pos_err(g.positions(), o.positions(), box) <= POS_ATOL
     eg, eo = g.energies(), o.energies()
     assert eg.ke == pytest.approx(eo.ke, rel=ENERGY_RTOL) and eg.pe == pytest.approx(eo.pe, rel=ENERGY_RTOL)
+
+
+TILE_GEOMS = [dict(S=1, R=1, RZ=1, THREADS=128), dict(S=2, R=3, RZ=1, THREADS=128), dict(S=3, R=2, RZ=3, THREADS=256),
+              dict(S=1000, R=3, RZ=3, THREADS=512), dict(S=4, R=1, RZ=2, THREADS=256), dict(S=5, R=2, RZ=2, THREADS=128)]
+
+
+@pytest.mark.parametrize("case", ["wca_ragged_1000", "wca_dr05_13824", "lj_6912", "chains_4096"])
+@pytest.mark.parametrize("geom", range(len(TILE_GEOMS)))
+def test_tiled_w_any_box_shape(md, case, geom, monkeypatch):
+    """The tiled W layout must give the same matrix, forces and trajectory for every box shape S x R x RZ and
+    block size (boxes cut by the periodic faces, boxes wider than the system, blocks looping over their atoms)."""
+    cfg, _ = small_cases()[case]
+    for k, v in TILE_GEOMS[geom].items():
+        monkeypatch.setenv(f"MD_TILE_{k}", str(v))
+    monkeypatch.setenv("MD_TILE_CAP", "8192")
+    g, o, box = make_pair(md, cfg, 2, variant="full", mode="fused", state="jitter")
+    info = g.info()
+    assert info["w_layout"] == 1 and info["tile_cells"][1:] == [TILE_GEOMS[geom]["R"], TILE_GEOMS[geom]["RZ"]]
+    counts, lst = g.neighbors()
+    nbad, first = sets_equal(counts, lst, o)
+    assert nbad == 0, f"neighbor sets differ for {nbad} atoms (first: atom {first})"
+    assert force_rel_err(g.forces(), o.forces()) <= FORCE_RTOL
+    g.step(10)
+    o.step(10)
+    assert pos_err(g.positions(), o.positions(), box) <= POS_ATOL
+    eg, eo = g.energies(), o.energies()
+    assert eg.ke == pytest.approx(eo.ke, rel=ENERGY_RTOL) and eg.pe == pytest.approx(eo.pe, rel=ENERGY_RTOL)
+    g.close()
+
+
+def test_tile_overflow_is_reported(md, monkeypatch):
+    cfg = get_config("wca_4k")
+    monkeypatch.setenv("MD_TILE_CAP", "64")
+    r, v, _, box = make_state(cfg, 1, jitter_amp=0.1)
+    with pytest.raises(md.MDError):
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+        g.set_state(r, v)
