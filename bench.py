@@ -178,6 +178,7 @@ def main():
     ap.add_argument("--variant", default="full", choices=["full", "newton3"])
     ap.add_argument("--mode", default="fused", choices=["fused", "split"])
     ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--flags", type=int, default=0, help="md_params.flags: 1 = no CUDA graph, 2 = global-index W layout")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -213,7 +214,7 @@ def main():
     seed = 1 + rank
     r0, v0, bonds, box = make_state(cfg, seed)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=args.variant,
-                    step_mode=args.mode if args.variant == "full" else "split", block_size=args.block)
+                    step_mode=args.mode if args.variant == "full" else "split", block_size=args.block, flags=args.flags)
     g.set_state(r0, v0)
     if bonds is not None:
         g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)

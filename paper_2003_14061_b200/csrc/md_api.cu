@@ -65,6 +65,14 @@ struct md_system {
     // profiling
     bool profiling = false;
     std::vector<EvPair> pending, pool;
+    // CUDA graph of one fused step: force+kick+drift -> decide -> IF(need_rebuild){cells, reorder, build}
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    cudaStream_t cap_stream = nullptr;
+    bool graph_tried = false;
+    int chain_kernels = 0;         // kernels inside the conditional body
+    int rebuilds_seen = 0;
+    int64_t graph_steps = 0;       // steps run through the graph since the last status read         // ctrl->n_rebuilds at the last status read (launch accounting)
     double t_ms[MD_T_COUNT] = {0};
     int64_t t_n[MD_T_COUNT] = {0};
 };
@@ -139,6 +147,12 @@ int check_device_status(md_system *s)
 {
     int rc = fetch_ctrl(s);
     if (rc) return rc;
+    if (s->graph_steps > 0) {      // kernels of the conditional bodies that actually ran
+        const int d = s->h_ctrl->n_rebuilds - s->rebuilds_seen;
+        if (d > 0) s->launches += (int64_t)std::min<int64_t>(d, s->graph_steps) * s->chain_kernels;
+        s->graph_steps = 0;
+    }
+    s->rebuilds_seen = s->h_ctrl->n_rebuilds;
     const int err = s->h_ctrl->err;
     if (err) {
         switch (err) {
@@ -165,10 +179,71 @@ void enqueue_rebuild(md_system *s)
     { Timed t(s, MD_T_NEBR, 1); if (s->P.tiled) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
-void enqueue_force(md_system *s, int mode)
+void enqueue_force(md_system *s, int mode, unsigned long long cond = 0ull)
 {
-    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream);
-    else mdk_force(s->P, s->lc, mode, s->stream);
+    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream, cond);
+    else mdk_force(s->P, s->lc, mode, s->stream, cond);
+}
+
+void drop_graph(md_system *s)
+{
+    if (s->gexec) cudaGraphExecDestroy(s->gexec);
+    if (s->graph) cudaGraphDestroy(s->graph);
+    s->gexec = nullptr; s->graph = nullptr; s->graph_tried = false;
+}
+
+// One fused time step as a CUDA graph.  The rebuild chain sits in the body of an IF node whose condition
+// k_decide sets on the device (cudaGraphSetConditional), so a step without a rebuild launches 2 kernels
+// instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision on the host every step).
+// Returns false (and leaves no graph) if any step of the construction is refused; md_step then launches
+// the kernels one by one.
+bool build_step_graph(md_system *s)
+{
+    s->graph_tried = true;
+    cudaStream_t st = s->stream;
+    if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+    cudaGraph_t g = nullptr;
+    bool capturing = false, ok = false;
+    do {
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        capturing = true;
+        cudaStreamCaptureStatus status;
+        const cudaGraphNode_t *deps = nullptr;
+        size_t ndeps = 0;
+        if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
+        cudaGraphConditionalHandle h;
+        if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
+        enqueue_force(s, 1, (unsigned long long)h);
+        if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
+        cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
+        cp.conditional.handle = h;
+        cp.conditional.type = cudaGraphCondTypeIf;
+        cp.conditional.size = 1;
+        cudaGraphNode_t cnode;
+        if (cudaGraphAddNode(&cnode, g, deps, ndeps, &cp) != cudaSuccess) break;
+        cudaGraph_t body = cp.conditional.phGraph_out[0];
+        if (cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        mdk_cells(s->P, s->lc, s->cap_stream);
+        mdk_reorder(s->P, s->lc, s->cap_stream);
+        if (s->P.tiled) mdk_tile_build(s->P, s->cap_stream); else mdk_build(s->P, s->lc, s->cap_stream);
+        cudaGraph_t body_out = nullptr;
+        if (cudaStreamEndCapture(s->cap_stream, &body_out) != cudaSuccess) break;
+        if (cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) break;
+        capturing = false;
+        if (cudaStreamEndCapture(st, &g) != cudaSuccess) { g = nullptr; break; }
+        s->graph = g;
+        if (cudaGraphInstantiate(&s->gexec, g, 0) != cudaSuccess) break;
+        ok = true;
+    } while (0);
+    if (!ok) {
+        if (capturing) { cudaGraph_t junk = nullptr; cudaStreamEndCapture(st, &junk); if (junk) cudaGraphDestroy(junk); }
+        cudaGetLastError();
+        if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+        if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+        return false;
+    }
+    s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1;
+    return true;
 }
 
 void enqueue_forces_only(md_system *s)
@@ -192,6 +267,7 @@ int install_state(md_system *s)
     if (rc) return rc;
     // the initial build is not counted as a rebuild
     s->h_ctrl->n_rebuilds = 0;
+    s->rebuilds_seen = 0;
     CK(cudaMemsetAsync(&s->P.ctrl->n_rebuilds, 0, sizeof(int), s->stream));
     return MD_OK;
 }
@@ -297,6 +373,8 @@ void md_destroy(md_system *s)
     if (s->stream) cudaStreamSynchronize(s->stream);
     for (EvPair &e : s->pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (EvPair &e : s->pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    drop_graph(s);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     dev_free_all(s);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_stage) cudaFreeHost(s->h_stage);
@@ -342,6 +420,7 @@ md_system *md_create_ex(const md_params *pp)
         const double ideal = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         p.max_neighbors = 16 * (int)ceil((1.35 * ideal + 12.0) / 16.0);
     }
+    p.max_neighbors = (p.max_neighbors + 1) & ~1;          // W rows are stored in pairs in the tiled layout
     if (p.lattice == MD_LATTICE_AUTO) {
         p.lattice = md_init_pick_lattice(p.n_atoms);
         if (!p.lattice) { set_error("n_atoms fits neither a simple-cubic nor an FCC lattice"); return nullptr; }
@@ -391,10 +470,11 @@ md_system *md_create_ex(const md_params *pp)
     s->lc.grid_atoms = (P.N + p.block_size - 1) / p.block_size;
 
     P.tiled = 0;
+    P.dbg = env_int("MD_DEBUG_EXP", 0);
     if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
         if (!choose_tile(P, prop.sharedMemPerBlockOptin)) { md_destroy(s); return nullptr; }
     }
-    P.max_grid = std::max((P.N + 255) / 256, P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
+    P.max_grid = std::max((P.N + 63) / 64, P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
 
     const size_t np = (size_t)P.N_pad;
     bool ok = true;
@@ -414,6 +494,7 @@ md_system *md_create_ex(const md_params *pp)
     P.block_sums = (int *)A(((size_t)P.scan_blocks + 1) * sizeof(int));
     P.W = (int *)A((size_t)(P.tiled ? P.Mmax / 2 : P.Mmax) * np * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
+    P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
     if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
@@ -482,6 +563,7 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
     }
     CK(cudaMemcpyAsync(P.bond_orig, tab.data(), 2 * n * sizeof(int), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream));
+    drop_graph(s);                 // the captured kernel arguments (MdDev by value) change
     P.has_bonds = n_bonds > 0;
     P.fene_k = k;
     P.fene_R02 = R0 * R0;
@@ -494,6 +576,7 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
     int rc = check_device_status(s);
     if (rc) return rc;
     CK(cudaMemsetAsync(&P.ctrl->n_rebuilds, 0, sizeof(int), s->stream));
+    s->rebuilds_seen = 0;
     return MD_OK;
 }
 
@@ -517,16 +600,24 @@ int md_step(md_system *s, int64_t n)
     cudaStream_t st = s->stream;
     if (s->prm.step_mode == MD_STEP_FUSED) {
         // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
-        { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+        { Timed t(s, MD_T_INTEGRATE, 2); mdk_kick_drift(P, s->lc, st); }
         enqueue_rebuild(s);
-        for (int64_t k = 1; k < n; k++) {
-            { Timed t(s, MD_T_FUSED_STEP, 1); enqueue_force(s, 1); }
-            enqueue_rebuild(s);
+        const bool want_graph = !s->profiling && !(s->prm.flags & MD_FLAG_NO_GRAPH) && n > 1;
+        if (want_graph && !s->gexec && !s->graph_tried) build_step_graph(s);
+        if (want_graph && s->gexec) {
+            for (int64_t k = 1; k < n; k++) CK(cudaGraphLaunch(s->gexec, st));
+            s->graph_steps += n - 1;
+            s->launches += 2 * (n - 1);                  // + the rebuild chains, added in check_device_status
+        } else {
+            for (int64_t k = 1; k < n; k++) {
+                { Timed t(s, MD_T_FUSED_STEP, 2); enqueue_force(s, 1); }
+                enqueue_rebuild(s);
+            }
         }
         { Timed t(s, MD_T_FORCE, 1); enqueue_force(s, 2); }
     } else {
         for (int64_t k = 0; k < n; k++) {
-            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+            { Timed t(s, MD_T_INTEGRATE, 2); mdk_kick_drift(P, s->lc, st); }
             enqueue_rebuild(s);
             enqueue_forces_only(s);
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick(P, s->lc, st); }
@@ -644,6 +735,7 @@ int md_get_info(md_system *s, md_info *out)
         out->tile_cells[0] = s->P.tg.S; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }
+    out->use_graph = s->gexec ? 1 : 0;
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

@@ -129,14 +129,15 @@ __device__ __forceinline__ double block_max(double v, double *sm)
     return v;
 }
 
-// The rebuild decision (R8), taken by ONE thread of the last block of the kernel
-// that drifted the positions.  It also fixes which buffers the rebuild kernels read and write, so the host
-// never needs to know whether a rebuild happened.
-__device__ void decide(const MdDev &P, bool pos_pingpong)
+// The rebuild decision (R8), taken on the device by k_decide from the per-block maxima of
+// v^2 that the drifting kernel left in blk_vmax2.  It also fixes which buffers the rebuild kernels read and
+// write, so the host never needs to know whether a rebuild happened.
+// (A "last block done" ticket inside the drifting kernel, was measured at ~7.5 ns per block on
+// B200 -- two same-address L2 atomics and a fence per block, ~75 us for the 10^4 blocks of N = 2M, more than
+// the rest of the kernel -- so the decision moved to a one-block kernel ordered by the stream.)
+__device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pingpong)
 {
     volatile DevCtrl *c = P.ctrl;
-    const double vmax2 = __longlong_as_double((long long)c->vmax2_bits);
-    c->vmax2_bits = 0ull;
     double acc = c->disp_acc + P.dt * sqrt(vmax2);
     const int need = acc > P.thresh;
     if (need) {
@@ -152,19 +153,6 @@ __device__ void decide(const MdDev &P, bool pos_pingpong)
     const int vs = c->v_dst;
     c->v_src = vs;
     c->v_dst = need ? (vs ^ 1) : vs;
-}
-
-// thread 0 of each block: publish the block's max v^2, then take a ticket; the last block decides.
-__device__ __forceinline__ void publish_vmax_and_decide(const MdDev &P, double bmax2, bool pos_pingpong)
-{
-    DevCtrl *c = P.ctrl;
-    atomicMax(&c->vmax2_bits, (unsigned long long)__double_as_longlong(bmax2));
-    __threadfence();
-    const unsigned t = atomicInc(&c->ticket[TK_INTEGRATE], gridDim.x - 1);
-    if (t == gridDim.x - 1) {
-        __threadfence();
-        decide(P, pos_pingpong);
-    }
 }
 
 __device__ __forceinline__ void set_err(const MdDev &P, int code) { atomicCAS(&P.ctrl->err, 0, code); }

@@ -31,7 +31,6 @@ __global__ void k_force_rebuild(const __grid_constant__ MdDev P)
     c->p_src = c->p_dst; c->p_dst ^= 1;
     c->v_src = c->v_dst; c->v_dst ^= 1;
     c->disp_acc = 0.0;
-    c->vmax2_bits = 0ull;
     c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
 }
 
@@ -90,7 +89,24 @@ __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDe
         if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
     }
     const double bm = block_max(v2, sm);
-    if (threadIdx.x == 0) publish_vmax_and_decide(P, bm, false);
+    if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+}
+
+// max over the per-block maxima of v^2, then the rebuild decision: one block, ordered after the drifting kernel
+// by the stream.  Inside md_step's CUDA graph it also sets the condition of the IF node that holds the rebuild chain.
+__global__ void __launch_bounds__(1024) k_decide(const __grid_constant__ MdDev P, int nblk, int pos_pingpong,
+                                                 cudaGraphConditionalHandle cond)
+{
+    __shared__ double sm[32];
+    double m = 0.0;
+    const double *__restrict__ v = P.blk_vmax2;
+#pragma unroll 8
+    for (int b = threadIdx.x; b < nblk; b += 1024) m = fmax(m, __ldcg(v + b));
+    m = block_max(m, sm);
+    if (threadIdx.x == 0) {
+        decide(P, m, pos_pingpong != 0);
+        if (cond) cudaGraphSetConditional(cond, (unsigned)P.ctrl->need_rebuild);
+    }
 }
 
 // second half kick
@@ -460,7 +476,7 @@ __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(c
     }
     if (MODE == 1) {
         const double bm = block_max(v2, sm);
-        if (threadIdx.x == 0) publish_vmax_and_decide(P, bm, true);
+        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 
@@ -576,7 +592,16 @@ void mdk_load_state(const MdDev &P, cudaStream_t st) { k_load_state<<<cdiv(P.N, 
 
 void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st) { k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset); }
 
-void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond)
+{
+    k_decide<<<1, 1024, 0, st>>>(P, nblk, pos_pingpong ? 1 : 0, (cudaGraphConditionalHandle)cond);
+}
+
+void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    k_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+    mdk_decide(P, cdiv(P.N, 256), false, st, 0ull);
+}
 
 void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
 
@@ -612,7 +637,7 @@ static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
     }
 }
 
-void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
+void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st, unsigned long long cond)
 {
     if (P.has_bonds) {
         if (mode == 0) launch_force_block<0, true>(P, lc.block, st);
@@ -623,6 +648,7 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
         else if (mode == 1) launch_force_block<1, false>(P, lc.block, st);
         else launch_force_block<2, false>(P, lc.block, st);
     }
+    if (mode == 1) mdk_decide(P, cdiv(P.N, lc.block), true, st, cond);
 }
 
 void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)

@@ -15,35 +15,27 @@
 // periodic-image flag bits of PAPER.md:163, packed two rows per 32-bit word.  The random accesses then hit
 // the shared-memory crossbar (128 B/cycle/SM, no tag look-ups) and W costs 2 bytes per neighbor.
 //
-// The tile layout is a pure function of (block index, cell_start); cell_start only changes at a rebuild,
-// so the build kernel and every later force / energy kernel reconstruct the same layout.
+// The tile layout is a pure function of (block index, cell_start); cell_start only changes at a rebuild, so the
+// build kernel computes it once per box, stores it as a TileDesc in global memory, and every later force /
+// energy kernel reads it back with one coalesced load.  Inside a block the global-memory latencies are
+// overlapped, not chained: descriptor -> {W words + velocities of the own atoms, position tile} -> compute.
 #include <algorithm>
 
 #include "md_device.cuh"
 
 namespace {
 
-struct TileMeta {
-    int n_own, T;                                       // atoms owned by the block, atoms in the tile
-    int own_base[TILE_OWN_MAX];                         // global index of the first own atom of own row k
-    int own_loc[TILE_OWN_MAX];                          // its index in the tile
-    int own_pre[TILE_OWN_MAX + 1];                      // exclusive prefix of the own-row lengths
-    int row_off[TILE_Q_MAX + 1];                        // tile index of the first atom of tile row q
-    int pg[TILE_Q_MAX][3], pn[TILE_Q_MAX][3];           // the (up to) 3 contiguous pieces of a tile row: start, length
-    int row_cell[TILE_Q_MAX];                           // linear index of the x = 0 cell of the (wrapped) row
-    int ysh[TILE_Q_MAX], zsh[TILE_Q_MAX];               // image shift of the row in units of L
+// what only the build kernel needs per tile row: the row's x = 0 cell and its image shift in units of L
+struct TileRowGeom {
+    int row_cell[TILE_Q_MAX], ysh[TILE_Q_MAX], zsh[TILE_Q_MAX];
 };
 
-// Build the tile of block blockIdx.x: fills M, copies positions into sx/sy/sz and (CELLS) the tile index of
-// the first atom of every tile cell into tcs[q * (S + 3) + k], k = 0 .. sxc + 2.  Returns false, with nothing
-// copied, when the tile would exceed the capacity.  All threads of the block must call it.
-template <bool CELLS>
-__device__ __forceinline__ bool tile_setup(const MdDev &P, const TileBox &B, const pos_t *__restrict__ pos, TileMeta &M,
-                                           double *sx, double *sy, double *sz, int *tcs)
+// Build kernel, step 1: the descriptor of box blockIdx.x from cell_start.  All threads of the block call it.
+__device__ __forceinline__ void tile_describe(const MdDev &P, const TileBox &B, TileDesc &M, TileRowGeom &X)
 {
     const int nc = P.nc;
     const int *__restrict__ cs = P.cell_start;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+    const int tid = threadIdx.x;
     if (tid < B.nq) {
         const int q = tid;
         int rowc, ysh, zsh, xa, xc;
@@ -51,58 +43,87 @@ __device__ __forceinline__ bool tile_setup(const MdDev &P, const TileBox &B, con
         const int gA = __ldg(cs + rowc + xa), nA = __ldg(cs + rowc + xa + 1) - gA;
         const int gB = __ldg(cs + rowc + B.x0), nB = __ldg(cs + rowc + B.x0 + B.sxc) - gB;
         const int gC = __ldg(cs + rowc + xc), nC = __ldg(cs + rowc + xc + 1) - gC;
-        M.pg[q][0] = gA; M.pg[q][1] = gB; M.pg[q][2] = gC;
-        M.pn[q][0] = nA; M.pn[q][1] = nB; M.pn[q][2] = nC;
-        M.row_cell[q] = rowc; M.ysh[q] = ysh; M.zsh[q] = zsh;
+        M.row[q].g[0] = gA; M.row[q].g[1] = gB; M.row[q].g[2] = gC;
+        M.row[q].n[0] = nA; M.row[q].n[1] = nB; M.row[q].n[2] = nC;
+        X.row_cell[q] = rowc; X.ysh[q] = ysh; X.zsh[q] = zsh;
+        // piece 0 is the far-face cell when the box starts at x = 0: d = (r_i - r_j) + L; piece 2 likewise with -L
+        const int xshA = B.x0 == 0 ? 1 : 0, xshC = B.x0 + B.sxc == nc ? -1 : 0;
+        M.row[q].sh = (ysh + 1) | ((zsh + 1) << 2) | ((xshA + 1) << 4) | ((xshC + 1) << 6);
     }
     __syncthreads();
     if (tid == 0) {
         int off = 0, own = 0, k = 0;
         for (int q = 0; q < B.nq; q++) {
-            M.row_off[q] = off;
+            M.row[q].off = off;
             const int qy = q % B.nyq, qz = q / B.nyq;
             if (qy >= 1 && qy <= B.ny && qz >= 1 && qz <= B.nz) {      // a row of the box itself
-                M.own_base[k] = M.pg[q][1];
-                M.own_loc[k] = off + M.pn[q][0];
+                M.own_base[k] = M.row[q].g[1];
+                M.own_loc[k] = off + M.row[q].n[0];
                 M.own_pre[k] = own;
-                own += M.pn[q][1];
+                own += M.row[q].n[1];
                 k++;
             }
-            off += M.pn[q][0] + M.pn[q][1] + M.pn[q][2];
+            off += M.row[q].n[0] + M.row[q].n[1] + M.row[q].n[2];
         }
-        M.row_off[B.nq] = off;
-        for (; k <= TILE_OWN_MAX; k++) M.own_pre[k] = own;
-        M.n_own = own;
-        M.T = off;
+        for (; k <= TILE_OWN_MAX; k++) {
+            M.own_pre[k] = own;
+            if (k < TILE_OWN_MAX) { M.own_base[k] = 0; M.own_loc[k] = 0; }
+        }
+        M.n_own = own; M.T = off; M.nq = B.nq; M.pad = 0;
     }
     __syncthreads();
-    if (M.T > P.tg.cap) return false;
-    for (int q = wid; q < B.nq; q += nw) {
-        const int off = M.row_off[q], nA = M.pn[q][0], nB = M.pn[q][1], nC = M.pn[q][2];
-        const int gA = M.pg[q][0], gB = M.pg[q][1], gC = M.pg[q][2];
-        const int tot = nA + nB + nC;
-        for (int u = lane; u < tot; u += 32) {
-            const int src = u < nA ? gA + u : (u < nA + nB ? gB + (u - nA) : gC + (u - nA - nB));
-            const pos_t p = ld_pos(pos + src);
-            sx[off + u] = p.x; sy[off + u] = p.y; sz[off + u] = p.z;
-        }
-        if (CELLS) {
-            const int rowc = M.row_cell[q];
-            for (int k = lane; k <= B.sxc + 2; k += 32) {
-                int v;
-                if (k == 0) v = off;
-                else if (k == B.sxc + 2) v = off + tot;
-                else v = off + nA + (__ldg(cs + rowc + B.x0 + k - 1) - gB);
-                tcs[q * (P.tg.S + 3) + k] = v;
+}
+
+// Copy the positions of the tile into shared memory as packed (x, y, z) triples: st[3 j + k].  One warp per
+// tile row, two rows and two 32-atom chunks of each in flight per lane (4 independent 256-bit loads) before
+// the first shared-memory store.
+// IMAGE: store the periodic IMAGE the box sees, r_j - shift (shift = 0 or +-L per axis, fixed per tile row and
+// piece), so that the pair loop needs no flag handling.  r - L is exact (Sterbenz) and r + L is rounded once at
+// magnitude L, the same size of error as the oracle's (r_i - r_j) at the far face: ~1e-16 relative to L, far
+// inside the 1e-10 force tolerance.  The build kernel stages raw positions (IMAGE = false) and applies the
+// shift to the difference, because its accept test must reproduce DESIGN.md R5 bit for bit.
+template <bool IMAGE>
+__device__ __forceinline__ void tile_stage(const TileDesc &M, const pos_t *__restrict__ pos, double *st, double L)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int nq = M.nq;
+    for (int qa = wid; qa < nq; qa += 2 * nw) {
+        const int qb = qa + nw < nq ? qa + nw : qa;
+        const TileDesc::Row &A = M.row[qa], &Bq = M.row[qb];
+        const int ta = A.n[0] + A.n[1] + A.n[2], tb = qb != qa ? Bq.n[0] + Bq.n[1] + Bq.n[2] : 0;
+        const int tmax = ta > tb ? ta : tb;
+        for (int u = lane; u < tmax; u += 64) {
+            pos_t p[4];
+            int dst[4];
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const TileDesc::Row &R = k < 2 ? A : Bq;
+                const int tot = k < 2 ? ta : tb, uu = u + (k & 1) * 32;
+                dst[k] = -1;
+                if (uu < tot) {
+                    const int piece = uu < R.n[0] ? 0 : (uu < R.n[0] + R.n[1] ? 1 : 2);
+                    const int src = piece == 0 ? R.g[0] + uu : (piece == 1 ? R.g[1] + (uu - R.n[0]) : R.g[2] + (uu - R.n[0] - R.n[1]));
+                    p[k] = ld_pos(pos + src);
+                    if (IMAGE) {
+                        const int sh = R.sh;
+                        const int xs = piece == 0 ? ((sh >> 4) & 3) - 1 : (piece == 2 ? ((sh >> 6) & 3) - 1 : 0);
+                        const int ys = (sh & 3) - 1, zs = ((sh >> 2) & 3) - 1;
+                        if (xs) p[k].x -= xs * L;
+                        if (ys) p[k].y -= ys * L;
+                        if (zs) p[k].z -= zs * L;
+                    }
+                    dst[k] = 3 * (R.off + uu);
+                }
             }
+#pragma unroll
+            for (int k = 0; k < 4; k++)
+                if (dst[k] >= 0) { st[dst[k]] = p[k].x; st[dst[k] + 1] = p[k].y; st[dst[k] + 2] = p[k].z; }
         }
     }
-    __syncthreads();
-    return true;
 }
 
 // own atom number t of the block -> global index i and tile index li
-__device__ __forceinline__ void own_atom(const TileMeta &M, int t, int &i, int &li)
+__device__ __forceinline__ void own_atom(const TileDesc &M, int t, int &i, int &li)
 {
     int k = 0;
 #pragma unroll
@@ -138,11 +159,11 @@ struct Emit {
 };
 
 template <bool SHIFT>
-__device__ __forceinline__ void tile_scan_run(const double *sx, const double *sy, const double *sz, double xi, double yi, double zi,
+__device__ __forceinline__ void tile_scan_run(const double *st, double xi, double yi, double zi,
                                               int li, int b, int e, double shx, double shy, double shz, unsigned fl, double rn2, Emit &em)
 {
     for (int j = b; j < e; j++) {
-        double dx = __dsub_rn(xi, sx[j]), dy = __dsub_rn(yi, sy[j]), dz = __dsub_rn(zi, sz[j]);
+        double dx = __dsub_rn(xi, st[3 * j]), dy = __dsub_rn(yi, st[3 * j + 1]), dz = __dsub_rn(zi, st[3 * j + 2]);
         if (SHIFT) { dx = __dadd_rn(dx, shx); dy = __dadd_rn(dy, shy); dz = __dadd_rn(dz, shz); }
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
         if (r2 < rn2 && j != li) em.put((unsigned)j | (fl << T_FLAG_SHIFT));
@@ -154,51 +175,71 @@ __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ Md
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     extern __shared__ double dsm[];
-    __shared__ TileMeta M;
+    __shared__ TileDesc M;
+    __shared__ TileRowGeom X;
     __shared__ int smx[32], ssum[32];
     const int cap = P.tg.cap;
-    double *sx = dsm, *sy = sx + cap, *sz = sy + cap;
-    int *tcs = (int *)(sz + cap);
+    double *st = dsm;
+    int *tcs = (int *)(st + 3 * cap);
     const int stride = P.tg.S + 3;
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    const int *__restrict__ cs = P.cell_start;
     const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
-    const bool ok = tile_setup<true>(P, B, pos, M, sx, sy, sz, tcs);
-    if (!ok) {
+    tile_describe(P, B, M, X);
+    {   // publish the descriptor for the force / energy kernels
+        int *d = P.tile_desc + (size_t)blockIdx.x * TILE_DESC_INTS;
+        const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
+        for (int k = threadIdx.x; k < n; k += BLOCK) d[k] = ((const int *)&M)[k];
+    }
+    if (M.T > cap) {
         if (threadIdx.x == 0) set_err(P, MD_ERR_TILE_OVERFLOW);
         return;
     }
+    tile_stage<false>(M, pos, st, P.L);
+    // tile index of the first atom of every tile cell: tcs[q * stride + k], k = 0 .. sxc + 2
+    for (int e = threadIdx.x; e < B.nq * stride; e += BLOCK) {
+        const int q = e / stride, k = e - q * stride;
+        if (k > B.sxc + 2) continue;
+        const TileDesc::Row &R = M.row[q];
+        int v;
+        if (k == 0) v = R.off;
+        else if (k == B.sxc + 2) v = R.off + R.n[0] + R.n[1] + R.n[2];
+        else v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - 1) - R.g[1]);
+        tcs[e] = v;
+    }
+    __syncthreads();
     const int nc = P.nc;
     const double L = P.L, rn2 = P.rn2;
     int tmax = 0, tsum = 0;
     for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
         int i, li;
         own_atom(M, t, i, li);
-        const double xi = sx[li], yi = sy[li], zi = sz[li];
+        const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
         const int cx = cell_coord(xi, P.inv_w, nc), cy = cell_coord(yi, P.inv_w, nc), cz = cell_coord(zi, P.inv_w, nc);
         Emit em = {(unsigned *)P.W + i, (size_t)P.N_pad, 0, P.Mmax, 0u};
         const int k0 = cx - B.x0;
         for (int dz = -1; dz <= 1; dz++) {
             for (int dy = -1; dy <= 1; dy++) {
                 const int q = (cy + dy - (B.y0 - 1)) + B.nyq * (cz + dz - (B.z0 - 1));
-                const int ysh = M.ysh[q], zsh = M.zsh[q];
+                const int ysh = X.ysh[q], zsh = X.zsh[q];
                 const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
                 const double shy = ysh * L, shz = zsh * L;
                 const int *tc = tcs + q * stride + k0;
                 const int b = tc[0], e = tc[3];
                 if (cx == 0) {
                     const int mid = tc[1];
-                    tile_scan_run<true>(sx, sy, sz, xi, yi, zi, li, b, mid, L, shy, shz, fl | 1u, rn2, em);
-                    if (fl) tile_scan_run<true>(sx, sy, sz, xi, yi, zi, li, mid, e, 0.0, shy, shz, fl, rn2, em);
-                    else tile_scan_run<false>(sx, sy, sz, xi, yi, zi, li, mid, e, 0.0, 0.0, 0.0, 0u, rn2, em);
+                    tile_scan_run<true>(st, xi, yi, zi, li, b, mid, L, shy, shz, fl | 1u, rn2, em);
+                    if (fl) tile_scan_run<true>(st, xi, yi, zi, li, mid, e, 0.0, shy, shz, fl, rn2, em);
+                    else tile_scan_run<false>(st, xi, yi, zi, li, mid, e, 0.0, 0.0, 0.0, 0u, rn2, em);
                 } else if (cx == nc - 1) {
                     const int mid = tc[2];
-                    if (fl) tile_scan_run<true>(sx, sy, sz, xi, yi, zi, li, b, mid, 0.0, shy, shz, fl, rn2, em);
-                    else tile_scan_run<false>(sx, sy, sz, xi, yi, zi, li, b, mid, 0.0, 0.0, 0.0, 0u, rn2, em);
-                    tile_scan_run<true>(sx, sy, sz, xi, yi, zi, li, mid, e, -L, shy, shz, fl | 1u, rn2, em);
+                    if (fl) tile_scan_run<true>(st, xi, yi, zi, li, b, mid, 0.0, shy, shz, fl, rn2, em);
+                    else tile_scan_run<false>(st, xi, yi, zi, li, b, mid, 0.0, 0.0, 0.0, 0u, rn2, em);
+                    tile_scan_run<true>(st, xi, yi, zi, li, mid, e, -L, shy, shz, fl | 1u, rn2, em);
                 } else if (fl) {
-                    tile_scan_run<true>(sx, sy, sz, xi, yi, zi, li, b, e, 0.0, shy, shz, fl, rn2, em);
+                    tile_scan_run<true>(st, xi, yi, zi, li, b, e, 0.0, shy, shz, fl, rn2, em);
                 } else {
-                    tile_scan_run<false>(sx, sy, sz, xi, yi, zi, li, b, e, 0.0, 0.0, 0.0, 0u, rn2, em);
+                    tile_scan_run<false>(st, xi, yi, zi, li, b, e, 0.0, 0.0, 0.0, 0u, rn2, em);
                 }
             }
         }
@@ -230,49 +271,90 @@ struct PairAccT {
     double fx, fy, fz, u, vir;
 };
 
+// One 32-bit word of W = two neighbors, evaluated together and branch-free so that their two dependent
+// fp64 chains interleave.  The tile holds image positions (tile_stage<true>), so the flag bits are not needed.
+// valid0 / valid1: the entry exists (n < m_i); an absent entry is index 0 of the tile, a harmless read.
 template <bool ENERGY>
-__device__ __forceinline__ void tile_pair(const MdDev &P, const double *sx, const double *sy, const double *sz, double xi, double yi,
-                                          double zi, unsigned e, PairAccT &a)
+__device__ __forceinline__ void tile_pair2(const MdDev &P, const double *st, double xi, double yi, double zi, unsigned w,
+                                           bool valid0, bool valid1, PairAccT &a)
 {
-    const unsigned l = e & T_INDEX_MASK, fl = e >> T_FLAG_SHIFT;
-    double dx = xi - sx[l], dy = yi - sy[l], dz = zi - sz[l];
-    if (fl) {                                   // only atoms next to a periodic face take this branch
-        if (fl & 1u) dx -= copysign(P.L, dx);
-        if (fl & 2u) dy -= copysign(P.L, dy);
-        if (fl & 4u) dz -= copysign(P.L, dz);
-    }
-    const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-    if (r2 < P.rc2) {
-        if (ENERGY) {
-            const double s = 1.0 / r2, s3 = s * s * s;
-            a.u += 4.0 * s3 * (s3 - 1.0) - P.uc;
-            a.vir += 48.0 * s3 * (s3 - 0.5);          // fc * r^2
-        } else {
-            const double s = fast_rcp(r2), s3 = s * s * s;
-            const double fc = s3 * (s3 - 0.5) * s;    // x 48 applied once to the sums
-            a.fx += fc * dx; a.fy += fc * dy; a.fz += fc * dz;
-        }
+    const double *p0 = st + 3 * (w & T_INDEX_MASK), *p1 = st + 3 * ((w >> 16) & T_INDEX_MASK);
+    const double dx0 = xi - p0[0], dy0 = yi - p0[1], dz0 = zi - p0[2];
+    const double dx1 = xi - p1[0], dy1 = yi - p1[1], dz1 = zi - p1[2];
+    const double q0 = __fma_rn(dz0, dz0, __fma_rn(dy0, dy0, __dmul_rn(dx0, dx0)));
+    const double q1 = __fma_rn(dz1, dz1, __fma_rn(dy1, dy1, __dmul_rn(dx1, dx1)));
+    const bool in0 = valid0 && q0 < P.rc2, in1 = valid1 && q1 < P.rc2;
+    if (!(in0 || in1)) return;
+    if (ENERGY) {
+        const double s0 = 1.0 / (in0 ? q0 : 1.0), s1 = 1.0 / (in1 ? q1 : 1.0);
+        const double c0 = s0 * s0 * s0, c1 = s1 * s1 * s1;
+        a.u += in0 ? 4.0 * c0 * (c0 - 1.0) - P.uc : 0.0;
+        a.u += in1 ? 4.0 * c1 * (c1 - 1.0) - P.uc : 0.0;
+        a.vir += in0 ? 48.0 * c0 * (c0 - 0.5) : 0.0;          // fc * r^2
+        a.vir += in1 ? 48.0 * c1 * (c1 - 0.5) : 0.0;
+    } else {
+        const double s0 = fast_rcp(in0 ? q0 : 1.0), s1 = fast_rcp(in1 ? q1 : 1.0);
+        const double c0 = s0 * s0 * s0, c1 = s1 * s1 * s1;
+        const double f0 = in0 ? c0 * (c0 - 0.5) * s0 : 0.0, f1 = in1 ? c1 * (c1 - 0.5) * s1 : 0.0;   // x 48 applied to the sums
+        a.fx += f0 * dx0; a.fy += f0 * dy0; a.fz += f0 * dz0;
+        a.fx += f1 * dx1; a.fy += f1 * dy1; a.fz += f1 * dz1;
     }
 }
 
-template <bool ENERGY>
-__device__ __forceinline__ PairAccT tile_column(const MdDev &P, const double *sx, const double *sy, const double *sz, double xi,
-                                                double yi, double zi, int i)
+// The first WPRE words (2 WPRE neighbors) of column i and its length, loaded BEFORE the position tile is staged
+// so that their HBM latency overlaps the staging.
+constexpr int WPRE = 4;
+struct ColPre {
+    int m;
+    unsigned w[WPRE];
+};
+
+__device__ __forceinline__ ColPre tile_column_preload(const MdDev &P, int i)
 {
-    const int m = P.nnb[i];
+    ColPre c;
+    const unsigned *__restrict__ w = (const unsigned *)P.W + i;
+    const int rows = P.Mmax >> 1;
+    c.m = P.nnb[i];
+#pragma unroll
+    for (int k = 0; k < WPRE; k++) c.w[k] = k < rows ? __ldcs(w + (size_t)k * P.N_pad) : 0u;
+    return c;
+}
+
+template <bool ENERGY>
+__device__ __forceinline__ PairAccT tile_column(const MdDev &P, const double *st, double xi, double yi, double zi, int i,
+                                                const ColPre &pre)
+{
+    const int m = pre.m;
     const unsigned *__restrict__ w = (const unsigned *)P.W + i;
     const size_t pitch = (size_t)P.N_pad;
     const int nw = (m + 1) >> 1;
     PairAccT a = {0.0, 0.0, 0.0, 0.0, 0.0};
-    unsigned cur = nw > 0 ? __ldcs(w) : 0u, nxt = nw > 1 ? __ldcs(w + pitch) : 0u;
-    for (int k = 0; k < nw; k++) {
-        const unsigned nn = k + 2 < nw ? __ldcs(w + (size_t)(k + 2) * pitch) : 0u;
-        tile_pair<ENERGY>(P, sx, sy, sz, xi, yi, zi, cur & 0xffffu, a);
-        if (2 * k + 1 < m) tile_pair<ENERGY>(P, sx, sy, sz, xi, yi, zi, cur >> 16, a);
-        cur = nxt; nxt = nn;
+    unsigned cur[WPRE];
+#pragma unroll
+    for (int k = 0; k < WPRE; k++) cur[k] = pre.w[k];
+    for (int base = 0; base < nw; base += WPRE) {
+        unsigned nxt[WPRE];
+#pragma unroll
+        for (int k = 0; k < WPRE; k++) nxt[k] = base + WPRE + k < nw ? __ldcs(w + (size_t)(base + WPRE + k) * pitch) : 0u;
+#pragma unroll
+        for (int k = 0; k < WPRE; k++) {
+            const int n0 = 2 * (base + k);
+            if (n0 < m) tile_pair2<ENERGY>(P, st, xi, yi, zi, cur[k], true, n0 + 1 < m, a);
+        }
+#pragma unroll
+        for (int k = 0; k < WPRE; k++) cur[k] = nxt[k];
     }
     if (!ENERGY) { a.fx *= 48.0; a.fy *= 48.0; a.fz *= 48.0; }
     return a;
+}
+
+// one coalesced load of the box descriptor written by the build kernel
+__device__ __forceinline__ void tile_load_desc(const MdDev &P, const TileBox &B, TileDesc &M)
+{
+    const int *__restrict__ d = P.tile_desc + (size_t)blockIdx.x * TILE_DESC_INTS;
+    const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) ((int *)&M)[k] = __ldg(d + k);
+    __syncthreads();
 }
 
 // FENE bonds: partners by global index, read from the position array (2 per atom at most)
@@ -305,46 +387,60 @@ template <int MODE, bool BONDS, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, 1024 / BLOCK) k_tile_force(const __grid_constant__ MdDev P)
 {
     extern __shared__ double dsm[];
-    __shared__ TileMeta M;
+    __shared__ TileDesc M;
     __shared__ double red[32];
     const int cap = P.tg.cap;
-    double *sx = dsm, *sy = sx + cap, *sz = sy + cap;
+    double *st = dsm;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pos = P.pos[pc];
+    double *__restrict__ vel = P.vel[vc];
+    const size_t np = (size_t)P.N_pad;
     const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
-    const bool ok = tile_setup<false>(P, B, pos, M, sx, sy, sz, nullptr);
-    double v2 = 0.0;
-    if (ok) {
-        for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
-            int i, li;
+    tile_load_desc(P, B, M);
+    const int n_own = M.T <= cap ? M.n_own : 0;          // an overflowing tile was reported by the build kernel
+    int t = threadIdx.x, i = 0, li = 0;
+    ColPre pre;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+    if (t < n_own) {
+        own_atom(M, t, i, li);
+        pre = tile_column_preload(P, i);
+        if (MODE != 0) { v0 = vel[i]; v1 = vel[np + i]; v2 = vel[2 * np + i]; }
+    }
+    if (n_own > 0 && !(P.dbg & 2)) tile_stage<true>(M, pos, st, P.L);
+    __syncthreads();
+    double vm2 = 0.0;
+    for (; t < n_own; t += BLOCK) {
+        if (t != (int)threadIdx.x) {                      // boxes with more atoms than threads: rare
             own_atom(M, t, i, li);
-            const double xi = sx[li], yi = sy[li], zi = sz[li];
-            PairAccT a = tile_column<false>(P, sx, sy, sz, xi, yi, zi, i);
-            double ub = 0.0;
-            if (BONDS) tile_bonds<false>(P, pos, xi, yi, zi, i, a, ub);
-            if (MODE == 0 || MODE == 2) {
-                double *f = P.frc + i;
-                f[0] = a.fx; f[P.N_pad] = a.fy; f[2 * (size_t)P.N_pad] = a.fz;
-            }
-            if (MODE == 2) {
-                double *v = P.vel[vc] + i;
-                v[0] += P.hdt * a.fx; v[P.N_pad] += P.hdt * a.fy; v[2 * (size_t)P.N_pad] += P.hdt * a.fz;
-            }
-            if (MODE == 1) {
-                double *v = P.vel[vc] + i;
-                const double vx = v[0] + P.dt * a.fx, vy = v[P.N_pad] + P.dt * a.fy, vz = v[2 * (size_t)P.N_pad] + P.dt * a.fz;
-                v[0] = vx; v[P.N_pad] = vy; v[2 * (size_t)P.N_pad] = vz;
-                const double x = xi + P.dt * vx, y = yi + P.dt * vy, z = zi + P.dt * vz;
-                st_pos(P.pos[pc ^ 1] + i, x, y, z);
-                double w2 = vx * vx + vy * vy + vz * vz;
-                if (!isfinite(w2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); w2 = 0.0; }
-                v2 = fmax(v2, w2);
-            }
+            pre = tile_column_preload(P, i);
+            if (MODE != 0) { v0 = vel[i]; v1 = vel[np + i]; v2 = vel[2 * np + i]; }
+        }
+        double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
+        if (P.dbg & 2) { const pos_t r = ld_pos(pos + i); xi = r.x; yi = r.y; zi = r.z; }
+        PairAccT a = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (!(P.dbg & 1)) a = tile_column<false>(P, st, xi, yi, zi, i, pre);
+        double ub = 0.0;
+        if (BONDS) tile_bonds<false>(P, pos, xi, yi, zi, i, a, ub);
+        if (MODE == 0 || MODE == 2) {
+            double *f = P.frc + i;
+            f[0] = a.fx; f[np] = a.fy; f[2 * np] = a.fz;
+        }
+        if (MODE == 2) {
+            vel[i] = v0 + P.hdt * a.fx; vel[np + i] = v1 + P.hdt * a.fy; vel[2 * np + i] = v2 + P.hdt * a.fz;
+        }
+        if (MODE == 1) {
+            const double vx = v0 + P.dt * a.fx, vy = v1 + P.dt * a.fy, vz = v2 + P.dt * a.fz;
+            vel[i] = vx; vel[np + i] = vy; vel[2 * np + i] = vz;
+            const double x = xi + P.dt * vx, y = yi + P.dt * vy, z = zi + P.dt * vz;
+            st_pos(P.pos[pc ^ 1] + i, x, y, z);
+            double w2 = vx * vx + vy * vy + vz * vz;
+            if (!isfinite(w2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); w2 = 0.0; }
+            vm2 = fmax(vm2, w2);
         }
     }
     if (MODE == 1) {
-        const double bm = block_max(v2, red);
-        if (threadIdx.x == 0) publish_vmax_and_decide(P, bm, true);
+        const double bm = block_max(vm2, red);
+        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 
@@ -352,34 +448,36 @@ template <bool BONDS, int BLOCK>
 __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ MdDev P)
 {
     extern __shared__ double dsm[];
-    __shared__ TileMeta M;
+    __shared__ TileDesc M;
     __shared__ RedSmem S;
     const int cap = P.tg.cap;
-    double *sx = dsm, *sy = sx + cap, *sz = sy + cap;
+    double *st = dsm;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pos = P.pos[pc];
     const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
-    const bool ok = tile_setup<false>(P, B, pos, M, sx, sy, sz, nullptr);
+    tile_load_desc(P, B, M);
+    const int n_own = M.T <= cap ? M.n_own : 0;
+    if (n_own > 0) tile_stage<true>(M, pos, st, P.L);
+    __syncthreads();
     double q[RED_N];
 #pragma unroll
     for (int k = 0; k < RED_N; k++) q[k] = 0.0;
-    if (ok) {
-        for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
-            int i, li;
-            own_atom(M, t, i, li);
-            const double xi = sx[li], yi = sy[li], zi = sz[li];
-            PairAccT a = tile_column<true>(P, sx, sy, sz, xi, yi, zi, i);
-            a.u *= 0.5; a.vir *= 0.5;               // full list: u_i counts every pair twice
-            double ub = 0.0;
-            if (BONDS) tile_bonds<true>(P, pos, xi, yi, zi, i, a, ub);
-            const double *v = P.vel[vc] + i;
-            const double vx = v[0], vy = v[P.N_pad], vz = v[2 * (size_t)P.N_pad];
-            const double w2 = vx * vx + vy * vy + vz * vz;
-            q[RED_PE] += a.u; q[RED_PEB] += ub; q[RED_VIR] += a.vir;
-            q[RED_KE] += 0.5 * w2;
-            q[RED_PX] += vx; q[RED_PY] += vy; q[RED_PZ] += vz;
-            q[RED_VMAX2] = fmax(q[RED_VMAX2], w2);
-        }
+    for (int t = threadIdx.x; t < n_own; t += BLOCK) {
+        int i, li;
+        own_atom(M, t, i, li);
+        const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
+        const ColPre pre = tile_column_preload(P, i);
+        PairAccT a = tile_column<true>(P, st, xi, yi, zi, i, pre);
+        a.u *= 0.5; a.vir *= 0.5;               // full list: u_i counts every pair twice
+        double ub = 0.0;
+        if (BONDS) tile_bonds<true>(P, pos, xi, yi, zi, i, a, ub);
+        const double *v = P.vel[vc] + i;
+        const double vx = v[0], vy = v[P.N_pad], vz = v[2 * (size_t)P.N_pad];
+        const double w2 = vx * vx + vy * vy + vz * vz;
+        q[RED_PE] += a.u; q[RED_PEB] += ub; q[RED_VIR] += a.vir;
+        q[RED_KE] += 0.5 * w2;
+        q[RED_PX] += vx; q[RED_PY] += vy; q[RED_PZ] += vz;
+        q[RED_VMAX2] = fmax(q[RED_VMAX2], w2);
     }
     reduce_finish(P, q, S);
 }
@@ -462,13 +560,14 @@ void mdk_tile_build(const MdDev &P, cudaStream_t st)
     }
 }
 
-void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st)
+void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long long cond)
 {
     switch (P.tg.threads) {
     case 128: launch_force<128>(P, mode, st); break;
     case 512: launch_force<512>(P, mode, st); break;
     default: launch_force<256>(P, mode, st); break;
     }
+    if (mode == 1) mdk_decide(P, tile_grid(P), true, st, cond);
 }
 
 void mdk_tile_energy(const MdDev &P, cudaStream_t st)

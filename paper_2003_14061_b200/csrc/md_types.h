@@ -28,7 +28,7 @@ struct DevCtrl {
     int max_occ;               // max k_c of the last binning
     int pad0;
     unsigned int ticket[6];    // "last block done" counters, one per kernel family
-    unsigned long long vmax2_bits;
+    unsigned long long reserved0;
     unsigned long long nnb_total;
     long long step;
     double disp_acc;           // accumulated dt * max|v| since the last rebuild
@@ -94,10 +94,13 @@ struct TileDesc {
     struct Row {
         int g[3], n[3];                                 // the (up to) 3 contiguous pieces of the row: start, length
         int off;                                        // tile index of the row's first atom
+        int sh;                                         // periodic-image shifts in units of L, 2 bits each, biased by 1:
+                                                        // bits 0-1 y, 2-3 z, 4-5 x of piece 0, 6-7 x of piece 2
     } row[TILE_Q_MAX];
 };
 constexpr int TILE_DESC_INTS = (int)(sizeof(TileDesc) / sizeof(int));
 constexpr int TILE_DESC_HEAD = 4 + 2 * TILE_OWN_MAX + TILE_OWN_MAX + 1;     // ints before row[]
+constexpr int TILE_ROW_INTS = 8;
 #define T_INDEX_MASK 0x1fffu
 #define T_FLAG_SHIFT 13
 
@@ -106,6 +109,7 @@ constexpr int TILE_DESC_HEAD = 4 + 2 * TILE_OWN_MAX + TILE_OWN_MAX + 1;     // i
 struct MdDev {
     int N, N_pad, Mmax, nc, NC;
     int has_bonds, half_list, scan_blocks;
+    int dbg;                            // MD_DEBUG_EXP bit mask: timing experiments only (results are wrong when set)
     int tiled, max_grid;                // W layout (1 = MD_W_TILED); row pitch of `partials`
     TileGeom tg;
     double L, half_L, inv_w;            // inv_w = nc / L
@@ -121,6 +125,7 @@ struct MdDev {
     int *W, *nnb;                       // neighbor matrix W[m * N_pad + i], counts m_i
                                         // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)
+    double *blk_vmax2;                  // max_grid per-block maxima of v^2 from the drifting kernel (input of k_decide)
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
@@ -134,13 +139,15 @@ struct MdLaunch {
 
 void mdk_force_rebuild(const MdDev &P, cudaStream_t st);
 void mdk_load_state(const MdDev &P, cudaStream_t st);                        // scratch(xyz | vxyz) -> pos/vel/id
-void mdk_kick_drift(const MdDev &P, const MdLaunch &lc, cudaStream_t st);     // v += dt/2 f; r += dt v; wrap; decide
+// rebuild decision from blk_vmax2[0..nblk); cond != 0: also set that CUDA-graph conditional handle to need_rebuild
+void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond);
+void mdk_kick_drift(const MdDev &P, const MdLaunch &lc, cudaStream_t st);     // v += dt/2 f; r += dt v; decide
 void mdk_kick(const MdDev &P, const MdLaunch &lc, cudaStream_t st);           // v += dt/2 f
 void mdk_cells(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // bin + scan + place       (N1-N4)
 void mdk_reorder(const MdDev &P, const MdLaunch &lc, cudaStream_t st);        // cell-order gather       (sec 2.4(4))
 void mdk_build(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // neighbor matrix         (N5)
 // mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, decide); 2: f and closing half kick
-void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
+void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st, unsigned long long cond = 0ull);
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    // 0 pos, 1 vel, 2 frc -> scratch + offset
@@ -148,7 +155,7 @@ void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    //
 int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
 size_t mdk_tile_smem(const TileGeom &G, bool with_cells);
 void mdk_tile_build(const MdDev &P, cudaStream_t st);
-void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st);
+void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long long cond = 0ull);
 void mdk_tile_energy(const MdDev &P, cudaStream_t st);
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,

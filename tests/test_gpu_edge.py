@@ -90,7 +90,7 @@ def test_info_and_timers(md):
     k0 = g.info()["kernel_launches"]
     g.step(50)
     t = g.timers()
-    assert t["fused_step"]["launches"] == 49 and t["fused_step"]["ms"] > 0
+    assert t["fused_step"]["launches"] == 2 * 49 and t["fused_step"]["ms"] > 0      # force kernel + k_decide
     assert t["nebr"]["launches"] == 50
     assert g.info()["kernel_launches"] - k0 == sum(x["launches"] for x in t.values())
 
@@ -104,3 +104,25 @@ def test_set_state_keeps_velocities_when_none(md):
     g.set_state(r)                                                     # velocities kept, order reset
     assert np.array_equal(g.velocities(), v)
     assert np.array_equal(g.positions(), r)
+
+
+def test_graph_and_direct_launch_agree_bitwise(md):
+    """md_step through the CUDA graph (conditional rebuild node) and with FLAG_NO_GRAPH run the same kernels in the
+    same order: states must be identical, rebuild counts too."""
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 4, jitter_amp=0.05)
+    out = []
+    for flags in (0, md.FLAG_NO_GRAPH, md.FLAG_GLOBAL_W, md.FLAG_GLOBAL_W | md.FLAG_NO_GRAPH):
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags)
+        g.set_state(r, v)
+        g.step(150)
+        g.step(1)
+        g.step(37)
+        e = g.energies()
+        assert g.info()["use_graph"] == (0 if flags & md.FLAG_NO_GRAPH else 1)
+        out.append((g.positions(), g.velocities(), e.n_rebuilds, g.info()["kernel_launches"]))
+        g.close()
+    for a, b in ((0, 1), (2, 3)):
+        assert np.array_equal(out[a][0], out[b][0]) and np.array_equal(out[a][1], out[b][1])
+        assert out[a][2] == out[b][2] > 10
+        assert out[a][3] < out[b][3]          # the graph skips the rebuild chain of steps that do not rebuild
