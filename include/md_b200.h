@@ -85,11 +85,12 @@ typedef struct md_params {
 } md_params;
 
 enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying a captured CUDA graph */
-       MD_FLAG_GLOBAL_W = 2u  /* W holds 29-bit global atom indices and partner positions are gathered through
-                                 L1/L2 (the paper's literal layout).  Default for variant A is the
-                                 tiled layout: every thread block stages the cell neighbourhood of its atoms in
-                                 shared memory and W holds 16-bit indices into that tile.
-                                 Variant B (Newton-3) always uses the global layout. */ };
+       MD_FLAG_GLOBAL_W = 2u, /* the paper's literal data path: W holds global atom indices and BOTH
+                                 the neighbor build and the force kernel gather partner positions through L1/L2.
+                                 Without this flag the build kernel stages the cell neighbourhood of each thread
+                                 block in shared memory; W is the same. */
+       MD_FLAG_TILED_W = 4u   /* W holds 16-bit indices into the per-block shared-memory tile, and the force / energy
+                                 kernels stage that tile too.  Variant A only. */ };
 enum { MD_W_GLOBAL = 0, MD_W_TILED = 1 };
 
 /* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */

@@ -176,7 +176,7 @@ void enqueue_rebuild(md_system *s)
 {
     { Timed t(s, MD_T_CELLS, mdk_launches_of(LK_CELLS)); mdk_cells(s->P, s->lc, s->stream); }
     { Timed t(s, MD_T_REORDER, s->P.has_bonds ? 2 : 1); mdk_reorder(s->P, s->lc, s->stream); }
-    { Timed t(s, MD_T_NEBR, 1); if (s->P.tiled) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_NEBR, 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
 void enqueue_force(md_system *s, int mode, unsigned long long cond = 0ull)
@@ -225,7 +225,7 @@ bool build_step_graph(md_system *s)
         if (cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
         mdk_cells(s->P, s->lc, s->cap_stream);
         mdk_reorder(s->P, s->lc, s->cap_stream);
-        if (s->P.tiled) mdk_tile_build(s->P, s->cap_stream); else mdk_build(s->P, s->lc, s->cap_stream);
+        if (s->P.tile_build) mdk_tile_build(s->P, s->cap_stream); else mdk_build(s->P, s->lc, s->cap_stream);
         cudaGraph_t body_out = nullptr;
         if (cudaStreamEndCapture(s->cap_stream, &body_out) != cudaSuccess) break;
         if (cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) break;
@@ -337,7 +337,6 @@ bool choose_tile(MdDev &P, size_t smem_optin)
     G.cap = cap;
     if (mean > 0.8 * cap) { set_error("tiled W: %.0f atoms per tile exceed the 13-bit tile index; use MD_FLAG_GLOBAL_W or smaller MD_TILE_S", mean); return false; }
     if (mdk_tile_smem(G, true) > smem_optin) { set_error("tiled W: tile of %d atoms does not fit shared memory", cap); return false; }
-    P.tiled = 1;
     if (mdk_tile_configure(P) != 0) { set_error("tiled W: cudaFuncSetAttribute failed: %s", cudaGetErrorString(cudaGetLastError())); return false; }
     return true;
 }
@@ -470,11 +469,20 @@ md_system *md_create_ex(const md_params *pp)
     s->lc.grid_atoms = (P.N + p.block_size - 1) / p.block_size;
 
     P.tiled = 0;
+    P.tile_build = 0;
     P.dbg = env_int("MD_DEBUG_EXP", 0);
     if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
-        if (!choose_tile(P, prop.sharedMemPerBlockOptin)) { md_destroy(s); return nullptr; }
+        // shared-memory staged neighbor build (both W layouts); the tiled W layout only on request
+        const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin);
+        if (!fits && (p.flags & MD_FLAG_TILED_W)) { md_destroy(s); return nullptr; }
+        P.tile_build = fits ? 1 : 0;
+        P.tiled = fits && (p.flags & MD_FLAG_TILED_W) ? 1 : 0;
+    } else if (p.flags & MD_FLAG_TILED_W) {
+        set_error("MD_FLAG_TILED_W needs the full-list force variant and excludes MD_FLAG_GLOBAL_W");
+        md_destroy(s);
+        return nullptr;
     }
-    P.max_grid = std::max((P.N + 63) / 64, P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
+    P.max_grid = std::max((P.N + 63) / 64, P.tile_build ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
 
     const size_t np = (size_t)P.N_pad;
     bool ok = true;
@@ -731,7 +739,7 @@ int md_get_info(md_system *s, md_info *out)
     out->force_variant = s->prm.force_variant; out->step_mode = s->prm.step_mode;
     out->n_bonds_per_atom_max = s->n_bonds_max;
     out->w_layout = s->P.tiled ? MD_W_TILED : MD_W_GLOBAL;
-    if (s->P.tiled) {
+    if (s->P.tile_build) {
         out->tile_cells[0] = s->P.tg.S; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }

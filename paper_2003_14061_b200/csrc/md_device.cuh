@@ -165,7 +165,7 @@ struct RedSmem {
     bool last;
 };
 
-__device__ __forceinline__ void reduce_finish(const MdDev &P, const double (&q)[RED_N], RedSmem &S)
+__device__ __forceinline__ void reduce_finish(const MdDev &P, const double (&q)[RED_N], RedSmem &S, int bid, int nblk)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
@@ -178,13 +178,13 @@ __device__ __forceinline__ void reduce_finish(const MdDev &P, const double (&q)[
         const int k = threadIdx.x;
         double r = S.v[k][0];
         for (int w = 1; w < nw; w++) r = k == RED_VMAX2 ? fmax(r, S.v[k][w]) : r + S.v[k][w];
-        P.partials[(size_t)k * P.max_grid + blockIdx.x] = r;
+        P.partials[(size_t)k * P.max_grid + bid] = r;
     }
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
-        const unsigned t = atomicInc(&P.ctrl->ticket[TK_ENERGY], gridDim.x - 1);
-        S.last = (t == gridDim.x - 1);
+        const unsigned t = atomicInc(&P.ctrl->ticket[TK_ENERGY], nblk - 1);
+        S.last = (t == (unsigned)(nblk - 1));
     }
     __syncthreads();
     if (!S.last) return;
@@ -193,7 +193,7 @@ __device__ __forceinline__ void reduce_finish(const MdDev &P, const double (&q)[
     for (int k = 0; k < RED_N; k++) {
         double r = 0.0;
         const volatile double *p = P.partials + (size_t)k * P.max_grid;
-        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) r = k == RED_VMAX2 ? fmax(r, p[b]) : r + p[b];
+        for (int b = threadIdx.x; b < nblk; b += blockDim.x) r = k == RED_VMAX2 ? fmax(r, p[b]) : r + p[b];
         r = k == RED_VMAX2 ? warp_max(r) : warp_sum(r);
         __syncthreads();
         if (lane == 0) S.v[0][wid] = r;

@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
         q[RED_PX] = vx; q[RED_PY] = vy; q[RED_PZ] = vz;
         q[RED_VMAX2] = v2;
     }
-    reduce_finish(P, q, S);
+    reduce_finish(P, q, S, blockIdx.x, gridDim.x);
 }
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }

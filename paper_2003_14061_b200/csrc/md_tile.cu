@@ -23,7 +23,13 @@
 
 #include "md_device.cuh"
 
+#ifndef MD_TILE_FORCE_THREADS
+#define MD_TILE_FORCE_THREADS 1024     // resident threads per SM the register allocation of k_tile_force must allow
+#endif
+
 namespace {
+
+__device__ __forceinline__ int tile_bid(const TileGeom &G) { return blockIdx.x + G.nsx * (blockIdx.y + G.nsy * blockIdx.z); }
 
 // what only the build kernel needs per tile row: the row's x = 0 cell and its image shift in units of L
 struct TileRowGeom {
@@ -74,6 +80,49 @@ __device__ __forceinline__ void tile_describe(const MdDev &P, const TileBox &B, 
     __syncthreads();
 }
 
+// one tile row's copy parameters in registers (the descriptor lives in shared memory, which the staging stores
+// alias, so the compiler would otherwise reload it inside the copy loop)
+struct RowCopy {
+    int tot, g0, n0, n01, b1, b2, off3;     // src = u + (u < n0 ? g0 : u < n01 ? b1 : b2);  dst = off3 + 3 u
+    bool contiguous, xwrap;
+    double shxA, shxC, shy, shz;            // image shifts (IMAGE only)
+};
+
+template <bool IMAGE>
+__device__ __forceinline__ RowCopy row_copy(const TileDesc::Row &R, double L)
+{
+    RowCopy c;
+    const int g0 = R.g[0], g1 = R.g[1], g2 = R.g[2], n0 = R.n[0], n1 = R.n[1], n2 = R.n[2], sh = R.sh;
+    c.tot = n0 + n1 + n2; c.g0 = g0; c.n0 = n0; c.n01 = n0 + n1;
+    c.b1 = g1 - n0; c.b2 = g2 - n0 - n1; c.off3 = 3 * R.off;
+    c.contiguous = g0 + n0 == g1 && g1 + n1 == g2;
+    c.xwrap = false; c.shxA = c.shxC = c.shy = c.shz = 0.0;
+    if (IMAGE) {
+        const int xa = ((sh >> 4) & 3) - 1, xc = ((sh >> 6) & 3) - 1;
+        c.xwrap = (xa | xc) != 0;
+        c.shxA = xa * L; c.shxC = xc * L; c.shy = ((sh & 3) - 1) * L; c.shz = (((sh >> 2) & 3) - 1) * L;
+    }
+    return c;
+}
+
+template <bool IMAGE>
+__device__ __forceinline__ pos_t row_load(const RowCopy &c, const pos_t *__restrict__ pos, int u)
+{
+    const int src = c.contiguous ? c.g0 + u : u + (u < c.n0 ? c.g0 : (u < c.n01 ? c.b1 : c.b2));
+    pos_t p = ld_pos(pos + src);
+    if (IMAGE) {
+        p.y -= c.shy; p.z -= c.shz;
+        if (c.xwrap) p.x -= u < c.n0 ? c.shxA : (u >= c.n01 ? c.shxC : 0.0);
+    }
+    return p;
+}
+
+__device__ __forceinline__ void row_store(const RowCopy &c, double *st, int u, const pos_t &p)
+{
+    double *d = st + c.off3 + 3 * u;
+    d[0] = p.x; d[1] = p.y; d[2] = p.z;
+}
+
 // Copy the positions of the tile into shared memory as packed (x, y, z) triples: st[3 j + k].  One warp per
 // tile row, two rows and two 32-atom chunks of each in flight per lane (4 independent 256-bit loads) before
 // the first shared-memory store.
@@ -88,36 +137,22 @@ __device__ __forceinline__ void tile_stage(const TileDesc &M, const pos_t *__res
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int nq = M.nq;
     for (int qa = wid; qa < nq; qa += 2 * nw) {
-        const int qb = qa + nw < nq ? qa + nw : qa;
-        const TileDesc::Row &A = M.row[qa], &Bq = M.row[qb];
-        const int ta = A.n[0] + A.n[1] + A.n[2], tb = qb != qa ? Bq.n[0] + Bq.n[1] + Bq.n[2] : 0;
-        const int tmax = ta > tb ? ta : tb;
+        const RowCopy A = row_copy<IMAGE>(M.row[qa], L);
+        RowCopy B = A;
+        B.tot = 0;
+        if (qa + nw < nq) B = row_copy<IMAGE>(M.row[qa + nw], L);
+        const int tmax = A.tot > B.tot ? A.tot : B.tot;
         for (int u = lane; u < tmax; u += 64) {
-            pos_t p[4];
-            int dst[4];
-#pragma unroll
-            for (int k = 0; k < 4; k++) {
-                const TileDesc::Row &R = k < 2 ? A : Bq;
-                const int tot = k < 2 ? ta : tb, uu = u + (k & 1) * 32;
-                dst[k] = -1;
-                if (uu < tot) {
-                    const int piece = uu < R.n[0] ? 0 : (uu < R.n[0] + R.n[1] ? 1 : 2);
-                    const int src = piece == 0 ? R.g[0] + uu : (piece == 1 ? R.g[1] + (uu - R.n[0]) : R.g[2] + (uu - R.n[0] - R.n[1]));
-                    p[k] = ld_pos(pos + src);
-                    if (IMAGE) {
-                        const int sh = R.sh;
-                        const int xs = piece == 0 ? ((sh >> 4) & 3) - 1 : (piece == 2 ? ((sh >> 6) & 3) - 1 : 0);
-                        const int ys = (sh & 3) - 1, zs = ((sh >> 2) & 3) - 1;
-                        if (xs) p[k].x -= xs * L;
-                        if (ys) p[k].y -= ys * L;
-                        if (zs) p[k].z -= zs * L;
-                    }
-                    dst[k] = 3 * (R.off + uu);
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < 4; k++)
-                if (dst[k] >= 0) { st[dst[k]] = p[k].x; st[dst[k] + 1] = p[k].y; st[dst[k] + 2] = p[k].z; }
+            pos_t a0, a1, b0, b1;
+            const bool va0 = u < A.tot, va1 = u + 32 < A.tot, vb0 = u < B.tot, vb1 = u + 32 < B.tot;
+            if (va0) a0 = row_load<IMAGE>(A, pos, u);
+            if (va1) a1 = row_load<IMAGE>(A, pos, u + 32);
+            if (vb0) b0 = row_load<IMAGE>(B, pos, u);
+            if (vb1) b1 = row_load<IMAGE>(B, pos, u + 32);
+            if (va0) row_store(A, st, u, a0);
+            if (va1) row_store(A, st, u + 32, a1);
+            if (vb0) row_store(B, st, u, b0);
+            if (vb1) row_store(B, st, u + 32, b1);
         }
     }
 }
@@ -137,40 +172,57 @@ __device__ __forceinline__ void own_atom(const TileDesc &M, int t, int &i, int &
 // ------------------------------------------------------------------------------------------------
 // N5 on the tile.  One thread per atom; the candidates of atom i in cell (cx, cy, cz) are, for
 // each of the 9 (dy, dz), the 3 consecutive tile cells cx-1 .. cx+1 of tile row (cy+dy, cz+dz): one contiguous
-// range of the shared arrays.  Lanes in the same cell read the same shared-memory words (broadcast).
+// range of the shared array.  Lanes in the same cell read the same shared-memory words (broadcast).
 // Accept test and image arithmetic are those of DESIGN.md R5, bit for bit: d = (r_i - r_j) rounded, + shift
 // rounded, r^2 = fma(dz,dz, fma(dy,dy, dx*dx)) < r_n^2.
+// LOCALW: W entries are 16-bit tile indices packed two per word (MD_W_TILED); otherwise 29-bit global atom
+// indices, one per word (MD_W_GLOBAL) -- the same kernel then feeds the gathering force kernels.
 // ------------------------------------------------------------------------------------------------
+// Appending to column i of W is written so that it compiles to predicated instructions, not a divergent
+// block: in a warp some lane accepts its candidate in most iterations, so a branch would be taken (by a few
+// lanes, the others idling) nearly every time.
+template <bool LOCALW>
 struct Emit {
-    unsigned *w;        // column i of W (32-bit words of two entries)
+    unsigned *wp;       // next free word of column i of W
     size_t pitch;
     int m, Mmax;
     unsigned pend;
-    __device__ __forceinline__ void put(unsigned e)
+    // candidate with tile index j; add = (flags << shift) + (global - tile index), constant over a run
+    __device__ __forceinline__ void put(bool acc, int j, unsigned add)
     {
-        if (m & 1) { if (m < Mmax) w[(size_t)(m >> 1) * pitch] = pend | (e << 16); }
-        else pend = e;
-        m++;
+        const unsigned e = (unsigned)j + add;
+        if (LOCALW) {
+            const bool odd = m & 1;
+            if (acc && odd && m < Mmax) *wp = pend | (e << 16);
+            wp += acc && odd ? pitch : 0;
+            pend = acc && !odd ? e : pend;
+        } else {
+            if (acc && m < Mmax) *wp = e;
+            wp += acc ? pitch : 0;
+        }
+        m += acc;
     }
     __device__ __forceinline__ void flush()
     {
-        if ((m & 1) && m < Mmax) w[(size_t)(m >> 1) * pitch] = pend;
+        if (LOCALW && (m & 1) && m < Mmax) *wp = pend;
     }
 };
 
-template <bool SHIFT>
-__device__ __forceinline__ void tile_scan_run(const double *st, double xi, double yi, double zi,
-                                              int li, int b, int e, double shx, double shy, double shz, unsigned fl, double rn2, Emit &em)
+template <bool SHIFT, bool LOCALW>
+__device__ __forceinline__ void tile_scan_run(const double *st, double xi, double yi, double zi, int li, int b, int e, double shx,
+                                              double shy, double shz, unsigned add, double rn2, Emit<LOCALW> &em)
 {
-    for (int j = b; j < e; j++) {
-        double dx = __dsub_rn(xi, st[3 * j]), dy = __dsub_rn(yi, st[3 * j + 1]), dz = __dsub_rn(zi, st[3 * j + 2]);
+    const double *p = st + 3 * b;
+#pragma unroll 2
+    for (int j = b; j < e; j++, p += 3) {
+        double dx = __dsub_rn(xi, p[0]), dy = __dsub_rn(yi, p[1]), dz = __dsub_rn(zi, p[2]);
         if (SHIFT) { dx = __dadd_rn(dx, shx); dy = __dadd_rn(dy, shy); dz = __dadd_rn(dz, shz); }
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-        if (r2 < rn2 && j != li) em.put((unsigned)j | (fl << T_FLAG_SHIFT));
+        em.put(r2 < rn2 && j != li, j, add);
     }
 }
 
-template <int BLOCK>
+template <int BLOCK, bool LOCALW>
 __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
@@ -184,10 +236,11 @@ __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ Md
     const int stride = P.tg.S + 3;
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
     const int *__restrict__ cs = P.cell_start;
-    const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
+    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const int bid = tile_bid(P.tg);
     tile_describe(P, B, M, X);
-    {   // publish the descriptor for the force / energy kernels
-        int *d = P.tile_desc + (size_t)blockIdx.x * TILE_DESC_INTS;
+    if (LOCALW) {   // publish the descriptor for the force / energy kernels
+        int *d = P.tile_desc + (size_t)bid * TILE_DESC_INTS;
         const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
         for (int k = threadIdx.x; k < n; k += BLOCK) d[k] = ((const int *)&M)[k];
     }
@@ -216,31 +269,34 @@ __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ Md
         own_atom(M, t, i, li);
         const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
         const int cx = cell_coord(xi, P.inv_w, nc), cy = cell_coord(yi, P.inv_w, nc), cz = cell_coord(zi, P.inv_w, nc);
-        Emit em = {(unsigned *)P.W + i, (size_t)P.N_pad, 0, P.Mmax, 0u};
+        Emit<LOCALW> em = {(unsigned *)P.W + i, (size_t)P.N_pad, 0, P.Mmax, 0u};
         const int k0 = cx - B.x0;
-        for (int dz = -1; dz <= 1; dz++) {
-            for (int dy = -1; dy <= 1; dy++) {
-                const int q = (cy + dy - (B.y0 - 1)) + B.nyq * (cz + dz - (B.z0 - 1));
-                const int ysh = X.ysh[q], zsh = X.zsh[q];
-                const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
-                const double shy = ysh * L, shz = zsh * L;
-                const int *tc = tcs + q * stride + k0;
-                const int b = tc[0], e = tc[3];
-                if (cx == 0) {
-                    const int mid = tc[1];
-                    tile_scan_run<true>(st, xi, yi, zi, li, b, mid, L, shy, shz, fl | 1u, rn2, em);
-                    if (fl) tile_scan_run<true>(st, xi, yi, zi, li, mid, e, 0.0, shy, shz, fl, rn2, em);
-                    else tile_scan_run<false>(st, xi, yi, zi, li, mid, e, 0.0, 0.0, 0.0, 0u, rn2, em);
-                } else if (cx == nc - 1) {
-                    const int mid = tc[2];
-                    if (fl) tile_scan_run<true>(st, xi, yi, zi, li, b, mid, 0.0, shy, shz, fl, rn2, em);
-                    else tile_scan_run<false>(st, xi, yi, zi, li, b, mid, 0.0, 0.0, 0.0, 0u, rn2, em);
-                    tile_scan_run<true>(st, xi, yi, zi, li, mid, e, -L, shy, shz, fl | 1u, rn2, em);
-                } else if (fl) {
-                    tile_scan_run<true>(st, xi, yi, zi, li, b, e, 0.0, shy, shz, fl, rn2, em);
-                } else {
-                    tile_scan_run<false>(st, xi, yi, zi, li, b, e, 0.0, 0.0, 0.0, 0u, rn2, em);
-                }
+        const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
+#pragma unroll 1
+        for (int r = 0; r < 9; r++) {
+            const int q = q0 + (r % 3) + B.nyq * (r / 3);
+            const int ysh = X.ysh[q], zsh = X.zsh[q];
+            const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
+            const double shy = ysh * L, shz = zsh * L;
+            const TileDesc::Row &R = M.row[q];
+            const int *tc = tcs + q * stride + k0;
+            const int b = tc[0], e = tc[3];
+            // split off the cell that is a periodic image along x (box at an x face, atom in the face cell)
+            int mid = cx == 0 ? tc[1] : (cx == nc - 1 ? tc[2] : e);
+            // global index = tile index + delta, constant over each contiguous piece of the row
+            const int e0 = R.off + R.n[0], e1 = e0 + R.n[1];
+            const int d0 = R.g[0] - R.off, d1 = R.g[1] - e0, d2 = R.g[2] - e1;
+            const int da = b < e0 ? d0 : (b < e1 ? d1 : d2), db = mid < e0 ? d0 : (mid < e1 ? d1 : d2);
+            const double shxa = cx == 0 ? L : 0.0, shxb = cx == nc - 1 ? -L : 0.0;
+            const unsigned fla = fl | (cx == 0 ? 1u : 0u), flb = fl | (cx == nc - 1 ? 1u : 0u);
+            // what is added to the tile index to make the W entry: the flag bits, and for global W the index offset
+            const unsigned adda = LOCALW ? fla << T_FLAG_SHIFT : (fla << W_FLAG_SHIFT) + (unsigned)da;
+            const unsigned addb = LOCALW ? flb << T_FLAG_SHIFT : (flb << W_FLAG_SHIFT) + (unsigned)db;
+            if (fla) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
+            else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, mid, 0.0, 0.0, 0.0, adda, rn2, em);
+            if (mid < e) {
+                if (flb) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
+                else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, mid, e, 0.0, 0.0, 0.0, addb, rn2, em);
             }
         }
         em.flush();
@@ -293,7 +349,7 @@ __device__ __forceinline__ void tile_pair2(const MdDev &P, const double *st, dou
         a.vir += in0 ? 48.0 * c0 * (c0 - 0.5) : 0.0;          // fc * r^2
         a.vir += in1 ? 48.0 * c1 * (c1 - 0.5) : 0.0;
     } else {
-        const double s0 = fast_rcp(in0 ? q0 : 1.0), s1 = fast_rcp(in1 ? q1 : 1.0);
+        const double s0 = fast_rcp(q0), s1 = fast_rcp(q1);     // q = 0 (an absent entry hitting the atom itself) gives inf / NaN, dropped by the select below
         const double c0 = s0 * s0 * s0, c1 = s1 * s1 * s1;
         const double f0 = in0 ? c0 * (c0 - 0.5) * s0 : 0.0, f1 = in1 ? c1 * (c1 - 0.5) * s1 : 0.0;   // x 48 applied to the sums
         a.fx += f0 * dx0; a.fy += f0 * dy0; a.fz += f0 * dz0;
@@ -349,9 +405,9 @@ __device__ __forceinline__ PairAccT tile_column(const MdDev &P, const double *st
 }
 
 // one coalesced load of the box descriptor written by the build kernel
-__device__ __forceinline__ void tile_load_desc(const MdDev &P, const TileBox &B, TileDesc &M)
+__device__ __forceinline__ void tile_load_desc(const MdDev &P, const TileBox &B, int bid, TileDesc &M)
 {
-    const int *__restrict__ d = P.tile_desc + (size_t)blockIdx.x * TILE_DESC_INTS;
+    const int *__restrict__ d = P.tile_desc + (size_t)bid * TILE_DESC_INTS;
     const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
     for (int k = threadIdx.x; k < n; k += blockDim.x) ((int *)&M)[k] = __ldg(d + k);
     __syncthreads();
@@ -384,7 +440,7 @@ __device__ __forceinline__ void tile_bonds(const MdDev &P, const pos_t *__restri
 // MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = r + dt v into the other position buffer,
 // max |v|, rebuild decision.  MODE 2: store f and apply the closing half kick v += dt/2 f.
 template <int MODE, bool BONDS, int BLOCK>
-__global__ void __launch_bounds__(BLOCK, 1024 / BLOCK) k_tile_force(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_force(const __grid_constant__ MdDev P)
 {
     extern __shared__ double dsm[];
     __shared__ TileDesc M;
@@ -395,8 +451,9 @@ __global__ void __launch_bounds__(BLOCK, 1024 / BLOCK) k_tile_force(const __grid
     const pos_t *__restrict__ pos = P.pos[pc];
     double *__restrict__ vel = P.vel[vc];
     const size_t np = (size_t)P.N_pad;
-    const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
-    tile_load_desc(P, B, M);
+    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const int bid = tile_bid(P.tg);
+    tile_load_desc(P, B, bid, M);
     const int n_own = M.T <= cap ? M.n_own : 0;          // an overflowing tile was reported by the build kernel
     int t = threadIdx.x, i = 0, li = 0;
     ColPre pre;
@@ -440,7 +497,7 @@ __global__ void __launch_bounds__(BLOCK, 1024 / BLOCK) k_tile_force(const __grid
     }
     if (MODE == 1) {
         const double bm = block_max(vm2, red);
-        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (threadIdx.x == 0) P.blk_vmax2[bid] = bm;
     }
 }
 
@@ -454,8 +511,9 @@ __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ M
     double *st = dsm;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pos = P.pos[pc];
-    const TileBox B = tile_box(P.tg, P.nc, blockIdx.x);
-    tile_load_desc(P, B, M);
+    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const int bid = tile_bid(P.tg);
+    tile_load_desc(P, B, bid, M);
     const int n_own = M.T <= cap ? M.n_own : 0;
     if (n_own > 0) tile_stage<true>(M, pos, st, P.L);
     __syncthreads();
@@ -479,7 +537,7 @@ __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ M
         q[RED_PX] += vx; q[RED_PY] += vy; q[RED_PZ] += vz;
         q[RED_VMAX2] = fmax(q[RED_VMAX2], w2);
     }
-    reduce_finish(P, q, S);
+    reduce_finish(P, q, S, bid, P.tg.nsx * P.tg.nsy * P.tg.nsz);
 }
 
 }  // namespace
@@ -497,6 +555,7 @@ size_t mdk_tile_smem(const TileGeom &G, bool with_cells)
 namespace {
 
 inline int tile_grid(const MdDev &P) { return P.tg.nsx * P.tg.nsy * P.tg.nsz; }
+inline dim3 tile_grid3(const MdDev &P) { return dim3(P.tg.nsx, P.tg.nsy, P.tg.nsz); }
 
 template <typename K>
 int opt_in(K kernel, size_t bytes)
@@ -509,7 +568,8 @@ int configure_block(const MdDev &P)
 {
     const size_t sf = mdk_tile_smem(P.tg, false), sb = mdk_tile_smem(P.tg, true);
     int rc = 0;
-    rc |= opt_in(k_tile_build<BLOCK>, sb);
+    rc |= opt_in(k_tile_build<BLOCK, true>, sb);
+    rc |= opt_in(k_tile_build<BLOCK, false>, sb);
     rc |= opt_in(k_tile_force<0, false, BLOCK>, sf);
     rc |= opt_in(k_tile_force<1, false, BLOCK>, sf);
     rc |= opt_in(k_tile_force<2, false, BLOCK>, sf);
@@ -524,7 +584,7 @@ int configure_block(const MdDev &P)
 template <int BLOCK>
 void launch_force(const MdDev &P, int mode, cudaStream_t st)
 {
-    const int g = tile_grid(P);
+    const dim3 g = tile_grid3(P);
     const size_t sm = mdk_tile_smem(P.tg, false);
     if (P.has_bonds) {
         if (mode == 0) k_tile_force<0, true, BLOCK><<<g, BLOCK, sm, st>>>(P);
@@ -551,13 +611,17 @@ int mdk_tile_configure(const MdDev &P)
 
 void mdk_tile_build(const MdDev &P, cudaStream_t st)
 {
-    const int g = tile_grid(P);
+    const dim3 g = tile_grid3(P);
     const size_t sm = mdk_tile_smem(P.tg, true);
+#define MD_TB(B)                                                            \
+    if (P.tiled) k_tile_build<B, true><<<g, B, sm, st>>>(P);               \
+    else k_tile_build<B, false><<<g, B, sm, st>>>(P)
     switch (P.tg.threads) {
-    case 128: k_tile_build<128><<<g, 128, sm, st>>>(P); break;
-    case 512: k_tile_build<512><<<g, 512, sm, st>>>(P); break;
-    default: k_tile_build<256><<<g, 256, sm, st>>>(P); break;
+    case 128: MD_TB(128); break;
+    case 512: MD_TB(512); break;
+    default: MD_TB(256); break;
     }
+#undef MD_TB
 }
 
 void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long long cond)
@@ -572,7 +636,7 @@ void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long lon
 
 void mdk_tile_energy(const MdDev &P, cudaStream_t st)
 {
-    const int g = tile_grid(P);
+    const dim3 g = tile_grid3(P);
     const size_t sm = mdk_tile_smem(P.tg, false);
 #define MD_TE(B)                                                            \
     if (P.has_bonds) k_tile_energy<true, B><<<g, B, sm, st>>>(P);          \

@@ -67,6 +67,17 @@ __host__ __device__ inline TileBox tile_box(const TileGeom &G, int nc, int b)
     return B;
 }
 
+__host__ __device__ inline TileBox tile_box3(const TileGeom &G, int nc, int bx, int by, int bz)
+{
+    TileBox B;
+    B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
+    B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
+    B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
+    B.nyq = B.ny + 2;
+    B.nq = B.nyq * (B.nz + 2);
+    return B;
+}
+
 // Tile row q of a box: the row of cells (y0-1 + q % nyq, z0-1 + q / nyq), wrapped periodically.
 // rowc = linear index of its x = 0 cell; ysh, zsh in {-1, 0, +1}: image shift of the row in units of L
 // (added to r_i - r_j); xa, xc = x index of the halo cells before / after the box (wrapped at the faces).
@@ -110,7 +121,7 @@ struct MdDev {
     int N, N_pad, Mmax, nc, NC;
     int has_bonds, half_list, scan_blocks;
     int dbg;                            // MD_DEBUG_EXP bit mask: timing experiments only (results are wrong when set)
-    int tiled, max_grid;                // W layout (1 = MD_W_TILED); row pitch of `partials`
+    int tiled, tile_build, max_grid;    // W layout (1 = MD_W_TILED); shared-memory staged build kernel in use; row pitch of `partials`
     TileGeom tg;
     double L, half_L, inv_w;            // inv_w = nc / L
     double rc2, rn2, uc;

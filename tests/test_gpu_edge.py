@@ -112,7 +112,7 @@ def test_graph_and_direct_launch_agree_bitwise(md):
     cfg = get_config("wca_4k")
     r, v, _, box = make_state(cfg, 4, jitter_amp=0.05)
     out = []
-    for flags in (0, md.FLAG_NO_GRAPH, md.FLAG_GLOBAL_W, md.FLAG_GLOBAL_W | md.FLAG_NO_GRAPH):
+    for flags in (0, md.FLAG_NO_GRAPH, md.FLAG_TILED_W, md.FLAG_TILED_W | md.FLAG_NO_GRAPH):
         g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags)
         g.set_state(r, v)
         g.step(150)

@@ -43,8 +43,10 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
         o.set_state(r, v)
         if bonds is not None:
             o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
-    if variant == "full-globalw":          # variant A on the paper's literal W layout (global indices, L1/L2 gathers)
+    if variant == "full-globalw":          # variant A on the paper's literal data path (global indices, L1/L2 gathers)
         variant, kw = "full", dict(kw, flags=md.FLAG_GLOBAL_W)
+    elif variant == "full-tiledw":         # variant A with 16-bit tile-local W entries and shared-memory force kernels
+        variant, kw = "full", dict(kw, flags=md.FLAG_TILED_W)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
                     step_mode=mode, **kw)
     g.set_state(r, v)
@@ -54,7 +56,7 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
 
 
 @pytest.mark.parametrize("case", list(small_cases()))
-@pytest.mark.parametrize("variant", ["full", "full-globalw", "newton3"])
+@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-tiledw", "newton3"])
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
 def test_neighbor_sets_and_forces(md, case, variant, state):
     cfg, _ = small_cases()[case]
@@ -86,7 +88,8 @@ def test_neighbor_sets_and_forces(md, case, variant, state):
 
 @pytest.mark.parametrize("case", list(small_cases()))
 @pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("full-globalw", "fused"),
-                                          ("full-globalw", "split"), ("newton3", "split")])
+                                          ("full-globalw", "split"), ("full-tiledw", "fused"), ("full-tiledw", "split"),
+                                          ("newton3", "split")])
 def test_ten_steps(md, case, variant, mode):
     cfg, _ = small_cases()[case]
     for seed in (1, 2, 3):
@@ -183,16 +186,17 @@ TILE_GEOMS = [dict(S=1, R=1, RZ=1, THREADS=128), dict(S=2, R=3, RZ=1, THREADS=12
 
 @pytest.mark.parametrize("case", ["wca_ragged_1000", "wca_dr05_13824", "lj_6912", "chains_4096"])
 @pytest.mark.parametrize("geom", range(len(TILE_GEOMS)))
-def test_tiled_w_any_box_shape(md, case, geom, monkeypatch):
-    """The tiled W layout must give the same matrix, forces and trajectory for every box shape S x R x RZ and
+@pytest.mark.parametrize("variant", ["full", "full-tiledw"])
+def test_tile_staging_any_box_shape(md, case, geom, variant, monkeypatch):
+    """The shared-memory staged build (default) and the tiled W layout must give the same matrix, forces and trajectory for every box shape S x R x RZ and
     block size (boxes cut by the periodic faces, boxes wider than the system, blocks looping over their atoms)."""
     cfg, _ = small_cases()[case]
     for k, v in TILE_GEOMS[geom].items():
         monkeypatch.setenv(f"MD_TILE_{k}", str(v))
     monkeypatch.setenv("MD_TILE_CAP", "8192")
-    g, o, box = make_pair(md, cfg, 2, variant="full", mode="fused", state="jitter")
+    g, o, box = make_pair(md, cfg, 2, variant=variant, mode="fused", state="jitter")
     info = g.info()
-    assert info["w_layout"] == 1 and info["tile_cells"][1:] == [TILE_GEOMS[geom]["R"], TILE_GEOMS[geom]["RZ"]]
+    assert info["w_layout"] == (1 if variant == "full-tiledw" else 0) and info["tile_cells"][1:] == [TILE_GEOMS[geom]["R"], TILE_GEOMS[geom]["RZ"]]
     counts, lst = g.neighbors()
     nbad, first = sets_equal(counts, lst, o)
     assert nbad == 0, f"neighbor sets differ for {nbad} atoms (first: atom {first})"
@@ -206,9 +210,29 @@ def test_tiled_w_any_box_shape(md, case, geom, monkeypatch):
 
 
 def test_tile_overflow_is_reported(md, monkeypatch):
+    """A tile that cannot hold the mean cell neighbourhood is refused at create (tiled W) or replaced by the gathering
+    build kernel (default layout); a neighbourhood that outgrows its tile at run time is an error code, never a
+    truncated matrix."""
     cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 1, jitter_amp=0.0)
     monkeypatch.setenv("MD_TILE_CAP", "64")
-    r, v, _, box = make_state(cfg, 1, jitter_amp=0.1)
     with pytest.raises(md.MDError):
-        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
-        g.set_state(r, v)
+        md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=md.FLAG_TILED_W)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g.set_state(r, v)
+    assert g.info()["tile_capacity"] == 0          # fell back to the gathering build kernel
+    g.close()
+    monkeypatch.delenv("MD_TILE_CAP")
+    squeezed = r.copy()
+    squeezed[:, 1] *= 0.5                          # density x 2 in half of the box (along y: a tile spans all of x)
+    for flags in (0, md.FLAG_TILED_W):
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags,
+                        max_neighbors=64)
+        with pytest.raises(md.MDError) as ei:
+            g.set_state(squeezed, v)
+        assert ei.value.code == md.binding.MD_ERR_TILE_OVERFLOW
+        g.close()
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=md.FLAG_GLOBAL_W,
+                    max_neighbors=64)
+    g.set_state(squeezed, v)                       # the literal path has no tile and takes any density
+    g.close()
