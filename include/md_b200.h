@@ -89,8 +89,11 @@ enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying 
                                  the neighbor build and the force kernel gather partner positions through L1/L2.
                                  Without this flag the build kernel stages the cell neighbourhood of each thread
                                  block in shared memory; W is the same. */
-       MD_FLAG_TILED_W = 4u   /* W holds 16-bit indices into the per-block shared-memory tile, and the force / energy
-                                 kernels stage that tile too.  Variant A only. */ };
+       MD_FLAG_TILED_W = 4u,  /* W holds 16-bit indices into the per-block shared-memory tile, and the force / energy
+                                 kernels stage that tile too.  Variant A only.  Without any of
+                                 these flags the library picks this layout when the expected number of neighbors per
+                                 atom is >= 32 (e.g. LJ with r_c = 2.5) and global indices otherwise. */
+       MD_FLAG_GATHER_W = 8u  /* never pick the tiled layout automatically (the build kernel still stages tiles) */ };
 enum { MD_W_GLOBAL = 0, MD_W_TILED = 1 };
 
 /* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */

@@ -476,7 +476,12 @@ md_system *md_create_ex(const md_params *pp)
         const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin);
         if (!fits && (p.flags & MD_FLAG_TILED_W)) { md_destroy(s); return nullptr; }
         P.tile_build = fits ? 1 : 0;
-        P.tiled = fits && (p.flags & MD_FLAG_TILED_W) ? 1 : 0;
+        // W layout: measured on B200, tile-local W wins once a column of W is long enough
+        // to amortise staging the tile (LJ r_c = 2.5: 76 neighbors, +17 %) and loses for the short WCA columns
+        // (12 neighbors, -17 %).  Estimated mean column length = ideal-gas count in the neighbor sphere.
+        const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
+        const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
+        P.tiled = fits && want_tiled ? 1 : 0;
     } else if (p.flags & MD_FLAG_TILED_W) {
         set_error("MD_FLAG_TILED_W needs the full-list force variant and excludes MD_FLAG_GLOBAL_W");
         md_destroy(s);

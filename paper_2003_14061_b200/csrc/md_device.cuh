@@ -53,17 +53,16 @@ __device__ __forceinline__ void st_pos(pos_t *p, double x, double y, double z)
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x), "d"(y), "d"(z), "d"(0.0) : "memory");
 }
 
-// 1/x to within ~1 ulp without the IEEE-division slow path: hardware seed + two Newton steps.
+// 1/x to within ~1 ulp without the IEEE-division slow path: hardware seed (relative error <= 2^-23) + one
+// third-order (Halley) step, y (1 + e + e^2) with e = 1 - x y: error e^3 ~ 2^-69, i.e. rounding only.
 // (Forces are compared with the oracle to 1e-10; the accept tests use r^2 itself.)
 __device__ __forceinline__ double fast_rcp(double x)
 {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    return y;
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
 }
 
 // Displacement r_i - r_j with the image correction frozen into the W entry (flag bit k set = subtract +-L

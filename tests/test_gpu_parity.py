@@ -45,6 +45,8 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
             o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
     if variant == "full-globalw":          # variant A on the paper's literal data path (global indices, L1/L2 gathers)
         variant, kw = "full", dict(kw, flags=md.FLAG_GLOBAL_W)
+    elif variant == "full-gatherw":        # tile-staged build, global W, gathering force kernel (the default for short columns)
+        variant, kw = "full", dict(kw, flags=md.FLAG_GATHER_W)
     elif variant == "full-tiledw":         # variant A with 16-bit tile-local W entries and shared-memory force kernels
         variant, kw = "full", dict(kw, flags=md.FLAG_TILED_W)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
@@ -56,7 +58,7 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
 
 
 @pytest.mark.parametrize("case", list(small_cases()))
-@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-tiledw", "newton3"])
+@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-gatherw", "full-tiledw", "newton3"])
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
 def test_neighbor_sets_and_forces(md, case, variant, state):
     cfg, _ = small_cases()[case]
@@ -186,7 +188,7 @@ TILE_GEOMS = [dict(S=1, R=1, RZ=1, THREADS=128), dict(S=2, R=3, RZ=1, THREADS=12
 
 @pytest.mark.parametrize("case", ["wca_ragged_1000", "wca_dr05_13824", "lj_6912", "chains_4096"])
 @pytest.mark.parametrize("geom", range(len(TILE_GEOMS)))
-@pytest.mark.parametrize("variant", ["full", "full-tiledw"])
+@pytest.mark.parametrize("variant", ["full-gatherw", "full-tiledw"])
 def test_tile_staging_any_box_shape(md, case, geom, variant, monkeypatch):
     """The shared-memory staged build (default) and the tiled W layout must give the same matrix, forces and trajectory for every box shape S x R x RZ and
     block size (boxes cut by the periodic faces, boxes wider than the system, blocks looping over their atoms)."""
@@ -225,7 +227,7 @@ def test_tile_overflow_is_reported(md, monkeypatch):
     monkeypatch.delenv("MD_TILE_CAP")
     squeezed = r.copy()
     squeezed[:, 1] *= 0.5                          # density x 2 in half of the box (along y: a tile spans all of x)
-    for flags in (0, md.FLAG_TILED_W):
+    for flags in (md.FLAG_GATHER_W, md.FLAG_TILED_W):
         g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags,
                         max_neighbors=64)
         with pytest.raises(md.MDError) as ei:
