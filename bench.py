@@ -238,7 +238,8 @@ def main():
     t_wall = time.perf_counter() - t_wall0
     ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop() if rank == 0 else None
-    launches = g.info()["kernel_launches"] - launches0
+    info_end = g.info()
+    launches = info_end["kernel_launches"] - launches0
     e_end = g.energies()
     if dist is not None:
         t = torch.tensor([ms], device="cuda", dtype=torch.float64)
@@ -256,24 +257,35 @@ def main():
     rebuilds_prof = e_prof.n_rebuilds - e_end.n_rebuilds
     mbar = 0.5 * (e_end.mean_neighbors + e_prof.mean_neighbors)
     peak, peak_src = load_peaks()
+    tiled = info["w_layout"] == 1
     if args.mode == "fused" and args.variant == "full":
-        kname, tk = "k_force<fused step>", timers["fused_step"]
-        bytes_per_atom = 28.0 * mbar + 100.0     # W 4m + m_i 4 + r_i 24 + gathers 24m + v r/w 48 + r' write 24
+        tk = timers["fused_step"]
+        if tiled:
+            kname = "k_tile_force<fused step>"
+            w_bytes = 2.0                        # 16-bit tile-local entries
+        else:
+            kname = "k_force<fused step>"
+            w_bytes = 4.0
+        # W w*m + m_i 4 + r_i 24 + gathers 24m + v read+write 48 + r' write 24   (north_star's accounting)
+        bytes_per_atom = (w_bytes + 24.0) * mbar + 100.0
+        floor_bytes = w_bytes * mbar + 100.0
     else:
         kname, tk = "k_force", timers["force"]
+        w_bytes = 4.0
         bytes_per_atom = 28.0 * mbar + 52.0      # SURVEY 8(d) B_ns: W 4m + m_i 4 + r_i 24 + gathers 24m + f write 24
+        floor_bytes = 4.0 * mbar + 52.0
         if args.variant == "newton3":
             tk = dict(tk, launches=tk["launches"] // 2)
     dur_ms = tk["ms"] / max(1, tk["launches"])
     achieved = bytes_per_atom * n / (dur_ms * 1e-3) / 1e9
-    floor_bytes = 4.0 * mbar + 100.0
     traffic = load_ncu_traffic(f"{args.config}:{kname}")
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_atom": bytes_per_atom, "mean_neighbors": mbar, "avg_launch_ms": dur_ms,
                 "accounting": "north_star B_ns (every gather charged 24 B)",
                 "frac_compulsory": floor_bytes * n / (dur_ms * 1e-3) / 1e9 / peak,
-                "compulsory_bytes_per_atom": floor_bytes}
+                "compulsory_bytes_per_atom": floor_bytes,
+                "timing": "CUDA events on the library's stream around each launch (md_set_profiling), second pass of K steps"}
     nebr = timers["nebr"]
     breakdown = {k: round(v["ms"] / args.steps, 6) for k, v in timers.items()}
     nebr_info = {"rebuilds": int(rebuilds_prof), "ms_per_rebuild": nebr["ms"] / max(1, rebuilds_prof),
@@ -321,6 +333,8 @@ def main():
                    "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
                    "force_variant": args.variant, "step_mode": args.mode, "block_size": info["block_size"],
                    "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
+                   "w_layout": "tiled16" if tiled else "global32", "tile_cells": info["tile_cells"],
+                   "cuda_graph": bool(info_end["use_graph"]),
                    "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                    "l2": "working set per step (positions 2x64 MB, velocities 48 MB, W rows ~100 MB) exceeds the 126 MB L2; no flush"},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,

@@ -128,7 +128,7 @@ typedef struct md_info {
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */
 enum { MD_T_INTEGRATE = 0, MD_T_CELLS = 1, MD_T_REORDER = 2, MD_T_NEBR = 3, MD_T_FORCE = 4, MD_T_ENERGY = 5,
-       MD_T_FUSED_STEP = 6, MD_T_COUNT = 8 };
+       MD_T_FUSED_STEP = 6, MD_T_DECIDE = 7, MD_T_COUNT = 8 };
 
 MD_API void md_params_default(md_params *p);
 

@@ -21,7 +21,7 @@ FLAG_NO_GRAPH, FLAG_GLOBAL_W, FLAG_TILED_W, FLAG_GATHER_W = 1, 2, 4, 8
 LATTICE = {"auto": 0, "sc": 1, "fcc": 2, "none": 3}
 FORCE_VARIANT = {"full": 0, "newton3": 1}
 STEP_MODE = {"fused": 0, "split": 1}
-TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "reserved")
+TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "decide")
 
 EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_step", "md_energies",
            "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",

@@ -179,10 +179,17 @@ void enqueue_rebuild(md_system *s)
     { Timed t(s, MD_T_NEBR, 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
-void enqueue_force(md_system *s, int mode, unsigned long long cond = 0ull)
+void enqueue_force(md_system *s, int mode)
 {
-    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream, cond);
-    else mdk_force(s->P, s->lc, mode, s->stream, cond);
+    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream);
+    else mdk_force(s->P, s->lc, mode, s->stream);
+}
+
+// rebuild decision after a drifting kernel; cond: conditional handle of the step graph or 0
+void enqueue_decide(md_system *s, bool fused_force, unsigned long long cond = 0ull)
+{
+    Timed t(s, MD_T_DECIDE, 1);
+    mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused_force), fused_force, s->stream, cond);
 }
 
 void drop_graph(md_system *s)
@@ -213,7 +220,8 @@ bool build_step_graph(md_system *s)
         if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
         cudaGraphConditionalHandle h;
         if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-        enqueue_force(s, 1, (unsigned long long)h);
+        enqueue_force(s, 1);
+        mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, true), true, st, (unsigned long long)h);
         if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
         cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
         cp.conditional.handle = h;
@@ -613,7 +621,8 @@ int md_step(md_system *s, int64_t n)
     cudaStream_t st = s->stream;
     if (s->prm.step_mode == MD_STEP_FUSED) {
         // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
-        { Timed t(s, MD_T_INTEGRATE, 2); mdk_kick_drift(P, s->lc, st); }
+        { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+        enqueue_decide(s, false);
         enqueue_rebuild(s);
         const bool want_graph = !s->profiling && !(s->prm.flags & MD_FLAG_NO_GRAPH) && n > 1;
         if (want_graph && !s->gexec && !s->graph_tried) build_step_graph(s);
@@ -623,14 +632,16 @@ int md_step(md_system *s, int64_t n)
             s->launches += 2 * (n - 1);                  // + the rebuild chains, added in check_device_status
         } else {
             for (int64_t k = 1; k < n; k++) {
-                { Timed t(s, MD_T_FUSED_STEP, 2); enqueue_force(s, 1); }
+                { Timed t(s, MD_T_FUSED_STEP, 1); enqueue_force(s, 1); }
+                enqueue_decide(s, true);
                 enqueue_rebuild(s);
             }
         }
         { Timed t(s, MD_T_FORCE, 1); enqueue_force(s, 2); }
     } else {
         for (int64_t k = 0; k < n; k++) {
-            { Timed t(s, MD_T_INTEGRATE, 2); mdk_kick_drift(P, s->lc, st); }
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+            enqueue_decide(s, false);
             enqueue_rebuild(s);
             enqueue_forces_only(s);
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick(P, s->lc, st); }

@@ -600,7 +600,6 @@ void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, un
 void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     k_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P);
-    mdk_decide(P, cdiv(P.N, 256), false, st, 0ull);
 }
 
 void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
@@ -637,7 +636,7 @@ static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
     }
 }
 
-void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st, unsigned long long cond)
+void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 {
     if (P.has_bonds) {
         if (mode == 0) launch_force_block<0, true>(P, lc.block, st);
@@ -648,7 +647,13 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st, un
         else if (mode == 1) launch_force_block<1, false>(P, lc.block, st);
         else launch_force_block<2, false>(P, lc.block, st);
     }
-    if (mode == 1) mdk_decide(P, cdiv(P.N, lc.block), true, st, cond);
+}
+
+// number of blocks (= entries of blk_vmax2) the drifting kernels write: input size of k_decide
+int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force)
+{
+    if (!fused_force) return cdiv(P.N, 256);
+    return P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : cdiv(P.N, lc.block);
 }
 
 void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)

@@ -624,14 +624,13 @@ void mdk_tile_build(const MdDev &P, cudaStream_t st)
 #undef MD_TB
 }
 
-void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long long cond)
+void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st)
 {
     switch (P.tg.threads) {
     case 128: launch_force<128>(P, mode, st); break;
     case 512: launch_force<512>(P, mode, st); break;
     default: launch_force<256>(P, mode, st); break;
     }
-    if (mode == 1) mdk_decide(P, tile_grid(P), true, st, cond);
 }
 
 void mdk_tile_energy(const MdDev &P, cudaStream_t st)

@@ -152,13 +152,14 @@ void mdk_force_rebuild(const MdDev &P, cudaStream_t st);
 void mdk_load_state(const MdDev &P, cudaStream_t st);                        // scratch(xyz | vxyz) -> pos/vel/id
 // rebuild decision from blk_vmax2[0..nblk); cond != 0: also set that CUDA-graph conditional handle to need_rebuild
 void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond);
-void mdk_kick_drift(const MdDev &P, const MdLaunch &lc, cudaStream_t st);     // v += dt/2 f; r += dt v; decide
+void mdk_kick_drift(const MdDev &P, const MdLaunch &lc, cudaStream_t st);     // v += dt/2 f; r += dt v; per-block max v^2
 void mdk_kick(const MdDev &P, const MdLaunch &lc, cudaStream_t st);           // v += dt/2 f
 void mdk_cells(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // bin + scan + place       (N1-N4)
 void mdk_reorder(const MdDev &P, const MdLaunch &lc, cudaStream_t st);        // cell-order gather       (sec 2.4(4))
 void mdk_build(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // neighbor matrix         (N5)
-// mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, decide); 2: f and closing half kick
-void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st, unsigned long long cond = 0ull);
+// mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, per-block max v^2; follow with mdk_decide); 2: f and closing half kick
+void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
+int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   // blocks writing blk_vmax2
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    // 0 pos, 1 vel, 2 frc -> scratch + offset
@@ -166,7 +167,7 @@ void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    //
 int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
 size_t mdk_tile_smem(const TileGeom &G, bool with_cells);
 void mdk_tile_build(const MdDev &P, cudaStream_t st);
-void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st, unsigned long long cond = 0ull);
+void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st);
 void mdk_tile_energy(const MdDev &P, cudaStream_t st);
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,
