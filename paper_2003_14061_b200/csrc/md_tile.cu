@@ -180,31 +180,32 @@ __device__ __forceinline__ void own_atom(const TileDesc &M, int t, int &i, int &
 // ------------------------------------------------------------------------------------------------
 // Appending to column i of W is written so that it compiles to predicated instructions, not a divergent
 // block: in a warp some lane accepts its candidate in most iterations, so a branch would be taken (by a few
-// lanes, the others idling) nearly every time.
+// lanes, the others idling) nearly every time.  Tiled layout: entry m of the column is the 16-bit half
+// (m & 1) of word (m >> 1) * pitch + i, written with a 16-bit store.
 template <bool LOCALW>
 struct Emit {
-    unsigned *wp;       // next free word of column i of W
-    size_t pitch;
+    char *wp;           // address of the next free entry of column i of W
+    long long pitch4;   // bytes between consecutive word rows
     int m, Mmax;
-    unsigned pend;
     // candidate with tile index j; add = (flags << shift) + (global - tile index), constant over a run
     __device__ __forceinline__ void put(bool acc, int j, unsigned add)
     {
         const unsigned e = (unsigned)j + add;
+        const bool st = acc && m < Mmax;
         if (LOCALW) {
-            const bool odd = m & 1;
-            if (acc && odd && m < Mmax) *wp = pend | (e << 16);
-            wp += acc && odd ? pitch : 0;
-            pend = acc && !odd ? e : pend;
+            if (st) *(unsigned short *)wp = (unsigned short)e;
+            const long long step = (m & 1) ? pitch4 - 2 : 2;
+            wp += acc ? step : 0;
         } else {
-            if (acc && m < Mmax) *wp = e;
-            wp += acc ? pitch : 0;
+            if (st) *(unsigned *)wp = e;
+            wp += acc ? pitch4 : 0;
         }
         m += acc;
     }
+    // an odd column leaves the upper half of its last word unwritten: clear it, the force kernel reads whole words
     __device__ __forceinline__ void flush()
     {
-        if (LOCALW && (m & 1) && m < Mmax) *wp = pend;
+        if (LOCALW && (m & 1) && m < Mmax) *(unsigned short *)wp = 0;
     }
 };
 
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ Md
         own_atom(M, t, i, li);
         const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
         const int cx = cell_coord(xi, P.inv_w, nc), cy = cell_coord(yi, P.inv_w, nc), cz = cell_coord(zi, P.inv_w, nc);
-        Emit<LOCALW> em = {(unsigned *)P.W + i, (size_t)P.N_pad, 0, P.Mmax, 0u};
+        Emit<LOCALW> em = {(char *)((unsigned *)P.W + i), 4ll * P.N_pad, 0, P.Mmax};
         const int k0 = cx - B.x0;
         const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
 #pragma unroll 1
