@@ -51,7 +51,7 @@ def load_ncu_traffic(kernel_key):
         for line in fh:
             line = line.split("#", 1)[0].strip()
             if line.startswith(kernel_key + " "):
-                return float(line.split()[1])
+                return float(line.rsplit(None, 1)[1])
     return None
 
 

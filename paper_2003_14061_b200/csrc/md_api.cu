@@ -66,8 +66,8 @@ struct md_system {
     bool profiling = false;
     std::vector<EvPair> pending, pool;
     // CUDA graph of one fused step: force+kick+drift -> decide -> IF(need_rebuild){cells, reorder, build}
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t gexec = nullptr;
+    cudaGraph_t graph[2] = {nullptr, nullptr};          // [0] kick+drift step head, [1] fused force+kick+drift step
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     cudaStream_t cap_stream = nullptr;
     bool graph_tried = false;
     int chain_kernels = 0;         // kernels inside the conditional body
@@ -194,19 +194,22 @@ void enqueue_decide(md_system *s, bool fused_force, unsigned long long cond = 0u
 
 void drop_graph(md_system *s)
 {
-    if (s->gexec) cudaGraphExecDestroy(s->gexec);
-    if (s->graph) cudaGraphDestroy(s->graph);
-    s->gexec = nullptr; s->graph = nullptr; s->graph_tried = false;
+    for (int k = 0; k < 2; k++) {
+        if (s->gexec[k]) cudaGraphExecDestroy(s->gexec[k]);
+        if (s->graph[k]) cudaGraphDestroy(s->graph[k]);
+        s->gexec[k] = nullptr; s->graph[k] = nullptr;
+    }
+    s->graph_tried = false;
 }
 
-// One fused time step as a CUDA graph.  The rebuild chain sits in the body of an IF node whose condition
-// k_decide sets on the device (cudaGraphSetConditional), so a step without a rebuild launches 2 kernels
-// instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision on the host every step).
-// Returns false (and leaves no graph) if any step of the construction is refused; md_step then launches
-// the kernels one by one.
-bool build_step_graph(md_system *s)
+// The drifting part of a time step as a CUDA graph: kind 0 = opening half kick + drift (k_kick_drift), kind 1 =
+// fused force + kick + drift (k_force<1> / k_tile_force<1>); then k_decide; then the rebuild chain in the body
+// of an IF node whose condition k_decide sets on the device (cudaGraphSetConditional).  A step without a
+// rebuild so launches 2 kernels instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision
+// on the host every step).  Returns false (and leaves no graph) if any step of the construction is refused;
+// md_step then launches the kernels one by one.
+bool build_step_graph(md_system *s, int kind)
 {
-    s->graph_tried = true;
     cudaStream_t st = s->stream;
     if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
     cudaGraph_t g = nullptr;
@@ -220,8 +223,9 @@ bool build_step_graph(md_system *s)
         if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
         cudaGraphConditionalHandle h;
         if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-        enqueue_force(s, 1);
-        mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, true), true, st, (unsigned long long)h);
+        if (kind == 1) enqueue_force(s, 1);
+        else mdk_kick_drift(s->P, s->lc, st);
+        mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, kind == 1), kind == 1, st, (unsigned long long)h);
         if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
         cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
         cp.conditional.handle = h;
@@ -239,19 +243,35 @@ bool build_step_graph(md_system *s)
         if (cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) break;
         capturing = false;
         if (cudaStreamEndCapture(st, &g) != cudaSuccess) { g = nullptr; break; }
-        s->graph = g;
-        if (cudaGraphInstantiate(&s->gexec, g, 0) != cudaSuccess) break;
+        s->graph[kind] = g;
+        if (cudaGraphInstantiate(&s->gexec[kind], g, 0) != cudaSuccess) break;
         ok = true;
     } while (0);
     if (!ok) {
         if (capturing) { cudaGraph_t junk = nullptr; cudaStreamEndCapture(st, &junk); if (junk) cudaGraphDestroy(junk); }
         cudaGetLastError();
-        if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
-        if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+        if (s->gexec[kind]) { cudaGraphExecDestroy(s->gexec[kind]); s->gexec[kind] = nullptr; }
+        if (s->graph[kind]) { cudaGraphDestroy(s->graph[kind]); s->graph[kind] = nullptr; }
         return false;
     }
     s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1;
     return true;
+}
+
+// both graphs, once; all or nothing
+bool have_graphs(md_system *s)
+{
+    if (s->profiling || (s->prm.flags & MD_FLAG_NO_GRAPH)) return false;
+    if (!s->graph_tried) {
+        s->graph_tried = true;
+        const bool fused = s->prm.step_mode == MD_STEP_FUSED;
+        if (!build_step_graph(s, 0) || (fused && !build_step_graph(s, 1))) {
+            const bool tried = true;
+            drop_graph(s);
+            s->graph_tried = tried;
+        }
+    }
+    return s->gexec[0] != nullptr;
 }
 
 void enqueue_forces_only(md_system *s)
@@ -621,16 +641,16 @@ int md_step(md_system *s, int64_t n)
     cudaStream_t st = s->stream;
     if (s->prm.step_mode == MD_STEP_FUSED) {
         // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
-        { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
-        enqueue_decide(s, false);
-        enqueue_rebuild(s);
-        const bool want_graph = !s->profiling && !(s->prm.flags & MD_FLAG_NO_GRAPH) && n > 1;
-        if (want_graph && !s->gexec && !s->graph_tried) build_step_graph(s);
-        if (want_graph && s->gexec) {
-            for (int64_t k = 1; k < n; k++) CK(cudaGraphLaunch(s->gexec, st));
-            s->graph_steps += n - 1;
-            s->launches += 2 * (n - 1);                  // + the rebuild chains, added in check_device_status
+        const bool graphs = have_graphs(s);
+        if (graphs) {
+            CK(cudaGraphLaunch(s->gexec[0], st));
+            for (int64_t k = 1; k < n; k++) CK(cudaGraphLaunch(s->gexec[1], st));
+            s->graph_steps += n;
+            s->launches += 2 * n;                        // + the rebuild chains, added in check_device_status
         } else {
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+            enqueue_decide(s, false);
+            enqueue_rebuild(s);
             for (int64_t k = 1; k < n; k++) {
                 { Timed t(s, MD_T_FUSED_STEP, 1); enqueue_force(s, 1); }
                 enqueue_decide(s, true);
@@ -639,10 +659,17 @@ int md_step(md_system *s, int64_t n)
         }
         { Timed t(s, MD_T_FORCE, 1); enqueue_force(s, 2); }
     } else {
+        const bool graphs = have_graphs(s);
         for (int64_t k = 0; k < n; k++) {
-            { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
-            enqueue_decide(s, false);
-            enqueue_rebuild(s);
+            if (graphs) {
+                CK(cudaGraphLaunch(s->gexec[0], st));
+                s->graph_steps += 1;
+                s->launches += 2;
+            } else {
+                { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
+                enqueue_decide(s, false);
+                enqueue_rebuild(s);
+            }
             enqueue_forces_only(s);
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick(P, s->lc, st); }
         }
@@ -759,7 +786,7 @@ int md_get_info(md_system *s, md_info *out)
         out->tile_cells[0] = s->P.tg.S; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }
-    out->use_graph = s->gexec ? 1 : 0;
+    out->use_graph = s->gexec[0] ? 1 : 0;
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

@@ -238,3 +238,38 @@ def test_tile_overflow_is_reported(md, monkeypatch):
                     max_neighbors=64)
     g.set_state(squeezed, v)                       # the literal path has no tile and takes any density
     g.close()
+
+
+@pytest.mark.parametrize("name", ["wca_2m", "wca_2m_dr03", "wca_2m_dr05", "lj_1m", "chains_1m"])
+def test_full_size_sampled_against_definitions(md, name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (default flags, fused steps, CUDA graph):
+    after 40 steps from the seeded start, sampled atoms are checked one by one against the all-pairs definitions
+    (neighbor sets exact, forces 1e-10), and the conserved quantities against the start."""
+    cfg = get_config(name)
+    r, v, bonds, box = make_state(cfg, 1)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g.set_state(r, v)
+    if bonds is not None:
+        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    n = cfg.n_atoms
+    e0 = g.energies()
+    g.step(40)
+    e1 = g.energies()
+    assert g.info()["use_graph"] == 1 and e1.n_rebuilds >= 2
+    assert abs(e1.total - e0.total) / n < 2e-3
+    assert max(abs(e1.px), abs(e1.py), abs(e1.pz)) < 1e-9 * np.sqrt(n) * 10
+    g.rebuild_neighbors()                       # W and forces for the current (wrapped) positions
+    pos = g.positions()
+    assert pos.min() >= 0.0 and pos.max() < box
+    rng = np.random.default_rng(7)
+    idx = np.sort(rng.choice(n, 400, replace=False))
+    counts, lst = g.neighbors()
+    want = brute_neighbors_sample(pos, box, cfg.r_cut + cfg.r_shell, idx)
+    for k, i in enumerate(idx):
+        got = np.sort(lst[i, :counts[i]])
+        assert np.array_equal(got, want[k]), f"neighbor set of atom {i} differs"
+    del lst
+    if bonds is None:                           # the all-pairs definition has no bond term
+        fb, _, _ = brute_forces_sample(pos, box, cfg.r_cut, idx)
+        assert force_rel_err(g.forces()[idx], fb) <= FORCE_RTOL
+    g.close()
