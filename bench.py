@@ -294,17 +294,21 @@ def main():
     # ---- end to end through the C ABI with HOST buffers: H2D state, one step, D2H positions + energies ------
     e2e = None
     if not args.no_e2e:
-        rh, vh = g.positions(), g.velocities()
-        out = np.empty_like(rh)
+        def pinned(shape):                # page-locked host buffers: the library copies to / from them directly
+            return torch.empty(shape, dtype=torch.float64, pin_memory=True).numpy()
+        rh, vh, out, vout = pinned((n, 3)), pinned((n, 3)), pinned((n, 3)), pinned((n, 3))
+        g.positions(rh)
+        g.velocities(vh)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
             g.set_state(rh, vh)          # host -> device (pinned staging inside the library), rebuild, forces
             g.step(1)
             g.positions(out)             # device -> host
-            vh = g.velocities()
+            g.velocities(vout)
             en = g.energies()
-            rh = out
+            rh, out = out, rh
+            vh, vout = vout, vh
         barrier()
         dt = time.perf_counter() - t0
         if dist is not None:
@@ -313,7 +317,7 @@ def main():
             dt = float(t.item())
         e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
                "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
-               "what": "md_set_state(host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
+               "what": "md_set_state(pinned host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
 
     if rank != 0:
         if dist is not None:

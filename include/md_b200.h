@@ -17,6 +17,8 @@
  * Conventions
  *   - Reduced units (sigma = epsilon = m = 1).  Cubic periodic box [0, L)^3.  All arithmetic is fp64.
  *   - Every array argument is a HOST pointer owned by the caller unless its name ends in `_device`.
+ *     Page-locked (cudaHostAlloc / cudaHostRegister) arrays are copied to and from directly on the stream;
+ *     pageable ones go through a pinned staging buffer inside the library.
  *     Layout of per-atom vectors at the boundary: xyz[3*i + k], i = ORIGINAL atom id (the device keeps
  *     atoms in cell order and re-sorts them at every rebuild; that is invisible here).
  *   - No C++ exceptions cross the boundary.  Functions returning int give MD_OK (0) or a negative

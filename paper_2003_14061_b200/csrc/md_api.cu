@@ -300,6 +300,15 @@ int install_state(md_system *s)
     return MD_OK;
 }
 
+// page-locked host memory can be the source / target of the asynchronous copies directly; anything else goes
+// through the library's pinned staging buffer
+bool is_pinned(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost;
+}
+
 int upload_state(md_system *s, const double *xyz, const double *vxyz)
 {
     const size_t n3 = 3 * (size_t)s->P.N;
@@ -308,11 +317,13 @@ int upload_state(md_system *s, const double *xyz, const double *vxyz)
         s->launches += 1;
         mdk_export(s->P, 1, n3, s->stream);
     }
-    memcpy(s->h_stage, xyz, n3 * sizeof(double));
-    CK(cudaMemcpyAsync(s->P.scratch, s->h_stage, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    const double *src = xyz;
+    if (!is_pinned(xyz)) { memcpy(s->h_stage, xyz, n3 * sizeof(double)); src = s->h_stage; }
+    CK(cudaMemcpyAsync(s->P.scratch, src, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     if (vxyz) {
-        memcpy(s->h_stage + n3, vxyz, n3 * sizeof(double));
-        CK(cudaMemcpyAsync(s->P.scratch + n3, s->h_stage + n3, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+        src = vxyz;
+        if (!is_pinned(vxyz)) { memcpy(s->h_stage + n3, vxyz, n3 * sizeof(double)); src = s->h_stage + n3; }
+        CK(cudaMemcpyAsync(s->P.scratch + n3, src, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     }
     return install_state(s);
 }
@@ -324,10 +335,11 @@ int download(md_system *s, int what, double *out)
     const size_t n3 = 3 * (size_t)s->P.N;
     s->launches += 1;
     mdk_export(s->P, what, 0, s->stream);
-    CK(cudaMemcpyAsync(s->h_stage, s->P.scratch, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    const bool direct = is_pinned(out);
+    CK(cudaMemcpyAsync(direct ? out : s->h_stage, s->P.scratch, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     CK(cudaGetLastError());
-    memcpy(out, s->h_stage, n3 * sizeof(double));
+    if (!direct) memcpy(out, s->h_stage, n3 * sizeof(double));
     return MD_OK;
 }
 
@@ -571,8 +583,12 @@ int md_set_state(md_system *s, const double *xyz, const double *vxyz)
 {
     if (!s || !xyz) { set_error("md_set_state: null argument"); return MD_ERR_INVALID; }
     const double L = s->P.L;
-    for (size_t i = 0; i < 3 * (size_t)s->P.N; i++)
-        if (!(xyz[i] >= 0.0 && xyz[i] <= L)) { set_error("md_set_state: coordinate %zu = %g outside [0, L]", i, xyz[i]); return MD_ERR_INVALID; }
+    const size_t n3 = 3 * (size_t)s->P.N;
+    int bad = 0;
+    for (size_t i = 0; i < n3; i++) bad |= !(xyz[i] >= 0.0 && xyz[i] <= L);      // branch-free: vectorises
+    if (bad)
+        for (size_t i = 0; i < n3; i++)
+            if (!(xyz[i] >= 0.0 && xyz[i] <= L)) { set_error("md_set_state: coordinate %zu = %g outside [0, L]", i, xyz[i]); return MD_ERR_INVALID; }
     return upload_state(s, xyz, vxyz);
 }
 

@@ -127,3 +127,24 @@ def test_graph_and_direct_launch_agree_bitwise(md):
         assert np.array_equal(out[a][0], out[b][0]) and np.array_equal(out[a][1], out[b][1])
         assert out[a][2] == out[b][2] > 10
         assert out[a][3] < out[b][3]          # the graph skips the rebuild chain of steps that do not rebuild
+
+
+def test_pinned_host_buffers_take_the_direct_copy_path(md):
+    import torch
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 2, jitter_amp=0.05)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    rp = torch.empty(r.shape, dtype=torch.float64, pin_memory=True).numpy()
+    vp = torch.empty(v.shape, dtype=torch.float64, pin_memory=True).numpy()
+    rp[:], vp[:] = r, v
+    g.set_state(rp, vp)
+    g.step(5)
+    out = torch.empty(r.shape, dtype=torch.float64, pin_memory=True).numpy()
+    g.positions(out)
+    assert np.array_equal(out, g.positions())
+    g.velocities(out)
+    assert np.array_equal(out, g.velocities())
+    g2 = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g2.set_state(r, v)
+    g2.step(5)
+    assert np.array_equal(g2.positions(), g.positions())
