@@ -510,7 +510,6 @@ md_system *md_create_ex(const md_params *pp)
 
     P.tiled = 0;
     P.tile_build = 0;
-    P.dbg = env_int("MD_DEBUG_EXP", 0);
     if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
         // shared-memory staged neighbor build (both W layouts); the tiled W layout only on request
         const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin);

@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_f
         pre = tile_column_preload(P, i);
         if (MODE != 0) { v0 = vel[i]; v1 = vel[np + i]; v2 = vel[2 * np + i]; }
     }
-    if (n_own > 0 && !(P.dbg & 2)) tile_stage<true>(M, pos, st, P.L);
+    if (n_own > 0) tile_stage<true>(M, pos, st, P.L);
     __syncthreads();
     double vm2 = 0.0;
     for (; t < n_own; t += BLOCK) {
@@ -473,10 +473,8 @@ __global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_f
             pre = tile_column_preload(P, i);
             if (MODE != 0) { v0 = vel[i]; v1 = vel[np + i]; v2 = vel[2 * np + i]; }
         }
-        double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
-        if (P.dbg & 2) { const pos_t r = ld_pos(pos + i); xi = r.x; yi = r.y; zi = r.z; }
-        PairAccT a = {0.0, 0.0, 0.0, 0.0, 0.0};
-        if (!(P.dbg & 1)) a = tile_column<false>(P, st, xi, yi, zi, i, pre);
+        const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
+        PairAccT a = tile_column<false>(P, st, xi, yi, zi, i, pre);
         double ub = 0.0;
         if (BONDS) tile_bonds<false>(P, pos, xi, yi, zi, i, a, ub);
         if (MODE == 0 || MODE == 2) {

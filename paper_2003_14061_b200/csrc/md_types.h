@@ -120,7 +120,6 @@ constexpr int TILE_ROW_INTS = 8;
 struct MdDev {
     int N, N_pad, Mmax, nc, NC;
     int has_bonds, half_list, scan_blocks;
-    int dbg;                            // MD_DEBUG_EXP bit mask: timing experiments only (results are wrong when set)
     int tiled, tile_build, max_grid;    // W layout (1 = MD_W_TILED); shared-memory staged build kernel in use; row pitch of `partials`
     TileGeom tg;
     double L, half_L, inv_w;            // inv_w = nc / L
