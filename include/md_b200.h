@@ -95,7 +95,9 @@ enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying 
                                  kernels stage that tile too.  Variant A only.  Without any of
                                  these flags the library picks this layout when the expected number of neighbors per
                                  atom is >= 32 (e.g. LJ with r_c = 2.5) and global indices otherwise. */
-       MD_FLAG_GATHER_W = 8u  /* never pick the tiled layout automatically (the build kernel still stages tiles) */ };
+       MD_FLAG_GATHER_W = 8u, /* never pick the tiled layout automatically (the build kernel still stages tiles) */
+       MD_FLAG_W_TRANSPOSED = 16u /* ablation of PAPER.md:165-167: store W atom-index-SLOWEST, W[i * Mmax + m], so that
+                                 the threads of a warp no longer read consecutive words (global-index layout only) */ };
 enum { MD_W_GLOBAL = 0, MD_W_TILED = 1 };
 
 /* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */

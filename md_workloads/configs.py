@@ -47,6 +47,10 @@ CONFIGS = {
     # configs[4]
     "chains_1m": MDConfig("chains_1m", 16384 * 64, "chains", 0.85, 1.0, R_WCA, 0.4, 0.005, 500,
                           chain_len=64, n_chains=16384, fene_k=30.0, fene_r0=1.5),
+    # Context only (not BASELINE.json configs): the paper's OWN state points and shell at the
+    # N = 128^3 row of its Table 1, cubic-grid start, for a line next to that table in BASELINE.md.
+    "paper_sp_2m": MDConfig("paper_sp_2m", 128 ** 3, "sc", 0.8, 1.0, R_WCA, 0.6, 0.005, 500),
+    "paper_lj_2m": MDConfig("paper_lj_2m", 128 ** 3, "sc", 0.38, 1.2, 2.5, 0.6, 0.005, 500),
 }
 
 

@@ -526,6 +526,11 @@ md_system *md_create_ex(const md_params *pp)
         md_destroy(s);
         return nullptr;
     }
+    P.w_row = P.N_pad; P.w_col = 1;
+    if (p.flags & MD_FLAG_W_TRANSPOSED) {
+        if (P.tiled) { set_error("MD_FLAG_W_TRANSPOSED applies to the global-index W layout only"); md_destroy(s); return nullptr; }
+        P.w_row = 1; P.w_col = P.Mmax;
+    }
     P.max_grid = std::max((P.N + 63) / 64, P.tile_build ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
 
     const size_t np = (size_t)P.N_pad;
@@ -730,7 +735,7 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
     const int N = P.N, M = P.Mmax;
     const size_t np = (size_t)P.N_pad;
     const int nrows = std::min(M, std::max(1, s->h_ctrl->max_nnb));
-    const int rows = P.tiled ? (nrows + 1) / 2 : nrows;      // tiled: two 16-bit entries per 32-bit word
+    const int rows = P.tiled ? (nrows + 1) / 2 : (P.w_col == 1 ? nrows : M);      // tiled: two 16-bit entries per 32-bit word
     std::vector<int> nnb(N), id(N), W((size_t)rows * np);
     CK(cudaMemcpy(nnb.data(), P.nnb, N * sizeof(int), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(id.data(), P.id[s->h_ctrl->v_dst], N * sizeof(int), cudaMemcpyDeviceToHost));
@@ -774,7 +779,7 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
     } else {
         for (int p = 0; p < N; p++)
             for (int m = 0; m < nnb[p]; m++) {
-                const int i = id[p], j = id[(unsigned)W[(size_t)m * np + p] & 0x1fffffffu];   // top 3 bits: image flags
+                const int i = id[p], j = id[(unsigned)W[(size_t)m * P.w_row + (size_t)p * P.w_col] & 0x1fffffffu];   // top 3 bits: image flags
                 add(i, j);
                 if (P.half_list) add(j, i);
             }

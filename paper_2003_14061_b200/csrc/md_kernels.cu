@@ -318,7 +318,7 @@ __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict
         if (SHIFT) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
         if (r2 < P.rn2 && (HALF ? (j > i) : (j != i))) {
-            if (m < P.Mmax) P.W[(size_t)m * P.N_pad + i] = (int)((unsigned)j | (fl << W_FLAG_SHIFT));
+            if (m < P.Mmax) P.W[(size_t)m * P.w_row + (size_t)i * P.w_col] = (int)((unsigned)j | (fl << W_FLAG_SHIFT));
             m++;
         }
     }
@@ -419,8 +419,8 @@ template <int U>
 __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i)
 {
     const int m = P.nnb[i];
-    const int *__restrict__ w = P.W + i;
-    const size_t pitch = (size_t)P.N_pad;
+    const int *__restrict__ w = P.W + (size_t)i * P.w_col;
+    const size_t pitch = (size_t)P.w_row;
     PairAcc a = {0.0, 0.0, 0.0};
     unsigned cur[U], nxt[U];
 #pragma unroll
@@ -489,12 +489,12 @@ __global__ void __launch_bounds__(256) k_force_n3(const __grid_constant__ MdDev 
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
     const pos_t ri = ld_pos(pos + i);
     const int m = P.nnb[i];
-    const int *__restrict__ w = P.W + i;
+    const int *__restrict__ w = P.W + (size_t)i * P.w_col;
     double *fx = P.frc, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
     PairAcc a = {0.0, 0.0, 0.0};
 #pragma unroll 2
     for (int k = 0; k < m; k++) {
-        const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.N_pad);
+        const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.w_row);
         const int j = (int)(en & W_INDEX_MASK);
         const pos_t rj = ld_pos(pos + j);
         double dx, dy, dz;
@@ -534,11 +534,11 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
     if (i < P.N) {
         const pos_t ri = ld_pos(pos + i);
         const int m = P.nnb[i];
-        const int *__restrict__ w = P.W + i;
+        const int *__restrict__ w = P.W + (size_t)i * P.w_col;
         double u = 0.0, vir = 0.0;
 #pragma unroll 2
         for (int k = 0; k < m; k++) {
-            const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.N_pad);
+            const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.w_row);
             const pos_t rj = ld_pos(pos + (en & W_INDEX_MASK));
             double dx, dy, dz;
             const double r2 = disp2(ri, rj, en >> W_FLAG_SHIFT, P.L, dx, dy, dz);

@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ Md
         own_atom(M, t, i, li);
         const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
         const int cx = cell_coord(xi, P.inv_w, nc), cy = cell_coord(yi, P.inv_w, nc), cz = cell_coord(zi, P.inv_w, nc);
-        Emit<LOCALW> em = {(char *)((unsigned *)P.W + i), 4ll * P.N_pad, 0, P.Mmax};
+        Emit<LOCALW> em = {(char *)((unsigned *)P.W + (size_t)i * P.w_col), 4ll * P.w_row, 0, P.Mmax};
         const int k0 = cx - B.x0;
         const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
 #pragma unroll 1

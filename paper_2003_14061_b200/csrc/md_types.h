@@ -132,6 +132,7 @@ struct MdDev {
     int *id[2];                         // device slot -> original atom id
     int *cell_of, *slot, *cell_count, *cell_start, *perm, *block_sums;
     int *tile_desc;                     // tiled layout: TileDesc per box
+    int w_row, w_col;                   // W[m * w_row + i * w_col]: (N_pad, 1) = atom-index-fastest; (1, Mmax) = transposed (ablation)
     int *W, *nnb;                       // neighbor matrix W[m * N_pad + i], counts m_i
                                         // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)

@@ -47,6 +47,8 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
         variant, kw = "full", dict(kw, flags=md.FLAG_GLOBAL_W)
     elif variant == "full-gatherw":        # tile-staged build, global W, gathering force kernel (the default for short columns)
         variant, kw = "full", dict(kw, flags=md.FLAG_GATHER_W)
+    elif variant == "full-transposed":     # ablation: W stored atom-index-slowest
+        variant, kw = "full", dict(kw, flags=md.FLAG_W_TRANSPOSED | md.FLAG_GATHER_W)
     elif variant == "full-tiledw":         # variant A with 16-bit tile-local W entries and shared-memory force kernels
         variant, kw = "full", dict(kw, flags=md.FLAG_TILED_W)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
@@ -58,7 +60,7 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
 
 
 @pytest.mark.parametrize("case", list(small_cases()))
-@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-gatherw", "full-tiledw", "newton3"])
+@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-gatherw", "full-tiledw", "full-transposed", "newton3"])
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
 def test_neighbor_sets_and_forces(md, case, variant, state):
     cfg, _ = small_cases()[case]
@@ -90,7 +92,7 @@ def test_neighbor_sets_and_forces(md, case, variant, state):
 
 @pytest.mark.parametrize("case", list(small_cases()))
 @pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("full-globalw", "fused"),
-                                          ("full-globalw", "split"), ("full-tiledw", "fused"), ("full-tiledw", "split"),
+                                          ("full-globalw", "split"), ("full-tiledw", "fused"), ("full-tiledw", "split"), ("full-transposed", "fused"),
                                           ("newton3", "split")])
 def test_ten_steps(md, case, variant, mode):
     cfg, _ = small_cases()[case]
