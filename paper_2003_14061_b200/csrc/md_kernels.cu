@@ -414,29 +414,44 @@ __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restri
     }
 }
 
-// sum of pair forces on atom i over column i of W
-template <int U>
+// Sum of pair forces on atom i over column i of W.
+// Two dependent streams feed the loop: the rows of W come from HBM (W is far larger than L2 and read once per
+// step), the partner positions from L1/L2.  With the index loads only U rows ahead, every U rows waited one
+// full HBM latency (measured: ~7 us per row of W at N = 2M, whatever the gathers touched).  So the W rows are
+// loaded a block of D at a time, one block ahead: the next D rows are in flight while the gathers of the current
+// block run U at a time.
+#ifndef MD_FORCE_D
+#define MD_FORCE_D 8
+#endif
+template <int U, int D>
 __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i)
 {
-    const int m = P.nnb[i];
+    static_assert(D % U == 0, "D must be a multiple of U");
     const int *__restrict__ w = P.W + (size_t)i * P.w_col;
     const size_t pitch = (size_t)P.w_row;
     PairAcc a = {0.0, 0.0, 0.0};
-    unsigned cur[U], nxt[U];
+    unsigned cur[D], nxt[D];
+    // the first block of rows does not wait for the column length: rows < Mmax exist, entries >= m are never used
 #pragma unroll
-    for (int u = 0; u < U; u++) cur[u] = u < m ? (unsigned)__ldcs(w + u * pitch) : 0u;
-    for (int k = 0; k < m; k += U) {
-        pos_t rj[U];
+    for (int d = 0; d < D; d++) cur[d] = d < P.Mmax ? (unsigned)__ldcs(w + d * pitch) : 0u;
+    const int m = P.nnb[i];
+    for (int base = 0; base < m; base += D) {
 #pragma unroll
-        for (int u = 0; u < U; u++)
-            if (k + u < m) rj[u] = ld_pos(pos + (cur[u] & W_INDEX_MASK));
+        for (int d = 0; d < D; d++) nxt[d] = base + D + d < m ? (unsigned)__ldcs(w + (base + D + d) * pitch) : 0u;
 #pragma unroll
-        for (int u = 0; u < U; u++) nxt[u] = k + U + u < m ? (unsigned)__ldcs(w + (k + U + u) * pitch) : 0u;
+        for (int g = 0; g < D; g += U) {
+            if (base + g < m) {
+                pos_t rj[U];
 #pragma unroll
-        for (int u = 0; u < U; u++)
-            if (k + u < m) pair_force(P, ri, rj[u], cur[u] >> W_FLAG_SHIFT, a);
+                for (int u = 0; u < U; u++)
+                    if (base + g + u < m) rj[u] = ld_pos(pos + (cur[g + u] & W_INDEX_MASK));
 #pragma unroll
-        for (int u = 0; u < U; u++) cur[u] = nxt[u];
+                for (int u = 0; u < U; u++)
+                    if (base + g + u < m) pair_force(P, ri, rj[u], cur[g + u] >> W_FLAG_SHIFT, a);
+            }
+        }
+#pragma unroll
+        for (int d = 0; d < D; d++) cur[d] = nxt[d];
     }
     a.fx *= 48.0; a.fy *= 48.0; a.fz *= 48.0;
     return a;
@@ -454,20 +469,22 @@ __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(c
     double v2 = 0.0;
     if (i < P.N) {
         const pos_t ri = ld_pos(pos + i);
-        PairAcc a = column_force<MD_FORCE_U>(P, pos, ri, i);
+        const size_t np = (size_t)P.N_pad;
+        double *v = P.vel[vc] + i;
+        double v0 = 0.0, v1 = 0.0, v2i = 0.0;
+        if (MODE != 0) { v0 = v[0]; v1 = v[np]; v2i = v[2 * np]; }     // in flight while the column is walked
+        PairAcc a = column_force<MD_FORCE_U, MD_FORCE_D>(P, pos, ri, i);
         if (BONDS) bond_force<true>(P, pos, ri, i, a);
         if (MODE == 0 || MODE == 2) {
             double *f = P.frc + i;
-            f[0] = a.fx; f[P.N_pad] = a.fy; f[2 * (size_t)P.N_pad] = a.fz;
+            f[0] = a.fx; f[np] = a.fy; f[2 * np] = a.fz;
         }
         if (MODE == 2) {
-            double *v = P.vel[vc] + i;
-            v[0] += P.hdt * a.fx; v[P.N_pad] += P.hdt * a.fy; v[2 * (size_t)P.N_pad] += P.hdt * a.fz;
+            v[0] = v0 + P.hdt * a.fx; v[np] = v1 + P.hdt * a.fy; v[2 * np] = v2i + P.hdt * a.fz;
         }
         if (MODE == 1) {
-            double *v = P.vel[vc] + i;
-            const double vx = v[0] + P.dt * a.fx, vy = v[P.N_pad] + P.dt * a.fy, vz = v[2 * (size_t)P.N_pad] + P.dt * a.fz;
-            v[0] = vx; v[P.N_pad] = vy; v[2 * (size_t)P.N_pad] = vz;
+            const double vx = v0 + P.dt * a.fx, vy = v1 + P.dt * a.fy, vz = v2i + P.dt * a.fz;
+            v[0] = vx; v[np] = vy; v[2 * np] = vz;
             const double x = ri.x + P.dt * vx, y = ri.y + P.dt * vy, z = ri.z + P.dt * vz;
             st_pos(P.pos[pc ^ 1] + i, x, y, z);
             v2 = vx * vx + vy * vy + vz * vz;
