@@ -445,7 +445,7 @@ md_system *md_create_ex(const md_params *pp)
     if (p.force_variant != MD_FORCE_FULL_LIST && p.force_variant != MD_FORCE_NEWTON3_ATOMICS) { set_error("bad force_variant"); return nullptr; }
     if (p.force_variant == MD_FORCE_NEWTON3_ATOMICS) p.step_mode = MD_STEP_SPLIT;
     if (p.step_mode != MD_STEP_FUSED && p.step_mode != MD_STEP_SPLIT) { set_error("bad step_mode"); return nullptr; }
-    if (p.block_size == 0) p.block_size = 256;
+    if (p.block_size == 0) p.block_size = 128;     // measured best by a small margin (the paper: 3 % spread)
     if (p.block_size != 64 && p.block_size != 128 && p.block_size != 256 && p.block_size != 512) {
         set_error("block_size must be 64, 128, 256 or 512");
         return nullptr;
