@@ -57,25 +57,32 @@ __device__ __forceinline__ void tile_describe(const MdDev &P, const TileBox &B, 
         M.row[q].sh = (ysh + 1) | ((zsh + 1) << 2) | ((xshA + 1) << 4) | ((xshC + 1) << 6);
     }
     __syncthreads();
-    if (tid == 0) {
-        int off = 0, own = 0, k = 0;
-        for (int q = 0; q < B.nq; q++) {
-            M.row[q].off = off;
-            const int qy = q % B.nyq, qz = q / B.nyq;
-            if (qy >= 1 && qy <= B.ny && qz >= 1 && qz <= B.nz) {      // a row of the box itself
-                M.own_base[k] = M.row[q].g[1];
-                M.own_loc[k] = off + M.row[q].n[0];
-                M.own_pre[k] = own;
-                own += M.row[q].n[1];
-                k++;
-            }
-            off += M.row[q].n[0] + M.row[q].n[1] + M.row[q].n[2];
+    if (tid < 32) {
+        // prefix sums over the <= 25 tile rows by warp 0: tile offset of each row, and for the rows of the box itself
+        // (own rows) their rank k and the prefix of their lengths
+        const int q = tid;
+        const bool in = q < B.nq;
+        const int nA = in ? M.row[q].n[0] : 0, nB = in ? M.row[q].n[1] : 0, nC = in ? M.row[q].n[2] : 0;
+        const int qy = q % B.nyq, qz = q / B.nyq;
+        const bool own_row = in && qy >= 1 && qy <= B.ny && qz >= 1 && qz <= B.nz;
+        const int tot = nA + nB + nC, ownn = own_row ? nB : 0;
+        int inc = tot, oinc = ownn;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t1 = __shfl_up_sync(FULL_MASK, inc, o), t2 = __shfl_up_sync(FULL_MASK, oinc, o);
+            if (tid >= o) { inc += t1; oinc += t2; }
         }
-        for (; k <= TILE_OWN_MAX; k++) {
-            M.own_pre[k] = own;
-            if (k < TILE_OWN_MAX) { M.own_base[k] = 0; M.own_loc[k] = 0; }
+        const int off = inc - tot, opre = oinc - ownn;
+        const unsigned ownmask = __ballot_sync(FULL_MASK, own_row);
+        const int k = __popc(ownmask & ((1u << tid) - 1u)), nown_rows = __popc(ownmask);
+        const int T = __shfl_sync(FULL_MASK, inc, 31), n_own = __shfl_sync(FULL_MASK, oinc, 31);
+        if (in) M.row[q].off = off;
+        if (own_row) { M.own_base[k] = M.row[q].g[1]; M.own_loc[k] = off + nA; M.own_pre[k] = opre; }
+        if (tid >= nown_rows && tid <= TILE_OWN_MAX) {
+            M.own_pre[tid] = n_own;
+            if (tid < TILE_OWN_MAX) { M.own_base[tid] = 0; M.own_loc[tid] = 0; }
         }
-        M.n_own = own; M.T = off; M.nq = B.nq; M.pad = 0;
+        if (tid == 0) { M.n_own = n_own; M.T = T; M.nq = B.nq; M.pad = 0; }
     }
     __syncthreads();
 }
