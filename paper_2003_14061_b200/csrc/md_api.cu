@@ -360,7 +360,7 @@ bool choose_tile(MdDev &P, size_t smem_optin)
     G.R = std::min(std::max(env_int("MD_TILE_R", 2), 1), 3);
     G.RZ = std::min(std::max(env_int("MD_TILE_RZ", 2), 1), 3);
     G.threads = env_int("MD_TILE_THREADS", per_cell > 8.0 ? 512 : 256);
-    if (G.threads != 128 && G.threads != 256 && G.threads != 512) { set_error("MD_TILE_THREADS must be 128, 256 or 512"); return false; }
+    if (G.threads < 64 || G.threads > 512 || G.threads % 32) { set_error("MD_TILE_THREADS must be a multiple of 32 in [64, 512]"); return false; }
     int S = env_int("MD_TILE_S", 0);
     if (S <= 0) S = (int)lround(0.8 * G.threads / (G.R * G.RZ * per_cell));
     S = std::min(std::max(S, 1), nc);
@@ -377,7 +377,6 @@ bool choose_tile(MdDev &P, size_t smem_optin)
     G.cap = cap;
     if (mean > 0.8 * cap) { set_error("tiled W: %.0f atoms per tile exceed the 13-bit tile index; use MD_FLAG_GLOBAL_W or smaller MD_TILE_S", mean); return false; }
     if (mdk_tile_smem(G, true) > smem_optin) { set_error("tiled W: tile of %d atoms does not fit shared memory", cap); return false; }
-    if (mdk_tile_configure(P) != 0) { set_error("tiled W: cudaFuncSetAttribute failed: %s", cudaGetErrorString(cudaGetLastError())); return false; }
     return true;
 }
 
@@ -521,6 +520,11 @@ md_system *md_create_ex(const md_params *pp)
         const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
         P.tiled = fits && want_tiled ? 1 : 0;
+        if (fits && mdk_tile_configure(P) != 0) {
+            set_error("tile kernels: %d threads per block not available for this W layout, or cudaFuncSetAttribute failed", P.tg.threads);
+            md_destroy(s);
+            return nullptr;
+        }
     } else if (p.flags & MD_FLAG_TILED_W) {
         set_error("MD_FLAG_TILED_W needs the full-list force variant and excludes MD_FLAG_GLOBAL_W");
         md_destroy(s);

@@ -230,9 +230,12 @@ __device__ __forceinline__ void tile_scan_run(const double *st, double xi, doubl
     }
 }
 
-template <int BLOCK, bool LOCALW>
-__global__ void __launch_bounds__(BLOCK) k_tile_build(const __grid_constant__ MdDev P)
+// The block size is a run-time value (any multiple of 32 up to 512): it is picked so that the own atoms of a box
+// fill the block's warps.
+template <bool LOCALW>
+__global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDev P)
 {
+    const int BLOCK = blockDim.x;
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     extern __shared__ double dsm[];
     __shared__ TileDesc M;
@@ -574,8 +577,6 @@ int configure_block(const MdDev &P)
 {
     const size_t sf = mdk_tile_smem(P.tg, false), sb = mdk_tile_smem(P.tg, true);
     int rc = 0;
-    rc |= opt_in(k_tile_build<BLOCK, true>, sb);
-    rc |= opt_in(k_tile_build<BLOCK, false>, sb);
     rc |= opt_in(k_tile_force<0, false, BLOCK>, sf);
     rc |= opt_in(k_tile_force<1, false, BLOCK>, sf);
     rc |= opt_in(k_tile_force<2, false, BLOCK>, sf);
@@ -607,6 +608,9 @@ void launch_force(const MdDev &P, int mode, cudaStream_t st)
 
 int mdk_tile_configure(const MdDev &P)
 {
+    const size_t sb = mdk_tile_smem(P.tg, true);
+    if (opt_in(k_tile_build<true>, sb) || opt_in(k_tile_build<false>, sb)) return -1;
+    if (!P.tiled) return 0;                          // the force / energy kernels exist for 128, 256 and 512 threads
     switch (P.tg.threads) {
     case 128: return configure_block<128>(P);
     case 256: return configure_block<256>(P);
@@ -619,15 +623,8 @@ void mdk_tile_build(const MdDev &P, cudaStream_t st)
 {
     const dim3 g = tile_grid3(P);
     const size_t sm = mdk_tile_smem(P.tg, true);
-#define MD_TB(B)                                                            \
-    if (P.tiled) k_tile_build<B, true><<<g, B, sm, st>>>(P);               \
-    else k_tile_build<B, false><<<g, B, sm, st>>>(P)
-    switch (P.tg.threads) {
-    case 128: MD_TB(128); break;
-    case 512: MD_TB(512); break;
-    default: MD_TB(256); break;
-    }
-#undef MD_TB
+    if (P.tiled) k_tile_build<true><<<g, P.tg.threads, sm, st>>>(P);
+    else k_tile_build<false><<<g, P.tg.threads, sm, st>>>(P);
 }
 
 void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st)
