@@ -566,10 +566,16 @@ namespace {
 inline int tile_grid(const MdDev &P) { return P.tg.nsx * P.tg.nsy * P.tg.nsz; }
 inline dim3 tile_grid3(const MdDev &P) { return dim3(P.tg.nsx, P.tg.nsy, P.tg.nsz); }
 
+// The attribute belongs to the kernel, not to one md_system: opt in to the device maximum, so that systems with
+// different tile capacities can coexist in a process.  `bytes` only checks that this system fits.
 template <typename K>
 int opt_in(K kernel, size_t bytes)
 {
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess ? 0 : -1;
+    int dev = 0, optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return -1;
+    optin -= 8192;                                   // room for the kernels' static shared memory (< 4 KB)
+    if (optin < 0 || (size_t)optin < bytes) return -1;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin) == cudaSuccess ? 0 : -1;
 }
 
 template <int BLOCK>

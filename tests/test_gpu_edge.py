@@ -148,3 +148,27 @@ def test_pinned_host_buffers_take_the_direct_copy_path(md):
     g2.set_state(r, v)
     g2.step(5)
     assert np.array_equal(g2.positions(), g.positions())
+
+
+def test_two_systems_with_different_tiles_coexist(md):
+    """The dynamic shared-memory opt-in is a property of the kernels, not of one system: a dense (large tile) and a
+    dilute (small tile) system must both keep working when alive at the same time."""
+    from oracle.md_oracle import OracleMD
+    big = scaled_config("lj_1m", 4 * 12 ** 3)
+    small = get_config("wca_4k")
+    systems = []
+    for cfg in (big, small, big):
+        r, v, _, box = make_state(cfg, 1, jitter_amp=0.1)
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+        g.set_state(r, v)
+        o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+        o.set_state(r, v)
+        systems.append((g, o, box))
+    for g, o, box in systems:
+        g.step(10)
+        o.step(10)
+    for g, o, box in systems:
+        d = g.positions() - o.positions()
+        d -= box * np.round(d / box)
+        assert np.abs(d).max() <= 1e-9
+        g.close()
