@@ -102,6 +102,21 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def replica_seed(rank: int) -> int:
+    """Replicas only: every rank runs an independent system; only the seed differs."""
+    return 1 + rank
+
+
+def max_over_ranks(x: float, dist, device) -> float:
+    """The one collective of the multi-GPU path: the timed region of the job is that of its slowest replica."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def oracle_rate(cfg, seed, budget_s, steps=None, n_atoms=None):
     """Time the oracle as it stands on a bounded sample: returns (atom-steps/s, sample text, threads, steps, N)."""
     from oracle.md_oracle import OracleMD, get_threads
@@ -178,6 +193,8 @@ def main():
     ap.add_argument("--variant", default="full", choices=["full", "newton3"])
     ap.add_argument("--mode", default="fused", choices=["fused", "split"])
     ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--systems", type=int, default=1,
+                    help="batch of independent systems of the workload run by the same launches (md_params.n_systems)")
     ap.add_argument("--flags", type=int, default=0, help="md_params.flags: 1 = no CUDA graph, 2 = global-index W layout")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -211,15 +228,19 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    seed = 1 + rank
-    r0, v0, bonds, box = make_state(cfg, seed)
+    seed = replica_seed(rank)
+    nsys = max(1, args.systems)
+    states = [make_state(cfg, seed + 1000 * b) for b in range(nsys)]
+    box = states[0][3]
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=args.variant,
-                    step_mode=args.mode if args.variant == "full" else "split", block_size=args.block, flags=args.flags)
-    g.set_state(r0, v0)
-    if bonds is not None:
-        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+                    step_mode=args.mode if args.variant == "full" else "split", block_size=args.block, flags=args.flags,
+                    n_systems=nsys)
+    g.set_state(np.concatenate([s[0] for s in states]), np.concatenate([s[1] for s in states]))
+    if states[0][2] is not None:
+        g.set_bonds(np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)]), cfg.fene_k, cfg.fene_r0)
+    del states
     info = g.info()
-    n = cfg.n_atoms
+    n = cfg.n_atoms * nsys                  # atoms advanced per step
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps --------------------------
     g.step(args.warmup)
@@ -241,10 +262,7 @@ def main():
     info_end = g.info()
     launches = info_end["kernel_launches"] - launches0
     e_end = g.energies()
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     value = world * n * args.steps / (ms * 1e-3)
 
     # ---- per-kernel-class device timers over a second pass of K steps (Table 2 of the paper; roofline) ----
@@ -287,6 +305,25 @@ def main():
                 "compulsory_bytes_per_atom": floor_bytes,
                 "timing": "CUDA events on the library's stream around each launch (md_set_profiling), second pass of K steps"}
     nebr = timers["nebr"]
+    # the neighbor-matrix build on its own: 5 forced rebuilds, each exactly one working launch of the build kernel
+    g.set_profiling(True)
+    g.reset_timers()
+    for _ in range(5):
+        g.rebuild_neighbors()
+    tb = g.timers()["nebr"]
+    g.set_profiling(False)
+    build_ms = tb["ms"] / max(1, tb["launches"])
+    cand = 27.0 * (n / nsys) / info["cells_per_edge"] ** 3                   # candidates examined per atom (27-cell stencil)
+    nb_floor = 24.0 + w_bytes * mbar + 4.0                            # r_i + W written + m_i
+    nb_ns = nb_floor + 24.0 * cand                                    # + 24 B per candidate position read
+    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else "k_build",
+                         "avg_launch_ms": build_ms, "candidates_per_atom": cand,
+                         "achieved": nb_ns * n / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": nb_ns * n / (build_ms * 1e-3) / 1e9 / peak,
+                         "frac_compulsory": nb_floor * n / (build_ms * 1e-3) / 1e9 / peak,
+                         "algorithmic_bytes_per_atom": nb_ns, "compulsory_bytes_per_atom": nb_floor,
+                         "accounting": "north_star style: every candidate position charged 24 B (they are read from the "
+                                       "shared-memory tile); the kernel is instruction-issue bound, not HBM bound"}
     breakdown = {k: round(v["ms"] / args.steps, 6) for k, v in timers.items()}
     nebr_info = {"rebuilds": int(rebuilds_prof), "ms_per_rebuild": nebr["ms"] / max(1, rebuilds_prof),
                  "steps_per_rebuild": args.steps / max(1, rebuilds_prof)}
@@ -311,10 +348,7 @@ def main():
             vh, vout = vout, vh
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dist, "cuda")
         e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
                "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
                "what": "md_set_state(pinned host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
@@ -325,7 +359,7 @@ def main():
         return
 
     cpu = None
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline and world == 1 and nsys == 1:
         rate, sample, cores, _, _ = oracle_rate(cfg, 1, args.cpu_seconds)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
@@ -333,7 +367,8 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "n_atoms": n, "lattice": cfg.lattice, "density": cfg.density,
+        "config": {"workload": cfg.name if nsys == 1 else f"{nsys} x {cfg.name}", "n_atoms": n, "n_systems": nsys,
+                   "lattice": cfg.lattice, "density": cfg.density,
                    "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
                    "force_variant": args.variant, "step_mode": args.mode, "block_size": info["block_size"],
                    "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
@@ -341,7 +376,7 @@ def main():
                    "cuda_graph": bool(info_end["use_graph"]),
                    "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                    "l2": "working set per step (positions 2x64 MB, velocities 48 MB, W rows ~100 MB) exceeds the 126 MB L2; no flush"},
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": roofline, "roofline_neighbor": roofline_neighbor, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "wall_s": t_wall, "rebuilds_in_timed_region": int(e_end.n_rebuilds - e_start.n_rebuilds),
         "energy_per_atom": {"start": e_start.total / n, "end": e_end.total / n},
         "temperature_end": e_end.ke / (1.5 * (n - 1)),

@@ -84,6 +84,13 @@ typedef struct md_params {
     int32_t  device;         /* CUDA device ordinal; -1 = current */
     void    *stream;         /* cudaStream_t to run on; NULL = the library creates its own */
     uint32_t flags;          /* MD_FLAG_* */
+    int32_t  n_systems;      /* batch of independent, mutually invisible systems run by the same kernel launches
+                                ("many separate simulations within a single run" to fill the GPU with
+                                small systems); 0 or 1 = one.  n_atoms, box, density are PER SYSTEM; every per-atom
+                                array at this boundary then has n_systems * n_atoms rows, system-major, and atom ids
+                                (bond lists, md_get_neighbors) are global: id = system * n_atoms + i.  System b starts
+                                from the same lattice with velocity seed + b.  One rebuild decision (the largest
+                                velocity of any system) serves all; md_energies returns sums over all systems. */
 } md_params;
 
 enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying a captured CUDA graph */
@@ -116,7 +123,7 @@ typedef struct md_energy {
 } md_energy;
 
 typedef struct md_info {
-    int64_t n_atoms, n_pad;     /* n_pad: row pitch of W (atoms rounded up to 128) */
+    int64_t n_atoms, n_pad;     /* n_atoms PER SYSTEM; n_pad: row pitch of W (all atoms, rounded up to 128) */
     double  box, r_neighbor, cell_width;
     int32_t cells_per_edge, max_neighbors, block_size, force_variant, step_mode, n_bonds_per_atom_max;
     int64_t device_bytes;       /* device memory held by this system */
@@ -127,7 +134,7 @@ typedef struct md_info {
     int32_t tile_capacity;      /* tiled: atoms the shared-memory tile can hold */
     int32_t tile_threads;       /* tiled: threads per block of the build / force kernels */
     int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node */
-    int32_t reserved_[1];
+    int32_t n_systems;
 } md_info;
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */

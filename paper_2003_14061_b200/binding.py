@@ -40,7 +40,7 @@ class _Params(C.Structure):
                 ("r_shell", C.c_double), ("dt", C.c_double), ("seed", C.c_uint64), ("temperature", C.c_double),
                 ("lattice", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
                 ("max_neighbors", C.c_int32), ("block_size", C.c_int32), ("device", C.c_int32),
-                ("stream", C.c_void_p), ("flags", C.c_uint32)]
+                ("stream", C.c_void_p), ("flags", C.c_uint32), ("n_systems", C.c_int32)]
 
 
 class _Energy(C.Structure):
@@ -57,7 +57,7 @@ class _Info(C.Structure):
                 ("n_bonds_per_atom_max", C.c_int32), ("device_bytes", C.c_int64), ("kernel_launches", C.c_int64),
                 ("device_name", C.c_char * 64), ("w_layout", C.c_int32), ("tile_cells", C.c_int32 * 3),
                 ("tile_capacity", C.c_int32), ("tile_threads", C.c_int32), ("use_graph", C.c_int32),
-                ("reserved_", C.c_int32 * 1)]
+                ("n_systems", C.c_int32)]
 
 
 @dataclass
@@ -159,7 +159,7 @@ class MDSystem:
 
     def __init__(self, n_atoms, r_cut, r_shell, dt, box=0.0, density=0.0, seed=1, temperature=1.0, lattice="auto",
                  force_variant="full", step_mode="fused", max_neighbors=0, block_size=0, device=-1,
-                 torch_memory=True, flags=0):
+                 torch_memory=True, flags=0, n_systems=1):
         import torch
         if not torch.cuda.is_available():
             raise MDError(MD_ERR_CUDA, "no CUDA device: the MD path has no CPU fallback")
@@ -172,12 +172,13 @@ class MDSystem:
         p.seed, p.temperature = int(seed), temperature
         p.lattice, p.force_variant, p.step_mode = LATTICE[lattice], FORCE_VARIANT[force_variant], STEP_MODE[step_mode]
         p.max_neighbors, p.block_size, p.device, p.flags = max_neighbors, block_size, device, flags
+        p.n_systems = int(n_systems)
         p.stream = torch.cuda.current_stream().cuda_stream or None
         self._L = L
         self._h = L.md_create_ex(C.byref(p))
         if not self._h:
             raise MDError(MD_ERR_INVALID, _err(L))
-        self.n = int(n_atoms)
+        self.n = int(n_atoms) * int(n_systems)          # rows of every per-atom array at the boundary
 
     @classmethod
     def from_config(cls, cfg, **kw):
@@ -258,7 +259,7 @@ class MDSystem:
         d = {k: getattr(i, k) for k, _ in _Info._fields_}
         d["device_name"] = d["device_name"].decode()
         d["tile_cells"] = list(d["tile_cells"])
-        d.pop("reserved_", None)
+
         return d
 
     def set_profiling(self, on: bool):

@@ -352,7 +352,7 @@ int env_int(const char *name, int dflt)
 // Box of cells per thread block, block size and tile capacity of the tiled W layout (md_types.h: TileGeom).
 // Defaults aim at ~0.8 own atoms per thread and a 2 x 2 cross-section in y, z (halo factor ~4.5 for the WCA
 // configs); MD_TILE_S / _R / _RZ / _THREADS / _CAP override them for tuning runs.
-bool choose_tile(MdDev &P, size_t smem_optin)
+bool choose_tile(MdDev &P, size_t smem_optin, bool for_tiled_w)
 {
     TileGeom &G = P.tg;
     const int nc = P.nc;
@@ -367,8 +367,16 @@ bool choose_tile(MdDev &P, size_t smem_optin)
     G.nsx = (nc + S - 1) / S;
     G.S = (nc + G.nsx - 1) / G.nsx;                 // balance the boxes along x
     G.nsx = (nc + G.S - 1) / G.S;
+    if (!env_int("MD_TILE_THREADS", 0)) {
+        // small boxes (few cells per edge): S was clipped to the row, so shrink the block to the atoms a box owns
+        const double own = (double)G.S * G.R * G.RZ * per_cell;
+        int t = 32 * (int)ceil(1.12 * own / 32.0);
+        if (for_tiled_w) t = t <= 128 ? 128 : (t <= 256 ? 256 : 512);      // instantiated sizes of the tiled force kernels
+        G.threads = std::min(G.threads, std::max(64, t));
+    }
     G.nsy = (nc + G.R - 1) / G.R;
     G.nsz = (nc + G.RZ - 1) / G.RZ;
+    G.nsys = P.n_sys;
     const double mean = (double)(G.S + 2) * (G.R + 2) * (G.RZ + 2) * per_cell;
     int cap = env_int("MD_TILE_CAP", 0);
     if (cap <= 0) cap = (int)(1.35 * mean + 6.0 * sqrt(mean) + 32.0);
@@ -424,7 +432,8 @@ md_system *md_create_ex(const md_params *pp)
 {
     if (!pp) { set_error("md_create_ex: null params"); return nullptr; }
     md_params p = *pp;
-    if (p.n_atoms <= 0 || p.n_atoms >= (1ll << 29)) { set_error("n_atoms must be in [1, 2^29)"); return nullptr; }
+    if (p.n_systems <= 0) p.n_systems = 1;
+    if (p.n_atoms <= 0 || p.n_atoms * p.n_systems >= (1ll << 29)) { set_error("n_atoms * n_systems must be in [1, 2^29)"); return nullptr; }
     if (!(p.r_cut > 0) || !(p.r_shell >= 0) || !(p.dt > 0) || !(p.temperature >= 0)) {
         set_error("r_cut, dt must be > 0; r_shell, temperature >= 0");
         return nullptr;
@@ -453,7 +462,7 @@ md_system *md_create_ex(const md_params *pp)
     int nc = (int)floor(p.box / rn);
     if (nc >= 1 && p.box / nc - rn < 1e-9 * rn) nc -= 1;     // keep the cell strictly wider than r_n
     if (nc < 3) { set_error("box too small: %d cells per edge (need >= 3)", nc); return nullptr; }
-    if ((int64_t)nc * nc * nc > (1ll << 30)) { set_error("too many cells"); return nullptr; }
+    if ((int64_t)nc * nc * nc * std::max(1, p.n_systems) > (1ll << 30)) { set_error("too many cells"); return nullptr; }
     if (p.max_neighbors <= 0) {
         const double ideal = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         p.max_neighbors = 16 * (int)ceil((1.35 * ideal + 12.0) / 16.0);
@@ -491,11 +500,14 @@ md_system *md_create_ex(const md_params *pp)
 
     MdDev &P = s->P;
     memset(&P, 0, sizeof(P));
-    P.N = (int)p.n_atoms;
+    P.n_sys = p.n_systems;
+    P.N1 = (int)p.n_atoms;
+    P.N = P.N1 * P.n_sys;
     P.N_pad = (P.N + 127) & ~127;
     P.Mmax = p.max_neighbors;
     P.nc = nc;
-    P.NC = nc * nc * nc;
+    P.NC1 = nc * nc * nc;
+    P.NC = P.NC1 * P.n_sys;
     P.half_list = p.force_variant == MD_FORCE_NEWTON3_ATOMICS;
     P.scan_blocks = (P.NC + 2047) / 2048;
     P.L = p.box; P.half_L = 0.5 * p.box; P.inv_w = (double)nc / p.box;
@@ -511,14 +523,14 @@ md_system *md_create_ex(const md_params *pp)
     P.tile_build = 0;
     if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
         // shared-memory staged neighbor build (both W layouts); the tiled W layout only on request
-        const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin);
+        const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
+        const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
+        const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin, want_tiled);
         if (!fits && (p.flags & MD_FLAG_TILED_W)) { md_destroy(s); return nullptr; }
         P.tile_build = fits ? 1 : 0;
         // W layout: measured on B200, tile-local W wins once a column of W is long enough
         // to amortise staging the tile (LJ r_c = 2.5: 76 neighbors, +17 %) and loses for the short WCA columns
         // (12 neighbors, -17 %).  Estimated mean column length = ideal-gas count in the neighbor sphere.
-        const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
-        const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
         P.tiled = fits && want_tiled ? 1 : 0;
         if (fits && mdk_tile_configure(P) != 0) {
             set_error("tile kernels: %d threads per block not available for this W layout, or cudaFuncSetAttribute failed", P.tg.threads);
@@ -535,7 +547,7 @@ md_system *md_create_ex(const md_params *pp)
         if (P.tiled) { set_error("MD_FLAG_W_TRANSPOSED applies to the global-index W layout only"); md_destroy(s); return nullptr; }
         P.w_row = 1; P.w_col = P.Mmax;
     }
-    P.max_grid = std::max((P.N + 63) / 64, P.tile_build ? P.tg.nsx * P.tg.nsy * P.tg.nsz : 0);
+    P.max_grid = std::max((P.N + 63) / 64, P.tile_build ? P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys : 0);
 
     const size_t np = (size_t)P.N_pad;
     bool ok = true;
@@ -556,7 +568,7 @@ md_system *md_create_ex(const md_params *pp)
     P.W = (int *)A((size_t)(P.tiled ? P.Mmax / 2 : P.Mmax) * np * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
     P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
-    if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * sizeof(TileDesc));
+    if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
     if (!ok) { set_error("device allocation failed (%.1f MB so far)", s->bytes / 1048576.0); md_destroy(s); return nullptr; }
@@ -566,12 +578,15 @@ md_system *md_create_ex(const md_params *pp)
 
     if (p.lattice != MD_LATTICE_NONE) {
         std::vector<double> xyz(3 * (size_t)P.N), v(3 * (size_t)P.N);
-        if (!md_init_lattice(p.lattice, p.n_atoms, p.box, xyz.data())) {
-            set_error("n_atoms = %lld does not fit lattice %d", (long long)p.n_atoms, p.lattice);
-            md_destroy(s);
-            return nullptr;
+        for (int b = 0; b < P.n_sys; b++) {      // every system: the same lattice, its own velocities (seed + b)
+            const size_t o = 3 * (size_t)b * P.N1;
+            if (!md_init_lattice(p.lattice, p.n_atoms, p.box, xyz.data() + o)) {
+                set_error("n_atoms = %lld does not fit lattice %d", (long long)p.n_atoms, p.lattice);
+                md_destroy(s);
+                return nullptr;
+            }
+            md_init_velocities(p.n_atoms, p.temperature, p.seed + (uint64_t)b, v.data() + o);
         }
-        md_init_velocities(p.n_atoms, p.temperature, p.seed, v.data());
         if (upload_state(s, xyz.data(), v.data()) != MD_OK) { md_destroy(s); return nullptr; }
     } else if (cudaStreamSynchronize(s->stream) != cudaSuccess) {
         return fail("cudaStreamSynchronize");
@@ -756,7 +771,7 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
         // rebuild every block's tile layout from cell_start exactly as the kernels do (md_tile.cu: tile_setup)
         std::vector<int> cs((size_t)P.NC + 1), map;
         CK(cudaMemcpy(cs.data(), P.cell_start, cs.size() * sizeof(int), cudaMemcpyDeviceToHost));
-        const int nblocks = P.tg.nsx * P.tg.nsy * P.tg.nsz;
+        const int nblocks = P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys;
         for (int b = 0; b < nblocks; b++) {
             const TileBox B = tile_box(P.tg, P.nc, b);
             map.clear();
@@ -800,7 +815,7 @@ int md_get_info(md_system *s, md_info *out)
 {
     if (!s || !out) { set_error("md_get_info: null argument"); return MD_ERR_INVALID; }
     memset(out, 0, sizeof(*out));
-    out->n_atoms = s->P.N; out->n_pad = s->P.N_pad;
+    out->n_atoms = s->P.N1; out->n_pad = s->P.N_pad; out->n_systems = s->P.n_sys;
     out->box = s->P.L; out->r_neighbor = s->r_n; out->cell_width = s->cell_w;
     out->cells_per_edge = s->P.nc; out->max_neighbors = s->P.Mmax; out->block_size = s->lc.block;
     out->force_variant = s->prm.force_variant; out->step_mode = s->prm.step_mode;

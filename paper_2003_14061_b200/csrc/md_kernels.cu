@@ -129,11 +129,14 @@ __global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_src)];
+    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_src)];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
         const pos_t r = ld_pos(pos + i);
         const int cx = cell_coord(wrap1(r.x, P.L), P.inv_w, P.nc), cy = cell_coord(wrap1(r.y, P.L), P.inv_w, P.nc),
                   cz = cell_coord(wrap1(r.z, P.L), P.inv_w, P.nc);
-        const int c = cx + P.nc * (cy + P.nc * cz);
+        // batched independent systems: each has its own block of cells, found from the permanent id
+        const int sys = P.n_sys > 1 ? __ldg(idv + i) / P.N1 : 0;
+        const int c = sys * P.NC1 + cx + P.nc * (cy + P.nc * cz);
         P.cell_of[i] = c;
         P.slot[i] = atomicAdd(&P.cell_count[c], 1);  // l_i; "incrementing k_c requires an atomic operation" (N2)
     }
@@ -332,6 +335,7 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
     __shared__ int ssum[4];
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
     const int *__restrict__ cs = P.cell_start;
+    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
     const int nc = P.nc;
     const double L = P.L;
     int tmax = 0, tsum = 0;
@@ -339,6 +343,7 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
         const pos_t ri = ld_pos(pos + i);
         const int cx = cell_coord(ri.x, P.inv_w, nc), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
         const int xa = cx == 0 ? 0 : cx - 1, xb = cx == nc - 1 ? nc - 1 : cx + 1;
+        const int cell_base = P.n_sys > 1 ? (__ldg(idv + i) / P.N1) * P.NC1 : 0;     // the atom's own system of cells
         int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
             int z = cz + dz;
@@ -350,7 +355,7 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
                 double sy = 0.0;
                 unsigned fl = fz;
                 if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
-                const int row = nc * (y + nc * z);
+                const int row = cell_base + nc * (y + nc * z);
                 const int b = __ldg(cs + row + xa), e = __ldg(cs + row + xb + 1);
                 if (fl) scan_run<HALF, true>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m);
                 else scan_run<HALF, false>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m);

@@ -546,7 +546,7 @@ __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ M
         q[RED_PX] += vx; q[RED_PY] += vy; q[RED_PZ] += vz;
         q[RED_VMAX2] = fmax(q[RED_VMAX2], w2);
     }
-    reduce_finish(P, q, S, bid, P.tg.nsx * P.tg.nsy * P.tg.nsz);
+    reduce_finish(P, q, S, bid, P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys);
 }
 
 }  // namespace
@@ -563,8 +563,8 @@ size_t mdk_tile_smem(const TileGeom &G, bool with_cells)
 
 namespace {
 
-inline int tile_grid(const MdDev &P) { return P.tg.nsx * P.tg.nsy * P.tg.nsz; }
-inline dim3 tile_grid3(const MdDev &P) { return dim3(P.tg.nsx, P.tg.nsy, P.tg.nsz); }
+inline int tile_grid(const MdDev &P) { return P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys; }
+inline dim3 tile_grid3(const MdDev &P) { return dim3(P.tg.nsx, P.tg.nsy, P.tg.nsz * P.tg.nsys); }
 
 // The attribute belongs to the kernel, not to one md_system: opt in to the device maximum, so that systems with
 // different tile capacities can coexist in a process.  `bytes` only checks that this system fits.

@@ -45,7 +45,8 @@ enum { TK_INTEGRATE = 0, TK_ENERGY = 1, TK_FORCE = 2 };
 // into that tile + the 3 periodic-image flag bits of PAPER.md:163.
 struct TileGeom {
     int S, R, RZ;            // cells per box along x, y, z
-    int nsx, nsy, nsz;       // boxes per axis
+    int nsx, nsy, nsz;       // boxes per axis of ONE system
+    int nsys;                // independent systems stacked along the grid's z axis (box index bz = sys * nsz + local)
     int cap;                 // tile capacity in atoms (<= 8192: 13 index bits)
     int threads;             // block size of the tile kernels
 };
@@ -53,23 +54,28 @@ struct TileGeom {
 struct TileBox {
     int x0, sxc, y0, ny, z0, nz;   // first cell and number of cells of the box along each axis
     int nyq, nq;                   // tile rows per z plane (ny + 2) and in total
+    int cell_base;                 // index of the first cell of the system the box belongs to (batched systems)
 };
 
 __host__ __device__ inline TileBox tile_box(const TileGeom &G, int nc, int b)
 {
     TileBox B;
-    const int bx = b % G.nsx, by = (b / G.nsx) % G.nsy, bz = b / (G.nsx * G.nsy);
+    const int bx = b % G.nsx, by = (b / G.nsx) % G.nsy, bzg = b / (G.nsx * G.nsy);
+    const int sys = bzg / G.nsz, bz = bzg - sys * G.nsz;
     B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
     B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
     B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
     B.nyq = B.ny + 2;
     B.nq = B.nyq * (B.nz + 2);
+    B.cell_base = sys * nc * nc * nc;
     return B;
 }
 
-__host__ __device__ inline TileBox tile_box3(const TileGeom &G, int nc, int bx, int by, int bz)
+__host__ __device__ inline TileBox tile_box3(const TileGeom &G, int nc, int bx, int by, int bzg)
 {
     TileBox B;
+    const int sys = bzg / G.nsz, bz = bzg - sys * G.nsz;
+    B.cell_base = sys * nc * nc * nc;
     B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
     B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
     B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
@@ -87,7 +93,7 @@ __host__ __device__ inline void tile_row(const TileBox &B, int nc, int q, int &r
     ysh = 0; zsh = 0;
     if (y < 0) { y += nc; ysh = 1; } else if (y >= nc) { y -= nc; ysh = -1; }
     if (z < 0) { z += nc; zsh = 1; } else if (z >= nc) { z -= nc; zsh = -1; }
-    rowc = nc * (y + nc * z);
+    rowc = B.cell_base + nc * (y + nc * z);
     xa = B.x0 == 0 ? nc - 1 : B.x0 - 1;
     xc = B.x0 + B.sxc == nc ? 0 : B.x0 + B.sxc;
 }
@@ -118,7 +124,8 @@ constexpr int TILE_ROW_INTS = 8;
 // The unvarying parameter block.  The paper copies it to constant memory; here it is a
 // __grid_constant__ kernel argument, which lives in the same constant bank without a separate copy.
 struct MdDev {
-    int N, N_pad, Mmax, nc, NC;
+    int N, N_pad, Mmax, nc, NC;         // N, NC: atoms and cells of ALL systems; nc: cells per edge of one
+    int n_sys, N1, NC1;                 // batched independent systems: count, atoms and cells of one
     int has_bonds, half_list, scan_blocks;
     int tiled, tile_build, max_grid;    // W layout (1 = MD_W_TILED); shared-memory staged build kernel in use; row pitch of `partials`
     TileGeom tg;

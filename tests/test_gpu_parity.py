@@ -275,3 +275,68 @@ def test_full_size_sampled_against_definitions(md, name):
         fb, _, _ = brute_forces_sample(pos, box, cfg.r_cut, idx)
         assert force_rel_err(g.forces()[idx], fb) <= FORCE_RTOL
     g.close()
+
+
+@pytest.mark.parametrize("case,n_sys", [("wca_ragged_1000", 5), ("wca_4k", 3), ("lj_6912", 2), ("chains_4096", 2)])
+@pytest.mark.parametrize("variant", ["full", "full-globalw", "full-tiledw", "newton3"])
+def test_batched_independent_systems(md, case, n_sys, variant):
+    """n_systems mutually invisible systems in one set of kernel launches: every system must follow its
+    own oracle exactly as if it were alone -- neighbor sets exact (global ids), forces 1e-10, 10 steps 1e-9."""
+    cfg, _ = small_cases()[case]
+    n = cfg.n_atoms
+    states = [make_state(cfg, 10 + b, jitter_amp=0.12 if cfg.lattice != "chains" else 0.0) for b in range(n_sys)]
+    box = states[0][3]
+    kw = {}
+    fv = variant
+    if variant == "full-globalw":
+        fv, kw = "full", dict(flags=md.FLAG_GLOBAL_W)
+    elif variant == "full-tiledw":
+        fv, kw = "full", dict(flags=md.FLAG_TILED_W)
+    g = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=fv,
+                    step_mode="fused" if fv == "full" else "split", n_systems=n_sys, **kw)
+    g.set_state(np.concatenate([s[0] for s in states]), np.concatenate([s[1] for s in states]))
+    oracles = []
+    for b, (r, v, bonds, _) in enumerate(states):
+        o = OracleMD(n, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+        o.set_state(r, v)
+        if bonds is not None:
+            assert o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0) == 0
+        oracles.append(o)
+    if states[0][2] is not None:
+        g.set_bonds(np.concatenate([s[2] + b * n for b, s in enumerate(states)]), cfg.fene_k, cfg.fene_r0)
+    assert g.info()["n_systems"] == n_sys and g.info()["n_atoms"] == n
+    counts, lst = g.neighbors()
+    fg = g.forces()
+    for b, o in enumerate(oracles):
+        sl = slice(b * n, (b + 1) * n)
+        rows = np.where(lst[sl] >= 0, lst[sl] - b * n, -1)
+        assert ((rows < n) | (lst[sl] < 0)).all() and (rows[lst[sl] >= 0] >= 0).all()      # no partner in another system
+        nbad, first = sets_equal(counts[sl], rows, o)
+        assert nbad == 0, f"system {b}: neighbor sets differ for {nbad} atoms (first: atom {first})"
+        assert force_rel_err(fg[sl], o.forces()) <= FORCE_RTOL
+    g.step(10)
+    pg, eg = g.positions(), g.energies()
+    ke = pe = 0.0
+    for b, o in enumerate(oracles):
+        assert o.step(10) == 0
+        assert pos_err(pg[b * n:(b + 1) * n], o.positions(), box) <= POS_ATOL
+        eo = o.energies()
+        ke, pe = ke + eo.ke, pe + eo.pe
+    assert eg.ke == pytest.approx(ke, rel=ENERGY_RTOL) and eg.pe == pytest.approx(pe, rel=ENERGY_RTOL)
+    g.close()
+
+
+def test_batched_systems_created_from_the_lattice(md):
+    cfg = get_config("wca_4k")
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, density=cfg.density, seed=5, temperature=1.0, n_systems=4)
+    r, v = g.positions(), g.velocities()
+    n = cfg.n_atoms
+    for b in range(4):
+        rb, vb, _, _ = make_state(cfg, 5 + b)
+        assert np.abs(r[b * n:(b + 1) * n] - rb).max() < 1e-12 and np.abs(v[b * n:(b + 1) * n] - vb).max() < 1e-12
+    e0 = g.energies()
+    assert e0.ke == pytest.approx(4 * 1.5 * (n - 1) * 1.0, rel=1e-12)          # every system at exactly T = 1
+    g.step(30)
+    e1 = g.energies()
+    assert abs(e1.total - e0.total) / (4 * n) < 2e-3 and e1.n_rebuilds >= 2
+    g.close()
