@@ -510,24 +510,45 @@ __global__ void __launch_bounds__(256) k_force_n3(const __grid_constant__ MdDev 
     if (i >= P.N) return;
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
     const pos_t ri = ld_pos(pos + i);
-    const int m = P.nnb[i];
     const int *__restrict__ w = P.W + (size_t)i * P.w_col;
+    const size_t pitch = (size_t)P.w_row;
     double *fx = P.frc, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
     PairAcc a = {0.0, 0.0, 0.0};
-#pragma unroll 2
-    for (int k = 0; k < m; k++) {
-        const unsigned en = (unsigned)__ldcs(w + (size_t)k * P.w_row);
-        const int j = (int)(en & W_INDEX_MASK);
-        const pos_t rj = ld_pos(pos + j);
-        double dx, dy, dz;
-        const double r2 = disp2(ri, rj, en >> W_FLAG_SHIFT, P.L, dx, dy, dz);
-        if (r2 < P.rc2) {
-            const double s = fast_rcp(r2), s3 = s * s * s;
-            const double fc = 48.0 * s3 * (s3 - 0.5) * s;
-            const double gx = fc * dx, gy = fc * dy, gz = fc * dz;
-            a.fx += gx; a.fy += gy; a.fz += gz;
-            atomicAdd(fx + j, -gx); atomicAdd(fy + j, -gy); atomicAdd(fz + j, -gz);
+    // same W prefetch as variant A (column_force): a block of D rows ahead, the first before the column length
+    constexpr int D = MD_FORCE_D, U = MD_FORCE_U;
+    unsigned cur[D], nxt[D];
+#pragma unroll
+    for (int d = 0; d < D; d++) cur[d] = d < P.Mmax ? (unsigned)__ldcs(w + d * pitch) : 0u;
+    const int m = P.nnb[i];
+    for (int base = 0; base < m; base += D) {
+#pragma unroll
+        for (int d = 0; d < D; d++) nxt[d] = base + D + d < m ? (unsigned)__ldcs(w + (base + D + d) * pitch) : 0u;
+#pragma unroll
+        for (int g = 0; g < D; g += U) {
+            if (base + g < m) {
+                pos_t rj[U];
+#pragma unroll
+                for (int u = 0; u < U; u++)
+                    if (base + g + u < m) rj[u] = ld_pos(pos + (cur[g + u] & W_INDEX_MASK));
+#pragma unroll
+                for (int u = 0; u < U; u++)
+                    if (base + g + u < m) {
+                        const unsigned en = cur[g + u];
+                        const int j = (int)(en & W_INDEX_MASK);
+                        double dx, dy, dz;
+                        const double r2 = disp2(ri, rj[u], en >> W_FLAG_SHIFT, P.L, dx, dy, dz);
+                        if (r2 < P.rc2) {
+                            const double s = fast_rcp(r2), s3 = s * s * s;
+                            const double fc = 48.0 * s3 * (s3 - 0.5) * s;
+                            const double gx = fc * dx, gy = fc * dy, gz = fc * dz;
+                            a.fx += gx; a.fy += gy; a.fz += gz;
+                            atomicAdd(fx + j, -gx); atomicAdd(fy + j, -gy); atomicAdd(fz + j, -gz);
+                        }
+                    }
+            }
         }
+#pragma unroll
+        for (int d = 0; d < D; d++) cur[d] = nxt[d];
     }
     if (BONDS) bond_force<true>(P, pos, ri, i, a);
     atomicAdd(fx + i, a.fx); atomicAdd(fy + i, a.fy); atomicAdd(fz + i, a.fz);
