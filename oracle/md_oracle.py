@@ -1,4 +1,5 @@
-"""ctypes front end of the CPU oracle (oracle/md_oracle.c).  TEST INFRASTRUCTURE ONLY.
+"""ctypes front end of the CPU oracles (oracle/md_oracle.c, fp64; oracle/md_oracle_sp.c, the single-precision
+variant of SURVEY.md 8(f) NEXT-1).  TEST INFRASTRUCTURE ONLY.
 
 Imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 `--impl reference` legs -- never by the product package.  Shares nothing with
@@ -16,14 +17,17 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "md_oracle.c")
 _LIB = os.path.join(_HERE, "libmd_oracle.so")
+_SRC_SP = os.path.join(_HERE, "md_oracle_sp.c")
+_LIB_SP = os.path.join(_HERE, "libmd_oracle_sp.so")
 
 
 def build(force: bool = False) -> str:
     """gcc -O2 build of the oracle (fp contraction off: every a*b+c rounds twice unless written fma())."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-std=c11", "-O2", "-march=native", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
-               "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
-        subprocess.run(cmd, check=True, cwd=_HERE)
+    for src, out in ((_SRC, _LIB), (_SRC_SP, _LIB_SP)):
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+            cmd = ["gcc", "-std=c11", "-O2", "-march=native", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+                   "-fPIC", "-shared", "-o", out, src, "-lm"]
+            subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
 
@@ -66,40 +70,69 @@ _ip = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
 _lp = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
 
 
+class _Prefixed:
+    """The functions of one oracle library under prefix-free names (orc_* / orcs_* share one signature set)."""
+
+    def __init__(self, L, prefix):
+        self._L, self._p = L, prefix
+
+    def __getattr__(self, name):
+        return getattr(self._L, self._p + name)
+
+
+def _declare_system_api(L, p):
+    f = lambda n: getattr(L, p + n)
+    f("create").restype = C.c_void_p
+    f("create").argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double]
+    f("destroy").argtypes = [C.c_void_p]
+    f("force_brute_search").argtypes = [C.c_void_p, C.c_int]
+    f("set_state").argtypes = [C.c_void_p, _dp, C.c_void_p]
+    f("set_bonds").argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
+    f("set_bonds").restype = C.c_int
+    f("rebuild_neighbors").argtypes = [C.c_void_p]
+    f("step").argtypes = [C.c_void_p, C.c_int64]
+    f("step").restype = C.c_int
+    f("energies").argtypes = [C.c_void_p, C.POINTER(_Energy)]
+    for name in ("get_positions", "get_velocities", "get_forces", "set_velocities"):
+        f(name).argtypes = [C.c_void_p, _dp]
+    f("get_atom_energies").argtypes = [C.c_void_p, _dp, _dp]
+    f("neighbor_total").argtypes = [C.c_void_p]
+    f("neighbor_total").restype = C.c_int64
+    f("get_neighbors").argtypes = [C.c_void_p, _ip, _ip]
+    f("set_threads").argtypes = [C.c_int]
+    f("get_threads").restype = C.c_int
+
+
+_lib_sp = None
+
+
+def lib_sp():
+    global _lib_sp
+    if _lib_sp is None:
+        build()
+        L = C.CDLL(_LIB_SP)
+        _declare_system_api(L, "orcs_")
+        _lib_sp = L
+    return _lib_sp
+
+
 def lib():
     global _lib
     if _lib is None:
         L = C.CDLL(build())
-        L.orc_create.restype = C.c_void_p
-        L.orc_create.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double]
-        L.orc_destroy.argtypes = [C.c_void_p]
-        L.orc_force_brute_search.argtypes = [C.c_void_p, C.c_int]
-        L.orc_set_state.argtypes = [C.c_void_p, _dp, C.c_void_p]
-        L.orc_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
-        L.orc_set_bonds.restype = C.c_int
-        L.orc_rebuild_neighbors.argtypes = [C.c_void_p]
-        L.orc_step.argtypes = [C.c_void_p, C.c_int64]
-        L.orc_step.restype = C.c_int
-        L.orc_energies.argtypes = [C.c_void_p, C.POINTER(_Energy)]
-        for name in ("orc_get_positions", "orc_get_velocities", "orc_get_forces", "orc_set_velocities"):
-            getattr(L, name).argtypes = [C.c_void_p, _dp]
-        L.orc_get_atom_energies.argtypes = [C.c_void_p, _dp, _dp]
-        L.orc_neighbor_total.argtypes = [C.c_void_p]
-        L.orc_neighbor_total.restype = C.c_int64
-        L.orc_get_neighbors.argtypes = [C.c_void_p, _ip, _ip]
+        _declare_system_api(L, "orc_")
         L.orc_brute_forces.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
         L.orc_brute_forces_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp, _dp, _dp, _dp]
         L.orc_brute_neighbors_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp,
                                                  C.c_int32, _ip, _ip]
         L.orc_brute_neighbors_sample.restype = C.c_int32
-        L.orc_set_threads.argtypes = [C.c_int]
-        L.orc_get_threads.restype = C.c_int
         _lib = L
     return _lib
 
 
 def set_threads(n: int) -> None:
     lib().orc_set_threads(int(n))
+    lib_sp().orcs_set_threads(int(n))
 
 
 def get_threads() -> int:
@@ -142,19 +175,24 @@ def brute_neighbors_sample(r, box, r_n, idx, cap=256):
 class OracleMD:
     """Plain CPU MD of the same model (see md_oracle.c header for the passages followed)."""
 
+    _prefix = "orc_"
+
+    def _load(self):
+        return lib()
+
     def __init__(self, n_atoms, box, r_cut, r_shell, dt, brute_search=False):
-        self._L = lib()
+        self._L = _Prefixed(self._load(), self._prefix)
         self.n = int(n_atoms)
         self.box, self.r_cut, self.r_shell, self.dt = float(box), float(r_cut), float(r_shell), float(dt)
-        self._h = self._L.orc_create(self.n, self.box, self.r_cut, self.r_shell, self.dt)
+        self._h = self._L.create(self.n, self.box, self.r_cut, self.r_shell, self.dt)
         if not self._h:
             raise ValueError("orc_create failed")
         if brute_search:
-            self._L.orc_force_brute_search(self._h, 1)
+            self._L.force_brute_search(self._h, 1)
 
     def close(self):
         if self._h:
-            self._L.orc_destroy(self._h)
+            self._L.destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -170,24 +208,24 @@ class OracleMD:
         if v is not None:
             v = _c(v)
             vp = v.ctypes.data_as(C.c_void_p)
-        self._L.orc_set_state(self._h, r, vp)
+        self._L.set_state(self._h, r, vp)
 
     def set_velocities(self, v):
-        self._L.orc_set_velocities(self._h, _c(v))
+        self._L.set_velocities(self._h, _c(v))
 
     def set_bonds(self, bonds, k, r0):
         b = _c(bonds, np.int32).reshape(-1, 2)
-        return self._L.orc_set_bonds(self._h, b.shape[0], b, float(k), float(r0))
+        return self._L.set_bonds(self._h, b.shape[0], b, float(k), float(r0))
 
     def rebuild_neighbors(self):
-        self._L.orc_rebuild_neighbors(self._h)
+        self._L.rebuild_neighbors(self._h)
 
     def step(self, n=1):
-        return self._L.orc_step(self._h, int(n))
+        return self._L.step(self._h, int(n))
 
     def energies(self) -> Energies:
         e = _Energy()
-        self._L.orc_energies(self._h, C.byref(e))
+        self._L.energies(self._h, C.byref(e))
         return Energies(**{k: getattr(e, k) for k, _ in _Energy._fields_})
 
     def _get(self, name):
@@ -196,28 +234,37 @@ class OracleMD:
         return out
 
     def positions(self):
-        return self._get("orc_get_positions")
+        return self._get("get_positions")
 
     def velocities(self):
-        return self._get("orc_get_velocities")
+        return self._get("get_velocities")
 
     def forces(self):
-        return self._get("orc_get_forces")
+        return self._get("get_forces")
 
     def atom_energies(self):
         u, w = np.empty(self.n), np.empty(self.n)
-        self._L.orc_get_atom_energies(self._h, u, w)
+        self._L.get_atom_energies(self._h, u, w)
         return u, w
 
     def neighbors(self):
         """(counts[N], flat list in CSR order)."""
-        tot = self._L.orc_neighbor_total(self._h)
+        tot = self._L.neighbor_total(self._h)
         counts = np.empty(self.n, np.int32)
         flat = np.empty(max(tot, 1), np.int32)
-        self._L.orc_get_neighbors(self._h, counts, flat)
+        self._L.get_neighbors(self._h, counts, flat)
         return counts, flat[:tot]
 
     def neighbor_sets(self):
         counts, flat = self.neighbors()
         off = np.concatenate([[0], np.cumsum(counts, dtype=np.int64)])
         return [np.sort(flat[off[i]:off[i + 1]]) for i in range(self.n)]
+
+
+class OracleMDSP(OracleMD):
+    """The single-precision variant (md_oracle_sp.c): binary32 state and pair arithmetic, binary64 energy sums.
+    Same interface; boundary arrays are float64 holding binary32 values."""
+    _prefix = "orcs_"
+
+    def _load(self):
+        return lib_sp()
