@@ -117,9 +117,11 @@ def max_over_ranks(x: float, dist, device) -> float:
     return float(t.item())
 
 
-def oracle_rate(cfg, seed, budget_s, steps=None, n_atoms=None):
+def oracle_rate(cfg, seed, budget_s, steps=None, n_atoms=None, precision="f64"):
     """Time the oracle as it stands on a bounded sample: returns (atom-steps/s, sample text, threads, steps, N)."""
-    from oracle.md_oracle import OracleMD, get_threads
+    from oracle.md_oracle import OracleMD, OracleMDSP, get_threads
+    if precision == "f32":
+        OracleMD = OracleMDSP
     scfg = cfg if not n_atoms or n_atoms == cfg.n_atoms else scaled_config(cfg.name, n_atoms)
     r, v, bonds, box = make_state(scfg, seed)
     o = OracleMD(scfg.n_atoms, box, scfg.r_cut, scfg.r_shell, scfg.dt)
@@ -145,11 +147,13 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle.md_oracle import OracleMD, get_threads
+    from oracle.md_oracle import OracleMD, OracleMDSP, get_threads
+    if args.precision == "f32":
+        OracleMD = OracleMDSP
     # calibrate on a small system, then pick the largest lattice that keeps (K + W) steps within ~150 s
     small = scaled_config(cfg.name, 32 ** 3) if cfg.lattice == "sc" else scaled_config(cfg.name, 4 * 16 ** 3) \
         if cfg.lattice == "fcc" else scaled_config(cfg.name, 64 * cfg.chain_len * 8)
-    rate0, _, _, _, _ = oracle_rate(small, 1, 2.0)
+    rate0, _, _, _, _ = oracle_rate(small, 1, 2.0, precision=args.precision)
     want = rate0 * 150.0 / max(1, args.steps + args.warmup)
     if cfg.lattice == "sc":
         side = int(min(round(cfg.n_atoms ** (1 / 3)), max(16, int(want ** (1 / 3)))))
@@ -172,15 +176,19 @@ def run_reference(args, cfg):
     value = scfg.n_atoms * args.steps / dt
     sample = f"each step = one oracle time step over N={scfg.n_atoms} atoms of {cfg.name}'s state point ({scfg.lattice} lattice start)"
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": metric_name(args), "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": cfg.n_atoms, "sample_n_atoms": scfg.n_atoms},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": get_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def metric_name(args):
+    return METRIC if args.precision == "f64" else "atom-timesteps/sec (fp32 state and pair arithmetic, fp64 energy sums)"
 
 
 def main():
@@ -196,6 +204,8 @@ def main():
     ap.add_argument("--systems", type=int, default=1,
                     help="batch of independent systems of the workload run by the same launches (md_params.n_systems)")
     ap.add_argument("--flags", type=int, default=0, help="md_params.flags: 1 = no CUDA graph, 2 = global-index W layout")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
+                    help="f32: the single-precision variant (md_params.precision = MD_PREC_F32; SURVEY 8(f) NEXT-1)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -234,7 +244,7 @@ def main():
     box = states[0][3]
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=args.variant,
                     step_mode=args.mode if args.variant == "full" else "split", block_size=args.block, flags=args.flags,
-                    n_systems=nsys)
+                    n_systems=nsys, precision=args.precision)
     g.set_state(np.concatenate([s[0] for s in states]), np.concatenate([s[1] for s in states]))
     if states[0][2] is not None:
         g.set_bonds(np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)]), cfg.fene_k, cfg.fene_r0)
@@ -276,22 +286,25 @@ def main():
     mbar = 0.5 * (e_end.mean_neighbors + e_prof.mean_neighbors)
     peak, peak_src = load_peaks()
     tiled = info["w_layout"] == 1
+    sp = args.precision == "f32"
+    rec = 16.0 if sp else 24.0               # bytes of one position / velocity / force record (float4 | 3 doubles)
     if args.mode == "fused" and args.variant == "full":
         tk = timers["fused_step"]
         if tiled:
             kname = "k_tile_force<fused step>"
             w_bytes = 2.0                        # 16-bit tile-local entries
         else:
-            kname = "k_force<fused step>"
+            kname = "k_sp_force<fused step>" if sp else "k_force<fused step>"
             w_bytes = 4.0
-        # W w*m + m_i 4 + r_i 24 + gathers 24m + v read+write 48 + r' write 24   (north_star's accounting)
-        bytes_per_atom = (w_bytes + 24.0) * mbar + 100.0
-        floor_bytes = w_bytes * mbar + 100.0
+        # W w*m + m_i 4 + r_i 24 + gathers 24m + v read+write 48 + r' write 24   (north_star's accounting);
+        # single precision: 16-byte float4 records instead of 24
+        bytes_per_atom = (w_bytes + rec) * mbar + 4.0 + 4.0 * rec
+        floor_bytes = w_bytes * mbar + 4.0 + 4.0 * rec
     else:
-        kname, tk = "k_force", timers["force"]
+        kname, tk = ("k_sp_force" if sp else "k_force"), timers["force"]
         w_bytes = 4.0
-        bytes_per_atom = 28.0 * mbar + 52.0      # SURVEY 8(d) B_ns: W 4m + m_i 4 + r_i 24 + gathers 24m + f write 24
-        floor_bytes = 4.0 * mbar + 52.0
+        bytes_per_atom = (4.0 + rec) * mbar + 4.0 + 2.0 * rec      # SURVEY 8(d) B_ns: W 4m + m_i 4 + r_i + gathers + f write
+        floor_bytes = 4.0 * mbar + 4.0 + 2.0 * rec
         if args.variant == "newton3":
             tk = dict(tk, launches=tk["launches"] // 2)
     dur_ms = tk["ms"] / max(1, tk["launches"])
@@ -300,7 +313,7 @@ def main():
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_atom": bytes_per_atom, "mean_neighbors": mbar, "avg_launch_ms": dur_ms,
-                "accounting": "north_star B_ns (every gather charged 24 B)",
+                "accounting": f"north_star B_ns (every gather charged {rec:.0f} B)",
                 "frac_compulsory": floor_bytes * n / (dur_ms * 1e-3) / 1e9 / peak,
                 "compulsory_bytes_per_atom": floor_bytes,
                 "timing": "CUDA events on the library's stream around each launch (md_set_profiling), second pass of K steps"}
@@ -314,9 +327,9 @@ def main():
     g.set_profiling(False)
     build_ms = tb["ms"] / max(1, tb["launches"])
     cand = 27.0 * (n / nsys) / info["cells_per_edge"] ** 3                   # candidates examined per atom (27-cell stencil)
-    nb_floor = 24.0 + w_bytes * mbar + 4.0                            # r_i + W written + m_i
-    nb_ns = nb_floor + 24.0 * cand                                    # + 24 B per candidate position read
-    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else "k_build",
+    nb_floor = rec + w_bytes * mbar + 4.0                             # r_i + W written + m_i
+    nb_ns = nb_floor + rec * cand                                     # + one record per candidate position read
+    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else ("k_sp_build" if sp else "k_build"),
                          "avg_launch_ms": build_ms, "candidates_per_atom": cand,
                          "achieved": nb_ns * n / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": nb_ns * n / (build_ms * 1e-3) / 1e9 / peak,
@@ -349,7 +362,7 @@ def main():
         barrier()
         dt = time.perf_counter() - t0
         dt = max_over_ranks(dt, dist, "cuda")
-        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
+        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT,  # the boundary arrays are double in both precisions "h2d_bytes_per_step": 2 * 3 * n * 8,
                "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
                "what": "md_set_state(pinned host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
 
@@ -360,17 +373,17 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline and world == 1 and nsys == 1:
-        rate, sample, cores, _, _ = oracle_rate(cfg, 1, args.cpu_seconds)
+        rate, sample, cores, _, _ = oracle_rate(cfg, 1, args.cpu_seconds, precision=args.precision)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": metric_name(args), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "dtype": args.precision, "data": "synthetic",
         "config": {"workload": cfg.name if nsys == 1 else f"{nsys} x {cfg.name}", "n_atoms": n, "n_systems": nsys,
                    "lattice": cfg.lattice, "density": cfg.density,
                    "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
-                   "force_variant": args.variant, "step_mode": args.mode, "block_size": info["block_size"],
+                   "force_variant": args.variant, "step_mode": args.mode, "precision": args.precision, "block_size": info["block_size"],
                    "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
                    "w_layout": "tiled16" if tiled else "global32", "tile_cells": info["tile_cells"],
                    "cuda_graph": bool(info_end["use_graph"]),

@@ -15,7 +15,8 @@
  * leapfrog; rebuild when the accumulated dt*max|v| exceeds r_shell/2) is fixed in DESIGN.md, "Readings".
  *
  * Conventions
- *   - Reduced units (sigma = epsilon = m = 1).  Cubic periodic box [0, L)^3.  All arithmetic is fp64.
+ *   - Reduced units (sigma = epsilon = m = 1).  Cubic periodic box [0, L)^3.  All arithmetic is fp64 unless
+ *     md_params.precision = MD_PREC_F32 selects the single-precision variant.
  *   - Every array argument is a HOST pointer owned by the caller unless its name ends in `_device`.
  *     Page-locked (cudaHostAlloc / cudaHostRegister) arrays are copied to and from directly on the stream;
  *     pageable ones go through a pinned staging buffer inside the library.
@@ -91,7 +92,14 @@ typedef struct md_params {
                                 (bond lists, md_get_neighbors) are global: id = system * n_atoms + i.  System b starts
                                 from the same lattice with velocity seed + b.  One rebuild decision (the largest
                                 velocity of any system) serves all; md_energies returns sums over all systems. */
+    int32_t  precision;      /* MD_PREC_F64 (default) or MD_PREC_F32: the paper's own precision with
+                                its float4 state arrays: coordinates, velocities, forces and the pair
+                                arithmetic in binary32, every sum of energies in binary64.  Boundary arrays stay double and
+                                are rounded to binary32 on entry; the box edge used is (float)box.  Variant A only
+                                (fused or split steps), global-index W. */
 } md_params;
+
+enum { MD_PREC_F64 = 0, MD_PREC_F32 = 1 };
 
 enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying a captured CUDA graph */
        MD_FLAG_GLOBAL_W = 2u, /* the paper's literal data path: W holds global atom indices and BOTH
@@ -135,6 +143,7 @@ typedef struct md_info {
     int32_t tile_threads;       /* tiled: threads per block of the build / force kernels */
     int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node */
     int32_t n_systems;
+    int32_t precision;          /* MD_PREC_* */
 } md_info;
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */

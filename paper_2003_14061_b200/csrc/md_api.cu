@@ -458,16 +458,23 @@ md_system *md_create_ex(const md_params *pp)
         set_error("block_size must be 64, 128, 256 or 512");
         return nullptr;
     }
+    if (p.precision != MD_PREC_F64 && p.precision != MD_PREC_F32) { set_error("bad precision"); return nullptr; }
+    const bool sp = p.precision == MD_PREC_F32;
+    if (sp && p.force_variant != MD_FORCE_FULL_LIST) { set_error("MD_PREC_F32 supports the full-list force variant only"); return nullptr; }
+    if (sp && (p.flags & MD_FLAG_TILED_W)) { set_error("MD_PREC_F32 uses the global-index W layout"); return nullptr; }
     const double rn = p.r_cut + p.r_shell;
-    int nc = (int)floor(p.box / rn);
-    if (nc >= 1 && p.box / nc - rn < 1e-9 * rn) nc -= 1;     // keep the cell strictly wider than r_n
+    // single precision: the box edge is the binary32 number, and cells keep a margin above the rounding error of a
+    // binary32 r^2 (~2e-7 relative) so that no accepted pair can lie outside the 27-cell stencil
+    const double box_eff = sp ? (double)(float)p.box : p.box;
+    int nc = (int)floor(box_eff / rn);
+    if (nc >= 1 && box_eff / nc - rn < (sp ? 1e-5 : 1e-9) * rn) nc -= 1;     // keep the cell strictly wider than r_n
     if (nc < 3) { set_error("box too small: %d cells per edge (need >= 3)", nc); return nullptr; }
     if ((int64_t)nc * nc * nc * std::max(1, p.n_systems) > (1ll << 30)) { set_error("too many cells"); return nullptr; }
     if (p.max_neighbors <= 0) {
         const double ideal = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         p.max_neighbors = 16 * (int)ceil((1.35 * ideal + 12.0) / 16.0);
     }
-    p.max_neighbors = (p.max_neighbors + 1) & ~1;          // W rows are stored in pairs in the tiled layout
+    p.max_neighbors = (p.max_neighbors + 3) & ~3;          // W rows are stored in pairs in the tiled layout, padded to fours in single precision
     if (p.lattice == MD_LATTICE_AUTO) {
         p.lattice = md_init_pick_lattice(p.n_atoms);
         if (!p.lattice) { set_error("n_atoms fits neither a simple-cubic nor an FCC lattice"); return nullptr; }
@@ -510,18 +517,24 @@ md_system *md_create_ex(const md_params *pp)
     P.NC = P.NC1 * P.n_sys;
     P.half_list = p.force_variant == MD_FORCE_NEWTON3_ATOMICS;
     P.scan_blocks = (P.NC + 2047) / 2048;
-    P.L = p.box; P.half_L = 0.5 * p.box; P.inv_w = (double)nc / p.box;
+    P.L = box_eff; P.half_L = 0.5 * box_eff; P.inv_w = (double)nc / box_eff;
+    P.sp = sp ? 1 : 0;
+    // padded columns pay once a column is long enough (measured: +14 % at 76 neighbors, -5 % at 12; md_sp.cu)
+    P.sp_pad = sp && 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density >= 32.0 ? 4 : 1;
+    P.Lf = (float)p.box; P.half_Lf = 0.5f * P.Lf;
+    P.rc2f = (float)(p.r_cut * p.r_cut); P.rn2f = (float)(rn * rn);
+    P.dtf = (float)p.dt; P.hdtf = (float)(0.5 * p.dt);
     P.rc2 = p.r_cut * p.r_cut;
     P.rn2 = rn * rn;
-    { const double sc = 1.0 / P.rc2, sc3 = sc * sc * sc; P.uc = 4.0 * sc3 * (sc3 - 1.0); }
+    { const double sc = 1.0 / P.rc2, sc3 = sc * sc * sc; P.uc = 4.0 * sc3 * (sc3 - 1.0); P.ucf = (float)P.uc; }
     P.dt = p.dt; P.hdt = 0.5 * p.dt; P.thresh = 0.5 * p.r_shell;
-    s->r_n = rn; s->cell_w = p.box / nc;
+    s->r_n = rn; s->cell_w = box_eff / nc;
     s->lc.block = p.block_size;
     s->lc.grid_atoms = (P.N + p.block_size - 1) / p.block_size;
 
     P.tiled = 0;
     P.tile_build = 0;
-    if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
+    if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W) && !sp) {
         // shared-memory staged neighbor build (both W layouts); the tiled W layout only on request
         const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
@@ -553,11 +566,17 @@ md_system *md_create_ex(const md_params *pp)
     bool ok = true;
     auto A = [&](size_t bytes) { void *q = dev_alloc(s, bytes); if (!q) ok = false; return q; };
     for (int k = 0; k < 2; k++) {
-        P.pos[k] = (pos_t *)A(np * sizeof(pos_t));
-        P.vel[k] = (double *)A(3 * np * sizeof(double));
+        if (sp) {
+            P.posf[k] = (float4 *)A(np * sizeof(float4));
+            P.velf[k] = (float4 *)A(np * sizeof(float4));
+        } else {
+            P.pos[k] = (pos_t *)A(np * sizeof(pos_t));
+            P.vel[k] = (double *)A(3 * np * sizeof(double));
+        }
         P.id[k] = (int *)A(np * sizeof(int));
     }
-    P.frc = (double *)A(3 * np * sizeof(double));
+    if (sp) P.frcf = (float4 *)A(np * sizeof(float4));
+    else P.frc = (double *)A(3 * np * sizeof(double));
     P.cell_of = (int *)A(np * sizeof(int));
     P.slot = (int *)A(np * sizeof(int));
     P.perm = (int *)A(np * sizeof(int));
@@ -605,7 +624,7 @@ md_system *md_create(int64_t n_atoms, double box, double density, double r_cut, 
 int md_set_state(md_system *s, const double *xyz, const double *vxyz)
 {
     if (!s || !xyz) { set_error("md_set_state: null argument"); return MD_ERR_INVALID; }
-    const double L = s->P.L;
+    const double L = s->prm.box;
     const size_t n3 = 3 * (size_t)s->P.N;
     int bad = 0;
     for (size_t i = 0; i < n3; i++) bad |= !(xyz[i] >= 0.0 && xyz[i] <= L);      // branch-free: vectorises
@@ -647,6 +666,8 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
     P.has_bonds = n_bonds > 0;
     P.fene_k = k;
     P.fene_R02 = R0 * R0;
+    P.fene_kf = (float)k;
+    P.fene_R02f = (float)(R0 * R0);
     s->n_bonds_max = mx;
     // a rebuild fills inv / bond_dev for the current order, then forces are re-evaluated
     s->launches += 1;
@@ -826,6 +847,7 @@ int md_get_info(md_system *s, md_info *out)
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }
     out->use_graph = s->gexec[0] ? 1 : 0;
+    out->precision = s->prm.precision;
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

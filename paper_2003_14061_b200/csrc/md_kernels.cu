@@ -631,9 +631,17 @@ inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdi
 // ------------------------------------------------------------------------------------------------
 void mdk_force_rebuild(const MdDev &P, cudaStream_t st) { k_force_rebuild<<<1, 1, 0, st>>>(P); }
 
-void mdk_load_state(const MdDev &P, cudaStream_t st) { k_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+void mdk_load_state(const MdDev &P, cudaStream_t st)
+{
+    if (P.sp) return mdk_sp_load_state(P, st);
+    k_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+}
 
-void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st) { k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset); }
+void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st)
+{
+    if (P.sp) return mdk_sp_export(P, what, offset, st);
+    k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset);
+}
 
 void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond)
 {
@@ -642,14 +650,20 @@ void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, un
 
 void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
+    if (P.sp) return mdk_sp_kick_drift(P, st);
     k_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P);
 }
 
-void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st) { k_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
+void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st)
+{
+    if (P.sp) return mdk_sp_kick(P, st);
+    k_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P);
+}
 
 void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
-    k_bin<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.sp) mdk_sp_bin(P, st);
+    else k_bin<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
     k_scan_reduce<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
     k_scan_top<<<1, 1024, 0, st>>>(P);
     k_scan_apply<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
@@ -658,12 +672,14 @@ void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
 
 void mdk_reorder(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
-    k_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.sp) mdk_sp_reorder(P, st);
+    else k_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
     if (P.has_bonds) k_bonds_remap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
 }
 
 void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
+    if (P.sp) return mdk_sp_build(P, st);
     if (P.half_list) k_build<true><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
     else k_build<false><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
 }
@@ -681,6 +697,7 @@ static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
 
 void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 {
+    if (P.sp) return mdk_sp_force(P, lc, mode, st);
     if (P.has_bonds) {
         if (mode == 0) launch_force_block<0, true>(P, lc.block, st);
         else if (mode == 1) launch_force_block<1, true>(P, lc.block, st);
@@ -708,6 +725,7 @@ void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)
 
 void mdk_energy(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
+    if (P.sp) return mdk_sp_energy(P, st);
     const int grid = cdiv(P.N, 256);
     if (P.has_bonds) k_energy<true><<<grid, 256, 0, st>>>(P);
     else k_energy<false><<<grid, 256, 0, st>>>(P);

@@ -147,6 +147,11 @@ struct MdDev {
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
+    // single-precision variant (md_sp.cu; MD_PREC_F32): float4 records r, v, f replace pos / vel / frc,
+    // which stay null; L and inv_w above are then those of the binary32 box edge (double)(float)L
+    int sp, sp_pad;                     // sp_pad = SP_PAD when the columns of W are padded with self entries (long columns), else 1
+    float Lf, half_Lf, rc2f, rn2f, ucf, dtf, hdtf, fene_kf, fene_R02f;
+    float4 *posf[2], *velf[2], *frcf;
 };
 
 // Launch wrappers (md_kernels.cu).  All are asynchronous on `st`.
@@ -176,6 +181,16 @@ size_t mdk_tile_smem(const TileGeom &G, bool with_cells);
 void mdk_tile_build(const MdDev &P, cudaStream_t st);
 void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st);
 void mdk_tile_energy(const MdDev &P, cudaStream_t st);
+// single-precision variant (md_sp.cu); the wrappers above dispatch to these when P.sp
+void mdk_sp_load_state(const MdDev &P, cudaStream_t st);
+void mdk_sp_export(const MdDev &P, int what, size_t offset, cudaStream_t st);
+void mdk_sp_kick_drift(const MdDev &P, cudaStream_t st);
+void mdk_sp_kick(const MdDev &P, cudaStream_t st);
+void mdk_sp_bin(const MdDev &P, cudaStream_t st);
+void mdk_sp_reorder(const MdDev &P, cudaStream_t st);
+void mdk_sp_build(const MdDev &P, cudaStream_t st);
+void mdk_sp_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
+void mdk_sp_energy(const MdDev &P, cudaStream_t st);
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,
        LK_ENERGY, LK_EXPORT };

@@ -25,11 +25,12 @@ def main():
     ap.add_argument("--mode", default="fused")
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--flags", type=int, default=0, help="md_params.flags (2 = MD_FLAG_GLOBAL_W)")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     a = ap.parse_args()
     cfg = get_config(a.config)
     r, v, bonds, box = make_state(cfg, 1)
     g = MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=a.variant,
-                 step_mode=a.mode if a.variant == "full" else "split", block_size=a.block, flags=a.flags)
+                 step_mode=a.mode if a.variant == "full" else "split", block_size=a.block, flags=a.flags, precision=a.precision)
     g.set_state(r, v)
     if bonds is not None:
         g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
