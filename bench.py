@@ -206,6 +206,11 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="md_params.flags: 1 = no CUDA graph, 2 = global-index W layout")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="f32: the single-precision variant (md_params.precision = MD_PREC_F32; SURVEY 8(f) NEXT-1)")
+    ap.add_argument("--reorder-interval", type=int, default=0,
+                    help="with --flags 32 (MD_FLAG_LAYER_H, the paper's cell x layer matrix): steps between sorts of the "
+                         "atoms into cell order; 0 = every rebuild, < 0 = never (PAPER.md:159)")
+    ap.add_argument("--shuffle", action="store_true",
+                    help="permute the atom numbering of the start state (a decorrelated storage order, for the sort ablation)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -242,9 +247,14 @@ def main():
     nsys = max(1, args.systems)
     states = [make_state(cfg, seed + 1000 * b) for b in range(nsys)]
     box = states[0][3]
+    if args.shuffle:
+        if nsys != 1 or states[0][2] is not None:
+            raise SystemExit("--shuffle: one system without bonds only")
+        perm = np.random.default_rng(12345).permutation(cfg.n_atoms)
+        states = [(states[0][0][perm], states[0][1][perm], None, box)]
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=args.variant,
                     step_mode=args.mode if args.variant == "full" else "split", block_size=args.block, flags=args.flags,
-                    n_systems=nsys, precision=args.precision)
+                    n_systems=nsys, precision=args.precision, reorder_interval=args.reorder_interval)
     g.set_state(np.concatenate([s[0] for s in states]), np.concatenate([s[1] for s in states]))
     if states[0][2] is not None:
         g.set_bonds(np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)]), cfg.fene_k, cfg.fene_r0)
@@ -329,7 +339,7 @@ def main():
     cand = 27.0 * (n / nsys) / info["cells_per_edge"] ** 3                   # candidates examined per atom (27-cell stencil)
     nb_floor = rec + w_bytes * mbar + 4.0                             # r_i + W written + m_i
     nb_ns = nb_floor + rec * cand                                     # + one record per candidate position read
-    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else ("k_sp_build" if sp else "k_build"),
+    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else ("k_sp_build" if sp else ("k_build_layers" if args.flags & 32 else "k_build")),
                          "avg_launch_ms": build_ms, "candidates_per_atom": cand,
                          "achieved": nb_ns * n / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": nb_ns * n / (build_ms * 1e-3) / 1e9 / peak,
@@ -383,7 +393,8 @@ def main():
         "config": {"workload": cfg.name if nsys == 1 else f"{nsys} x {cfg.name}", "n_atoms": n, "n_systems": nsys,
                    "lattice": cfg.lattice, "density": cfg.density,
                    "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
-                   "force_variant": args.variant, "step_mode": args.mode, "precision": args.precision, "block_size": info["block_size"],
+                   "force_variant": args.variant, "step_mode": args.mode, "precision": args.precision,
+                   "flags": args.flags, "reorder_interval": args.reorder_interval, "shuffled_ids": bool(args.shuffle), "block_size": info["block_size"],
                    "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
                    "w_layout": "tiled16" if tiled else "global32", "tile_cells": info["tile_cells"],
                    "cuda_graph": bool(info_end["use_graph"]),

@@ -55,8 +55,10 @@ typedef enum md_status {
     MD_ERR_CUDA = -5,           /* CUDA runtime error (text in md_last_error) */
     MD_ERR_UNSUPPORTED = -6,    /* e.g. fewer than 3 cells per edge, more than 2 bonds per atom */
     MD_ERR_NOMEM = -7,
-    MD_ERR_TILE_OVERFLOW = -8   /* tiled W: a block's cell neighbourhood holds more atoms than its shared-memory
+    MD_ERR_TILE_OVERFLOW = -8,  /* tiled W: a block's cell neighbourhood holds more atoms than its shared-memory
                                    tile (strongly inhomogeneous density); re-create with MD_FLAG_GLOBAL_W */
+    MD_ERR_CELL_OVERFLOW = -9   /* MD_FLAG_LAYER_H only: a cell holds more atoms than the layer count N_l of the dense
+                                   cell x layer matrix H (the CSR default has no such bound) */
 } md_status;
 
 enum { MD_LATTICE_AUTO = 0, MD_LATTICE_SC = 1, MD_LATTICE_FCC = 2, MD_LATTICE_NONE = 3 };
@@ -97,6 +99,10 @@ typedef struct md_params {
                                 arithmetic in binary32, every sum of energies in binary64.  Boundary arrays stay double and
                                 are rounded to binary32 on entry; the box edge used is (float)box.  Variant A only
                                 (fused or split steps), global-index W. */
+    int32_t  reorder_interval; /* MD_FLAG_LAYER_H only.  > 0: the atoms are re-sorted into cell order at the first rebuild
+                                that falls at least this many steps after the last sort (the paper: 100);
+                                0: at every rebuild; < 0: never (not even at the start).  Ignored without the flag: the
+                                default path sorts at every rebuild. */
 } md_params;
 
 enum { MD_PREC_F64 = 0, MD_PREC_F32 = 1 };
@@ -111,8 +117,13 @@ enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying 
                                  these flags the library picks this layout when the expected number of neighbors per
                                  atom is >= 32 (e.g. LJ with r_c = 2.5) and global indices otherwise. */
        MD_FLAG_GATHER_W = 8u, /* never pick the tiled layout automatically (the build kernel still stages tiles) */
-       MD_FLAG_W_TRANSPOSED = 16u /* ablation of PAPER.md:165-167: store W atom-index-SLOWEST, W[i * Mmax + m], so that
-                                 the threads of a warp no longer read consecutive words (global-index layout only) */ };
+       MD_FLAG_W_TRANSPOSED = 16u, /* ablation of PAPER.md:165-167: store W atom-index-SLOWEST, W[i * Mmax + m], so that
+                                 the threads of a warp no longer read consecutive words (global-index layout only) */
+       MD_FLAG_LAYER_H = 32u  /* ablation: the paper's own cell structure (steps N1-N5): a dense cell x
+                                 layer matrix H[c][l] = atom, filled from the atomic slot l_i, searched by the neighbor
+                                 build; atoms are re-sorted into cell order only every md_params.reorder_interval steps
+                                  and otherwise stay where they are.  Implies MD_FLAG_GLOBAL_W.  fp64,
+                                 variant A only.  A cell holding more than N_l atoms gives MD_ERR_CELL_OVERFLOW. */ };
 enum { MD_W_GLOBAL = 0, MD_W_TILED = 1 };
 
 /* Totals (not per atom) at the current, synchronised time: r, v and f belong to the same instant. */
@@ -144,6 +155,7 @@ typedef struct md_info {
     int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node */
     int32_t n_systems;
     int32_t precision;          /* MD_PREC_* */
+    int32_t n_layers;           /* MD_FLAG_LAYER_H: N_l, columns of H; else 0 */
 } md_info;
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */

@@ -16,8 +16,8 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libmd_b200.so")
 
 MD_OK, MD_ERR_INVALID, MD_ERR_NEBR_OVERFLOW, MD_ERR_BOND_BROKEN = 0, -1, -2, -3
-MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM, MD_ERR_TILE_OVERFLOW = -4, -5, -6, -7, -8
-FLAG_NO_GRAPH, FLAG_GLOBAL_W, FLAG_TILED_W, FLAG_GATHER_W, FLAG_W_TRANSPOSED = 1, 2, 4, 8, 16
+MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM, MD_ERR_TILE_OVERFLOW, MD_ERR_CELL_OVERFLOW = -4, -5, -6, -7, -8, -9
+FLAG_NO_GRAPH, FLAG_GLOBAL_W, FLAG_TILED_W, FLAG_GATHER_W, FLAG_W_TRANSPOSED, FLAG_LAYER_H = 1, 2, 4, 8, 16, 32
 LATTICE = {"auto": 0, "sc": 1, "fcc": 2, "none": 3}
 FORCE_VARIANT = {"full": 0, "newton3": 1}
 STEP_MODE = {"fused": 0, "split": 1}
@@ -42,7 +42,7 @@ class _Params(C.Structure):
                 ("lattice", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
                 ("max_neighbors", C.c_int32), ("block_size", C.c_int32), ("device", C.c_int32),
                 ("stream", C.c_void_p), ("flags", C.c_uint32), ("n_systems", C.c_int32),
-                ("precision", C.c_int32)]
+                ("precision", C.c_int32), ("reorder_interval", C.c_int32)]
 
 
 class _Energy(C.Structure):
@@ -59,7 +59,7 @@ class _Info(C.Structure):
                 ("n_bonds_per_atom_max", C.c_int32), ("device_bytes", C.c_int64), ("kernel_launches", C.c_int64),
                 ("device_name", C.c_char * 64), ("w_layout", C.c_int32), ("tile_cells", C.c_int32 * 3),
                 ("tile_capacity", C.c_int32), ("tile_threads", C.c_int32), ("use_graph", C.c_int32),
-                ("n_systems", C.c_int32), ("precision", C.c_int32)]
+                ("n_systems", C.c_int32), ("precision", C.c_int32), ("n_layers", C.c_int32)]
 
 
 @dataclass
@@ -161,7 +161,7 @@ class MDSystem:
 
     def __init__(self, n_atoms, r_cut, r_shell, dt, box=0.0, density=0.0, seed=1, temperature=1.0, lattice="auto",
                  force_variant="full", step_mode="fused", max_neighbors=0, block_size=0, device=-1,
-                 torch_memory=True, flags=0, n_systems=1, precision="f64"):
+                 torch_memory=True, flags=0, n_systems=1, precision="f64", reorder_interval=0):
         import torch
         if not torch.cuda.is_available():
             raise MDError(MD_ERR_CUDA, "no CUDA device: the MD path has no CPU fallback")
@@ -176,6 +176,7 @@ class MDSystem:
         p.max_neighbors, p.block_size, p.device, p.flags = max_neighbors, block_size, device, flags
         p.n_systems = int(n_systems)
         p.precision = PRECISION[precision]
+        p.reorder_interval = int(reorder_interval)
         p.stream = torch.cuda.current_stream().cuda_stream or None
         self._L = L
         self._h = L.md_create_ex(C.byref(p))

@@ -161,6 +161,9 @@ int check_device_status(md_system *s)
             break;
         case MD_ERR_BOND_BROKEN: set_error("FENE bond stretched to r >= R0"); break;
         case MD_ERR_NONFINITE: set_error("non-finite position or velocity"); break;
+        case MD_ERR_CELL_OVERFLOW:
+            set_error("MD_FLAG_LAYER_H: a cell holds more than N_l = %d atoms", s->P.n_layers);
+            break;
         case MD_ERR_TILE_OVERFLOW:
             set_error("tiled W: a block's cell neighbourhood holds more than %d atoms; re-create with MD_FLAG_GLOBAL_W", s->P.tg.cap);
             break;
@@ -175,8 +178,8 @@ int check_device_status(md_system *s)
 void enqueue_rebuild(md_system *s)
 {
     { Timed t(s, MD_T_CELLS, mdk_launches_of(LK_CELLS)); mdk_cells(s->P, s->lc, s->stream); }
-    { Timed t(s, MD_T_REORDER, s->P.has_bonds ? 2 : 1); mdk_reorder(s->P, s->lc, s->stream); }
-    { Timed t(s, MD_T_NEBR, 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_REORDER, (s->P.has_bonds ? 2 : 1) + (s->P.layer_H ? 1 : 0)); mdk_reorder(s->P, s->lc, s->stream); }
+    { Timed t(s, MD_T_NEBR, s->P.layer_H ? 2 : 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
 void enqueue_force(md_system *s, int mode)
@@ -254,7 +257,7 @@ bool build_step_graph(md_system *s, int kind)
         if (s->graph[kind]) { cudaGraphDestroy(s->graph[kind]); s->graph[kind] = nullptr; }
         return false;
     }
-    s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1;
+    s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1 + (s->P.layer_H ? 2 : 0);
     return true;
 }
 
@@ -462,6 +465,15 @@ md_system *md_create_ex(const md_params *pp)
     const bool sp = p.precision == MD_PREC_F32;
     if (sp && p.force_variant != MD_FORCE_FULL_LIST) { set_error("MD_PREC_F32 supports the full-list force variant only"); return nullptr; }
     if (sp && (p.flags & MD_FLAG_TILED_W)) { set_error("MD_PREC_F32 uses the global-index W layout"); return nullptr; }
+    if (p.flags & MD_FLAG_LAYER_H) {
+        if (sp || p.force_variant != MD_FORCE_FULL_LIST || p.n_systems > 1 || (p.flags & MD_FLAG_TILED_W)) {
+            set_error("MD_FLAG_LAYER_H: fp64, full-list variant, one system, global-index W only");
+            return nullptr;
+        }
+        p.flags |= MD_FLAG_GLOBAL_W;
+    } else {
+        p.reorder_interval = 0;
+    }
     const double rn = p.r_cut + p.r_shell;
     // single precision: the box edge is the binary32 number, and cells keep a margin above the rounding error of a
     // binary32 r^2 (~2e-7 relative) so that no accepted pair can lie outside the 27-cell stencil
@@ -555,6 +567,13 @@ md_system *md_create_ex(const md_params *pp)
         md_destroy(s);
         return nullptr;
     }
+    if (p.flags & MD_FLAG_LAYER_H) {
+        // N_l: the paper sizes H by the measured maximum occupancy (N3); here a fixed bound from the mean
+        const double mean_occ = (double)P.N1 / P.NC1;
+        P.layer_H = 1;
+        P.n_layers = 8 * (int)ceil((2.0 * mean_occ + 8.0) / 8.0);
+        P.reorder_interval = p.reorder_interval;
+    }
     P.w_row = P.N_pad; P.w_col = 1;
     if (p.flags & MD_FLAG_W_TRANSPOSED) {
         if (P.tiled) { set_error("MD_FLAG_W_TRANSPOSED applies to the global-index W layout only"); md_destroy(s); return nullptr; }
@@ -585,6 +604,7 @@ md_system *md_create_ex(const md_params *pp)
     P.cell_start = (int *)A(((size_t)P.NC + 1) * sizeof(int));
     P.block_sums = (int *)A(((size_t)P.scan_blocks + 1) * sizeof(int));
     P.W = (int *)A((size_t)(P.tiled ? P.Mmax / 2 : P.Mmax) * np * sizeof(int));
+    if (P.layer_H) P.H = (int *)A((size_t)P.NC * P.n_layers * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
     P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
     if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys * sizeof(TileDesc));
@@ -848,6 +868,7 @@ int md_get_info(md_system *s, md_info *out)
     }
     out->use_graph = s->gexec[0] ? 1 : 0;
     out->precision = s->prm.precision;
+    out->n_layers = s->P.n_layers;
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

@@ -139,10 +139,16 @@ __device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pi
     volatile DevCtrl *c = P.ctrl;
     double acc = c->disp_acc + P.dt * sqrt(vmax2);
     const int need = acc > P.thresh;
+    const int since = c->since_reorder + 1;
+    c->since_reorder = since;
     if (need) {
         acc = 0.0;
         c->n_rebuilds += 1;
         c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+        // the paper sorts the atoms only every ~100 steps; the default path at every rebuild
+        const int ro = !P.layer_H || P.reorder_interval == 0 || (P.reorder_interval > 0 && since >= P.reorder_interval);
+        c->do_reorder = ro;
+        if (ro) c->since_reorder = 0;
     }
     c->disp_acc = acc;
     c->need_rebuild = need;

@@ -32,6 +32,8 @@ __global__ void k_force_rebuild(const __grid_constant__ MdDev P)
     c->v_src = c->v_dst; c->v_dst ^= 1;
     c->disp_acc = 0.0;
     c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+    c->do_reorder = !P.layer_H || P.reorder_interval >= 0;      // a forced rebuild sorts unless the system never does
+    c->since_reorder = 0;
 }
 
 // scratch = [xyz (3N) | vxyz (3N)] in original-id order -> device arrays in identity order
@@ -249,6 +251,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ M
 __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    if (P.layer_H && !__ldcg(&P.ctrl->do_reorder)) return;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x)
         P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
 }
@@ -260,6 +263,7 @@ __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
 __global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    if (P.layer_H && !__ldcg(&P.ctrl->do_reorder)) return;
     const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
     const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pin = P.pos[ps];
@@ -369,6 +373,117 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
         tsum += m;
     }
     // statistics of the matrix (md_energy.max_neighbors / mean_neighbors)
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int mx = 0, sm = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        atomicMax(&P.ctrl->max_nnb, mx);
+        atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Ablation MD_FLAG_LAYER_H: the paper's own cell structure and sort schedule.
+//   N1/N2  k_bin as above: c_i and the layer l_i = atomicAdd(k_c)
+//   N3     max occupancy from the scan kernels (ctrl->max_occ); H has a fixed N_l = P.n_layers columns
+//   N4     k_layer_fill: H[c_i][l_i] = i
+//   N5     k_build_layers: for every cell of the stencil, for every layer l < k_c: i' = H[c][l]
+// The atoms are re-sorted into cell order only when decide() says so (every reorder_interval steps); at the
+// other rebuilds k_copy_wrap moves them to the other buffers in place (the rebuild chain always changes buffers).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_copy_wrap(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild) || __ldcg(&P.ctrl->do_reorder)) return;
+    const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
+    const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
+    const size_t np = (size_t)P.N_pad;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        const pos_t r = ld_pos(P.pos[ps] + i);
+        st_pos(P.pos[pd] + i, wrap1(r.x, P.L), wrap1(r.y, P.L), wrap1(r.z, P.L));
+        const double *vi = P.vel[vs] + i;
+        double *vo = P.vel[vd] + i;
+        vo[0] = vi[0]; vo[np] = vi[np]; vo[2 * np] = vi[2 * np];
+        const int id = P.id[vs][i];
+        P.id[vd][i] = id;
+        if (P.has_bonds) P.inv[id] = i;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_layer_fill(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    const bool sorted = __ldcg(&P.ctrl->do_reorder) != 0;
+    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        int c, l;
+        if (sorted) {        // after the sort the layer is the atom's rank inside its cell
+            const pos_t r = ld_pos(pos + i);
+            c = cell_coord(r.x, P.inv_w, P.nc) + P.nc * (cell_coord(r.y, P.inv_w, P.nc) + P.nc * cell_coord(r.z, P.inv_w, P.nc));
+            l = i - P.cell_start[c];
+        } else {             // atoms stayed in place: c_i and the atomic slot l_i of k_bin
+            c = P.cell_of[i];
+            l = P.slot[i];
+        }
+        if (l >= P.n_layers) { set_err(P, MD_ERR_CELL_OVERFLOW); continue; }
+        P.H[(size_t)c * P.n_layers + l] = i;
+    }
+}
+
+__global__ void __launch_bounds__(128) k_build_layers(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    __shared__ int smx[4];
+    __shared__ int ssum[4];
+    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    const int *__restrict__ cs = P.cell_start;
+    const int nc = P.nc, NL = P.n_layers;
+    const double L = P.L;
+    int tmax = 0, tsum = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        const pos_t ri = ld_pos(pos + i);
+        const int cx = cell_coord(ri.x, P.inv_w, nc), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
+        int m = 0;
+        for (int dz = -1; dz <= 1; dz++) {
+            int z = cz + dz;
+            double sz = 0.0;
+            unsigned fz = 0u;
+            if (z < 0) { z += nc; sz = L; fz = 4u; } else if (z >= nc) { z -= nc; sz = -L; fz = 4u; }
+            for (int dy = -1; dy <= 1; dy++) {
+                int y = cy + dy;
+                double sy = 0.0;
+                unsigned fy = fz;
+                if (y < 0) { y += nc; sy = L; fy |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fy |= 2u; }
+                for (int dx = -1; dx <= 1; dx++) {
+                    int x = cx + dx;
+                    double sx = 0.0;
+                    unsigned fl = fy;
+                    if (x < 0) { x += nc; sx = L; fl |= 1u; } else if (x >= nc) { x -= nc; sx = -L; fl |= 1u; }
+                    const int c = x + nc * (y + nc * z);
+                    const int kc = min(__ldg(cs + c + 1) - __ldg(cs + c), NL);        // k_c: occupancy from the scan
+                    const int *__restrict__ h = P.H + (size_t)c * NL;
+                    for (int l = 0; l < kc; l++) {
+                        const int j = __ldg(h + l);
+                        const pos_t rj = ld_pos(pos + j);
+                        // d = (r_i - r_j) + shift, each operation rounded once (+0.0 is exact): DESIGN.md R5
+                        const double ddx = __dadd_rn(__dsub_rn(ri.x, rj.x), sx), ddy = __dadd_rn(__dsub_rn(ri.y, rj.y), sy),
+                                     ddz = __dadd_rn(__dsub_rn(ri.z, rj.z), sz);
+                        const double r2 = __fma_rn(ddz, ddz, __fma_rn(ddy, ddy, __dmul_rn(ddx, ddx)));
+                        if (r2 < P.rn2 && j != i) {
+                            if (m < P.Mmax) P.W[(size_t)m * P.w_row + (size_t)i * P.w_col] = (int)((unsigned)j | (fl << W_FLAG_SHIFT));
+                            m++;
+                        }
+                    }
+                }
+            }
+        }
+        P.nnb[i] = m < P.Mmax ? m : P.Mmax;
+        if (m > P.Mmax) set_err(P, MD_ERR_NEBR_OVERFLOW);
+        tmax = max(tmax, m);
+        tsum += m;
+    }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
     if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
@@ -674,12 +789,18 @@ void mdk_reorder(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     if (P.sp) mdk_sp_reorder(P, st);
     else k_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.layer_H) k_copy_wrap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
     if (P.has_bonds) k_bonds_remap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
 }
 
 void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     if (P.sp) return mdk_sp_build(P, st);
+    if (P.layer_H) {
+        k_layer_fill<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+        k_build_layers<<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
+        return;
+    }
     if (P.half_list) k_build<true><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
     else k_build<false><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
 }

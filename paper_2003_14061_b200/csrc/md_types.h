@@ -26,9 +26,10 @@ struct DevCtrl {
     int n_rebuilds;
     int max_nnb;               // max m_i of the current matrix
     int max_occ;               // max k_c of the last binning
-    int pad0;
+    int do_reorder;            // MD_FLAG_LAYER_H: this rebuild re-sorts the atoms into cell order (else they stay in place)
     unsigned int ticket[6];    // "last block done" counters, one per kernel family
-    unsigned long long reserved0;
+    int since_reorder;         // steps since the last sort
+    int pad1;
     unsigned long long nnb_total;
     long long step;
     double disp_acc;           // accumulated dt * max|v| since the last rebuild
@@ -147,6 +148,10 @@ struct MdDev {
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
+    // ablation MD_FLAG_LAYER_H: the paper's dense cell x layer matrix H[c * n_layers + l] and its
+    // every-100-steps sort
+    int layer_H, n_layers, reorder_interval;
+    int *H;
     // single-precision variant (md_sp.cu; MD_PREC_F32): float4 records r, v, f replace pos / vel / frc,
     // which stay null; L and inv_w above are then those of the binary32 box edge (double)(float)L
     int sp, sp_pad;                     // sp_pad = SP_PAD when the columns of W are padded with self entries (long columns), else 1
