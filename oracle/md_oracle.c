@@ -22,6 +22,9 @@
  *   - rebuild rule: decided from the maximal atom velocity: accumulate dt * max|v| and
  *     rebuild when it exceeds delta/2 (reading R8).
  *   - bonds (polymer chains): FENE bond force between chain neighbours (R12).
+ *   - bond angles ("bond-angle torque"): PAPER.md gives no form; the textbook
+ *     cosine-harmonic U = k/2 (cos(theta) - cos(theta0))^2 at every atom with two bonded partners
+ *     (reading R19), forces by the chain rule on cos(theta) = d1.d2 / (|d1||d2|).
  *
  * Parity pins for every function here live in tests/test_oracle_pins.py (brute force on tiny
  * inputs, closed forms on the SC/FCC lattices, two-atom values, conservation laws, reversibility,
@@ -62,6 +65,10 @@ typedef struct orc_sys {
     double fene_k, fene_R0;
     double pe_bond, vir_bond;
     int bond_broken;
+    /* bond angles: partner table built from the bond list (-1 = none), potential constants */
+    int32_t *partner;       /* 2 x N */
+    int has_angles;
+    double ang_k, ang_c0, pe_angle;
     /* bookkeeping */
     double disp_acc;
     int64_t step, n_rebuilds;
@@ -209,7 +216,7 @@ void orc_destroy(orc_sys *s)
 {
     if (!s) return;
     free(s->r); free(s->v); free(s->f); free(s->u); free(s->w);
-    free(s->nb_start); free(s->nb); free(s->bonds);
+    free(s->nb_start); free(s->nb); free(s->bonds); free(s->partner);
     free(s);
 }
 
@@ -349,6 +356,31 @@ static void compute_forces(orc_sys *s)
         }
         s->pe_bond = pe + pc; s->vir_bond = vr + vc;
     }
+    /* bond angles (R19): vertex b with partners a, c; d1 = r_a - r_b, d2 = r_c - r_b (minimum image);
+     * c = d1.d2 / (|d1||d2|); U = k/2 (c - c0)^2; f_a = -dU/dc dc/dr_a, dc/dr_a = d2/(|d1||d2|) - c d1/|d1|^2;
+     * f_c likewise with 1 <-> 2; f_b = -(f_a + f_c).  cos(theta) is scale invariant: no virial contribution. */
+    s->pe_angle = 0;
+    if (s->has_angles) {
+        double pe = 0;
+        for (int64_t b = 0; b < N; b++) {
+            int64_t a = s->partner[b], c = s->partner[N + b];
+            if (a < 0 || c < 0) continue;
+            double d1[3], d2[3];
+            double n1 = dist2(s->r + 3 * a, s->r + 3 * b, L, half, d1);
+            double n2 = dist2(s->r + 3 * c, s->r + 3 * b, L, half, d2);
+            double dot = d1[0] * d2[0] + d1[1] * d2[1] + d1[2] * d2[2];
+            double inv12 = 1.0 / sqrt(n1 * n2);
+            double cs = dot * inv12;
+            double g = -s->ang_k * (cs - s->ang_c0);          /* -dU/dc */
+            for (int q = 0; q < 3; q++) {
+                double fa = g * (d2[q] * inv12 - cs * d1[q] / n1);
+                double fc = g * (d1[q] * inv12 - cs * d2[q] / n2);
+                s->f[3 * a + q] += fa; s->f[3 * c + q] += fc; s->f[3 * b + q] -= fa + fc;
+            }
+            pe += 0.5 * s->ang_k * (cs - s->ang_c0) * (cs - s->ang_c0);
+        }
+        s->pe_angle = pe;
+    }
 }
 
 static void rebuild(orc_sys *s)
@@ -375,8 +407,28 @@ int orc_set_bonds(orc_sys *s, int64_t nb, const int32_t *ij, double k, double R0
     s->bonds = (int32_t *)malloc(2 * nb * sizeof(int32_t));
     memcpy(s->bonds, ij, 2 * nb * sizeof(int32_t));
     s->n_bonds = nb; s->fene_k = k; s->fene_R0 = R0;
+    /* partner table (at most 2 per atom: linear chains) */
+    free(s->partner);
+    s->partner = (int32_t *)malloc(2 * s->N * sizeof(int32_t));
+    for (int64_t i = 0; i < 2 * s->N; i++) s->partner[i] = -1;
+    for (int64_t b = 0; b < nb; b++)
+        for (int side = 0; side < 2; side++) {
+            int32_t a = ij[2 * b + side], c = ij[2 * b + 1 - side];
+            if (s->partner[a] < 0) s->partner[a] = c;
+            else if (s->partner[s->N + a] < 0) s->partner[s->N + a] = c;
+            else return -6;
+        }
     compute_forces(s);
     return s->bond_broken ? -3 : 0;
+}
+
+/* bond-angle terms at every atom with two bonded partners; call after orc_set_bonds */
+int orc_set_angles(orc_sys *s, double k, double cos0)
+{
+    if (!s->partner) return -1;
+    s->has_angles = 1; s->ang_k = k; s->ang_c0 = cos0;
+    compute_forces(s);
+    return 0;
 }
 
 void orc_rebuild_neighbors(orc_sys *s) { rebuild(s); s->n_rebuilds--; compute_forces(s); }
@@ -440,7 +492,7 @@ void orc_energies(orc_sys *s, orc_energy *e)
     e->ke = 0.5 * nsum(v2, N, 1);
     free(v2);
     e->pe_pair = 0.5 * nsum(s->u, N, 1);
-    e->pe_bond = s->pe_bond;
+    e->pe_bond = s->pe_bond + s->pe_angle;      /* bonded energy: FENE + angle terms */
     e->virial = 0.5 * nsum(s->w, N, 1) + s->vir_bond;
     e->px = nsum(s->v, N, 3); e->py = nsum(s->v + 1, N, 3); e->pz = nsum(s->v + 2, N, 3);
     e->vmax = sqrt(vmax2);

@@ -121,6 +121,8 @@ def lib():
     if _lib is None:
         L = C.CDLL(build())
         _declare_system_api(L, "orc_")
+        L.orc_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orc_set_angles.restype = C.c_int
         L.orc_brute_forces.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
         L.orc_brute_forces_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp, _dp, _dp, _dp]
         L.orc_brute_neighbors_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp,
@@ -216,6 +218,10 @@ class OracleMD:
     def set_bonds(self, bonds, k, r0):
         b = _c(bonds, np.int32).reshape(-1, 2)
         return self._L.set_bonds(self._h, b.shape[0], b, float(k), float(r0))
+
+    def set_angles(self, k, cos0):
+        """Cosine-harmonic bond-angle terms (fp64 oracle only); after set_bonds."""
+        return self._L.set_angles(self._h, float(k), float(cos0))
 
     def rebuild_neighbors(self):
         self._L.rebuild_neighbors(self._h)

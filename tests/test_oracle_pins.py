@@ -360,3 +360,121 @@ def test_p9_paper_list_statistics(golden, col, n_side):
     t_meas = e2.ke / (1.5 * (n - 1))
     scaled = interval * math.sqrt(t_meas / g["temperature"][col]) * math.sqrt(math.log(n) / math.log(g["largest_n"][col]))
     assert scaled == pytest.approx(g["refresh_interval"][col], rel=0.12)
+
+
+# ---- P14: bond-angle terms (R19) ------------------------------------
+def np_angle_energy(r, box, triples, k, c0):
+    """U = k/2 (cos(theta) - c0)^2 summed over (a, b, c) with vertex b; cos from normalised bond vectors."""
+    e = 0.0
+    for a, b, c in triples:
+        u = r[a] - r[b]
+        u -= box * np.round(u / box)
+        w = r[c] - r[b]
+        w -= box * np.round(w / box)
+        cs = float(np.dot(u / np.linalg.norm(u), w / np.linalg.norm(w)))
+        e += 0.5 * k * (cs - c0) ** 2
+    return e
+
+
+def chain_system(n_chains=6, length=7, seed=4):
+    """Short kinked chains, dilute enough that pair terms do not matter for the angle pins."""
+    rng = np.random.default_rng(seed)
+    box = 30.0
+    r, bonds, triples = [], [], []
+    for ch in range(n_chains):
+        p = rng.uniform(5, 25, 3)
+        for s in range(length):
+            r.append(p.copy())
+            step = rng.normal(size=3)
+            p = p + 0.97 * step / np.linalg.norm(step)
+            i = ch * length + s
+            if s > 0:
+                bonds.append((i - 1, i))
+            if s > 1:
+                triples.append((i - 2, i - 1, i))
+    return np.mod(np.array(r), box), np.array(bonds, np.int32), triples, box
+
+
+def test_p14_angle_closed_forms():
+    box = 10.0
+    r = np.array([[3.0, 2, 2], [2.0, 2, 2], [2.0, 3, 2]])
+    o = OracleMD(3, box, R_WCA, 0.4, 0.005, brute_search=True)
+    o.set_state(r, np.zeros((3, 3)))
+    bonds = np.array([[0, 1], [1, 2]], np.int32)
+    assert o.set_bonds(bonds, 30.0, 1.5) == 0
+    f0, e0 = o.forces().copy(), o.energies()
+    assert o.set_angles(5.0, -1.0) == 0
+    # right angle, unit bonds: cos = 0, U = k/2 c0^2 = 2.5; f_a = -k (0 - c0) d2 = (0, -5, 0), f_c = (-5, 0, 0)
+    df = o.forces() - f0
+    assert np.allclose(df, [[0, -5, 0], [5, 5, 0], [-5, 0, 0]], atol=1e-13)
+    e1 = o.energies()
+    assert e1.pe_bond - e0.pe_bond == pytest.approx(2.5, abs=1e-13)
+    assert e1.virial == pytest.approx(e0.virial, abs=1e-12)          # cos(theta) is scale invariant: no virial
+    # straight chain across the periodic face with theta0 = pi: no energy, no force
+    r = np.array([[9.5, 2, 2], [0.45, 2, 2], [1.4, 2, 2]])
+    o = OracleMD(3, box, R_WCA, 0.4, 0.005, brute_search=True)
+    o.set_state(r, np.zeros((3, 3)))
+    o.set_bonds(bonds, 30.0, 1.5)
+    f0, e0 = o.forces().copy(), o.energies().pe_bond
+    o.set_angles(7.0, -1.0)
+    assert np.abs(o.forces() - f0).max() < 1e-12 and abs(o.energies().pe_bond - e0) < 1e-13
+
+
+def test_p14_angle_forces_are_minus_gradient_of_numpy_energy():
+    r, bonds, triples, box = chain_system()
+    n = r.shape[0]
+    k, c0 = 4.0, -0.8
+    o = OracleMD(n, box, R_WCA, 0.4, 0.005)
+    o.set_state(r, np.zeros_like(r))
+    assert o.set_bonds(bonds, 30.0, 1.5) == 0
+    f0, e0 = o.forces().copy(), o.energies().pe_bond
+    assert o.set_angles(k, c0) == 0
+    fa = o.forces() - f0                                             # the angle part alone
+    assert o.energies().pe_bond - e0 == pytest.approx(np_angle_energy(r, box, triples, k, c0), rel=1e-12)
+    h = 1e-6
+    rng = np.random.default_rng(0)
+    for i in rng.choice(n, 12, replace=False):
+        for q in range(3):
+            rp, rm = r.copy(), r.copy()
+            rp[i, q] += h
+            rm[i, q] -= h
+            g = (np_angle_energy(rp, box, triples, k, c0) - np_angle_energy(rm, box, triples, k, c0)) / (2 * h)
+            assert fa[i, q] == pytest.approx(-g, abs=2e-8 * max(1.0, np.abs(fa).max()))
+    # internal forces: no net force, no net torque (per chain the terms cancel; unwrap about the first bead)
+    # (fa is a difference of total forces that contain the stiff pair and FENE terms: scale the bounds by those)
+    scale = np.abs(o.forces()).sum()
+    assert np.abs(fa.sum(0)).max() < 1e-12 * scale
+    # torque about any point vanishes chain by chain; chains are compact (< box/2), so unwrap each about its head
+    length = 7
+    for ch in range(n // length):
+        sl = slice(ch * length, (ch + 1) * length)
+        dd = r[sl] - r[sl][0]
+        dd -= box * np.round(dd / box)
+        assert np.abs(np.cross(dd, fa[sl]).sum(0)).max() < 1e-11 * scale
+
+
+def test_p14_angle_run_conserves_energy_and_momentum():
+    cfg = scaled_config("chains_1m", 512, chain_len=16)
+    r, v, bonds, box = make_state(cfg, 3)
+    o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(r, v)
+    assert o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0) == 0
+    assert o.set_angles(2.0, -1.0) == 0
+    e0 = o.energies()
+    assert o.step(200) == 0
+    e1 = o.energies()
+    assert abs(e1.total - e0.total) / cfg.n_atoms < 2e-3              # same dt^2 bound as the pair + FENE system (R17)
+    assert max(abs(e1.px), abs(e1.py), abs(e1.pz)) < 1e-10
+    # halving dt quarters the fluctuation (P10's check, with the angle terms on)
+    def fluct(dt, steps):
+        q = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, dt)
+        q.set_state(r, v)
+        q.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+        q.set_angles(2.0, -1.0)
+        es = []
+        for _ in range(steps // 5):
+            q.step(5)
+            es.append(q.energies().total)
+        return np.std(es)
+    ratio = fluct(cfg.dt, 100) / fluct(cfg.dt / 2, 200)
+    assert 2.5 < ratio < 6.0
