@@ -24,7 +24,7 @@ STEP_MODE = {"fused": 0, "split": 1}
 PRECISION = {"f64": 0, "f32": 1}
 TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "decide")
 
-EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_step", "md_energies",
+EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_set_angles", "md_step", "md_energies",
            "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
            "md_set_allocator", "md_last_error", "md_version")
@@ -112,6 +112,7 @@ def load_library(path: str = LIB_PATH):
     L.md_create_ex.argtypes = [C.POINTER(_Params)]
     L.md_destroy.argtypes = [C.c_void_p]
     L.md_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
+    L.md_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_step.argtypes = [C.c_void_p, C.c_int64]
     L.md_energies.argtypes = [C.c_void_p, C.POINTER(_Energy)]
     for n in ("md_get_positions", "md_get_velocities", "md_get_forces"):
@@ -216,6 +217,9 @@ class MDSystem:
     def set_bonds(self, bonds, k, r0):
         b = np.ascontiguousarray(bonds, np.int32).reshape(-1, 2)
         self._ck(self._L.md_set_bonds(self._h, b.shape[0], b, float(k), float(r0)))
+
+    def set_angles(self, k_theta, cos_theta0):
+        self._ck(self._L.md_set_angles(self._h, float(k_theta), float(cos_theta0)))
 
     def step(self, n=1):
         self._ck(self._L.md_step(self._h, int(n)))

@@ -517,9 +517,56 @@ __device__ __forceinline__ void pair_force(const MdDev &P, const pos_t &ri, cons
     }
 }
 
+// minimum-image r_a - r_b (R5 arithmetic), squared length returned
+__device__ __forceinline__ double mi_disp(const MdDev &P, const pos_t &a, const pos_t &b, double &dx, double &dy, double &dz)
+{
+    dx = minimg(a.x - b.x, P.L, P.half_L); dy = minimg(a.y - b.y, P.L, P.half_L); dz = minimg(a.z - b.z, P.L, P.half_L);
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+}
+
+// Bond-angle terms ("bond-angle torque"; R19): U = k/2 (cos(theta) - c0)^2 at every atom with
+// two bonded partners.  "One thread per atom handles all its interactions": atom i collects its force
+// from the angle it is the vertex of and from the (up to two) angles it ends, found through its partners' partners.
+// With d1 = r_end - r_vertex, d2 = r_other_end - r_vertex, c = d1.d2/(|d1||d2|), g = -k (c - c0):
+//   force on the end atom of d1: g (d2/(|d1||d2|) - c d1/|d1|^2);  on the vertex: minus the sum of both ends.
+__device__ __forceinline__ void angle_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
+{
+    const int p[2] = {P.bond_dev[i], P.bond_dev[(size_t)P.N_pad + i]};
+    pos_t rp[2];
+#pragma unroll
+    for (int k = 0; k < 2; k++)
+        if (p[k] >= 0) rp[k] = ld_pos(pos + p[k]);
+    if (p[0] >= 0 && p[1] >= 0) {                       // i is the vertex
+        double x1, y1, z1, x2, y2, z2;
+        const double n1 = mi_disp(P, rp[0], ri, x1, y1, z1), n2 = mi_disp(P, rp[1], ri, x2, y2, z2);
+        const double inv12 = 1.0 / sqrt(n1 * n2), c = (x1 * x2 + y1 * y2 + z1 * z2) * inv12;
+        const double g = -P.ang_k * (c - P.ang_c0), u1 = c / n1, u2 = c / n2;
+        // -(f_a + f_c)
+        a.fx -= g * ((x2 * inv12 - u1 * x1) + (x1 * inv12 - u2 * x2));
+        a.fy -= g * ((y2 * inv12 - u1 * y1) + (y1 * inv12 - u2 * y2));
+        a.fz -= g * ((z2 * inv12 - u1 * z1) + (z1 * inv12 - u2 * z2));
+    }
+#pragma unroll
+    for (int k = 0; k < 2; k++) {                       // i ends the angle whose vertex is its partner p[k]
+        if (p[k] < 0) continue;
+        const int q0 = P.bond_dev[p[k]], q1 = P.bond_dev[(size_t)P.N_pad + p[k]];
+        const int q = q0 == i ? q1 : q0;
+        if (q < 0) continue;
+        const pos_t rq = ld_pos(pos + q);
+        double x1, y1, z1, x2, y2, z2;
+        const double n1 = mi_disp(P, ri, rp[k], x1, y1, z1), n2 = mi_disp(P, rq, rp[k], x2, y2, z2);
+        const double inv12 = 1.0 / sqrt(n1 * n2), c = (x1 * x2 + y1 * y2 + z1 * z2) * inv12;
+        const double g = -P.ang_k * (c - P.ang_c0), u1 = c / n1;
+        a.fx += g * (x2 * inv12 - u1 * x1);
+        a.fy += g * (y2 * inv12 - u1 * y1);
+        a.fz += g * (z2 * inv12 - u1 * z1);
+    }
+}
+
 template <bool CHECK>
 __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
 {
+    if (P.has_angles) angle_force(P, pos, ri, i, a);
 #pragma unroll
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
@@ -722,6 +769,15 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
                 const double x = 1.0 - r2 / P.fene_R02;
                 q[RED_PEB] += 0.5 * (-0.5 * P.fene_k * P.fene_R02 * log(x));
                 q[RED_VIR] += 0.5 * (-P.fene_k / x) * r2;
+            }
+            if (P.has_angles) {      // the angle i is the vertex of, counted once; cos(theta) is scale invariant: no virial
+                const int p0 = P.bond_dev[i], p1 = P.bond_dev[(size_t)P.N_pad + i];
+                if (p0 >= 0 && p1 >= 0) {
+                    double x1, y1, z1, x2, y2, z2;
+                    const double n1 = mi_disp(P, ld_pos(pos + p0), ri, x1, y1, z1), n2 = mi_disp(P, ld_pos(pos + p1), ri, x2, y2, z2);
+                    const double c = (x1 * x2 + y1 * y2 + z1 * z2) / sqrt(n1 * n2);
+                    q[RED_PEB] += 0.5 * P.ang_k * (c - P.ang_c0) * (c - P.ang_c0);
+                }
             }
         }
         const double *v = P.vel[vc] + i;

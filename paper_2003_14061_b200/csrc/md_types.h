@@ -134,6 +134,8 @@ struct MdDev {
     double rc2, rn2, uc;
     double dt, hdt, thresh;             // thresh = r_shell / 2
     double fene_k, fene_R02;
+    int has_angles;                     // bond-angle terms k/2 (cos(theta) - c0)^2 at atoms with two bonds (md_set_angles)
+    double ang_k, ang_c0;
     pos_t *pos[2];
     double *vel[2];                     // SoA: vx = vel, vy = vel + N_pad, vz = vel + 2 N_pad
     double *frc;                        // SoA, same pitch
