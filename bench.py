@@ -376,7 +376,8 @@ def main():
         barrier()
         dt = time.perf_counter() - t0
         dt = max_over_ranks(dt, dist, "cuda")
-        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT,  # the boundary arrays are double in both precisions "h2d_bytes_per_step": 2 * 3 * n * 8,
+        # the boundary arrays are binary64 in both precisions
+        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
                "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
                "what": "md_set_state(pinned host r,v) + md_step(1) + md_get_positions + md_get_velocities + md_energies per step"}
 

@@ -312,7 +312,8 @@ bool is_pinned(const void *p)
     return a.type == cudaMemoryTypeHost;
 }
 
-int upload_state(md_system *s, const double *xyz, const double *vxyz)
+// check: validate the coordinate range on the device (md_set_state) before anything of the old state is touched
+int upload_state(md_system *s, const double *xyz, const double *vxyz, bool check = false)
 {
     const size_t n3 = 3 * (size_t)s->P.N;
     if (!vxyz) {   // keep velocities: bring them to original order in the second half of scratch first
@@ -327,6 +328,19 @@ int upload_state(md_system *s, const double *xyz, const double *vxyz)
         src = vxyz;
         if (!is_pinned(vxyz)) { memcpy(s->h_stage + n3, vxyz, n3 * sizeof(double)); src = s->h_stage + n3; }
         CK(cudaMemcpyAsync(s->P.scratch + n3, src, n3 * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    }
+    if (check) {
+        s->launches += 1;
+        mdk_check_range(s->P, s->prm.box, s->stream);
+        int rc = fetch_ctrl(s);
+        if (rc) return rc;
+        if (s->h_ctrl->err == MD_ERR_INVALID) {
+            CK(cudaMemsetAsync(&s->P.ctrl->err, 0, sizeof(int), s->stream));
+            const double L = s->prm.box;
+            for (size_t i = 0; i < n3; i++)
+                if (!(xyz[i] >= 0.0 && xyz[i] <= L)) { set_error("md_set_state: coordinate %zu = %g outside [0, L]", i, xyz[i]); break; }
+            return MD_ERR_INVALID;
+        }
     }
     return install_state(s);
 }
@@ -644,14 +658,7 @@ md_system *md_create(int64_t n_atoms, double box, double density, double r_cut, 
 int md_set_state(md_system *s, const double *xyz, const double *vxyz)
 {
     if (!s || !xyz) { set_error("md_set_state: null argument"); return MD_ERR_INVALID; }
-    const double L = s->prm.box;
-    const size_t n3 = 3 * (size_t)s->P.N;
-    int bad = 0;
-    for (size_t i = 0; i < n3; i++) bad |= !(xyz[i] >= 0.0 && xyz[i] <= L);      // branch-free: vectorises
-    if (bad)
-        for (size_t i = 0; i < n3; i++)
-            if (!(xyz[i] >= 0.0 && xyz[i] <= L)) { set_error("md_set_state: coordinate %zu = %g outside [0, L]", i, xyz[i]); return MD_ERR_INVALID; }
-    return upload_state(s, xyz, vxyz);
+    return upload_state(s, xyz, vxyz, true);      // the range check [0, L] runs on the device, before the old state is touched
 }
 
 int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, double R0)

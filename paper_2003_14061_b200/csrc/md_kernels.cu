@@ -36,6 +36,19 @@ __global__ void k_force_rebuild(const __grid_constant__ MdDev P)
     c->since_reorder = 0;
 }
 
+// md_set_state's argument check, on the device: every coordinate of scratch[0 .. 3N) must lie in [0, box] (NaN fails).
+// (On the host this loop over 6.3 M doubles cost more than the H2D copy of the state at N = 2M.)
+__global__ void k_check_range(const __grid_constant__ MdDev P, double box)
+{
+    const size_t n3 = 3 * (size_t)P.N;
+    bool bad = false;
+    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < n3; k += (size_t)gridDim.x * blockDim.x) {
+        const double x = P.scratch[k];
+        bad |= !(x >= 0.0 && x <= box);
+    }
+    if (bad) set_err(P, MD_ERR_INVALID);
+}
+
 // scratch = [xyz (3N) | vxyz (3N)] in original-id order -> device arrays in identity order
 __global__ void k_load_state(const __grid_constant__ MdDev P)
 {
@@ -801,6 +814,11 @@ inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdi
 // launch wrappers
 // ------------------------------------------------------------------------------------------------
 void mdk_force_rebuild(const MdDev &P, cudaStream_t st) { k_force_rebuild<<<1, 1, 0, st>>>(P); }
+
+void mdk_check_range(const MdDev &P, double box, cudaStream_t st)
+{
+    k_check_range<<<std::min(cdiv(3LL * P.N, 256), 148 * 8), 256, 0, st>>>(P, box);
+}
 
 void mdk_load_state(const MdDev &P, cudaStream_t st)
 {

@@ -168,6 +168,7 @@ struct MdLaunch {
 };
 
 void mdk_force_rebuild(const MdDev &P, cudaStream_t st);
+void mdk_check_range(const MdDev &P, double box, cudaStream_t st);           // scratch xyz in [0, box] else ctrl->err = MD_ERR_INVALID
 void mdk_load_state(const MdDev &P, cudaStream_t st);                        // scratch(xyz | vxyz) -> pos/vel/id
 // rebuild decision from blk_vmax2[0..nblk); cond != 0: also set that CUDA-graph conditional handle to need_rebuild
 void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond);

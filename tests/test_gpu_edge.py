@@ -172,3 +172,28 @@ def test_two_systems_with_different_tiles_coexist(md):
         d -= box * np.round(d / box)
         assert np.abs(d).max() <= 1e-9
         g.close()
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_set_state_rejects_out_of_range_coordinates_and_keeps_the_old_state(md, precision):
+    """The range check of md_set_state runs on the device before anything of the old state is touched."""
+    cfg = get_config("wca_4k")
+    r, v, _, box = make_state(cfg, 1, jitter_amp=0.1)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", precision=precision)
+    g.set_state(r, v)
+    g.step(3)
+    p0, v0, e0 = g.positions(), g.velocities(), g.energies()
+    for bad_value in (box * 1.001, -1e-9, float("nan")):
+        bad = r.copy()
+        bad[1234, 2] = bad_value
+        with pytest.raises(md.MDError) as ei:
+            g.set_state(bad, v)
+        assert ei.value.code == md.binding.MD_ERR_INVALID and "coordinate" in str(ei.value)
+    assert np.array_equal(g.positions(), p0) and np.array_equal(g.velocities(), v0)
+    assert g.energies().total == e0.total and g.energies().step == 3
+    g.step(2)                                        # still usable
+    edge = r.copy()
+    edge[0, 0] = box                                 # x = L itself is accepted (wrapped to 0)
+    g.set_state(edge, v)
+    assert g.positions()[0, 0] == 0.0
+    g.close()
