@@ -182,7 +182,7 @@ MD_API int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double
  * no form: the textbook cosine-harmonic U = k_theta/2 (cos(theta) - cos_theta0)^2 is used, R19) at every
  * atom that has two bonded partners, theta the angle between its two bonds.  Call after md_set_bonds and before the
  * first md_step.  Forces and energies are re-evaluated; md_energy.pe_bond then holds FENE + angle energy (the terms
- * have no virial).  fp64, global-index W layouts only (MD_ERR_UNSUPPORTED otherwise). */
+ * have no virial).  Global-index W layouts only, either precision (MD_ERR_UNSUPPORTED with MD_FLAG_TILED_W). */
 MD_API int md_set_angles(md_system *s, double k_theta, double cos_theta0);
 
 /* Advance n time steps.  Asynchronous on the stream except for one status read at the end.

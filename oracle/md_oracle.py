@@ -112,6 +112,8 @@ def lib_sp():
         build()
         L = C.CDLL(_LIB_SP)
         _declare_system_api(L, "orcs_")
+        L.orcs_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orcs_set_angles.restype = C.c_int
         _lib_sp = L
     return _lib_sp
 
@@ -220,7 +222,7 @@ class OracleMD:
         return self._L.set_bonds(self._h, b.shape[0], b, float(k), float(r0))
 
     def set_angles(self, k, cos0):
-        """Cosine-harmonic bond-angle terms (fp64 oracle only); after set_bonds."""
+        """Cosine-harmonic bond-angle terms; after set_bonds."""
         return self._L.set_angles(self._h, float(k), float(cos0))
 
     def rebuild_neighbors(self):

@@ -48,6 +48,10 @@ typedef struct orcs_sys {
     float fene_kf, fene_R02f;
     double pe_bond, vir_bond;
     int bond_broken;
+    int32_t *partner;           /* 2 x N, from the bond list */
+    int has_angles;
+    float ang_kf, ang_c0f;
+    double pe_angle;
     double disp_acc;
     int64_t step, n_rebuilds;
     int32_t max_cell_occ;
@@ -122,7 +126,7 @@ void orcs_destroy(orcs_sys *s)
 {
     if (!s) return;
     free(s->r); free(s->v); free(s->f); free(s->u); free(s->w);
-    free(s->nb_start); free(s->nb); free(s->bonds);
+    free(s->nb_start); free(s->nb); free(s->bonds); free(s->partner);
     free(s);
 }
 
@@ -261,6 +265,30 @@ static void compute_forces(orcs_sys *s)
         }
         s->pe_bond = pe; s->vir_bond = vr;
     }
+    /* bond angles (R19) in binary32: the fp64 oracle's formulas, every operation rounded to binary32 */
+    s->pe_angle = 0;
+    if (s->has_angles) {
+        const float k = s->ang_kf, c0 = s->ang_c0f;
+        double pe = 0;
+        for (int64_t b = 0; b < N; b++) {
+            int64_t a = s->partner[b], c = s->partner[N + b];
+            if (a < 0 || c < 0) continue;
+            float d1[3], d2[3];
+            float n1 = dist2f(s->r + 3 * a, s->r + 3 * b, L, half, d1);
+            float n2 = dist2f(s->r + 3 * c, s->r + 3 * b, L, half, d2);
+            float dot = d1[0] * d2[0] + d1[1] * d2[1] + d1[2] * d2[2];
+            float inv12 = 1.0f / sqrtf(n1 * n2);
+            float cs = dot * inv12;
+            float g = -k * (cs - c0);
+            for (int q = 0; q < 3; q++) {
+                float fa = g * (d2[q] * inv12 - cs * d1[q] / n1);
+                float fc = g * (d1[q] * inv12 - cs * d2[q] / n2);
+                s->f[3 * a + q] += fa; s->f[3 * c + q] += fc; s->f[3 * b + q] -= fa + fc;
+            }
+            pe += (double)(0.5f * k * (cs - c0) * (cs - c0));
+        }
+        s->pe_angle = pe;
+    }
 }
 
 static void rebuild(orcs_sys *s)
@@ -286,8 +314,26 @@ int orcs_set_bonds(orcs_sys *s, int64_t nb, const int32_t *ij, double k, double 
     s->bonds = (int32_t *)malloc(2 * nb * sizeof(int32_t));
     memcpy(s->bonds, ij, 2 * nb * sizeof(int32_t));
     s->n_bonds = nb; s->fene_kf = (float)k; s->fene_R02f = (float)(R0 * R0);
+    free(s->partner);
+    s->partner = (int32_t *)malloc(2 * s->N * sizeof(int32_t));
+    for (int64_t i = 0; i < 2 * s->N; i++) s->partner[i] = -1;
+    for (int64_t b = 0; b < nb; b++)
+        for (int side = 0; side < 2; side++) {
+            int32_t a = ij[2 * b + side], c = ij[2 * b + 1 - side];
+            if (s->partner[a] < 0) s->partner[a] = c;
+            else if (s->partner[s->N + a] < 0) s->partner[s->N + a] = c;
+            else return -6;
+        }
     compute_forces(s);
     return s->bond_broken ? -3 : 0;
+}
+
+int orcs_set_angles(orcs_sys *s, double k, double cos0)
+{
+    if (!s->partner) return -1;
+    s->has_angles = 1; s->ang_kf = (float)k; s->ang_c0f = (float)cos0;
+    compute_forces(s);
+    return 0;
 }
 
 void orcs_rebuild_neighbors(orcs_sys *s) { rebuild(s); s->n_rebuilds--; compute_forces(s); }
@@ -335,7 +381,7 @@ void orcs_energies(orcs_sys *s, orcs_energy *e)
     }
     e->ke = 0.5 * ke;
     e->pe_pair = 0.5 * pe;
-    e->pe_bond = s->pe_bond;
+    e->pe_bond = s->pe_bond + s->pe_angle;
     e->virial = 0.5 * vir + s->vir_bond;
     e->px = px; e->py = py; e->pz = pz;
     e->vmax = sqrt(vmax2);

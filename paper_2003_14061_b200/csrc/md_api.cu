@@ -713,7 +713,7 @@ int md_set_angles(md_system *s, double k_theta, double cos_theta0)
     if (!s || !(k_theta >= 0) || !(cos_theta0 >= -1.0 && cos_theta0 <= 1.0)) { set_error("md_set_angles: bad argument"); return MD_ERR_INVALID; }
     if (!s->P.has_bonds) { set_error("md_set_angles: set the bond list first"); return MD_ERR_INVALID; }
     if (s->stepped) { set_error("md_set_angles: only before the first md_step"); return MD_ERR_INVALID; }
-    if (s->P.tiled || s->P.sp) { set_error("md_set_angles: fp64 global-index W layouts only (use MD_FLAG_GATHER_W)"); return MD_ERR_UNSUPPORTED; }
+    if (s->P.tiled) { set_error("md_set_angles: global-index W layouts only (use MD_FLAG_GATHER_W)"); return MD_ERR_UNSUPPORTED; }
     drop_graph(s);                 // the captured kernel arguments (MdDev by value) change
     s->P.has_angles = k_theta > 0;
     s->P.ang_k = k_theta;

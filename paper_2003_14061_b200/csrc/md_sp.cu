@@ -272,9 +272,52 @@ __device__ __forceinline__ void pair_force_f(const float4 &ri, const float4 &rj,
     a.fx = fmaf(fc, dx, a.fx); a.fy = fmaf(fc, dy, a.fy); a.fz = fmaf(fc, dz, a.fz);
 }
 
+__device__ __forceinline__ float mi_disp_f(const MdDev &P, const float4 &a, const float4 &b, float &dx, float &dy, float &dz)
+{
+    dx = minimgf(__fsub_rn(a.x, b.x), P.Lf, P.half_Lf); dy = minimgf(__fsub_rn(a.y, b.y), P.Lf, P.half_Lf);
+    dz = minimgf(__fsub_rn(a.z, b.z), P.Lf, P.half_Lf);
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+// bond-angle terms in binary32: md_kernels.cu:angle_force (R19)
+__device__ __forceinline__ void angle_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, PairAccF &a)
+{
+    const int p[2] = {P.bond_dev[i], P.bond_dev[(size_t)P.N_pad + i]};
+    const float k = (float)P.ang_k, c0 = (float)P.ang_c0;
+    float4 rp[2];
+#pragma unroll
+    for (int q = 0; q < 2; q++)
+        if (p[q] >= 0) rp[q] = ld4(pos + p[q]);
+    if (p[0] >= 0 && p[1] >= 0) {
+        float x1, y1, z1, x2, y2, z2;
+        const float n1 = mi_disp_f(P, rp[0], ri, x1, y1, z1), n2 = mi_disp_f(P, rp[1], ri, x2, y2, z2);
+        const float inv12 = 1.0f / sqrtf(n1 * n2), c = (x1 * x2 + y1 * y2 + z1 * z2) * inv12;
+        const float g = -k * (c - c0), u1 = c / n1, u2 = c / n2;
+        a.fx -= g * ((x2 * inv12 - u1 * x1) + (x1 * inv12 - u2 * x2));
+        a.fy -= g * ((y2 * inv12 - u1 * y1) + (y1 * inv12 - u2 * y2));
+        a.fz -= g * ((z2 * inv12 - u1 * z1) + (z1 * inv12 - u2 * z2));
+    }
+#pragma unroll
+    for (int q = 0; q < 2; q++) {
+        if (p[q] < 0) continue;
+        const int q0 = P.bond_dev[p[q]], q1 = P.bond_dev[(size_t)P.N_pad + p[q]];
+        const int o = q0 == i ? q1 : q0;
+        if (o < 0) continue;
+        const float4 ro = ld4(pos + o);
+        float x1, y1, z1, x2, y2, z2;
+        const float n1 = mi_disp_f(P, ri, rp[q], x1, y1, z1), n2 = mi_disp_f(P, ro, rp[q], x2, y2, z2);
+        const float inv12 = 1.0f / sqrtf(n1 * n2), c = (x1 * x2 + y1 * y2 + z1 * z2) * inv12;
+        const float g = -k * (c - c0), u1 = c / n1;
+        a.fx += g * (x2 * inv12 - u1 * x1);
+        a.fy += g * (y2 * inv12 - u1 * y1);
+        a.fz += g * (z2 * inv12 - u1 * z1);
+    }
+}
+
 template <bool CHECK>
 __device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, PairAccF &a)
 {
+    if (P.has_angles) angle_force_f(P, pos, ri, i, a);
 #pragma unroll
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
@@ -435,6 +478,16 @@ __global__ void __launch_bounds__(256) k_sp_energy(const __grid_constant__ MdDev
                 const float x = 1.0f - r2 / P.fene_R02f;
                 q[RED_PEB] += 0.5 * (double)(-0.5f * P.fene_kf * P.fene_R02f * logf(x));
                 q[RED_VIR] += 0.5 * (double)((-P.fene_kf / x) * r2);
+            }
+            if (P.has_angles) {
+                const int p0 = P.bond_dev[i], p1 = P.bond_dev[(size_t)P.N_pad + i];
+                if (p0 >= 0 && p1 >= 0) {
+                    float x1, y1, z1, x2, y2, z2;
+                    const float n1 = mi_disp_f(P, ld4(pos + p0), ri, x1, y1, z1), n2 = mi_disp_f(P, ld4(pos + p1), ri, x2, y2, z2);
+                    const float c = (x1 * x2 + y1 * y2 + z1 * z2) * (1.0f / sqrtf(n1 * n2));
+                    const float k = (float)P.ang_k, c0 = (float)P.ang_c0;
+                    q[RED_PEB] += (double)(0.5f * k * (c - c0) * (c - c0));
+                }
             }
         }
         const float4 v = P.velf[vc][i];

@@ -92,7 +92,7 @@ def test_angles_call_order_and_unsupported(md):
     with pytest.raises(md.MDError):                           # only before the first step
         g.set_angles(2.0, -1.0)
     g.close()
-    for kw in (dict(flags=md.FLAG_TILED_W), dict(precision="f32")):
+    for kw in (dict(flags=md.FLAG_TILED_W),):
         g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", **kw)
         g.set_state(r, v)
         g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
@@ -100,3 +100,32 @@ def test_angles_call_order_and_unsupported(md):
             g.set_angles(2.0, -1.0)
         assert ei.value.code == md.binding.MD_ERR_UNSUPPORTED
         g.close()
+
+
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("mode", ["fused", "split"])
+def test_angles_single_precision(md, case, mode):
+    """Binary32 variant against the binary32 oracle, bounds of tests/test_gpu_sp.py."""
+    from oracle.md_oracle import OracleMDSP
+    eps = 2.0 ** -24
+    n, clen = CASES[case]
+    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    r, v, bonds, box = make_state(cfg, 1)
+    o = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(r, v)
+    o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    assert o.set_angles(5.0, -0.5) == 0
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", step_mode=mode, precision="f32")
+    g.set_state(r, v)
+    g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    g.set_angles(5.0, -0.5)
+    fo = o.forces()
+    assert np.abs(g.forces() - fo).max() <= 64 * eps * 4 * np.abs(fo).max()
+    eg, eo = g.energies(), o.energies()
+    assert abs(eg.pe_bond - eo.pe_bond) <= 64 * eps * abs(eo.pe_bond)
+    g.step(10)
+    assert o.step(10) == 0
+    assert pos_err(g.positions(), o.positions(), float(np.float32(box))) <= 16 * float(np.spacing(np.float32(box)))
+    eg, eo = g.energies(), o.energies()
+    assert abs(eg.pe - eo.pe) <= 64 * eps * max(abs(eo.pe), eo.ke) * 4
+    g.close()
