@@ -25,6 +25,8 @@
  *   - bond angles ("bond-angle torque"): PAPER.md gives no form; the textbook
  *     cosine-harmonic U = k/2 (cos(theta) - cos(theta0))^2 at every atom with two bonded partners
  *     (reading R19), forces by the chain rule on cos(theta) = d1.d2 / (|d1||d2|).
+ *   - dihedral terms ("optional dihedral"): U = k/2 (cos(phi) - cos(phi0))^2 for every four consecutive
+ *     beads, cos(phi) = A.B/(|A||B|), A = b1 x b2, B = b2 x b3 (R19); forces by the chain rule through A, B.
  *
  * Parity pins for every function here live in tests/test_oracle_pins.py (brute force on tiny
  * inputs, closed forms on the SC/FCC lattices, two-atom values, conservation laws, reversibility,
@@ -69,6 +71,8 @@ typedef struct orc_sys {
     int32_t *partner;       /* 2 x N */
     int has_angles;
     double ang_k, ang_c0, pe_angle;
+    int has_dihedrals;
+    double dih_k, dih_c0, pe_dihedral;
     /* bookkeeping */
     double disp_acc;
     int64_t step, n_rebuilds;
@@ -381,6 +385,44 @@ static void compute_forces(orc_sys *s)
         }
         s->pe_angle = pe;
     }
+    /* dihedrals (R19): one per bond (b, c) whose ends both continue: a - b - c - d.
+     * b1 = r_b - r_a, b2 = r_c - r_b, b3 = r_d - r_c (minimum image); A = b1 x b2, B = b2 x b3; c = A.B/(|A||B|).
+     * gA = dc/dA = B/(|A||B|) - c A/|A|^2, gB likewise; dc/db1 = b2 x gA, dc/db2 = gA x b1 + b3 x gB, dc/db3 = gB x b2;
+     * dc/dr_a = -dc/db1, dc/dr_b = dc/db1 - dc/db2, dc/dr_c = dc/db2 - dc/db3, dc/dr_d = dc/db3;  f = -k (c - c0) dc/dr. */
+    s->pe_dihedral = 0;
+    if (s->has_dihedrals) {
+        double pe = 0;
+        for (int64_t q = 0; q < s->n_bonds; q++) {
+            int64_t b = s->bonds[2 * q], c = s->bonds[2 * q + 1];
+            int64_t a = s->partner[b] == c ? s->partner[N + b] : s->partner[b];
+            int64_t d = s->partner[c] == b ? s->partner[N + c] : s->partner[c];
+            if (a < 0 || d < 0) continue;
+            double b1[3], b2[3], b3[3], A[3], B[3], gA[3], gB[3], g1[3], g2[3], g3[3], t1[3], t2[3];
+            dist2(s->r + 3 * b, s->r + 3 * a, L, half, b1);
+            dist2(s->r + 3 * c, s->r + 3 * b, L, half, b2);
+            dist2(s->r + 3 * d, s->r + 3 * c, L, half, b3);
+#define CROSS(o, u, v) do { o[0] = u[1] * v[2] - u[2] * v[1]; o[1] = u[2] * v[0] - u[0] * v[2]; o[2] = u[0] * v[1] - u[1] * v[0]; } while (0)
+            CROSS(A, b1, b2); CROSS(B, b2, b3);
+            double nA = A[0] * A[0] + A[1] * A[1] + A[2] * A[2], nB = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+            double invAB = 1.0 / sqrt(nA * nB);
+            double cs = (A[0] * B[0] + A[1] * B[1] + A[2] * B[2]) * invAB;
+            for (int k = 0; k < 3; k++) { gA[k] = B[k] * invAB - cs * A[k] / nA; gB[k] = A[k] * invAB - cs * B[k] / nB; }
+            CROSS(g1, b2, gA);                       /* dc/db1 */
+            CROSS(t1, gA, b1); CROSS(t2, b3, gB);    /* dc/db2 = t1 + t2 */
+            CROSS(g3, gB, b2);                       /* dc/db3 */
+            for (int k = 0; k < 3; k++) g2[k] = t1[k] + t2[k];
+#undef CROSS
+            double g = -s->dih_k * (cs - s->dih_c0);
+            for (int k = 0; k < 3; k++) {
+                s->f[3 * a + k] += g * (-g1[k]);
+                s->f[3 * b + k] += g * (g1[k] - g2[k]);
+                s->f[3 * c + k] += g * (g2[k] - g3[k]);
+                s->f[3 * d + k] += g * g3[k];
+            }
+            pe += 0.5 * s->dih_k * (cs - s->dih_c0) * (cs - s->dih_c0);
+        }
+        s->pe_dihedral = pe;
+    }
 }
 
 static void rebuild(orc_sys *s)
@@ -420,6 +462,15 @@ int orc_set_bonds(orc_sys *s, int64_t nb, const int32_t *ij, double k, double R0
         }
     compute_forces(s);
     return s->bond_broken ? -3 : 0;
+}
+
+/* dihedral terms for every four consecutive bonded atoms; call after orc_set_bonds */
+int orc_set_dihedrals(orc_sys *s, double k, double cos0)
+{
+    if (!s->partner) return -1;
+    s->has_dihedrals = 1; s->dih_k = k; s->dih_c0 = cos0;
+    compute_forces(s);
+    return 0;
 }
 
 /* bond-angle terms at every atom with two bonded partners; call after orc_set_bonds */
@@ -492,7 +543,7 @@ void orc_energies(orc_sys *s, orc_energy *e)
     e->ke = 0.5 * nsum(v2, N, 1);
     free(v2);
     e->pe_pair = 0.5 * nsum(s->u, N, 1);
-    e->pe_bond = s->pe_bond + s->pe_angle;      /* bonded energy: FENE + angle terms */
+    e->pe_bond = s->pe_bond + s->pe_angle + s->pe_dihedral;      /* bonded energy: FENE + angle + dihedral terms */
     e->virial = 0.5 * nsum(s->w, N, 1) + s->vir_bond;
     e->px = nsum(s->v, N, 3); e->py = nsum(s->v + 1, N, 3); e->pz = nsum(s->v + 2, N, 3);
     e->vmax = sqrt(vmax2);

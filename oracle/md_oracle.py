@@ -125,6 +125,8 @@ def lib():
         _declare_system_api(L, "orc_")
         L.orc_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orc_set_angles.restype = C.c_int
+        L.orc_set_dihedrals.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orc_set_dihedrals.restype = C.c_int
         L.orc_brute_forces.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, _dp, _dp, _dp]
         L.orc_brute_forces_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp, _dp, _dp, _dp]
         L.orc_brute_neighbors_sample.argtypes = [C.c_int64, C.c_double, _dp, C.c_double, C.c_int64, _lp,
@@ -224,6 +226,10 @@ class OracleMD:
     def set_angles(self, k, cos0):
         """Cosine-harmonic bond-angle terms; after set_bonds."""
         return self._L.set_angles(self._h, float(k), float(cos0))
+
+    def set_dihedrals(self, k, cos0):
+        """Cosine-harmonic dihedral terms (fp64 oracle only); after set_bonds."""
+        return self._L.set_dihedrals(self._h, float(k), float(cos0))
 
     def rebuild_neighbors(self):
         self._L.rebuild_neighbors(self._h)

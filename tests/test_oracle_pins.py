@@ -478,3 +478,75 @@ def test_p14_angle_run_conserves_energy_and_momentum():
         return np.std(es)
     ratio = fluct(cfg.dt, 100) / fluct(cfg.dt / 2, 200)
     assert 2.5 < ratio < 6.0
+
+
+# ---- P15: dihedral terms (R19) ---------------------------------------
+def np_dihedral_energy(r, box, quads, k, c0):
+    """U = k/2 (cos(phi) - c0)^2; cos(phi) from the unit normals of the planes (a,b,c) and (b,c,d)."""
+    e = 0.0
+    for a, b, c, d in quads:
+        def mi(u):
+            return u - box * np.round(u / box)
+        b1, b2, b3 = mi(r[b] - r[a]), mi(r[c] - r[b]), mi(r[d] - r[c])
+        n1, n2 = np.cross(b1, b2), np.cross(b2, b3)
+        cs = float(np.dot(n1 / np.linalg.norm(n1), n2 / np.linalg.norm(n2)))
+        e += 0.5 * k * (cs - c0) ** 2
+    return e
+
+
+def test_p15_dihedral_closed_forms():
+    box = 12.0
+    bonds = np.array([[0, 1], [1, 2], [2, 3]], np.int32)
+    def run(r, k, c0):
+        o = OracleMD(4, box, R_WCA, 0.4, 0.005, brute_search=True)
+        o.set_state(np.array(r, float), np.zeros((4, 3)))
+        assert o.set_bonds(bonds, 30.0, 1.5) == 0
+        f0, e0 = o.forces().copy(), o.energies().pe_bond
+        assert o.set_dihedrals(k, c0) == 0
+        return o.forces() - f0, o.energies().pe_bond - e0
+    # planar zig-zag (trans): the two plane normals are antiparallel, cos(phi) = -1: nothing for phi0 = pi
+    df, de = run([[2, 2, 2], [3, 2.2, 2], [4, 2, 2], [5, 2.2, 2]], 3.0, -1.0)
+    assert np.abs(df).max() < 1e-12 and abs(de) < 1e-14
+    # planar cis: normals parallel, cos(phi) = +1: U = k/2 (1 - c0)^2 = 6, and a planar arrangement is stationary
+    df, de = run([[2, 2.2, 2], [3, 2, 2], [4, 2, 2], [5, 2.2, 2]], 3.0, -1.0)
+    assert de == pytest.approx(6.0, abs=1e-12) and np.abs(df).max() < 1e-9
+    # quarter twist: cos(phi) = 0: U = k/2 c0^2; end atoms are pushed perpendicular to their own planes
+    df, de = run([[2, 3, 2], [2, 2, 2], [3, 2, 2], [3, 2, 3]], 4.0, -1.0)
+    assert de == pytest.approx(2.0, abs=1e-13)
+    # a (2,3,2): plane normal of (a,b,c) is z; force on a along -/+ z only, magnitude k |c - c0| / |b1| = 4
+    assert abs(abs(df[0, 2]) - 4.0) < 1e-12 and np.abs(df[0, :2]).max() < 1e-12
+    assert abs(abs(df[3, 1]) - 4.0) < 1e-12 and np.abs(df[3, [0, 2]]).max() < 1e-12
+    assert np.abs(df.sum(0)).max() < 1e-12
+
+
+def test_p15_dihedral_forces_are_minus_gradient_of_numpy_energy():
+    r, bonds, triples, box = chain_system(n_chains=5, length=8, seed=9)
+    n, length = r.shape[0], 8
+    quads = [(c * length + s, c * length + s + 1, c * length + s + 2, c * length + s + 3)
+             for c in range(n // length) for s in range(length - 3)]
+    k, c0 = 3.0, -0.7
+    o = OracleMD(n, box, R_WCA, 0.4, 0.005)
+    o.set_state(r, np.zeros_like(r))
+    assert o.set_bonds(bonds, 30.0, 1.5) == 0
+    f0, e0 = o.forces().copy(), o.energies()
+    assert o.set_dihedrals(k, c0) == 0
+    fd = o.forces() - f0
+    e1 = o.energies()
+    assert e1.pe_bond - e0.pe_bond == pytest.approx(np_dihedral_energy(r, box, quads, k, c0), rel=1e-12)
+    assert e1.virial == pytest.approx(e0.virial, rel=1e-13)          # scale invariant: no virial
+    h = 1e-6
+    rng = np.random.default_rng(1)
+    for i in rng.choice(n, 12, replace=False):
+        for q in range(3):
+            rp, rm = r.copy(), r.copy()
+            rp[i, q] += h
+            rm[i, q] -= h
+            g = (np_dihedral_energy(rp, box, quads, k, c0) - np_dihedral_energy(rm, box, quads, k, c0)) / (2 * h)
+            assert fd[i, q] == pytest.approx(-g, abs=5e-8 * max(1.0, np.abs(fd).max()))
+    scale = np.abs(o.forces()).sum()
+    assert np.abs(fd.sum(0)).max() < 1e-12 * scale
+    for ch in range(n // length):
+        sl = slice(ch * length, (ch + 1) * length)
+        dd = r[sl] - r[sl][0]
+        dd -= box * np.round(dd / box)
+        assert np.abs(np.cross(dd, fd[sl]).sum(0)).max() < 1e-11 * scale
