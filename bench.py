@@ -213,6 +213,11 @@ def main():
                     help="permute the atom numbering of the start state (a decorrelated storage order, for the sort ablation)")
     ap.add_argument("--angles", type=float, default=0.0,
                     help="chain workloads: bond-angle stiffness k_theta of md_set_angles (cos theta0 = -1), 0 = off")
+    ap.add_argument("--angle-cos0", type=float, default=-1.0)
+    ap.add_argument("--dihedrals", type=float, default=0.0,
+                    help="chain workloads: dihedral stiffness k_phi of md_set_dihedrals, 0 = off (the cosine form is singular "
+                         "for collinear bonds: combine with stiff bent angles, e.g. --angles 40 --angle-cos0 -0.5)")
+    ap.add_argument("--dihedral-cos0", type=float, default=-0.6)
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -261,7 +266,9 @@ def main():
     if states[0][2] is not None:
         g.set_bonds(np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)]), cfg.fene_k, cfg.fene_r0)
         if args.angles > 0:
-            g.set_angles(args.angles, -1.0)
+            g.set_angles(args.angles, args.angle_cos0)
+        if args.dihedrals > 0:
+            g.set_dihedrals(args.dihedrals, args.dihedral_cos0)
     del states
     info = g.info()
     n = cfg.n_atoms * nsys                  # atoms advanced per step
@@ -399,7 +406,7 @@ def main():
                    "lattice": cfg.lattice, "density": cfg.density,
                    "r_cut": cfg.r_cut, "r_shell": cfg.r_shell, "dt": cfg.dt, "temperature": cfg.temperature,
                    "force_variant": args.variant, "step_mode": args.mode, "precision": args.precision,
-                   "angle_k": args.angles, "flags": args.flags, "reorder_interval": args.reorder_interval, "shuffled_ids": bool(args.shuffle), "block_size": info["block_size"],
+                   "angle_k": args.angles, "dihedral_k": args.dihedrals, "flags": args.flags, "reorder_interval": args.reorder_interval, "shuffled_ids": bool(args.shuffle), "block_size": info["block_size"],
                    "max_neighbors": info["max_neighbors"], "cells_per_edge": info["cells_per_edge"],
                    "w_layout": "tiled16" if tiled else "global32", "tile_cells": info["tile_cells"],
                    "cuda_graph": bool(info_end["use_graph"]),

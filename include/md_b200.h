@@ -185,6 +185,11 @@ MD_API int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double
  * have no virial).  Global-index W layouts only, either precision (MD_ERR_UNSUPPORTED with MD_FLAG_TILED_W). */
 MD_API int md_set_angles(md_system *s, double k_theta, double cos_theta0);
 
+/* Optional dihedral terms ("optional dihedral"; R19): U = k_phi/2 (cos(phi) - cos_phi0)^2 for
+ * every four consecutive bonded atoms a-b-c-d, phi the angle between the planes (a,b,c) and (b,c,d) (cos(phi) = -1 for a
+ * planar zig-zag).  Same call order and reporting as md_set_angles.  fp64, global-index W layouts only. */
+MD_API int md_set_dihedrals(md_system *s, double k_phi, double cos_phi0);
+
 /* Advance n time steps.  Asynchronous on the stream except for one status read at the end.
  * After an error other than MD_ERR_INVALID the state is undefined; only md_destroy is valid. */
 MD_API int md_step(md_system *s, int64_t n);

@@ -24,7 +24,7 @@ STEP_MODE = {"fused": 0, "split": 1}
 PRECISION = {"f64": 0, "f32": 1}
 TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "decide")
 
-EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_set_angles", "md_step", "md_energies",
+EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
            "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
            "md_set_allocator", "md_last_error", "md_version")
@@ -113,6 +113,7 @@ def load_library(path: str = LIB_PATH):
     L.md_destroy.argtypes = [C.c_void_p]
     L.md_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
     L.md_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
+    L.md_set_dihedrals.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_step.argtypes = [C.c_void_p, C.c_int64]
     L.md_energies.argtypes = [C.c_void_p, C.POINTER(_Energy)]
     for n in ("md_get_positions", "md_get_velocities", "md_get_forces"):
@@ -220,6 +221,9 @@ class MDSystem:
 
     def set_angles(self, k_theta, cos_theta0):
         self._ck(self._L.md_set_angles(self._h, float(k_theta), float(cos_theta0)))
+
+    def set_dihedrals(self, k_phi, cos_phi0):
+        self._ck(self._L.md_set_dihedrals(self._h, float(k_phi), float(cos_phi0)))
 
     def step(self, n=1):
         self._ck(self._L.md_step(self._h, int(n)))

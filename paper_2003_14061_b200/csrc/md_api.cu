@@ -722,6 +722,20 @@ int md_set_angles(md_system *s, double k_theta, double cos_theta0)
     return check_device_status(s);
 }
 
+int md_set_dihedrals(md_system *s, double k_phi, double cos_phi0)
+{
+    if (!s || !(k_phi >= 0) || !(cos_phi0 >= -1.0 && cos_phi0 <= 1.0)) { set_error("md_set_dihedrals: bad argument"); return MD_ERR_INVALID; }
+    if (!s->P.has_bonds) { set_error("md_set_dihedrals: set the bond list first"); return MD_ERR_INVALID; }
+    if (s->stepped) { set_error("md_set_dihedrals: only before the first md_step"); return MD_ERR_INVALID; }
+    if (s->P.tiled || s->P.sp) { set_error("md_set_dihedrals: fp64 global-index W layouts only"); return MD_ERR_UNSUPPORTED; }
+    drop_graph(s);
+    s->P.has_dihedrals = k_phi > 0;
+    s->P.dih_k = k_phi;
+    s->P.dih_c0 = cos_phi0;
+    enqueue_forces_only(s);
+    return check_device_status(s);
+}
+
 int md_rebuild_neighbors(md_system *s)
 {
     if (!s || !s->has_state) { set_error("md_rebuild_neighbors: no state"); return MD_ERR_INVALID; }

@@ -576,10 +576,79 @@ __device__ __forceinline__ void angle_force(const MdDev &P, const pos_t *__restr
     }
 }
 
-template <bool CHECK>
+// Dihedral terms ("optional dihedral"; R19): U = k/2 (cos(phi) - c0)^2 for every four consecutive
+// beads a-b-c-d, cos(phi) = A.B/(|A||B|), A = b1 x b2, B = b2 x b3, b1 = r_b - r_a, b2 = r_c - r_b, b3 = r_d - r_c.
+// With gA = B/(|A||B|) - c A/|A|^2, gB = A/(|A||B|) - c B/|B|^2:
+//   dc/db1 = b2 x gA, dc/db2 = gA x b1 + b3 x gB, dc/db3 = gB x b2,
+//   dc/dr_a = -dc/db1, dc/dr_b = dc/db1 - dc/db2, dc/dr_c = dc/db2 - dc/db3, dc/dr_d = dc/db3;  f = -k (c - c0) dc/dr.
+struct V3 {
+    double x, y, z;
+};
+__device__ __forceinline__ V3 cross3(const V3 &u, const V3 &v) { return {u.y * v.z - u.z * v.y, u.z * v.x - u.x * v.z, u.x * v.y - u.y * v.x}; }
+__device__ __forceinline__ V3 mi_vec(const MdDev &P, const pos_t &a, const pos_t &b)
+{
+    V3 d;
+    mi_disp(P, a, b, d.x, d.y, d.z);
+    return d;
+}
+
+// cos(phi) of a-b-c-d and, if WHICH >= 0, the force on atom WHICH (0 = a .. 3 = d) added to acc
+__device__ __forceinline__ double dihedral_term(const MdDev &P, const pos_t &ra, const pos_t &rb, const pos_t &rc, const pos_t &rd, int which,
+                                                PairAcc &acc)
+{
+    const V3 b1 = mi_vec(P, rb, ra), b2 = mi_vec(P, rc, rb), b3 = mi_vec(P, rd, rc);
+    const V3 A = cross3(b1, b2), B = cross3(b2, b3);
+    const double nA = A.x * A.x + A.y * A.y + A.z * A.z, nB = B.x * B.x + B.y * B.y + B.z * B.z;
+    const double invAB = 1.0 / sqrt(nA * nB), c = (A.x * B.x + A.y * B.y + A.z * B.z) * invAB;
+    if (which < 0) return c;
+    const double uA = c / nA, uB = c / nB;
+    const V3 gA = {B.x * invAB - uA * A.x, B.y * invAB - uA * A.y, B.z * invAB - uA * A.z};
+    const V3 gB = {A.x * invAB - uB * B.x, A.y * invAB - uB * B.y, A.z * invAB - uB * B.z};
+    const V3 g1 = cross3(b2, gA), t1 = cross3(gA, b1), t2 = cross3(b3, gB), g3 = cross3(gB, b2);
+    const V3 g2 = {t1.x + t2.x, t1.y + t2.y, t1.z + t2.z};
+    V3 d;
+    if (which == 0) d = {-g1.x, -g1.y, -g1.z};
+    else if (which == 1) d = {g1.x - g2.x, g1.y - g2.y, g1.z - g2.z};
+    else if (which == 2) d = {g2.x - g3.x, g2.y - g3.y, g2.z - g3.z};
+    else d = g3;
+    const double g = -P.dih_k * (c - P.dih_c0);
+    acc.fx += g * d.x; acc.fy += g * d.y; acc.fz += g * d.z;
+    return c;
+}
+
+// the partner of x other than prev (-1 at a chain end)
+__device__ __forceinline__ int chain_next(const MdDev &P, int x, int prev)
+{
+    const int q0 = P.bond_dev[x], q1 = P.bond_dev[(size_t)P.N_pad + x];
+    return q0 == prev ? q1 : q0;
+}
+
+// atom i collects its force from the (up to four) dihedrals it belongs to, found by walking three bonds either way.
+// Not inlined: its ~60 live fp64 values would otherwise spill inside the force kernels even when the terms are off.
+__device__ __noinline__ void dihedral_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
+{
+    const int L1 = P.bond_dev[i], R1 = P.bond_dev[(size_t)P.N_pad + i];
+    const int L2 = L1 >= 0 ? chain_next(P, L1, i) : -1, L3 = L2 >= 0 ? chain_next(P, L2, L1) : -1;
+    const int R2 = R1 >= 0 ? chain_next(P, R1, i) : -1, R3 = R2 >= 0 ? chain_next(P, R2, R1) : -1;
+    pos_t l1, l2, l3, r1, r2, r3;
+    if (L1 >= 0) l1 = ld_pos(pos + L1);
+    if (L2 >= 0) l2 = ld_pos(pos + L2);
+    if (L3 >= 0) l3 = ld_pos(pos + L3);
+    if (R1 >= 0) r1 = ld_pos(pos + R1);
+    if (R2 >= 0) r2 = ld_pos(pos + R2);
+    if (R3 >= 0) r3 = ld_pos(pos + R3);
+    if (L3 >= 0) dihedral_term(P, l3, l2, l1, ri, 3, a);
+    if (L2 >= 0 && R1 >= 0) dihedral_term(P, l2, l1, ri, r1, 2, a);
+    if (L1 >= 0 && R2 >= 0) dihedral_term(P, l1, ri, r1, r2, 1, a);
+    if (R3 >= 0) dihedral_term(P, ri, r1, r2, r3, 0, a);
+}
+
+// EXTRAS: the angle / dihedral code is compiled in (kernels instantiated without it keep the registers of the FENE-only path)
+template <bool CHECK, bool EXTRAS = true>
 __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
 {
-    if (P.has_angles) angle_force(P, pos, ri, i, a);
+    if (EXTRAS && P.has_angles) angle_force(P, pos, ri, i, a);
+    if (EXTRAS && P.has_dihedrals) dihedral_force(P, pos, ri, i, a);
 #pragma unroll
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
@@ -639,7 +708,8 @@ __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__r
 
 // MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = r + dt v into the other position
 // buffer, max |v|, rebuild decision.  MODE 2: store f and apply the closing half kick v += dt/2 f.
-template <int MODE, bool BONDS, int BLOCK>
+// BONDS: 0 none, 1 FENE bonds, 2 FENE + angle / dihedral terms
+template <int MODE, int BONDS, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
@@ -654,7 +724,8 @@ __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(c
         double v0 = 0.0, v1 = 0.0, v2i = 0.0;
         if (MODE != 0) { v0 = v[0]; v1 = v[np]; v2i = v[2 * np]; }     // in flight while the column is walked
         PairAcc a = column_force<MD_FORCE_U, MD_FORCE_D>(P, pos, ri, i);
-        if (BONDS) bond_force<true>(P, pos, ri, i, a);
+        if (BONDS == 1) bond_force<true, false>(P, pos, ri, i, a);
+        if (BONDS == 2) bond_force<true, true>(P, pos, ri, i, a);
         if (MODE == 0 || MODE == 2) {
             double *f = P.frc + i;
             f[0] = a.fx; f[np] = a.fy; f[2 * np] = a.fz;
@@ -783,6 +854,18 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
                 q[RED_PEB] += 0.5 * (-0.5 * P.fene_k * P.fene_R02 * log(x));
                 q[RED_VIR] += 0.5 * (-P.fene_k / x) * r2;
             }
+            if (P.has_dihedrals) {   // the dihedral around the bond (i, partner), counted by the end with the smaller index
+#pragma unroll
+                for (int k = 0; k < 2; k++) {
+                    const int pk = P.bond_dev[(size_t)k * P.N_pad + i], qk = P.bond_dev[(size_t)(1 - k) * P.N_pad + i];
+                    if (pk < 0 || qk < 0 || i > pk) continue;
+                    const int o = chain_next(P, pk, i);
+                    if (o < 0) continue;
+                    PairAcc dummy = {0.0, 0.0, 0.0};
+                    const double c = dihedral_term(P, ld_pos(pos + qk), ri, ld_pos(pos + pk), ld_pos(pos + o), -1, dummy);
+                    q[RED_PEB] += 0.5 * P.dih_k * (c - P.dih_c0) * (c - P.dih_c0);
+                }
+            }
             if (P.has_angles) {      // the angle i is the vertex of, counted once; cos(theta) is scale invariant: no virial
                 const int p0 = P.bond_dev[i], p1 = P.bond_dev[(size_t)P.N_pad + i];
                 if (p0 >= 0 && p1 >= 0) {
@@ -879,7 +962,7 @@ void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
     else k_build<false><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
 }
 
-template <int MODE, bool BONDS>
+template <int MODE, int BONDS>
 static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
 {
     switch (block) {
@@ -893,14 +976,18 @@ static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
 void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 {
     if (P.sp) return mdk_sp_force(P, lc, mode, st);
-    if (P.has_bonds) {
-        if (mode == 0) launch_force_block<0, true>(P, lc.block, st);
-        else if (mode == 1) launch_force_block<1, true>(P, lc.block, st);
-        else launch_force_block<2, true>(P, lc.block, st);
+    if (P.has_bonds && (P.has_angles || P.has_dihedrals)) {
+        if (mode == 0) launch_force_block<0, 2>(P, lc.block, st);
+        else if (mode == 1) launch_force_block<1, 2>(P, lc.block, st);
+        else launch_force_block<2, 2>(P, lc.block, st);
+    } else if (P.has_bonds) {
+        if (mode == 0) launch_force_block<0, 1>(P, lc.block, st);
+        else if (mode == 1) launch_force_block<1, 1>(P, lc.block, st);
+        else launch_force_block<2, 1>(P, lc.block, st);
     } else {
-        if (mode == 0) launch_force_block<0, false>(P, lc.block, st);
-        else if (mode == 1) launch_force_block<1, false>(P, lc.block, st);
-        else launch_force_block<2, false>(P, lc.block, st);
+        if (mode == 0) launch_force_block<0, 0>(P, lc.block, st);
+        else if (mode == 1) launch_force_block<1, 0>(P, lc.block, st);
+        else launch_force_block<2, 0>(P, lc.block, st);
     }
 }
 

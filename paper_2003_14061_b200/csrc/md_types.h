@@ -136,6 +136,8 @@ struct MdDev {
     double fene_k, fene_R02;
     int has_angles;                     // bond-angle terms k/2 (cos(theta) - c0)^2 at atoms with two bonds (md_set_angles)
     double ang_k, ang_c0;
+    int has_dihedrals;                  // dihedral terms k/2 (cos(phi) - c0)^2 for every four consecutive beads (md_set_dihedrals)
+    double dih_k, dih_c0;
     pos_t *pos[2];
     double *vel[2];                     // SoA: vx = vel, vy = vel + N_pad, vz = vel + 2 N_pad
     double *frc;                        // SoA, same pitch

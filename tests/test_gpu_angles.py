@@ -129,3 +129,66 @@ def test_angles_single_precision(md, case, mode):
     eg, eo = g.energies(), o.energies()
     assert abs(eg.pe - eo.pe) <= 64 * eps * max(abs(eo.pe), eo.ke) * 4
     g.close()
+
+
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("variant,mode,flags", [("full", "fused", 0), ("full", "split", 0), ("full", "fused", 2),
+                                                ("newton3", "split", 0), ("full", "fused", 32)])
+@pytest.mark.parametrize("with_angles", [False, True])
+def test_dihedrals_forces_energy_and_ten_steps(md, case, variant, mode, flags, with_angles):
+    """Dihedral terms (md_set_dihedrals, R19), alone and together with the angle terms."""
+    n, clen = CASES[case]
+    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    for seed, thermal in ((1, False), (2, True)):
+        r, v, bonds, box = make_state(cfg, seed)
+        o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+        o.set_state(r, v)
+        assert o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0) == 0
+        if with_angles:
+            assert o.set_angles(3.0, -0.8) == 0          # bent equilibrium keeps the chains away from collinear bonds
+        assert o.set_dihedrals(1.5, -0.6) == 0
+        if thermal:
+            assert o.step(150) == 0
+            r, v = o.positions(), o.velocities()
+            o.set_state(r, v)
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=variant,
+                        step_mode=mode, flags=flags)
+        g.set_state(r, v)
+        g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+        if with_angles:
+            g.set_angles(3.0, -0.8)
+        g.set_dihedrals(1.5, -0.6)
+        assert force_rel_err(g.forces(), o.forces()) <= FORCE_RTOL
+        eg, eo = g.energies(), o.energies()
+        assert eg.pe_bond == pytest.approx(eo.pe_bond, rel=ENERGY_RTOL)
+        assert eg.virial == pytest.approx(eo.virial, rel=ENERGY_RTOL, abs=1e-7)
+        g.step(10)
+        assert o.step(10) == 0
+        assert pos_err(g.positions(), o.positions(), box) <= POS_ATOL
+        eg, eo = g.energies(), o.energies()
+        assert eg.ke == pytest.approx(eo.ke, rel=ENERGY_RTOL)
+        assert eg.pe == pytest.approx(eo.pe, rel=ENERGY_RTOL)
+        g.close()
+
+
+def test_dihedrals_change_the_forces_and_unsupported(md):
+    cfg = scaled_config("chains_1m", 1000, chain_len=10)
+    r, v, bonds, box = make_state(cfg, 1)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g.set_state(r, v)
+    with pytest.raises(md.MDError):
+        g.set_dihedrals(1.0, -1.0)                          # no bond list yet
+    g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    f0, e0 = g.forces(), g.energies().pe_bond
+    g.set_dihedrals(2.0, 0.5)
+    assert np.abs(g.forces() - f0).max() > 1e-2 and g.energies().pe_bond > e0
+    g.set_dihedrals(0.0, 0.5)
+    assert np.array_equal(g.forces(), f0)
+    g.close()
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", precision="f32")
+    g.set_state(r, v)
+    g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    with pytest.raises(md.MDError) as ei:
+        g.set_dihedrals(1.0, -1.0)
+    assert ei.value.code == md.binding.MD_ERR_UNSUPPORTED
+    g.close()
