@@ -114,6 +114,8 @@ def lib_sp():
         _declare_system_api(L, "orcs_")
         L.orcs_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orcs_set_angles.restype = C.c_int
+        L.orcs_set_dihedrals.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orcs_set_dihedrals.restype = C.c_int
         _lib_sp = L
     return _lib_sp
 
@@ -228,7 +230,7 @@ class OracleMD:
         return self._L.set_angles(self._h, float(k), float(cos0))
 
     def set_dihedrals(self, k, cos0):
-        """Cosine-harmonic dihedral terms (fp64 oracle only); after set_bonds."""
+        """Cosine-harmonic dihedral terms; after set_bonds."""
         return self._L.set_dihedrals(self._h, float(k), float(cos0))
 
     def rebuild_neighbors(self):

@@ -52,6 +52,9 @@ typedef struct orcs_sys {
     int has_angles;
     float ang_kf, ang_c0f;
     double pe_angle;
+    int has_dihedrals;
+    float dih_kf, dih_c0f;
+    double pe_dihedral;
     double disp_acc;
     int64_t step, n_rebuilds;
     int32_t max_cell_occ;
@@ -289,6 +292,40 @@ static void compute_forces(orcs_sys *s)
         }
         s->pe_angle = pe;
     }
+    /* dihedrals (R19) in binary32: the fp64 oracle's formulas, every operation rounded to binary32 */
+    s->pe_dihedral = 0;
+    if (s->has_dihedrals) {
+        const float k = s->dih_kf, c0 = s->dih_c0f;
+        double pe = 0;
+        for (int64_t q = 0; q < s->n_bonds; q++) {
+            int64_t b = s->bonds[2 * q], c = s->bonds[2 * q + 1];
+            int64_t a = s->partner[b] == c ? s->partner[N + b] : s->partner[b];
+            int64_t d = s->partner[c] == b ? s->partner[N + c] : s->partner[c];
+            if (a < 0 || d < 0) continue;
+            float b1[3], b2[3], b3[3], A[3], B[3], gA[3], gB[3], g1[3], g2[3], g3[3], t1[3], t2[3];
+            dist2f(s->r + 3 * b, s->r + 3 * a, L, half, b1);
+            dist2f(s->r + 3 * c, s->r + 3 * b, L, half, b2);
+            dist2f(s->r + 3 * d, s->r + 3 * c, L, half, b3);
+#define CROSS(o, u, v) do { o[0] = u[1] * v[2] - u[2] * v[1]; o[1] = u[2] * v[0] - u[0] * v[2]; o[2] = u[0] * v[1] - u[1] * v[0]; } while (0)
+            CROSS(A, b1, b2); CROSS(B, b2, b3);
+            float nA = A[0] * A[0] + A[1] * A[1] + A[2] * A[2], nB = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+            float invAB = 1.0f / sqrtf(nA * nB);
+            float cs = (A[0] * B[0] + A[1] * B[1] + A[2] * B[2]) * invAB;
+            for (int m = 0; m < 3; m++) { gA[m] = B[m] * invAB - cs * A[m] / nA; gB[m] = A[m] * invAB - cs * B[m] / nB; }
+            CROSS(g1, b2, gA); CROSS(t1, gA, b1); CROSS(t2, b3, gB); CROSS(g3, gB, b2);
+            for (int m = 0; m < 3; m++) g2[m] = t1[m] + t2[m];
+#undef CROSS
+            float g = -k * (cs - c0);
+            for (int m = 0; m < 3; m++) {
+                s->f[3 * a + m] += g * (-g1[m]);
+                s->f[3 * b + m] += g * (g1[m] - g2[m]);
+                s->f[3 * c + m] += g * (g2[m] - g3[m]);
+                s->f[3 * d + m] += g * g3[m];
+            }
+            pe += (double)(0.5f * k * (cs - c0) * (cs - c0));
+        }
+        s->pe_dihedral = pe;
+    }
 }
 
 static void rebuild(orcs_sys *s)
@@ -326,6 +363,14 @@ int orcs_set_bonds(orcs_sys *s, int64_t nb, const int32_t *ij, double k, double 
         }
     compute_forces(s);
     return s->bond_broken ? -3 : 0;
+}
+
+int orcs_set_dihedrals(orcs_sys *s, double k, double cos0)
+{
+    if (!s->partner) return -1;
+    s->has_dihedrals = 1; s->dih_kf = (float)k; s->dih_c0f = (float)cos0;
+    compute_forces(s);
+    return 0;
 }
 
 int orcs_set_angles(orcs_sys *s, double k, double cos0)
@@ -381,7 +426,7 @@ void orcs_energies(orcs_sys *s, orcs_energy *e)
     }
     e->ke = 0.5 * ke;
     e->pe_pair = 0.5 * pe;
-    e->pe_bond = s->pe_bond + s->pe_angle;
+    e->pe_bond = s->pe_bond + s->pe_angle + s->pe_dihedral;
     e->virial = 0.5 * vir + s->vir_bond;
     e->px = px; e->py = py; e->pz = pz;
     e->vmax = sqrt(vmax2);

@@ -225,3 +225,24 @@ def test_sp7_angles_match_fp64_oracle_at_rounded_coordinates():
     assert np.abs(dfo).max() > 1.0
     assert np.abs(dfs - dfo).max() < 256 * EPS32 * np.abs(fo0).max()
     assert abs((s.energies().pe_bond - es0) - (o.energies().pe_bond - eo0)) < 64 * EPS32 * abs(o.energies().pe_bond)
+
+
+def test_sp8_dihedrals_match_fp64_oracle_at_rounded_coordinates():
+    """Dihedral terms (R19) in binary32 against the fp64 oracle (pinned by P15) from the same rounded state.
+    ~80 binary32 operations per term; 1/|A|^2 amplifies rounding where consecutive bonds are nearly collinear, hence the
+    bound relative to the largest dihedral force."""
+    cfg = scaled_config("chains_1m", 1000, chain_len=10)
+    r, v, bonds, box = make_state(cfg, 3)
+    box32 = float(np.float32(box))
+    s = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    s.set_state(r, v)
+    s.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    o = OracleMD(cfg.n_atoms, box32, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(np.mod(round32(r), box32), round32(v))
+    o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    fs0, fo0, es0, eo0 = s.forces(), o.forces(), s.energies().pe_bond, o.energies().pe_bond
+    assert s.set_dihedrals(2.0, 0.3) == 0 and o.set_dihedrals(2.0, 0.3) == 0
+    dfs, dfo = s.forces() - fs0, o.forces() - fo0
+    assert np.abs(dfo).max() > 0.5
+    assert np.abs(dfs - dfo).max() < 1024 * EPS32 * max(np.abs(dfo).max(), np.abs(fo0).max())
+    assert abs((s.energies().pe_bond - es0) - (o.energies().pe_bond - eo0)) < 256 * EPS32 * abs(o.energies().pe_bond)
