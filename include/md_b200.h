@@ -187,7 +187,7 @@ MD_API int md_set_angles(md_system *s, double k_theta, double cos_theta0);
 
 /* Optional dihedral terms ("optional dihedral"; R19): U = k_phi/2 (cos(phi) - cos_phi0)^2 for
  * every four consecutive bonded atoms a-b-c-d, phi the angle between the planes (a,b,c) and (b,c,d) (cos(phi) = -1 for a
- * planar zig-zag).  Same call order and reporting as md_set_angles.  fp64, global-index W layouts only. */
+ * planar zig-zag).  Same call order, reporting and restrictions as md_set_angles. */
 MD_API int md_set_dihedrals(md_system *s, double k_phi, double cos_phi0);
 
 /* Advance n time steps.  Asynchronous on the stream except for one status read at the end.

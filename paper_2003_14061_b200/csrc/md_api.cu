@@ -727,7 +727,7 @@ int md_set_dihedrals(md_system *s, double k_phi, double cos_phi0)
     if (!s || !(k_phi >= 0) || !(cos_phi0 >= -1.0 && cos_phi0 <= 1.0)) { set_error("md_set_dihedrals: bad argument"); return MD_ERR_INVALID; }
     if (!s->P.has_bonds) { set_error("md_set_dihedrals: set the bond list first"); return MD_ERR_INVALID; }
     if (s->stepped) { set_error("md_set_dihedrals: only before the first md_step"); return MD_ERR_INVALID; }
-    if (s->P.tiled || s->P.sp) { set_error("md_set_dihedrals: fp64 global-index W layouts only"); return MD_ERR_UNSUPPORTED; }
+    if (s->P.tiled) { set_error("md_set_dihedrals: global-index W layouts only (use MD_FLAG_GATHER_W)"); return MD_ERR_UNSUPPORTED; }
     drop_graph(s);
     s->P.has_dihedrals = k_phi > 0;
     s->P.dih_k = k_phi;

@@ -314,10 +314,71 @@ __device__ __forceinline__ void angle_force_f(const MdDev &P, const float4 *__re
     }
 }
 
-template <bool CHECK>
+// dihedral terms in binary32: md_kernels.cu:dihedral_term / dihedral_force (R19)
+struct V3f {
+    float x, y, z;
+};
+__device__ __forceinline__ V3f cross3f(const V3f &u, const V3f &v) { return {u.y * v.z - u.z * v.y, u.z * v.x - u.x * v.z, u.x * v.y - u.y * v.x}; }
+__device__ __forceinline__ V3f mi_vec_f(const MdDev &P, const float4 &a, const float4 &b)
+{
+    V3f d;
+    mi_disp_f(P, a, b, d.x, d.y, d.z);
+    return d;
+}
+
+__device__ __forceinline__ float dihedral_term_f(const MdDev &P, const float4 &ra, const float4 &rb, const float4 &rc, const float4 &rd, int which,
+                                                 PairAccF &acc)
+{
+    const V3f b1 = mi_vec_f(P, rb, ra), b2 = mi_vec_f(P, rc, rb), b3 = mi_vec_f(P, rd, rc);
+    const V3f A = cross3f(b1, b2), B = cross3f(b2, b3);
+    const float nA = A.x * A.x + A.y * A.y + A.z * A.z, nB = B.x * B.x + B.y * B.y + B.z * B.z;
+    const float invAB = 1.0f / sqrtf(nA * nB), c = (A.x * B.x + A.y * B.y + A.z * B.z) * invAB;
+    if (which < 0) return c;
+    const float uA = c / nA, uB = c / nB;
+    const V3f gA = {B.x * invAB - uA * A.x, B.y * invAB - uA * A.y, B.z * invAB - uA * A.z};
+    const V3f gB = {A.x * invAB - uB * B.x, A.y * invAB - uB * B.y, A.z * invAB - uB * B.z};
+    const V3f g1 = cross3f(b2, gA), t1 = cross3f(gA, b1), t2 = cross3f(b3, gB), g3 = cross3f(gB, b2);
+    const V3f g2 = {t1.x + t2.x, t1.y + t2.y, t1.z + t2.z};
+    V3f d;
+    if (which == 0) d = {-g1.x, -g1.y, -g1.z};
+    else if (which == 1) d = {g1.x - g2.x, g1.y - g2.y, g1.z - g2.z};
+    else if (which == 2) d = {g2.x - g3.x, g2.y - g3.y, g2.z - g3.z};
+    else d = g3;
+    const float g = -(float)P.dih_k * (c - (float)P.dih_c0);
+    acc.fx += g * d.x; acc.fy += g * d.y; acc.fz += g * d.z;
+    return c;
+}
+
+__device__ __forceinline__ int chain_next_f(const MdDev &P, int x, int prev)
+{
+    const int q0 = P.bond_dev[x], q1 = P.bond_dev[(size_t)P.N_pad + x];
+    return q0 == prev ? q1 : q0;
+}
+
+__device__ __noinline__ void dihedral_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, PairAccF &a)
+{
+    const int L1 = P.bond_dev[i], R1 = P.bond_dev[(size_t)P.N_pad + i];
+    const int L2 = L1 >= 0 ? chain_next_f(P, L1, i) : -1, L3 = L2 >= 0 ? chain_next_f(P, L2, L1) : -1;
+    const int R2 = R1 >= 0 ? chain_next_f(P, R1, i) : -1, R3 = R2 >= 0 ? chain_next_f(P, R2, R1) : -1;
+    float4 l1, l2, l3, r1, r2, r3;
+    if (L1 >= 0) l1 = ld4(pos + L1);
+    if (L2 >= 0) l2 = ld4(pos + L2);
+    if (L3 >= 0) l3 = ld4(pos + L3);
+    if (R1 >= 0) r1 = ld4(pos + R1);
+    if (R2 >= 0) r2 = ld4(pos + R2);
+    if (R3 >= 0) r3 = ld4(pos + R3);
+    if (L3 >= 0) dihedral_term_f(P, l3, l2, l1, ri, 3, a);
+    if (L2 >= 0 && R1 >= 0) dihedral_term_f(P, l2, l1, ri, r1, 2, a);
+    if (L1 >= 0 && R2 >= 0) dihedral_term_f(P, l1, ri, r1, r2, 1, a);
+    if (R3 >= 0) dihedral_term_f(P, ri, r1, r2, r3, 0, a);
+}
+
+// EXTRAS: angle / dihedral code compiled in (the FENE-only instantiation keeps its registers)
+template <bool CHECK, bool EXTRAS = true>
 __device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, PairAccF &a)
 {
-    if (P.has_angles) angle_force_f(P, pos, ri, i, a);
+    if (EXTRAS && P.has_angles) angle_force_f(P, pos, ri, i, a);
+    if (EXTRAS && P.has_dihedrals) dihedral_force_f(P, pos, ri, i, a);
 #pragma unroll
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
@@ -400,7 +461,8 @@ __device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 
 #ifndef MD_SP_MIN_THREADS
 #define MD_SP_MIN_THREADS 1280       // resident threads per SM the register allocation must allow
 #endif
-template <int MODE, bool BONDS, int BLOCK, bool PADDED>
+// BONDS: 0 none, 1 FENE bonds, 2 FENE + angle / dihedral terms
+template <int MODE, int BONDS, int BLOCK, bool PADDED>
 __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
@@ -413,7 +475,8 @@ __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(c
         float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (MODE != 0) v = P.velf[vc][i];               // in flight while the column is walked
         PairAccF a = column_force_f<MD_SP_FORCE_D, PADDED>(P, pos, ri, i);
-        if (BONDS) bond_force_f<true>(P, pos, ri, i, a);
+        if (BONDS == 1) bond_force_f<true, false>(P, pos, ri, i, a);
+        if (BONDS == 2) bond_force_f<true, true>(P, pos, ri, i, a);
         if (MODE == 0 || MODE == 2) P.frcf[i] = make_float4(a.fx, a.fy, a.fz, 0.0f);
         if (MODE == 2) {
             v.x = __fadd_rn(v.x, __fmul_rn(P.hdtf, a.fx)); v.y = __fadd_rn(v.y, __fmul_rn(P.hdtf, a.fy)); v.z = __fadd_rn(v.z, __fmul_rn(P.hdtf, a.fz));
@@ -479,6 +542,19 @@ __global__ void __launch_bounds__(256) k_sp_energy(const __grid_constant__ MdDev
                 q[RED_PEB] += 0.5 * (double)(-0.5f * P.fene_kf * P.fene_R02f * logf(x));
                 q[RED_VIR] += 0.5 * (double)((-P.fene_kf / x) * r2);
             }
+            if (P.has_dihedrals) {
+#pragma unroll
+                for (int k = 0; k < 2; k++) {
+                    const int pk = P.bond_dev[(size_t)k * P.N_pad + i], qk = P.bond_dev[(size_t)(1 - k) * P.N_pad + i];
+                    if (pk < 0 || qk < 0 || i > pk) continue;
+                    const int o = chain_next_f(P, pk, i);
+                    if (o < 0) continue;
+                    PairAccF dummy = {0.0f, 0.0f, 0.0f};
+                    const float c = dihedral_term_f(P, ld4(pos + qk), ri, ld4(pos + pk), ld4(pos + o), -1, dummy);
+                    const float kf = (float)P.dih_k, c0 = (float)P.dih_c0;
+                    q[RED_PEB] += (double)(0.5f * kf * (c - c0) * (c - c0));
+                }
+            }
             if (P.has_angles) {
                 const int p0 = P.bond_dev[i], p1 = P.bond_dev[(size_t)P.N_pad + i];
                 if (p0 >= 0 && p1 >= 0) {
@@ -503,7 +579,7 @@ __global__ void __launch_bounds__(256) k_sp_energy(const __grid_constant__ MdDev
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdiv(n, block), 148 * per_sm); }
 
-template <int MODE, bool BONDS, bool PADDED>
+template <int MODE, int BONDS, bool PADDED>
 void launch_sp_force_p(const MdDev &P, int block, cudaStream_t st)
 {
     switch (block) {
@@ -514,7 +590,7 @@ void launch_sp_force_p(const MdDev &P, int block, cudaStream_t st)
     }
 }
 
-template <int MODE, bool BONDS>
+template <int MODE, int BONDS>
 void launch_sp_force(const MdDev &P, int block, cudaStream_t st)
 {
     if (P.sp_pad > 1) launch_sp_force_p<MODE, BONDS, true>(P, block, st);
@@ -533,14 +609,18 @@ void mdk_sp_build(const MdDev &P, cudaStream_t st) { k_sp_build<<<capped_grid(P.
 
 void mdk_sp_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 {
-    if (P.has_bonds) {
-        if (mode == 0) launch_sp_force<0, true>(P, lc.block, st);
-        else if (mode == 1) launch_sp_force<1, true>(P, lc.block, st);
-        else launch_sp_force<2, true>(P, lc.block, st);
+    if (P.has_bonds && (P.has_angles || P.has_dihedrals)) {
+        if (mode == 0) launch_sp_force<0, 2>(P, lc.block, st);
+        else if (mode == 1) launch_sp_force<1, 2>(P, lc.block, st);
+        else launch_sp_force<2, 2>(P, lc.block, st);
+    } else if (P.has_bonds) {
+        if (mode == 0) launch_sp_force<0, 1>(P, lc.block, st);
+        else if (mode == 1) launch_sp_force<1, 1>(P, lc.block, st);
+        else launch_sp_force<2, 1>(P, lc.block, st);
     } else {
-        if (mode == 0) launch_sp_force<0, false>(P, lc.block, st);
-        else if (mode == 1) launch_sp_force<1, false>(P, lc.block, st);
-        else launch_sp_force<2, false>(P, lc.block, st);
+        if (mode == 0) launch_sp_force<0, 0>(P, lc.block, st);
+        else if (mode == 1) launch_sp_force<1, 0>(P, lc.block, st);
+        else launch_sp_force<2, 0>(P, lc.block, st);
     }
 }
 

@@ -185,10 +185,41 @@ def test_dihedrals_change_the_forces_and_unsupported(md):
     g.set_dihedrals(0.0, 0.5)
     assert np.array_equal(g.forces(), f0)
     g.close()
-    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", precision="f32")
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=md.FLAG_TILED_W)
     g.set_state(r, v)
     g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
     with pytest.raises(md.MDError) as ei:
         g.set_dihedrals(1.0, -1.0)
     assert ei.value.code == md.binding.MD_ERR_UNSUPPORTED
+    g.close()
+
+
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("mode", ["fused", "split"])
+def test_dihedrals_single_precision(md, case, mode):
+    """Binary32 variant with angle + dihedral terms against the binary32 oracle.  Forces: the dihedral gradient divides by
+    |b x b'|^2, so its binary32 rounding is bounded relative to the largest force, 1024 eps (the oracle's own pin SP8)."""
+    from oracle.md_oracle import OracleMDSP
+    eps = 2.0 ** -24
+    n, clen = CASES[case]
+    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    r, v, bonds, box = make_state(cfg, 1)
+    o = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(r, v)
+    o.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    assert o.set_angles(3.0, -0.8) == 0 and o.set_dihedrals(1.5, -0.6) == 0
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", step_mode=mode, precision="f32")
+    g.set_state(r, v)
+    g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+    g.set_angles(3.0, -0.8)
+    g.set_dihedrals(1.5, -0.6)
+    fo = o.forces()
+    assert np.abs(g.forces() - fo).max() <= 1024 * eps * np.abs(fo).max()
+    eg, eo = g.energies(), o.energies()
+    assert abs(eg.pe_bond - eo.pe_bond) <= 256 * eps * abs(eo.pe_bond)
+    g.step(10)
+    assert o.step(10) == 0
+    assert pos_err(g.positions(), o.positions(), float(np.float32(box))) <= 16 * float(np.spacing(np.float32(box)))
+    eg, eo = g.energies(), o.energies()
+    assert abs(eg.pe - eo.pe) <= 256 * eps * max(abs(eo.pe), eo.ke) * 4
     g.close()
