@@ -350,7 +350,7 @@ def main():
     cand = 27.0 * (n / nsys) / info["cells_per_edge"] ** 3                   # candidates examined per atom (27-cell stencil)
     nb_floor = rec + w_bytes * mbar + 4.0                             # r_i + W written + m_i
     nb_ns = nb_floor + rec * cand                                     # + one record per candidate position read
-    roofline_neighbor = {"bound": "hbm", "kernel": "k_tile_build" if info["tile_capacity"] else ("k_sp_build" if sp else ("k_build_layers" if args.flags & 32 else "k_build")),
+    roofline_neighbor = {"bound": "hbm", "kernel": ("k_sp_tile_build" if sp else "k_tile_build") if info["tile_capacity"] else ("k_sp_build" if sp else ("k_build_layers" if args.flags & 32 else "k_build")),
                          "avg_launch_ms": build_ms, "candidates_per_atom": cand,
                          "achieved": nb_ns * n / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": nb_ns * n / (build_ms * 1e-3) / 1e9 / peak,

@@ -560,10 +560,11 @@ md_system *md_create_ex(const md_params *pp)
 
     P.tiled = 0;
     P.tile_build = 0;
-    if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W) && !sp) {
+    if (!P.half_list && !(p.flags & MD_FLAG_GLOBAL_W)) {
         // shared-memory staged neighbor build (both W layouts); the tiled W layout only on request
         const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
-        const bool want_tiled = (p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0);
+        // (single precision: the tile-staged BUILD only; its force kernel gathers float4 records)
+        const bool want_tiled = !sp && ((p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0));
         const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin, want_tiled);
         if (!fits && (p.flags & MD_FLAG_TILED_W)) { md_destroy(s); return nullptr; }
         P.tile_build = fits ? 1 : 0;

@@ -331,6 +331,132 @@ __global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDe
 }
 
 // ------------------------------------------------------------------------------------------------
+// N5 on the tile for the single-precision variant (md_sp.cu; R18): the same box decomposition, descriptor
+// and candidate order as k_tile_build<false>, the tile held as packed binary32 triples, the accept test in the binary32
+// arithmetic of R18 (d = fl(a - b), + shift rounded once, r2 = fmaf(dz,dz, fmaf(dy,dy, fl(dx dx))) < (float)(r_n^2)).
+// W holds global indices; long columns are padded with self entries (P.sp_pad) as k_sp_build does.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tile_stage_f(const TileDesc &M, const float4 *__restrict__ pos, float *st)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int q = wid; q < M.nq; q += nw) {
+        const RowCopy A = row_copy<false>(M.row[q], 0.0);
+        for (int u = lane; u < A.tot; u += 64) {
+            const int u1 = u + 32;
+            const int s0 = A.contiguous ? A.g0 + u : u + (u < A.n0 ? A.g0 : (u < A.n01 ? A.b1 : A.b2));
+            const int s1 = A.contiguous ? A.g0 + u1 : u1 + (u1 < A.n0 ? A.g0 : (u1 < A.n01 ? A.b1 : A.b2));
+            const float4 p0 = __ldg(pos + s0);
+            float4 p1 = p0;
+            if (u1 < A.tot) p1 = __ldg(pos + s1);
+            float *d = st + A.off3 + 3 * u;
+            d[0] = p0.x; d[1] = p0.y; d[2] = p0.z;
+            if (u1 < A.tot) { d[96] = p1.x; d[97] = p1.y; d[98] = p1.z; }
+        }
+    }
+}
+
+template <bool SHIFT>
+__device__ __forceinline__ void tile_scan_run_f(const float *st, float xi, float yi, float zi, int li, int b, int e, float shx, float shy,
+                                                float shz, unsigned add, float rn2, Emit<false> &em)
+{
+    const float *p = st + 3 * b;
+#pragma unroll 2
+    for (int j = b; j < e; j++, p += 3) {
+        float dx = __fsub_rn(xi, p[0]), dy = __fsub_rn(yi, p[1]), dz = __fsub_rn(zi, p[2]);
+        if (SHIFT) { dx = __fadd_rn(dx, shx); dy = __fadd_rn(dy, shy); dz = __fadd_rn(dz, shz); }
+        const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+        em.put(r2 < rn2 && j != li, j, add);
+    }
+}
+
+__global__ void __launch_bounds__(512) k_sp_tile_build(const __grid_constant__ MdDev P)
+{
+    const int BLOCK = blockDim.x;
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    extern __shared__ double dsm[];
+    __shared__ TileDesc M;
+    __shared__ TileRowGeom X;
+    __shared__ int smx[32], ssum[32];
+    const int cap = P.tg.cap;
+    float *st = (float *)dsm;
+    int *tcs = (int *)(st + 3 * cap);
+    const int stride = P.tg.S + 3;
+    const float4 *__restrict__ pos = P.posf[__ldcg(&P.ctrl->p_dst)];
+    const int *__restrict__ cs = P.cell_start;
+    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    tile_describe(P, B, M, X);
+    if (M.T > cap) {
+        if (threadIdx.x == 0) set_err(P, MD_ERR_TILE_OVERFLOW);
+        return;
+    }
+    tile_stage_f(M, pos, st);
+    for (int e = threadIdx.x; e < B.nq * stride; e += BLOCK) {
+        const int q = e / stride, k = e - q * stride;
+        if (k > B.sxc + 2) continue;
+        const TileDesc::Row &R = M.row[q];
+        int v;
+        if (k == 0) v = R.off;
+        else if (k == B.sxc + 2) v = R.off + R.n[0] + R.n[1] + R.n[2];
+        else v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - 1) - R.g[1]);
+        tcs[e] = v;
+    }
+    __syncthreads();
+    const int nc = P.nc;
+    const float L = P.Lf, rn2 = P.rn2f;
+    int tmax = 0, tsum = 0;
+    for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
+        int i, li;
+        own_atom(M, t, i, li);
+        const float xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
+        const int cx = cell_coord((double)xi, P.inv_w, nc), cy = cell_coord((double)yi, P.inv_w, nc), cz = cell_coord((double)zi, P.inv_w, nc);
+        Emit<false> em = {(char *)((unsigned *)P.W + (size_t)i * P.w_col), 4ll * P.w_row, 0, P.Mmax};
+        const int k0 = cx - B.x0;
+        const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);
+#pragma unroll 1
+        for (int r = 0; r < 9; r++) {
+            const int q = q0 + (r % 3) + B.nyq * (r / 3);
+            const int ysh = X.ysh[q], zsh = X.zsh[q];
+            const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
+            const float shy = ysh * L, shz = zsh * L;
+            const TileDesc::Row &R = M.row[q];
+            const int *tc = tcs + q * stride + k0;
+            const int b = tc[0], e = tc[3];
+            int mid = cx == 0 ? tc[1] : (cx == nc - 1 ? tc[2] : e);
+            const int e0 = R.off + R.n[0], e1 = e0 + R.n[1];
+            const int d0 = R.g[0] - R.off, d1 = R.g[1] - e0, d2 = R.g[2] - e1;
+            const int da = b < e0 ? d0 : (b < e1 ? d1 : d2), db = mid < e0 ? d0 : (mid < e1 ? d1 : d2);
+            const float shxa = cx == 0 ? L : 0.0f, shxb = cx == nc - 1 ? -L : 0.0f;
+            const unsigned fla = fl | (cx == 0 ? 1u : 0u), flb = fl | (cx == nc - 1 ? 1u : 0u);
+            const unsigned adda = (fla << W_FLAG_SHIFT) + (unsigned)da, addb = (flb << W_FLAG_SHIFT) + (unsigned)db;
+            if (fla) tile_scan_run_f<true>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
+            else tile_scan_run_f<false>(st, xi, yi, zi, li, b, mid, 0.0f, 0.0f, 0.0f, adda, rn2, em);
+            if (mid < e) {
+                if (flb) tile_scan_run_f<true>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
+                else tile_scan_run_f<false>(st, xi, yi, zi, li, mid, e, 0.0f, 0.0f, 0.0f, addb, rn2, em);
+            }
+        }
+        const int m = em.m;
+        if (P.sp_pad > 1)
+            for (int k = m; k < ((m + P.sp_pad - 1) / P.sp_pad) * P.sp_pad && k < P.Mmax; k++)
+                P.W[(size_t)k * P.w_row + (size_t)i * P.w_col] = i;
+        P.nnb[i] = m < P.Mmax ? m : P.Mmax;
+        if (m > P.Mmax) set_err(P, MD_ERR_NEBR_OVERFLOW);
+        tmax = max(tmax, m);
+        tsum += m;
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int mx = 0, sm = 0;
+        for (int w = 0; w < BLOCK / 32; w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        atomicMax(&P.ctrl->max_nnb, mx);
+        atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // F1 on the tile.  Thread i walks column i of W (coalesced 32-bit words, two neighbors each, streamed from HBM
 // two words ahead of their use); the partner positions come from the shared-memory tile.
 // ------------------------------------------------------------------------------------------------
@@ -615,7 +741,7 @@ void launch_force(const MdDev &P, int mode, cudaStream_t st)
 int mdk_tile_configure(const MdDev &P)
 {
     const size_t sb = mdk_tile_smem(P.tg, true);
-    if (opt_in(k_tile_build<true>, sb) || opt_in(k_tile_build<false>, sb)) return -1;
+    if (opt_in(k_tile_build<true>, sb) || opt_in(k_tile_build<false>, sb) || opt_in(k_sp_tile_build, sb)) return -1;
     if (!P.tiled) return 0;                          // the force / energy kernels exist for 128, 256 and 512 threads
     switch (P.tg.threads) {
     case 128: return configure_block<128>(P);
@@ -629,7 +755,11 @@ void mdk_tile_build(const MdDev &P, cudaStream_t st)
 {
     const dim3 g = tile_grid3(P);
     const size_t sm = mdk_tile_smem(P.tg, true);
-    if (P.tiled) k_tile_build<true><<<g, P.tg.threads, sm, st>>>(P);
+    if (P.sp) {      // same launch shape; the binary32 tile needs half the bytes
+        const size_t smf = 3 * (size_t)P.tg.cap * sizeof(float) + (size_t)TILE_Q_MAX * (P.tg.S + 3) * sizeof(int);
+        k_sp_tile_build<<<g, P.tg.threads, smf, st>>>(P);
+    }
+    else if (P.tiled) k_tile_build<true><<<g, P.tg.threads, sm, st>>>(P);
     else k_tile_build<false><<<g, P.tg.threads, sm, st>>>(P);
 }
 

@@ -65,13 +65,14 @@ def make_pair(md, cfg, seed, mode="fused", state="jitter", flags=0, **kw):
 
 @pytest.mark.parametrize("case", list(cases()))
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
-def test_sp_neighbor_sets_and_forces(md, case, state):
+@pytest.mark.parametrize("build_flags", [0, 2])          # tile-staged build (default) / gather build (MD_FLAG_GLOBAL_W)
+def test_sp_neighbor_sets_and_forces(md, case, state, build_flags):
     cfg = cases()[case]
     if state == "lattice" and cfg.lattice == "chains":
         pytest.skip("chain start has no separate lattice state")
     for seed in (1, 2, 3) if state != "thermal" else (1,):
-        g, o, box = make_pair(md, cfg, seed, mode="split", state=state)
-        assert g.info()["precision"] == 1
+        g, o, box = make_pair(md, cfg, seed, mode="split", state=state, flags=build_flags)
+        assert g.info()["precision"] == 1 and (g.info()["tile_capacity"] > 0) == (build_flags == 0)
         counts, lst = g.neighbors()
         nbad, first = sets_equal(counts, lst, o)
         assert nbad == 0, f"neighbor sets differ for {nbad} atoms (first: atom {first})"
@@ -97,7 +98,7 @@ def test_sp_neighbor_sets_and_forces(md, case, state):
 
 
 @pytest.mark.parametrize("case", list(cases()))
-@pytest.mark.parametrize("mode,flags", [("fused", 0), ("split", 0), ("fused", 1), ("fused", 16)])
+@pytest.mark.parametrize("mode,flags", [("fused", 0), ("split", 0), ("fused", 1), ("fused", 16), ("fused", 2), ("fused", 2 | 16)])
 def test_sp_ten_steps(md, case, mode, flags):
     cfg = cases()[case]
     for seed in (1, 2, 3):
