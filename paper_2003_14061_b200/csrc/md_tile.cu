@@ -355,13 +355,54 @@ __device__ __forceinline__ void tile_stage_f(const TileDesc &M, const float4 *__
     }
 }
 
+// Packed binary32 arithmetic of sm_100 (FFMA2 / FADD2: two IEEE-rounded lanes per instruction): the accept test of TWO
+// consecutive candidates at once.  Lane-wise the operations are those of DESIGN.md R18 (d = fl(x_i - x_j) as
+// fma(-1, x_j, x_i), one rounding; + shift rounded once; r2 = fma(dz,dz, fma(dy,dy, fl(dx dx)))), so the sets stay exact.
+__device__ __forceinline__ unsigned long long pack2(float a, float b)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 template <bool SHIFT>
 __device__ __forceinline__ void tile_scan_run_f(const float *st, float xi, float yi, float zi, int li, int b, int e, float shx, float shy,
                                                 float shz, unsigned add, float rn2, Emit<false> &em)
 {
+    const unsigned long long m1 = pack2(-1.0f, -1.0f), x2 = pack2(xi, xi), y2 = pack2(yi, yi), z2 = pack2(zi, zi);
+    const unsigned long long sx2 = pack2(shx, shx), sy2 = pack2(shy, shy), sz2 = pack2(shz, shz);
     const float *p = st + 3 * b;
+    int j = b;
 #pragma unroll 2
-    for (int j = b; j < e; j++, p += 3) {
+    for (; j + 1 < e; j += 2, p += 6) {
+        unsigned long long dx = fma2(m1, pack2(p[0], p[3]), x2), dy = fma2(m1, pack2(p[1], p[4]), y2), dz = fma2(m1, pack2(p[2], p[5]), z2);
+        if (SHIFT) { dx = add2(dx, sx2); dy = add2(dy, sy2); dz = add2(dz, sz2); }
+        const unsigned long long r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        float ra, rb;
+        unpack2(r2, ra, rb);
+        em.put(ra < rn2 && j != li, j, add);
+        em.put(rb < rn2 && j + 1 != li, j + 1, add);
+    }
+    if (j < e) {
         float dx = __fsub_rn(xi, p[0]), dy = __fsub_rn(yi, p[1]), dz = __fsub_rn(zi, p[2]);
         if (SHIFT) { dx = __fadd_rn(dx, shx); dy = __fadd_rn(dy, shy); dz = __fadd_rn(dz, shz); }
         const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
