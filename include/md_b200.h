@@ -178,6 +178,35 @@ MD_API void md_destroy(md_system *s);
  * Forces and energies are re-evaluated. */
 MD_API int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, double R0);
 
+/* Chain start "grown as seeded random walks then pushed apart" (BASELINE.json configs[4]; R12).
+ * INITIALISATION, not part of the time-step path: xyz (host, 3*N, original-id order, in [0, L]) is an OVERLAPPING start,
+ * e.g. random walks; the library runs its own MD kernels on it with the pair force capped (for r < r_cap the force keeps
+ * the magnitude it has at r_cap), r_cap ramped from r_cap_start to r_cap_end over ramp_steps, the FENE force clamped
+ * short of its pole, no atom moving more than max_move per step, and the velocities rescaled to `temperature` every
+ * step, until the smallest distance between atoms that are not bonded exceeds min_nonbonded and the longest bond is
+ * below max_bond (checked every check_interval steps once the ramp is over).  Then it loads the pushed-off positions,
+ * fresh velocities (the generator of md_create with `seed`: Gaussian, zero net momentum, sum v^2 = 3(N-1)T) and the bond
+ * list into `s` exactly as md_set_state + md_set_bonds would.  The work runs in a temporary system of its own (global-index
+ * W with room for the crowded start), so `s` may have any layout or precision.  Zero fields of opts take the defaults
+ * given below; opts may be NULL.  MD_ERR_UNSUPPORTED if the criteria are not met within max_steps. */
+typedef struct md_pushoff_opts {
+    double   r_cap_start, r_cap_end;   /* 1.0, 0.8 */
+    int32_t  ramp_steps;               /* 3000 */
+    int32_t  max_steps;                /* 40000 */
+    int32_t  check_interval;           /* 100 */
+    double   min_nonbonded, max_bond;  /* 0.85, 1.3 */
+    double   max_move;                 /* 0.05 */
+    double   temperature;              /* 1.0 */
+    uint64_t seed;                     /* fresh velocities after the push-off; the push-off itself starts from seed + 1 */
+} md_pushoff_opts;
+typedef struct md_pushoff_report {
+    int64_t steps;                     /* push-off steps run */
+    double  min_nonbonded, max_bond;   /* of the state loaded into s */
+    double  min_nonbonded_start;       /* of the overlapping start */
+} md_pushoff_report;
+MD_API int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *ij, double k, double R0,
+                      const md_pushoff_opts *opts, md_pushoff_report *report);
+
 /* Optional bond-angle terms for the chain workload ("bond force, bond-angle torque"; the paper gives
  * no form: the textbook cosine-harmonic U = k_theta/2 (cos(theta) - cos_theta0)^2 is used, R19) at every
  * atom that has two bonded partners, theta the angle between its two bonds.  Call after md_set_bonds and before the
@@ -222,8 +251,10 @@ MD_API int md_set_profiling(md_system *s, int enabled);
 MD_API int md_get_timers(md_system *s, double *ms, int64_t *launches);
 MD_API int md_reset_timers(md_system *s);
 
-/* Device-memory hooks (process-wide; set before md_create*).  alloc(bytes, stream, user) returns a device
- * pointer or NULL; free_(ptr, user).  The Python binding routes these to torch's caching allocator. */
+/* Device-memory hooks for the systems created AFTER the call (each system records the pair in force at its creation
+ * and frees through it, so systems created under different hooks can coexist).  alloc(bytes, stream, user) returns a
+ * device pointer or NULL; free_(ptr, user).  NULL, NULL = cudaMalloc / cudaFree.  The Python binding routes these to
+ * torch's caching allocator. */
 typedef void *(*md_alloc_fn)(size_t bytes, void *stream, void *user);
 typedef void (*md_free_fn)(void *ptr, void *user);
 MD_API void md_set_allocator(md_alloc_fn alloc, md_free_fn free_, void *user);

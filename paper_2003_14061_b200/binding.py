@@ -24,7 +24,7 @@ STEP_MODE = {"fused": 0, "split": 1}
 PRECISION = {"f64": 0, "f32": 1}
 TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "decide")
 
-EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
+EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_pushoff", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
            "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
            "md_set_allocator", "md_last_error", "md_version")
@@ -60,6 +60,17 @@ class _Info(C.Structure):
                 ("device_name", C.c_char * 64), ("w_layout", C.c_int32), ("tile_cells", C.c_int32 * 3),
                 ("tile_capacity", C.c_int32), ("tile_threads", C.c_int32), ("use_graph", C.c_int32),
                 ("n_systems", C.c_int32), ("precision", C.c_int32), ("n_layers", C.c_int32)]
+
+
+class _PushoffOpts(C.Structure):
+    _fields_ = [("r_cap_start", C.c_double), ("r_cap_end", C.c_double), ("ramp_steps", C.c_int32), ("max_steps", C.c_int32),
+                ("check_interval", C.c_int32), ("min_nonbonded", C.c_double), ("max_bond", C.c_double),
+                ("max_move", C.c_double), ("temperature", C.c_double), ("seed", C.c_uint64)]
+
+
+class _PushoffReport(C.Structure):
+    _fields_ = [("steps", C.c_int64), ("min_nonbonded", C.c_double), ("max_bond", C.c_double),
+                ("min_nonbonded_start", C.c_double)]
 
 
 @dataclass
@@ -112,6 +123,8 @@ def load_library(path: str = LIB_PATH):
     L.md_create_ex.argtypes = [C.POINTER(_Params)]
     L.md_destroy.argtypes = [C.c_void_p]
     L.md_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
+    L.md_pushoff.argtypes = [C.c_void_p, _dp, C.c_int64, _ip, C.c_double, C.c_double, C.POINTER(_PushoffOpts),
+                             C.POINTER(_PushoffReport)]
     L.md_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_set_dihedrals.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_step.argtypes = [C.c_void_p, C.c_int64]
@@ -149,9 +162,14 @@ def use_torch_allocator():
         except Exception:
             pass
 
-    a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
-    _keep.extend([a, f])
-    L.md_set_allocator(C.cast(a, C.c_void_p), C.cast(f, C.c_void_p), None)
+    if not _keep:
+        _keep.extend([_ALLOC_FN(_alloc), _FREE_FN(_free)])
+    L.md_set_allocator(C.cast(_keep[0], C.c_void_p), C.cast(_keep[1], C.c_void_p), None)
+
+
+def use_cuda_allocator():
+    """Back to cudaMalloc / cudaFree for systems created from now on (existing systems keep the hooks they were created with)."""
+    load_library().md_set_allocator(None, None, None)
 
 
 def _err(L):
@@ -168,8 +186,11 @@ class MDSystem:
         if not torch.cuda.is_available():
             raise MDError(MD_ERR_CUDA, "no CUDA device: the MD path has no CPU fallback")
         L = load_library()
-        if torch_memory and not _keep:
+        # the library records the hooks in force at creation inside the handle, so systems of either kind can coexist
+        if torch_memory:
             use_torch_allocator()
+        else:
+            use_cuda_allocator()
         p = _Params()
         L.md_params_default(C.byref(p))
         p.n_atoms, p.box, p.density, p.r_cut, p.r_shell, p.dt = int(n_atoms), box, density, r_cut, r_shell, dt
@@ -218,6 +239,19 @@ class MDSystem:
     def set_bonds(self, bonds, k, r0):
         b = np.ascontiguousarray(bonds, np.int32).reshape(-1, 2)
         self._ck(self._L.md_set_bonds(self._h, b.shape[0], b, float(k), float(r0)))
+
+    def pushoff(self, r, bonds, k, r0, temperature=1.0, seed=1, **opts) -> dict:
+        """md_pushoff: push an overlapping chain start apart inside the library and load the result (fresh velocities,
+        bonds) into this system.  opts: fields of md_pushoff_opts.  Returns the report as a dict."""
+        r = np.ascontiguousarray(r, np.float64)
+        b = np.ascontiguousarray(bonds, np.int32).reshape(-1, 2)
+        o = _PushoffOpts()
+        o.temperature, o.seed = float(temperature), int(seed)
+        for key, val in opts.items():
+            setattr(o, key, val)
+        rep = _PushoffReport()
+        self._ck(self._L.md_pushoff(self._h, r, b.shape[0], b, float(k), float(r0), C.byref(o), C.byref(rep)))
+        return {key: getattr(rep, key) for key, _ in _PushoffReport._fields_}
 
     def set_angles(self, k_theta, cos_theta0):
         self._ck(self._L.md_set_angles(self._h, float(k_theta), float(cos_theta0)))

@@ -53,6 +53,9 @@ struct md_system {
     int device = 0;
     char device_name[64] = "";
     std::vector<void *> allocs;
+    md_alloc_fn alloc = nullptr;   // the hooks in force when the system was created: its memory goes back the way it came
+    md_free_fn free_ = nullptr;
+    void *alloc_user = nullptr;
     int64_t bytes = 0;
     DevCtrl *h_ctrl = nullptr;     // pinned
     double *h_stage = nullptr;     // pinned staging, 6 N doubles
@@ -83,7 +86,7 @@ void *dev_alloc(md_system *s, size_t bytes)
 {
     void *p = nullptr;
     bytes = (bytes + 255) & ~(size_t)255;
-    if (g_alloc) p = g_alloc(bytes, (void *)s->stream, g_alloc_user);
+    if (s->alloc) p = s->alloc(bytes, (void *)s->stream, s->alloc_user);
     else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
     if (!p) return nullptr;
     s->allocs.push_back(p);
@@ -95,7 +98,7 @@ void *dev_alloc(md_system *s, size_t bytes)
 void dev_free_all(md_system *s)
 {
     for (void *p : s->allocs) {
-        if (g_free) g_free(p, g_alloc_user);
+        if (s->alloc) { if (s->free_) s->free_(p, s->alloc_user); }
         else cudaFree(p);
     }
     s->allocs.clear();
@@ -514,6 +517,7 @@ md_system *md_create_ex(const md_params *pp)
     }
     md_system *s = new md_system();
     s->prm = p;
+    s->alloc = g_alloc; s->free_ = g_free; s->alloc_user = g_alloc_user;
     auto fail = [&](const char *what) -> md_system * {
         if (what) set_error("%s: %s", what, cudaGetErrorString(cudaGetLastError()));
         md_destroy(s);
@@ -677,6 +681,8 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
     for (int64_t b = 0; b < n_bonds; b++) {
         const int i = ij[2 * b], j = ij[2 * b + 1];
         if (i < 0 || j < 0 || i >= P.N || j >= P.N || i == j) { set_error("md_set_bonds: bad pair (%d, %d)", i, j); return MD_ERR_INVALID; }
+        if (i / P.N1 != j / P.N1) { set_error("md_set_bonds: pair (%d, %d) joins two independent systems", i, j); return MD_ERR_INVALID; }
+        if (tab[i] == j || tab[n + i] == j) { set_error("md_set_bonds: pair (%d, %d) listed twice", i, j); return MD_ERR_INVALID; }
         for (int side = 0; side < 2; side++) {
             const int a = side ? j : i, c = side ? i : j;
             if (tab[a] < 0) tab[a] = c;
@@ -710,6 +716,106 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
     CK(cudaMemsetAsync(&P.ctrl->n_rebuilds, 0, sizeof(int), s->stream));
     s->rebuilds_seen = 0;
     return MD_OK;
+}
+
+// Push-off of an overlapping chain start (include/md_b200.h; R12): initialisation, run in a temporary system.
+int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *ij, double k, double R0,
+               const md_pushoff_opts *opts, md_pushoff_report *report)
+{
+    if (!s || !xyz || n_bonds < 0 || (n_bonds > 0 && !ij) || !(R0 > 0)) { set_error("md_pushoff: bad argument"); return MD_ERR_INVALID; }
+    md_pushoff_opts o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    if (!(o.r_cap_start > 0)) o.r_cap_start = 1.0;
+    if (!(o.r_cap_end > 0)) o.r_cap_end = 0.8;
+    if (o.ramp_steps <= 0) o.ramp_steps = 3000;
+    if (o.max_steps <= 0) o.max_steps = 40000;
+    if (o.check_interval <= 0) o.check_interval = 100;
+    if (!(o.min_nonbonded > 0)) o.min_nonbonded = 0.85;
+    if (!(o.max_bond > 0)) o.max_bond = 1.3;
+    if (!(o.max_move > 0)) o.max_move = 0.05;
+    if (!(o.temperature > 0)) o.temperature = 1.0;
+    if (o.r_cap_end > o.r_cap_start || o.min_nonbonded >= s->prm.r_cut) { set_error("md_pushoff: bad options"); return MD_ERR_INVALID; }
+
+    // temporary system: same box and model, global-index W built by the gathering kernel (no tile capacity to exceed),
+    // twice the rows of W for the crowded start, split steps launched one by one
+    md_params tp = s->prm;
+    tp.lattice = MD_LATTICE_NONE;
+    tp.precision = MD_PREC_F64;
+    tp.force_variant = MD_FORCE_FULL_LIST;
+    tp.step_mode = MD_STEP_SPLIT;
+    tp.flags = MD_FLAG_GLOBAL_W | MD_FLAG_NO_GRAPH;
+    tp.max_neighbors = 2 * s->P.Mmax;
+    tp.reorder_interval = 0;
+    tp.stream = (void *)s->stream;
+    tp.device = s->device;
+    const md_alloc_fn a0 = g_alloc; const md_free_fn f0 = g_free; void *u0 = g_alloc_user;
+    g_alloc = s->alloc; g_free = s->free_; g_alloc_user = s->alloc_user;       // the temporary system allocates the way s does
+    md_system *t = md_create_ex(&tp);
+    g_alloc = a0; g_free = f0; g_alloc_user = u0;
+    if (!t) return MD_ERR_CUDA;
+    const size_t n3 = 3 * (size_t)s->P.N;
+    std::vector<double> v(n3), r(n3);
+    int rc = MD_OK;
+    unsigned long long *d_chk = nullptr, h_chk[2] = {0, 0};
+    md_pushoff_report rep;
+    memset(&rep, 0, sizeof(rep));
+    auto bits_to_len = [](unsigned long long b) { double d; memcpy(&d, &b, sizeof(d)); return std::sqrt(d); };
+    auto check = [&]() -> int {
+        mdk_po_check(t->P, d_chk, t->stream);
+        CK(cudaMemcpyAsync(h_chk, d_chk, sizeof(h_chk), cudaMemcpyDeviceToHost, t->stream));
+        return check_device_status(t);
+    };
+    do {
+        for (int b = 0; b < s->P.n_sys; b++)
+            md_init_velocities(s->P.N1, o.temperature, o.seed + 1 + (uint64_t)b, v.data() + 3 * (size_t)b * s->P.N1);
+        if ((rc = upload_state(t, xyz, v.data(), true)) != MD_OK) break;
+        if (n_bonds > 0 && (rc = md_set_bonds(t, n_bonds, ij, k, R0)) != MD_OK) break;
+        d_chk = (unsigned long long *)dev_alloc(t, 2 * sizeof(unsigned long long));
+        if (!d_chk) { set_error("md_pushoff: device allocation failed"); rc = MD_ERR_NOMEM; break; }
+        if ((rc = check()) != MD_OK) break;
+        rep.min_nonbonded_start = bits_to_len(h_chk[0]);
+        const MdDev &P = t->P;
+        const double ke_target = 1.5 * (double)(P.N - P.n_sys) * o.temperature;
+        const double vlim = o.max_move / P.dt;
+        double rcap = o.r_cap_start;
+        mdk_po_force(P, rcap * rcap, t->stream);
+        bool done = false;
+        int64_t step = 0;
+        while (!done && step < o.max_steps) {
+            for (int c = 0; c < o.check_interval; c++, step++) {
+                const double x = std::min(1.0, (double)step / o.ramp_steps);
+                rcap = o.r_cap_start + x * (o.r_cap_end - o.r_cap_start);
+                mdk_po_kick_drift(P, rcap * rcap, vlim * vlim, ke_target, step == 0, t->stream);
+                mdk_decide(P, mdk_drift_blocks(P, t->lc, false), false, t->stream, 0ull);
+                enqueue_rebuild(t);
+                mdk_po_force(P, rcap * rcap, t->stream);
+                mdk_po_kick(P, t->stream);
+            }
+            t->launches += 12 * (int64_t)o.check_interval;
+            if ((rc = check()) != MD_OK) break;
+            rep.min_nonbonded = bits_to_len(h_chk[0]);
+            rep.max_bond = bits_to_len(h_chk[1]);
+            done = step >= o.ramp_steps && rep.min_nonbonded > o.min_nonbonded && (n_bonds == 0 || rep.max_bond < o.max_bond);
+        }
+        rep.steps = step;
+        if (rc != MD_OK) break;
+        if (!done) {
+            set_error("md_pushoff: after %lld steps the smallest non-bonded distance is %.4f (want > %.3f) and the longest bond %.4f (want < %.3f)",
+                      (long long)step, rep.min_nonbonded, o.min_nonbonded, rep.max_bond, o.max_bond);
+            rc = MD_ERR_UNSUPPORTED;
+            break;
+        }
+        if ((rc = download(t, 0, r.data())) != MD_OK) break;
+    } while (0);
+    s->launches += t->launches;
+    md_destroy(t);
+    if (report) *report = rep;
+    if (rc != MD_OK) return rc;
+    for (int b = 0; b < s->P.n_sys; b++)
+        md_init_velocities(s->P.N1, o.temperature, o.seed + (uint64_t)b, v.data() + 3 * (size_t)b * s->P.N1);
+    if ((rc = upload_state(s, r.data(), v.data(), true)) != MD_OK) return rc;
+    return n_bonds > 0 ? md_set_bonds(s, n_bonds, ij, k, R0) : MD_OK;
 }
 
 int md_set_angles(md_system *s, double k_theta, double cos_theta0)

@@ -995,7 +995,7 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force)
 {
     if (!fused_force) return cdiv(P.N, 256);
-    return P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz : cdiv(P.N, lc.block);
+    return P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys : cdiv(P.N, lc.block);   // every box of every system writes its maximum
 }
 
 void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)

@@ -201,6 +201,11 @@ void mdk_sp_reorder(const MdDev &P, cudaStream_t st);
 void mdk_sp_build(const MdDev &P, cudaStream_t st);
 void mdk_sp_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
 void mdk_sp_energy(const MdDev &P, cudaStream_t st);
+// push-off of an overlapping chain start (md_pushoff.cu; initialisation, not the hot path)
+void mdk_po_kick_drift(const MdDev &P, double rcap2, double vlim2, double ke_target, int first, cudaStream_t st);
+void mdk_po_force(const MdDev &P, double rcap2, cudaStream_t st);
+void mdk_po_kick(const MdDev &P, cudaStream_t st);                             // + kinetic energy -> ctrl->red[RED_KE]
+void mdk_po_check(const MdDev &P, unsigned long long *out, cudaStream_t st);  // out[0] min non-bonded r^2, out[1] max bond r^2 (bit patterns)
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,
        LK_ENERGY, LK_EXPORT };

@@ -3,6 +3,8 @@ import math
 
 import numpy as np
 
+from md_workloads import make_state
+
 FORCE_RTOL = 1e-10      # per-atom max relative force error (SURVEY 8(c) A11 norm)
 POS_ATOL = 1e-9         # positions after 10 steps, sigma units, component-wise modulo L
 ENERGY_RTOL = 1e-9      # ke, pe separately after 10 steps
@@ -41,3 +43,18 @@ def sets_equal(gpu_counts, gpu_list, oracle):
         return 0, -1
     bad_rows = np.unique(rows[gflat != oflat_sorted])
     return len(bad_rows), int(bad_rows[0])
+
+
+def prepared_state(md, cfg, seed=1, jitter_amp=0.0):
+    """(r, v, bonds, box) of a config as BOTH sides receive it.  Lattice starts come straight from md_workloads.  The
+    random-walk chain start (cfg.lattice == "walk") overlaps; it is pushed apart by the library's md_pushoff --
+    initialisation, outside the parity-checked path -- and the result is handed to the oracle as data."""
+    r, v, bonds, box = make_state(cfg, seed, jitter_amp=jitter_amp)
+    if cfg.lattice != "walk":
+        return r, v, bonds, box
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    rep = g.pushoff(r, bonds, cfg.fene_k, cfg.fene_r0, temperature=cfg.temperature, seed=seed)
+    assert rep["min_nonbonded"] > 0.85 and rep["max_bond"] < 1.3, rep
+    r, v = g.positions(), g.velocities()
+    g.close()
+    return r, v, bonds, box

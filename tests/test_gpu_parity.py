@@ -340,3 +340,39 @@ def test_batched_systems_created_from_the_lattice(md):
     e1 = g.energies()
     assert abs(e1.total - e0.total) / (4 * n) < 2e-3 and e1.n_rebuilds >= 2
     g.close()
+
+
+@pytest.mark.parametrize("variant,mode", [("full", "fused"), ("full", "split"), ("full-globalw", "fused"), ("full-tiledw", "fused"),
+                                          ("full-tiledw", "split"), ("newton3", "split")])
+@pytest.mark.parametrize("hot", [0, 2])
+def test_batched_rebuild_follows_the_hottest_system(md, variant, mode, hot):
+    """One rebuild decision serves all systems of a batch (include/md_b200.h: "the largest velocity of any system").
+    Three systems, one of them hot and the others at rest: the rebuild count must be the HOT system's oracle count
+    whichever slot it sits in, and after the run every system's matrix must still hold all its interacting pairs
+    (forces against the all-pairs definition)."""
+    cfg = scaled_config("wca_4k", 1000)
+    n, n_sys = cfg.n_atoms, 3
+    states = [make_state(cfg, 20 + b, jitter_amp=0.05) for b in range(n_sys)]
+    box = states[0][3]
+    vel = [s[1] * (2.0 if b == hot else 0.0) for b, s in enumerate(states)]
+    kw, fv = {}, variant
+    if variant == "full-globalw":
+        fv, kw = "full", dict(flags=md.FLAG_GLOBAL_W)
+    elif variant == "full-tiledw":
+        fv, kw = "full", dict(flags=md.FLAG_TILED_W)
+    g = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", force_variant=fv, step_mode=mode,
+                    n_systems=n_sys, **kw)
+    g.set_state(np.concatenate([s[0] for s in states]), np.concatenate(vel))
+    o = OracleMD(n, box, cfg.r_cut, cfg.r_shell, cfg.dt)
+    o.set_state(states[hot][0], vel[hot])
+    steps = 60
+    g.step(steps)
+    assert o.step(steps) == 0
+    eg, eo = g.energies(), o.energies()
+    assert eo.n_rebuilds >= 5 and eg.n_rebuilds == eo.n_rebuilds
+    pos, fg = g.positions(), g.forces()
+    assert pos_err(pos[hot * n:(hot + 1) * n], o.positions(), box) <= 1e-7      # 60 steps: chaos-limited, not 1e-9
+    for b in range(n_sys):
+        fb, _, _ = brute_forces_sample(pos[b * n:(b + 1) * n], box, cfg.r_cut, np.arange(n))
+        assert force_rel_err(fg[b * n:(b + 1) * n], fb) <= FORCE_RTOL
+    g.close()

@@ -307,7 +307,17 @@ def test_p11_translation_and_permutation():
     t = oracle_for(np.mod(r + shift, box), box, rc, dr)
     assert rel_err(t.forces(), f0) < 1e-12
     st = t.neighbor_sets()
-    assert sum(not np.array_equal(a, b) for a, b in zip(s0, st)) <= 1   # a pair at r_n +- 1e-15 may flip
+    # Translation re-rounds every coordinate, so a pair whose r^2 sits within rounding of r_n^2 may change sides.  Any
+    # set that differs must differ by exactly such pairs: name them and show |r^2 - r_n^2| is at rounding level
+    # ("the comparator must print r^2 - r_n^2 for any mismatching pair").
+    rn2 = (rc + dr) ** 2
+    flipped = [(i, int(j)) for i, (a, b) in enumerate(zip(s0, st)) if not np.array_equal(a, b) for j in np.setxor1d(a, b)]
+    assert len(flipped) <= 2, f"{len(flipped)} neighbor entries changed under translation"        # one pair = two entries
+    for i, j in flipped:
+        d = r[i] - r[j]
+        d -= box * np.round(d / box)
+        gap = abs(float(d @ d) - rn2)
+        assert gap <= 64 * np.finfo(float).eps * box * box, f"pair ({i}, {j}) flipped with |r^2 - r_n^2| = {gap:.3e}"
     perm = np.random.default_rng(1).permutation(r.shape[0])
     p = oracle_for(r[perm], box, rc, dr)
     assert rel_err(p.forces(), f0[perm]) < 1e-12
@@ -550,3 +560,41 @@ def test_p15_dihedral_forces_are_minus_gradient_of_numpy_energy():
         dd = r[sl] - r[sl][0]
         dd -= box * np.round(dd / box)
         assert np.abs(np.cross(dd, fd[sl]).sum(0)).max() < 1e-11 * scale
+
+
+# ---- P16: the largest speed (S7's output, S8's input) and the rebuild rule it drives (R8) ----------
+def test_p16_vmax_is_the_largest_of_known_speeds_and_drives_the_rebuild_count():
+    """vmax against speeds fixed by construction, and the rebuild rule against its own arithmetic on a case where it
+    can be counted by hand: atoms too far apart to interact (no forces, constant velocities), ONE of them moving at speed
+    s.  Then disp_acc grows by exactly dt*s per step, a rebuild falls on every k0-th step with k0 the first k for which
+    k*dt*s > delta/2, and n steps give n // k0 rebuilds -- whatever atom carries the speed and whichever way it points."""
+    n_side, a = 6, 3.0
+    n, box = n_side ** 3, n_side * 3.0
+    r = sc_lattice(n, box)
+    rng = np.random.default_rng(5)
+    speeds = np.linspace(0.01, 0.02, n)
+    rng.shuffle(speeds)
+    u = rng.normal(size=(n, 3))
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    dt, delta = 0.005, 0.4
+    for fast, s_fast in ((0, 7.0), (n // 2, 3.3), (n - 1, 12.5)):
+        sp = speeds.copy()
+        sp[fast] = s_fast
+        v = u * sp[:, None]
+        o = oracle_for(r, box, R_WCA, delta, dt, v)
+        e = o.energies()
+        assert e.vmax == pytest.approx(s_fast, rel=1e-14)
+        assert e.ke == pytest.approx(0.5 * float((sp * sp).sum()), rel=1e-13)
+        k0 = int(math.floor(0.5 * delta / (dt * s_fast))) + 1          # first k with k dt s > delta/2
+        assert abs(k0 * dt * s_fast - 0.5 * delta) > 1e-9             # not a knife-edge case
+        for steps in (k0 - 1, k0, 5 * k0 + 2):
+            o.set_state(r, v)
+            assert o.step(steps) == 0
+            e = o.energies()
+            assert e.n_rebuilds == steps // k0
+            assert e.vmax == pytest.approx(s_fast, rel=1e-14)          # no forces: speeds do not change
+    # all atoms at rest: vmax = 0, never a rebuild
+    o = oracle_for(r, box, R_WCA, delta, dt, np.zeros((n, 3)))
+    o.step(50)
+    e = o.energies()
+    assert e.vmax == 0.0 and e.n_rebuilds == 0
