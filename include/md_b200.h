@@ -103,6 +103,13 @@ typedef struct md_params {
                                 that falls at least this many steps after the last sort (the paper: 100);
                                 0: at every rebuild; < 0: never (not even at the start).  Ignored without the flag: the
                                 default path sorts at every rebuild. */
+    int32_t  cell_split_x;   /* cells are >= r_n wide along y and z and this many times finer along x, the direction atoms
+                                are contiguous in after the cell-order sort, which shortens the candidate runs of the
+                                neighbor build; 1 = the paper's cubic cells; 0 = auto (4; 1 with
+                                MD_FLAG_LAYER_H).  1 .. 8. */
+    int32_t  tile_cells[3];  /* shared-memory staged kernels: r_n-wide cells per thread block along x, y, z (y, z: 1..3); 0 = auto */
+    int32_t  tile_threads;   /* their block size (multiple of 32 in [64, 512]; tiled W: 128, 256 or 512); 0 = auto */
+    int32_t  tile_capacity;  /* atoms the shared-memory tile holds (<= 8192); 0 = auto (1.35 x mean + 6 sigma) */
 } md_params;
 
 enum { MD_PREC_F64 = 0, MD_PREC_F32 = 1 };
@@ -156,6 +163,10 @@ typedef struct md_info {
     int32_t n_systems;
     int32_t precision;          /* MD_PREC_* */
     int32_t n_layers;           /* MD_FLAG_LAYER_H: N_l, columns of H; else 0 */
+    int32_t cells_x;            /* cells per edge along x (the direction atoms are contiguous in): cell_split_x * cells_per_edge */
+    int32_t cell_split_x;       /* fine cells per r_n-wide cell along x; the build scans up to +-cell_split_x of them per row */
+    int32_t sm_count;
+    double  candidates_per_atom;/* mean number of candidates the neighbor build tests per atom with this cell geometry (upper bound) */
 } md_info;
 
 /* Kernel classes of md_get_timers, after Table 2 of the paper. */
@@ -207,6 +218,25 @@ typedef struct md_pushoff_report {
 MD_API int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *ij, double k, double R0,
                       const md_pushoff_opts *opts, md_pushoff_report *report);
 
+/* Rigid molecules (sec. 4.3(1): "rigid bodies with multiple interaction sites ... e.g., four SP spheres
+ * in a rigid tetrahedral configuration ... rotation matrices ... a generalization of the symplectic leapfrog"; the paper
+ * gives no equations: DESIGN.md R20 states the textbook forms used).  The n_atoms atoms of the system become the
+ * interaction SITES of n_atoms / n_sites molecules: molecule m owns the atoms m*n_sites .. m*n_sites + n_sites - 1 (original
+ * ids), unit mass each, at the fixed body-frame positions body_xyz[3*k .. 3*k+2] (host; centre of mass at the origin,
+ * axes = principal axes, all three moments > 0, else MD_ERR_INVALID).  Sites of different molecules interact through the
+ * system's pair potential; sites of one molecule do not.  After this call load a state with md_set_rigid_state; md_step
+ * then integrates the molecules (half kick of V and of the body-frame angular momentum, free rotation of the rotation matrix
+ * by the splitting Rx Ry Rz Ry Rx, drift, rebuild decision from a bound on the largest site speed, site forces, half kick).
+ * md_energies: ke = translational + rotational kinetic energy, vmax = the largest site speed; md_get_positions /
+ * _velocities / _forces return the sites.  fp64, full-list forces, global-index W, one system, no bond terms
+ * (MD_ERR_UNSUPPORTED otherwise). */
+MD_API int md_set_rigid(md_system *s, int32_t n_sites, const double *body_xyz);
+/* Molecule state, all host arrays in molecule order: com[3*m], rot[9*m] (row-major rotation matrix A, body -> space: site k
+ * of molecule m sits at com + A b_k), vcom[3*m], angmom_body[3*m] (angular momentum in the body frame).  Setting a state
+ * bins the sites, builds W and evaluates the forces, like md_set_state. */
+MD_API int md_set_rigid_state(md_system *s, const double *com, const double *rot, const double *vcom, const double *angmom_body);
+MD_API int md_get_rigid_state(md_system *s, double *com, double *rot, double *vcom, double *angmom_body);
+
 /* Optional bond-angle terms for the chain workload ("bond force, bond-angle torque"; the paper gives
  * no form: the textbook cosine-harmonic U = k_theta/2 (cos(theta) - cos_theta0)^2 is used, R19) at every
  * atom that has two bonded partners, theta the angle between its two bonds.  Call after md_set_bonds and before the
@@ -231,10 +261,23 @@ MD_API int md_get_positions(md_system *s, double *xyz);
 MD_API int md_get_velocities(md_system *s, double *xyz);
 MD_API int md_get_forces(md_system *s, double *xyz);
 
+/* Positions and velocities in one call (one synchronisation; a single device-to-host transfer when vxyz == xyz + 3*N
+ * and the array is page-locked). */
+MD_API int md_get_state(md_system *s, double *xyz, double *vxyz);
+
+/* Zero-copy read-out: the same arrays (3*N doubles, original-id order, positions wrapped into [0, L)) written by one
+ * kernel into a caller-owned DEVICE buffer, e.g. the data_ptr() of a torch tensor on the system's device.  Enqueued on
+ * the system's stream and NOT synchronised: order later work after that stream.  MD_ERR_INVALID for a host pointer. */
+MD_API int md_get_positions_device(md_system *s, double *xyz_device);
+MD_API int md_get_velocities_device(md_system *s, double *xyz_device);
+MD_API int md_get_forces_device(md_system *s, double *xyz_device);
+
 /* Replace positions and velocities (host, 3*N each, original-id order; vxyz may be NULL = keep).
  * Positions must lie in [0, L].  Re-bins, rebuilds W, re-evaluates forces, resets step and rebuild
  * counters and the displacement accumulator; bonds are kept. */
 MD_API int md_set_state(md_system *s, const double *xyz, const double *vxyz);
+/* The same from DEVICE arrays (e.g. torch tensors on the system's device): no host transfer.  vxyz_device may be NULL. */
+MD_API int md_set_state_device(md_system *s, const double *xyz_device, const double *vxyz_device);
 
 /* Test hooks.  md_rebuild_neighbors forces a rebuild now.  md_get_neighbors returns the matrix by ORIGINAL
  * ids: counts[N]; list[N * max_neighbors] with row i = neighbors of atom i (unordered, -1 padded); for the
@@ -250,6 +293,16 @@ MD_API int md_get_info(md_system *s, md_info *out);
 MD_API int md_set_profiling(md_system *s, int enabled);
 MD_API int md_get_timers(md_system *s, double *ms, int64_t *launches);
 MD_API int md_reset_timers(md_system *s);
+
+/* Arithmetic ceilings of the device, MEASURED with register-resident FMA loops (CUDA events on the system's stream):
+ * the denominators for kernels bound by the fp64 pipe / instruction issue rather than HBM.  Not on the time-step path. */
+typedef struct md_peaks {
+    double  fp64_tflops;        /* DFMA loop, 2 flops per instruction */
+    double  fp32_tflops;        /* FFMA loop */
+    int32_t sm_count;
+    int32_t sm_clock_khz;       /* cudaDevAttrClockRate */
+} md_peaks;
+MD_API int md_measure_peaks(md_system *s, md_peaks *out);
 
 /* Device-memory hooks for the systems created AFTER the call (each system records the pair in force at its creation
  * and frees through it, so systems created under different hooks can coexist).  alloc(bytes, stream, user) returns a

@@ -12,14 +12,20 @@ BASELINE.json configs; see DESIGN.md "Input recipe".
 """
 from .configs import CONFIGS, MDConfig, get_config, scaled_config
 from .generators import (
+    body_inertia,
     box_edge,
     chain_melt,
+    chain_walks,
+    cross_body,
     fcc_lattice,
     gaussian_velocities,
     jitter,
     make_state,
+    random_rotations,
+    rigid_state,
     sc_lattice,
     splitmix64,
+    tetrahedron_body,
     uniform01,
 )
 
@@ -28,13 +34,19 @@ __all__ = [
     "MDConfig",
     "get_config",
     "scaled_config",
+    "body_inertia",
     "box_edge",
     "chain_melt",
+    "chain_walks",
+    "cross_body",
     "fcc_lattice",
     "gaussian_velocities",
     "jitter",
     "make_state",
+    "random_rotations",
+    "rigid_state",
     "sc_lattice",
     "splitmix64",
+    "tetrahedron_body",
     "uniform01",
 ]

@@ -16,7 +16,7 @@ R_WCA = 2.0 ** (1.0 / 6.0)
 class MDConfig:
     name: str
     n_atoms: int
-    lattice: str          # "sc" | "fcc" | "chains"
+    lattice: str          # "sc" | "fcc" | "chains" (zig-zag rows) | "walk" (overlapping random walks)
     density: float
     temperature: float
     r_cut: float
@@ -44,9 +44,14 @@ CONFIGS = {
     "wca_2m_dr05": MDConfig("wca_2m_dr05", 128 ** 3, "sc", 0.8, 1.0, R_WCA, 0.5, 0.005, 500),
     # configs[3]
     "lj_1m": MDConfig("lj_1m", 4 * 64 ** 3, "fcc", 0.8442, 0.72, 2.5, 0.3, 0.004, 500),
-    # configs[4]
-    "chains_1m": MDConfig("chains_1m", 16384 * 64, "chains", 0.85, 1.0, R_WCA, 0.4, 0.005, 500,
+    # configs[4]: 16,384 chains x 64 beads grown as seeded random walks (md_workloads.chain_walks); the overlapping start
+    # is pushed apart by the library (md_pushoff) before any timed or parity-checked step
+    "chains_1m": MDConfig("chains_1m", 16384 * 64, "walk", 0.85, 1.0, R_WCA, 0.4, 0.005, 500,
                           chain_len=64, n_chains=16384, fene_k=30.0, fene_r0=1.5),
+    # extra input, not a BASELINE.json config: the same melt started from overlap-free zig-zag rows (md_workloads.chain_melt),
+    # usable without a push-off (CPU-only tests, small parity cases)
+    "chains_rows_1m": MDConfig("chains_rows_1m", 16384 * 64, "chains", 0.85, 1.0, R_WCA, 0.4, 0.005, 500,
+                               chain_len=64, n_chains=16384, fene_k=30.0, fene_r0=1.5),
     # Context only (not BASELINE.json configs): the paper's OWN state points and shell at the
     # N = 128^3 row of its Table 1, cubic-grid start, for a line next to that table in BASELINE.md.
     "paper_sp_2m": MDConfig("paper_sp_2m", 128 ** 3, "sc", 0.8, 1.0, R_WCA, 0.6, 0.005, 500),
@@ -62,7 +67,7 @@ def scaled_config(name: str, n_atoms: int, **overrides) -> MDConfig:
     """Same state point, smaller system (for parity cases the oracle finishes in seconds)."""
     cfg = CONFIGS[name]
     kw = dict(n_atoms=n_atoms, name=f"{cfg.name}@{n_atoms}")
-    if cfg.lattice == "chains":
+    if cfg.lattice in ("chains", "walk"):
         chain_len = overrides.pop("chain_len", cfg.chain_len)
         if n_atoms % chain_len:
             raise ValueError("n_atoms must be a multiple of chain_len")

@@ -147,9 +147,8 @@ def chain_melt(n_chains: int, chain_len: int, density: float, seed: int,
     offset; a seeded jitter breaks the symmetry.  Returns (r, bonds, box) with
     atom id = chain * chain_len + bead and bonds (n_bonds, 2) int32.
 
-    This stands in for "chains grown as seeded random walks then pushed apart"
-    (BASELINE.json configs[4]): a push-off needs force evaluations, which this
-    module must not contain (reading R12).
+    An extra, crystalline chain input (configs "chains_rows_*"): it needs no push-off, so the CPU-only tests and
+    the small parity cases can use it.  BASELINE.json configs[4] itself is `chain_walks` + the library's push-off.
     """
     n = n_chains * chain_len
     box = box_edge(n, density)
@@ -189,6 +188,111 @@ def chain_melt(n_chains: int, chain_len: int, density: float, seed: int,
     return r, bonds, box
 
 
+_WALK_BASE = 1 << 42          # counter range of the random walks (velocities use [0, 6N), jitter 2^40.., rows 2^41..)
+_WALK_ATTEMPTS = 64
+
+
+def _unit_vectors(seed: int, ctr) -> np.ndarray:
+    """Uniform directions on the sphere from counters ctr, ctr + 1: z = 2u1 - 1, phi = 2 pi u2."""
+    ctr = np.asarray(ctr, dtype=np.uint64)
+    z = 2.0 * uniform01(seed, ctr) - 1.0
+    phi = 2.0 * math.pi * uniform01(seed, ctr + np.uint64(1))
+    s = np.sqrt(np.maximum(0.0, 1.0 - z * z))
+    return np.stack([s * np.cos(phi), s * np.sin(phi), z], axis=1)
+
+
+def chain_walks(n_chains: int, chain_len: int, density: float, seed: int,
+                bond: float = 0.97, min_second: float = 1.02):
+    """Chains "grown as seeded random walks" (BASELINE.json configs[4]).
+
+    Each chain starts at a seeded point uniform in the box and takes chain_len - 1 steps of length `bond` in uniformly
+    random directions; a step is redrawn while it would bring bead k+1 closer than `min_second` to bead k-1.  Chains
+    ignore one another, so the start OVERLAPS: it must be pushed apart before use (the library's md_pushoff --
+    pure geometry here, no forces).  Returns (r wrapped into the box, bonds, box), atom id = chain * chain_len + bead.
+    """
+    n = n_chains * chain_len
+    box = box_edge(n, density)
+    chain = np.arange(n_chains, dtype=np.uint64)
+    base = np.uint64(_WALK_BASE)
+    per_chain = np.uint64(4 + 2 * _WALK_ATTEMPTS * chain_len)
+    c0 = base + chain * per_chain
+    pos = np.empty((n_chains, chain_len, 3), dtype=np.float64)
+    for k in range(3):
+        pos[:, 0, k] = uniform01(seed, c0 + np.uint64(k)) * box
+    for b in range(1, chain_len):
+        pending = np.arange(n_chains)
+        for attempt in range(_WALK_ATTEMPTS):
+            ctr = c0[pending] + np.uint64(4 + 2 * (_WALK_ATTEMPTS * b + attempt))
+            cand = pos[pending, b - 1] + bond * _unit_vectors(seed, ctr)
+            if b >= 2:
+                d = cand - pos[pending, b - 2]
+                ok = (d * d).sum(1) >= min_second * min_second
+            else:
+                ok = np.ones(len(pending), dtype=bool)
+            pos[pending[ok], b] = cand[ok]
+            pending = pending[~ok]
+            if len(pending) == 0:
+                break
+        else:
+            raise RuntimeError("chain_walks: a step was rejected %d times" % _WALK_ATTEMPTS)
+    r = wrap(pos.reshape(n, 3), box)
+    ids = np.arange(n, dtype=np.int64)
+    first = ids[ids % chain_len < chain_len - 1]
+    bonds = np.stack([first, first + 1], axis=1).astype(np.int32)
+    return r, bonds, box
+
+
+# ---- rigid molecules (PAPER.md:183-185; DESIGN.md R20): geometry and seeded random numbers only -----------------------
+_ROT_BASE = 1 << 43
+
+
+def tetrahedron_body(edge: float = 0.9) -> np.ndarray:
+    """Four unit-mass sites at the corners of a regular tetrahedron ("four SP spheres in a rigid tetrahedral configuration,
+    spaced to overlap slightly"), centre of mass at the origin; the inertia tensor is isotropic (2 edge^2)."""
+    a = edge / (2.0 * math.sqrt(2.0))
+    return a * np.array([[1.0, 1.0, 1.0], [1.0, -1.0, -1.0], [-1.0, 1.0, -1.0], [-1.0, -1.0, 1.0]])
+
+
+def cross_body(a: float = 0.55, b: float = 0.4, c: float = 0.25) -> np.ndarray:
+    """Six unit-mass sites at (+-a,0,0), (0,+-b,0), (0,0,+-c): an asymmetric top in its principal frame
+    (moments 2(b^2+c^2), 2(a^2+c^2), 2(a^2+b^2))."""
+    return np.array([[a, 0, 0], [-a, 0, 0], [0, b, 0], [0, -b, 0], [0, 0, c], [0, 0, -c]], dtype=np.float64)
+
+
+def body_inertia(body: np.ndarray) -> np.ndarray:
+    """Principal moments of unit-mass sites given in their principal frame."""
+    b2 = (body * body).sum(1)
+    return np.array([(b2 - body[:, k] ** 2).sum() for k in range(3)])
+
+
+def random_rotations(n: int, seed: int) -> np.ndarray:
+    """n rotation matrices, uniform on SO(3): unit quaternions from four Gaussians of the counter generator."""
+    c = np.uint64(_ROT_BASE) + 2 * np.arange(4 * n, dtype=np.uint64)
+    g = (np.sqrt(-2.0 * np.log(uniform01(seed, c))) * np.cos(2.0 * math.pi * uniform01(seed, c + np.uint64(1)))).reshape(n, 4)
+    q = g / np.linalg.norm(g, axis=1)[:, None]
+    w, x, y, z = q[:, 0], q[:, 1], q[:, 2], q[:, 3]
+    A = np.empty((n, 3, 3))
+    A[:, 0, 0] = 1 - 2 * (y * y + z * z); A[:, 0, 1] = 2 * (x * y - w * z); A[:, 0, 2] = 2 * (x * z + w * y)
+    A[:, 1, 0] = 2 * (x * y + w * z); A[:, 1, 1] = 1 - 2 * (x * x + z * z); A[:, 1, 2] = 2 * (y * z - w * x)
+    A[:, 2, 0] = 2 * (x * z - w * y); A[:, 2, 1] = 2 * (y * z + w * x); A[:, 2, 2] = 1 - 2 * (x * x + y * y)
+    return A
+
+
+def rigid_state(n_mol: int, body: np.ndarray, mol_density: float, temperature: float, seed: int):
+    """Rigid molecules on a simple-cubic grid of centres with seeded random orientations: (R, A, V, pi, box).
+    V: Gaussian with variance T / M per component, zero net momentum; body-frame angular momentum pi_k: Gaussian with
+    variance I_k T (equipartition)."""
+    box = box_edge(n_mol, mol_density)
+    R = sc_lattice(n_mol, box)
+    A = random_rotations(n_mol, seed)
+    M = float(body.shape[0])
+    V = gaussian_velocities(n_mol, temperature / M, seed)
+    I = body_inertia(body)
+    g = gaussian_velocities(n_mol, 1.0, seed + 104729)          # unit-variance Gaussians (mean removed: harmless)
+    pi = g * np.sqrt(I * temperature)[None, :]
+    return R, A, V, pi, box
+
+
 def make_state(cfg: MDConfig, seed: int = 1, jitter_amp: float = 0.0):
     """(r, v, bonds, box) for a config.  `jitter_amp` > 0 displaces the lattice
     sites (a cheap non-trivial state for force/neighbor parity at full size)."""
@@ -200,6 +304,8 @@ def make_state(cfg: MDConfig, seed: int = 1, jitter_amp: float = 0.0):
         r = fcc_lattice(cfg.n_atoms, box)
     elif cfg.lattice == "chains":
         r, bonds, box = chain_melt(cfg.n_chains, cfg.chain_len, cfg.density, seed)
+    elif cfg.lattice == "walk":          # OVERLAPPING: to be pushed apart by the library's md_pushoff before use
+        r, bonds, box = chain_walks(cfg.n_chains, cfg.chain_len, cfg.density, seed)
     else:
         raise ValueError(cfg.lattice)
     if jitter_amp > 0.0:

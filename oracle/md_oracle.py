@@ -19,11 +19,13 @@ _SRC = os.path.join(_HERE, "md_oracle.c")
 _LIB = os.path.join(_HERE, "libmd_oracle.so")
 _SRC_SP = os.path.join(_HERE, "md_oracle_sp.c")
 _LIB_SP = os.path.join(_HERE, "libmd_oracle_sp.so")
+_SRC_RIGID = os.path.join(_HERE, "md_oracle_rigid.c")
+_LIB_RIGID = os.path.join(_HERE, "libmd_oracle_rigid.so")
 
 
 def build(force: bool = False) -> str:
     """gcc -O2 build of the oracle (fp contraction off: every a*b+c rounds twice unless written fma())."""
-    for src, out in ((_SRC, _LIB), (_SRC_SP, _LIB_SP)):
+    for src, out in ((_SRC, _LIB), (_SRC_SP, _LIB_SP), (_SRC_RIGID, _LIB_RIGID)):
         if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
             cmd = ["gcc", "-std=c11", "-O2", "-march=native", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
                    "-fPIC", "-shared", "-o", out, src, "-lm"]
@@ -284,3 +286,130 @@ class OracleMDSP(OracleMD):
 
     def _load(self):
         return lib_sp()
+
+
+# ---- rigid molecules (oracle/md_oracle_rigid.c; R20) ----------------------------------------------------
+class _RigidEnergy(C.Structure):
+    _fields_ = [("ke_trans", C.c_double), ("ke_rot", C.c_double), ("pe", C.c_double), ("virial", C.c_double),
+                ("px", C.c_double), ("py", C.c_double), ("pz", C.c_double), ("vbound", C.c_double),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
+                ("step", C.c_int64), ("n_rebuilds", C.c_int64), ("max_neighbors", C.c_int32), ("mean_neighbors", C.c_double)]
+
+
+@dataclass
+class RigidEnergies:
+    ke_trans: float
+    ke_rot: float
+    pe: float
+    virial: float
+    px: float
+    py: float
+    pz: float
+    vbound: float
+    lx: float
+    ly: float
+    lz: float
+    step: int
+    n_rebuilds: int
+    max_neighbors: int
+    mean_neighbors: float
+
+    @property
+    def ke(self) -> float:
+        return self.ke_trans + self.ke_rot
+
+    @property
+    def total(self) -> float:
+        return self.ke_trans + self.ke_rot + self.pe
+
+
+_lib_rigid = None
+
+
+def lib_rigid():
+    global _lib_rigid
+    if _lib_rigid is None:
+        build()
+        L = C.CDLL(_LIB_RIGID)
+        L.orr_create.restype = C.c_void_p
+        L.orr_create.argtypes = [C.c_int64, C.c_int, _dp, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.orr_destroy.argtypes = [C.c_void_p]
+        L.orr_set_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+        L.orr_get_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+        L.orr_step.argtypes = [C.c_void_p, C.c_int64]
+        L.orr_step.restype = C.c_int
+        L.orr_energies.argtypes = [C.c_void_p, C.POINTER(_RigidEnergy)]
+        for name in ("orr_get_sites", "orr_get_site_forces", "orr_get_inertia"):
+            getattr(L, name).argtypes = [C.c_void_p, _dp]
+        L.orr_get_force_torque.argtypes = [C.c_void_p, _dp, _dp]
+        L.orr_neighbor_total.argtypes = [C.c_void_p]
+        L.orr_neighbor_total.restype = C.c_int64
+        L.orr_get_neighbors.argtypes = [C.c_void_p, _ip, _ip]
+        _lib_rigid = L
+    return _lib_rigid
+
+
+class OracleRigid:
+    """Rigid molecules of n_sites unit-mass sites each (md_oracle_rigid.c header for the model and its sources)."""
+
+    def __init__(self, n_mol, body, box, r_cut, r_shell, dt):
+        self._L = lib_rigid()
+        body = _c(body).reshape(-1, 3)
+        self.nm, self.ns = int(n_mol), body.shape[0]
+        self._h = self._L.orr_create(self.nm, self.ns, body, float(box), float(r_cut), float(r_shell), float(dt))
+        if not self._h:
+            raise ValueError("orr_create failed: body frame must be the principal frame about the centre of mass, moments > 0")
+
+    def close(self):
+        if self._h:
+            self._L.orr_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, R, A, V, pi):
+        self._L.orr_set_state(self._h, _c(R), _c(A).reshape(self.nm, 9), _c(V), _c(pi))
+
+    def state(self):
+        R, A, V, pi = np.empty((self.nm, 3)), np.empty((self.nm, 9)), np.empty((self.nm, 3)), np.empty((self.nm, 3))
+        self._L.orr_get_state(self._h, R, A, V, pi)
+        return R, A.reshape(self.nm, 3, 3), V, pi
+
+    def step(self, n=1):
+        return self._L.orr_step(self._h, int(n))
+
+    def energies(self) -> RigidEnergies:
+        e = _RigidEnergy()
+        self._L.orr_energies(self._h, C.byref(e))
+        return RigidEnergies(**{k: getattr(e, k) for k, _ in _RigidEnergy._fields_})
+
+    def sites(self):
+        out = np.empty((self.nm * self.ns, 3))
+        self._L.orr_get_sites(self._h, out)
+        return out
+
+    def site_forces(self):
+        out = np.empty((self.nm * self.ns, 3))
+        self._L.orr_get_site_forces(self._h, out)
+        return out
+
+    def force_torque(self):
+        F, T = np.empty((self.nm, 3)), np.empty((self.nm, 3))
+        self._L.orr_get_force_torque(self._h, F, T)
+        return F, T
+
+    def inertia(self):
+        out = np.empty(3)
+        self._L.orr_get_inertia(self._h, out)
+        return out
+
+    def neighbors(self):
+        tot = self._L.orr_neighbor_total(self._h)
+        counts = np.empty(self.nm * self.ns, np.int32)
+        flat = np.empty(max(tot, 1), np.int32)
+        self._L.orr_get_neighbors(self._h, counts, flat)
+        return counts, flat[:tot]

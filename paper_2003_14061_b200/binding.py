@@ -24,8 +24,10 @@ STEP_MODE = {"fused": 0, "split": 1}
 PRECISION = {"f64": 0, "f32": 1}
 TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fused_step", "decide")
 
-EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_pushoff", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
-           "md_get_positions", "md_get_velocities", "md_get_forces", "md_set_state", "md_rebuild_neighbors",
+EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_pushoff", "md_set_rigid", "md_set_rigid_state", "md_get_rigid_state", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
+           "md_get_positions", "md_get_velocities", "md_get_forces", "md_get_state", "md_get_positions_device",
+           "md_get_velocities_device", "md_get_forces_device", "md_set_state", "md_set_state_device", "md_measure_peaks",
+           "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
            "md_set_allocator", "md_last_error", "md_version")
 
@@ -42,7 +44,8 @@ class _Params(C.Structure):
                 ("lattice", C.c_int32), ("force_variant", C.c_int32), ("step_mode", C.c_int32),
                 ("max_neighbors", C.c_int32), ("block_size", C.c_int32), ("device", C.c_int32),
                 ("stream", C.c_void_p), ("flags", C.c_uint32), ("n_systems", C.c_int32),
-                ("precision", C.c_int32), ("reorder_interval", C.c_int32)]
+                ("precision", C.c_int32), ("reorder_interval", C.c_int32), ("cell_split_x", C.c_int32), ("tile_cells", C.c_int32 * 3),
+                ("tile_threads", C.c_int32), ("tile_capacity", C.c_int32)]
 
 
 class _Energy(C.Structure):
@@ -59,7 +62,12 @@ class _Info(C.Structure):
                 ("n_bonds_per_atom_max", C.c_int32), ("device_bytes", C.c_int64), ("kernel_launches", C.c_int64),
                 ("device_name", C.c_char * 64), ("w_layout", C.c_int32), ("tile_cells", C.c_int32 * 3),
                 ("tile_capacity", C.c_int32), ("tile_threads", C.c_int32), ("use_graph", C.c_int32),
-                ("n_systems", C.c_int32), ("precision", C.c_int32), ("n_layers", C.c_int32)]
+                ("n_systems", C.c_int32), ("precision", C.c_int32), ("n_layers", C.c_int32), ("cells_x", C.c_int32),
+                ("cell_split_x", C.c_int32), ("sm_count", C.c_int32), ("candidates_per_atom", C.c_double)]
+
+
+class _Peaks(C.Structure):
+    _fields_ = [("fp64_tflops", C.c_double), ("fp32_tflops", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
 
 
 class _PushoffOpts(C.Structure):
@@ -125,6 +133,9 @@ def load_library(path: str = LIB_PATH):
     L.md_set_bonds.argtypes = [C.c_void_p, C.c_int64, _ip, C.c_double, C.c_double]
     L.md_pushoff.argtypes = [C.c_void_p, _dp, C.c_int64, _ip, C.c_double, C.c_double, C.POINTER(_PushoffOpts),
                              C.POINTER(_PushoffReport)]
+    L.md_set_rigid.argtypes = [C.c_void_p, C.c_int32, _dp]
+    L.md_set_rigid_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+    L.md_get_rigid_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
     L.md_set_angles.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_set_dihedrals.argtypes = [C.c_void_p, C.c_double, C.c_double]
     L.md_step.argtypes = [C.c_void_p, C.c_int64]
@@ -132,6 +143,11 @@ def load_library(path: str = LIB_PATH):
     for n in ("md_get_positions", "md_get_velocities", "md_get_forces"):
         getattr(L, n).argtypes = [C.c_void_p, _dp]
     L.md_set_state.argtypes = [C.c_void_p, _dp, C.c_void_p]
+    L.md_get_state.argtypes = [C.c_void_p, _dp, _dp]
+    for n in ("md_get_positions_device", "md_get_velocities_device", "md_get_forces_device"):
+        getattr(L, n).argtypes = [C.c_void_p, C.c_void_p]
+    L.md_set_state_device.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.md_measure_peaks.argtypes = [C.c_void_p, C.POINTER(_Peaks)]
     L.md_rebuild_neighbors.argtypes = [C.c_void_p]
     L.md_get_neighbors.argtypes = [C.c_void_p, _ip, C.c_void_p, C.POINTER(C.c_int32)]
     L.md_get_info.argtypes = [C.c_void_p, C.POINTER(_Info)]
@@ -181,7 +197,8 @@ class MDSystem:
 
     def __init__(self, n_atoms, r_cut, r_shell, dt, box=0.0, density=0.0, seed=1, temperature=1.0, lattice="auto",
                  force_variant="full", step_mode="fused", max_neighbors=0, block_size=0, device=-1,
-                 torch_memory=True, flags=0, n_systems=1, precision="f64", reorder_interval=0):
+                 torch_memory=True, flags=0, n_systems=1, precision="f64", reorder_interval=0,
+                 tile_cells=(0, 0, 0), tile_threads=0, tile_capacity=0, cell_split_x=0):
         import torch
         if not torch.cuda.is_available():
             raise MDError(MD_ERR_CUDA, "no CUDA device: the MD path has no CPU fallback")
@@ -200,6 +217,9 @@ class MDSystem:
         p.n_systems = int(n_systems)
         p.precision = PRECISION[precision]
         p.reorder_interval = int(reorder_interval)
+        p.tile_cells[0], p.tile_cells[1], p.tile_cells[2] = (int(x) for x in tile_cells)
+        p.tile_threads, p.tile_capacity = int(tile_threads), int(tile_capacity)
+        p.cell_split_x = int(cell_split_x)
         p.stream = torch.cuda.current_stream().cuda_stream or None
         self._L = L
         self._h = L.md_create_ex(C.byref(p))
@@ -253,6 +273,23 @@ class MDSystem:
         self._ck(self._L.md_pushoff(self._h, r, b.shape[0], b, float(k), float(r0), C.byref(o), C.byref(rep)))
         return {key: getattr(rep, key) for key, _ in _PushoffReport._fields_}
 
+    def set_rigid(self, body):
+        """md_set_rigid: the atoms become the sites of rigid molecules of len(body) sites (body: (n_sites, 3), principal frame)."""
+        b = np.ascontiguousarray(body, np.float64).reshape(-1, 3)
+        self._ck(self._L.md_set_rigid(self._h, b.shape[0], b))
+        self._n_sites = b.shape[0]
+
+    def set_rigid_state(self, com, rot, vcom, angmom_body):
+        nm = self.n // self._n_sites
+        a = [np.ascontiguousarray(x, np.float64).reshape(nm, k) for x, k in ((com, 3), (rot, 9), (vcom, 3), (angmom_body, 3))]
+        self._ck(self._L.md_set_rigid_state(self._h, *a))
+
+    def rigid_state(self):
+        nm = self.n // self._n_sites
+        R, A, V, pi = np.empty((nm, 3)), np.empty((nm, 9)), np.empty((nm, 3)), np.empty((nm, 3))
+        self._ck(self._L.md_get_rigid_state(self._h, R, A, V, pi))
+        return R, A.reshape(nm, 3, 3), V, pi
+
     def set_angles(self, k_theta, cos_theta0):
         self._ck(self._L.md_set_angles(self._h, float(k_theta), float(cos_theta0)))
 
@@ -284,6 +321,47 @@ class MDSystem:
 
     def forces(self, out=None):
         return self._get("md_get_forces", out)
+
+    def state(self, r_out=None, v_out=None):
+        """md_get_state: positions and velocities with one synchronisation.  Pass the two halves of ONE page-locked
+        (2, N, 3) array to get a single device-to-host transfer."""
+        if r_out is None or v_out is None:
+            both = np.empty((2, self.n, 3))
+            r_out, v_out = both[0], both[1]
+        self._ck(self._L.md_get_state(self._h, r_out, v_out))
+        return r_out, v_out
+
+    def _device_out(self, name, out):
+        import torch
+        if out is None:
+            out = torch.empty((self.n, 3), dtype=torch.float64, device="cuda")
+        if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 3 * self.n):
+            raise MDError(MD_ERR_INVALID, "need a contiguous float64 CUDA tensor of 3 N elements")
+        self._ck(getattr(self._L, name)(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def positions_device(self, out=None):
+        """Zero-copy read-out into a torch CUDA tensor (N, 3), original-id order; enqueued on the system's stream."""
+        return self._device_out("md_get_positions_device", out)
+
+    def velocities_device(self, out=None):
+        return self._device_out("md_get_velocities_device", out)
+
+    def forces_device(self, out=None):
+        return self._device_out("md_get_forces_device", out)
+
+    def set_state_device(self, r, v=None):
+        """md_set_state from torch CUDA tensors (float64, contiguous): no host transfer."""
+        import torch
+        for t in (r, v):
+            if t is not None and not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == 3 * self.n):
+                raise MDError(MD_ERR_INVALID, "need contiguous float64 CUDA tensors of 3 N elements")
+        self._ck(self._L.md_set_state_device(self._h, C.c_void_p(r.data_ptr()), C.c_void_p(v.data_ptr()) if v is not None else None))
+
+    def measure_peaks(self) -> dict:
+        p = _Peaks()
+        self._ck(self._L.md_measure_peaks(self._h, C.byref(p)))
+        return {k: getattr(p, k) for k, _ in _Peaks._fields_}
 
     def neighbors(self, with_list=True):
         """(counts[N], list[N, Mmax] of original ids, -1 padded)."""

@@ -51,6 +51,7 @@ struct md_system {
     cudaStream_t stream = nullptr;
     bool own_stream = false;
     int device = 0;
+    int sm_count = 0;
     char device_name[64] = "";
     std::vector<void *> allocs;
     md_alloc_fn alloc = nullptr;   // the hooks in force when the system was created: its memory goes back the way it came
@@ -322,7 +323,7 @@ int upload_state(md_system *s, const double *xyz, const double *vxyz, bool check
     if (!vxyz) {   // keep velocities: bring them to original order in the second half of scratch first
         if (!s->has_state) { set_error("md_set_state: no velocities to keep"); return MD_ERR_INVALID; }
         s->launches += 1;
-        mdk_export(s->P, 1, n3, s->stream);
+        mdk_export(s->P, 1, s->P.scratch + n3, s->stream);
     }
     const double *src = xyz;
     if (!is_pinned(xyz)) { memcpy(s->h_stage, xyz, n3 * sizeof(double)); src = s->h_stage; }
@@ -354,7 +355,7 @@ int download(md_system *s, int what, double *out)
     if (!s->has_state) { set_error("no state loaded"); return MD_ERR_INVALID; }
     const size_t n3 = 3 * (size_t)s->P.N;
     s->launches += 1;
-    mdk_export(s->P, what, 0, s->stream);
+    mdk_export(s->P, what, s->P.scratch, s->stream);
     const bool direct = is_pinned(out);
     CK(cudaMemcpyAsync(direct ? out : s->h_stage, s->P.scratch, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
@@ -363,48 +364,67 @@ int download(md_system *s, int what, double *out)
     return MD_OK;
 }
 
-int env_int(const char *name, int dflt)
+// positions / velocities / forces in original-id order into a caller-owned DEVICE buffer: one kernel, no copy, no sync
+int export_device(md_system *s, int what, double *dst)
 {
-    const char *v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
+    if (!s || !dst) { set_error("null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("no state loaded"); return MD_ERR_INVALID; }
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, dst) != cudaSuccess || (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged)) {
+        cudaGetLastError();
+        set_error("the *_device getters need a device pointer");
+        return MD_ERR_INVALID;
+    }
+    s->launches += 1;
+    mdk_export(s->P, what, dst, s->stream);
+    CK(cudaGetLastError());
+    return MD_OK;
 }
 
 // Box of cells per thread block, block size and tile capacity of the tiled W layout (md_types.h: TileGeom).
 // Defaults aim at ~0.8 own atoms per thread and a 2 x 2 cross-section in y, z (halo factor ~4.5 for the WCA
-// configs); MD_TILE_S / _R / _RZ / _THREADS / _CAP override them for tuning runs.
-bool choose_tile(MdDev &P, size_t smem_optin, bool for_tiled_w)
+// configs); md_params.tile_cells / tile_threads / tile_capacity override them (tuning runs, box-shape tests).
+bool choose_tile(MdDev &P, const md_params &prm, size_t smem_optin, bool for_tiled_w)
 {
     TileGeom &G = P.tg;
     const int nc = P.nc;
-    const double per_cell = (double)P.N / P.NC;
-    G.R = std::min(std::max(env_int("MD_TILE_R", 2), 1), 3);
-    G.RZ = std::min(std::max(env_int("MD_TILE_RZ", 2), 1), 3);
-    G.threads = env_int("MD_TILE_THREADS", per_cell > 8.0 ? 512 : 256);
-    if (G.threads < 64 || G.threads > 512 || G.threads % 32) { set_error("MD_TILE_THREADS must be a multiple of 32 in [64, 512]"); return false; }
-    int S = env_int("MD_TILE_S", 0);
+    const double per_cell = (double)P.N1 / ((double)nc * nc * nc);      // atoms per r_n-wide cell
+    auto knob = [](int v, int dflt) { return v > 0 ? v : dflt; };
+    G.R = std::min(std::max(knob(prm.tile_cells[1], 2), 1), 3);
+    G.RZ = std::min(std::max(knob(prm.tile_cells[2], 2), 1), 3);
+    G.threads = knob(prm.tile_threads, per_cell > 8.0 ? 512 : 256);
+    if (G.threads < 64 || G.threads > 512 || G.threads % 32) { set_error("tile_threads must be a multiple of 32 in [64, 512]"); return false; }
+    // box length along x in r_n-wide cells; in fine cells it is a multiple of kx, so every box starts at least kx cells
+    // from the row's ends or exactly at them: the halo of a box is then one contiguous range on either side (md_types.h)
+    int S = prm.tile_cells[0];
     if (S <= 0) S = (int)lround(0.8 * G.threads / (G.R * G.RZ * per_cell));
     S = std::min(std::max(S, 1), nc);
     G.nsx = (nc + S - 1) / S;
-    G.S = (nc + G.nsx - 1) / G.nsx;                 // balance the boxes along x
-    G.nsx = (nc + G.S - 1) / G.S;
-    if (!env_int("MD_TILE_THREADS", 0)) {
+    S = (nc + G.nsx - 1) / G.nsx;                   // balance the boxes along x
+    G.nsx = (nc + S - 1) / S;
+    if (prm.tile_threads <= 0) {
         // small boxes (few cells per edge): S was clipped to the row, so shrink the block to the atoms a box owns
-        const double own = (double)G.S * G.R * G.RZ * per_cell;
+        const double own = (double)S * G.R * G.RZ * per_cell;
         int t = 32 * (int)ceil(1.12 * own / 32.0);
         if (for_tiled_w) t = t <= 128 ? 128 : (t <= 256 ? 256 : 512);      // instantiated sizes of the tiled force kernels
         G.threads = std::min(G.threads, std::max(64, t));
     }
+    G.S = S * P.kx;
     G.nsy = (nc + G.R - 1) / G.R;
     G.nsz = (nc + G.RZ - 1) / G.RZ;
     G.nsys = P.n_sys;
-    const double mean = (double)(G.S + 2) * (G.R + 2) * (G.RZ + 2) * per_cell;
-    int cap = env_int("MD_TILE_CAP", 0);
+    const double mean = (double)(S + 2) * (G.R + 2) * (G.RZ + 2) * per_cell;
+    int cap = prm.tile_capacity;
     if (cap <= 0) cap = (int)(1.35 * mean + 6.0 * sqrt(mean) + 32.0);
     cap = (cap + 31) & ~31;
     if (cap > 8192) cap = 8192;
     G.cap = cap;
-    if (mean > 0.8 * cap) { set_error("tiled W: %.0f atoms per tile exceed the 13-bit tile index; use MD_FLAG_GLOBAL_W or smaller MD_TILE_S", mean); return false; }
-    if (mdk_tile_smem(G, true) > smem_optin) { set_error("tiled W: tile of %d atoms does not fit shared memory", cap); return false; }
+    // the largest tile the build kernel's shared memory holds (positions + cell table + index table for global-index W)
+    P.tiled = for_tiled_w ? 1 : 0;                  // mdk_tile_smem depends on the W layout
+    while (G.cap > 64 && mdk_tile_smem(P, true) + 8192 > smem_optin) G.cap -= 32;
+    cap = G.cap;
+    if (mean > 0.8 * cap) { set_error("tile build: %.0f atoms per tile exceed the tile capacity %d; use MD_FLAG_GLOBAL_W or a smaller tile_cells[0]", mean, cap); return false; }
+    if (mdk_tile_smem(P, true) + 8192 > smem_optin) { set_error("tile build: tile of %d atoms does not fit shared memory", cap); return false; }
     return true;
 }
 
@@ -498,7 +518,10 @@ md_system *md_create_ex(const md_params *pp)
     int nc = (int)floor(box_eff / rn);
     if (nc >= 1 && box_eff / nc - rn < (sp ? 1e-5 : 1e-9) * rn) nc -= 1;     // keep the cell strictly wider than r_n
     if (nc < 3) { set_error("box too small: %d cells per edge (need >= 3)", nc); return nullptr; }
-    if ((int64_t)nc * nc * nc * std::max(1, p.n_systems) > (1ll << 30)) { set_error("too many cells"); return nullptr; }
+    if (p.cell_split_x < 0 || p.cell_split_x > 8) { set_error("cell_split_x must be in [0, 8]"); return nullptr; }
+    if (p.cell_split_x == 0) p.cell_split_x = (p.flags & MD_FLAG_LAYER_H) ? 1 : 4;
+    if ((p.flags & MD_FLAG_LAYER_H) && p.cell_split_x != 1) { set_error("MD_FLAG_LAYER_H keeps the paper's cubic cells (cell_split_x = 1)"); return nullptr; }
+    if ((int64_t)nc * nc * nc * p.cell_split_x * std::max(1, p.n_systems) > (1ll << 30)) { set_error("too many cells"); return nullptr; }
     if (p.max_neighbors <= 0) {
         const double ideal = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         p.max_neighbors = 16 * (int)ceil((1.35 * ideal + 12.0) / 16.0);
@@ -528,6 +551,7 @@ md_system *md_create_ex(const md_params *pp)
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return fail("cudaGetDeviceProperties");
     snprintf(s->device_name, sizeof(s->device_name), "%.63s", prop.name);
+    s->sm_count = prop.multiProcessorCount;
     if (prop.major < 10) { set_error("device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); md_destroy(s); return nullptr; }
     if (p.stream) s->stream = (cudaStream_t)p.stream;
     else {
@@ -537,17 +561,25 @@ md_system *md_create_ex(const md_params *pp)
 
     MdDev &P = s->P;
     memset(&P, 0, sizeof(P));
+    P.sm_count = prop.multiProcessorCount;
     P.n_sys = p.n_systems;
     P.N1 = (int)p.n_atoms;
     P.N = P.N1 * P.n_sys;
     P.N_pad = (P.N + 127) & ~127;
     P.Mmax = p.max_neighbors;
     P.nc = nc;
-    P.NC1 = nc * nc * nc;
+    P.kx = p.cell_split_x;
+    P.ncx = nc * P.kx;
+    P.NC1 = P.ncx * nc * nc;
     P.NC = P.NC1 * P.n_sys;
     P.half_list = p.force_variant == MD_FORCE_NEWTON3_ATOMICS;
     P.scan_blocks = (P.NC + 2047) / 2048;
     P.L = box_eff; P.half_L = 0.5 * box_eff; P.inv_w = (double)nc / box_eff;
+    P.inv_wx = (double)P.ncx / box_eff;
+    // row pruning of the neighbor build: binary32 constants rounded to the safe side (md_device.cuh: row_halfwidth)
+    P.w_f = (float)(box_eff / nc * (1.0 - 1e-5));
+    P.inv_wx_f = (float)(P.inv_wx * (1.0 + 1e-5));
+    P.rn2_prune = (float)(rn * rn * (1.0 + 1e-5));
     P.sp = sp ? 1 : 0;
     // padded columns pay once a column is long enough (measured: +14 % at 76 neighbors, -5 % at 12; md_sp.cu)
     P.sp_pad = sp && 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density >= 32.0 ? 4 : 1;
@@ -569,16 +601,18 @@ md_system *md_create_ex(const md_params *pp)
         const double mbar_est = 4.0 / 3.0 * 3.14159265358979323846 * rn * rn * rn * p.density;
         // (single precision: the tile-staged BUILD only; its force kernel gathers float4 records)
         const bool want_tiled = !sp && ((p.flags & MD_FLAG_TILED_W) || (!(p.flags & MD_FLAG_GATHER_W) && mbar_est >= 32.0));
-        const bool fits = choose_tile(P, prop.sharedMemPerBlockOptin, want_tiled);
+        const bool fits = choose_tile(P, p, prop.sharedMemPerBlockOptin, want_tiled);
         if (!fits && (p.flags & MD_FLAG_TILED_W)) { md_destroy(s); return nullptr; }
         P.tile_build = fits ? 1 : 0;
+        // the tile build addresses W with 32-bit element offsets (md_tile.cu: Emit); larger matrices use the gather build
+        if ((uint64_t)p.max_neighbors * (uint64_t)((P.N + 127) & ~127) >= (1ull << 31)) P.tile_build = 0;
         // single precision, many small systems whose x-rows are shorter than the box length the tile wants: the gather
         // build is faster there (measured 64 / 512 x wca_4k: 6.90 vs 6.67 G and 13.75 vs 12.86 G atom-steps/s)
-        if (sp && fits && P.n_sys >= 32 && P.tg.S >= nc) P.tile_build = 0;
+        if (sp && fits && P.n_sys >= 32 && P.tg.S >= P.ncx) P.tile_build = 0;
         // W layout: measured on B200, tile-local W wins once a column of W is long enough
         // to amortise staging the tile (LJ r_c = 2.5: 76 neighbors, +17 %) and loses for the short WCA columns
         // (12 neighbors, -17 %).  Estimated mean column length = ideal-gas count in the neighbor sphere.
-        P.tiled = fits && want_tiled ? 1 : 0;
+        P.tiled = fits && P.tile_build && want_tiled ? 1 : 0;
         if (fits && mdk_tile_configure(P) != 0) {
             set_error("tile kernels: %d threads per block not available for this W layout, or cudaFuncSetAttribute failed", P.tg.threads);
             md_destroy(s);
@@ -666,7 +700,56 @@ md_system *md_create(int64_t n_atoms, double box, double density, double r_cut, 
 int md_set_state(md_system *s, const double *xyz, const double *vxyz)
 {
     if (!s || !xyz) { set_error("md_set_state: null argument"); return MD_ERR_INVALID; }
+    if (s->P.rigid) { set_error("md_set_state: a rigid-molecule system takes its state through md_set_rigid_state"); return MD_ERR_INVALID; }
     return upload_state(s, xyz, vxyz, true);      // the range check [0, L] runs on the device, before the old state is touched
+}
+
+int md_set_state_device(md_system *s, const double *xyz_device, const double *vxyz_device)
+{
+    if (!s || !xyz_device) { set_error("md_set_state_device: null argument"); return MD_ERR_INVALID; }
+    for (const double *p : {xyz_device, vxyz_device}) {
+        cudaPointerAttributes a;
+        if (p && (cudaPointerGetAttributes(&a, p) != cudaSuccess || (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged))) {
+            cudaGetLastError();
+            set_error("md_set_state_device needs device pointers");
+            return MD_ERR_INVALID;
+        }
+    }
+    const size_t n3 = 3 * (size_t)s->P.N;
+    if (!vxyz_device) {
+        if (!s->has_state) { set_error("md_set_state_device: no velocities to keep"); return MD_ERR_INVALID; }
+        s->launches += 1;
+        mdk_export(s->P, 1, s->P.scratch + n3, s->stream);
+    } else {
+        CK(cudaMemcpyAsync(s->P.scratch + n3, vxyz_device, n3 * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    }
+    CK(cudaMemcpyAsync(s->P.scratch, xyz_device, n3 * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    s->launches += 1;
+    mdk_check_range(s->P, s->prm.box, s->stream);
+    int rc = fetch_ctrl(s);
+    if (rc) return rc;
+    if (s->h_ctrl->err == MD_ERR_INVALID) {
+        CK(cudaMemsetAsync(&s->P.ctrl->err, 0, sizeof(int), s->stream));
+        set_error("md_set_state_device: a coordinate lies outside [0, L]");
+        return MD_ERR_INVALID;
+    }
+    return install_state(s);
+}
+
+int md_measure_peaks(md_system *s, md_peaks *out)
+{
+    if (!s || !out) { set_error("md_measure_peaks: null argument"); return MD_ERR_INVALID; }
+    memset(out, 0, sizeof(*out));
+    int clk = 0;
+    CK(cudaDeviceGetAttribute(&clk, cudaDevAttrClockRate, s->device));
+    out->sm_count = s->sm_count;
+    out->sm_clock_khz = clk;
+    CK(cudaStreamSynchronize(s->stream));
+    out->fp64_tflops = mdk_peak_fp64(s->stream, s->sm_count, s->P.partials);
+    out->fp32_tflops = mdk_peak_fp32(s->stream, s->sm_count, s->P.partials);
+    CK(cudaGetLastError());
+    if (!(out->fp64_tflops > 0)) { set_error("md_measure_peaks: timing failed"); return MD_ERR_CUDA; }
+    return MD_OK;
 }
 
 int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, double R0)
@@ -691,16 +774,18 @@ int md_set_bonds(md_system *s, int64_t n_bonds, const int32_t *ij, double k, dou
             mx = std::max(mx, tab[n + a] >= 0 ? 2 : 1);
         }
     }
+    if (s->P.rigid) { set_error("md_set_bonds: not with rigid molecules"); return MD_ERR_UNSUPPORTED; }
     if (!P.bond_orig) {
         P.bond_orig = (int *)dev_alloc(s, 2 * n * sizeof(int));
         P.bond_dev = (int *)dev_alloc(s, 2 * (size_t)P.N_pad * sizeof(int));
-        P.inv = (int *)dev_alloc(s, n * sizeof(int));
+        if (!P.inv) P.inv = (int *)dev_alloc(s, n * sizeof(int));
         if (!P.bond_orig || !P.bond_dev || !P.inv) { set_error("device allocation failed"); return MD_ERR_NOMEM; }
     }
     CK(cudaMemcpyAsync(P.bond_orig, tab.data(), 2 * n * sizeof(int), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     drop_graph(s);                 // the captured kernel arguments (MdDev by value) change
     P.has_bonds = n_bonds > 0;
+    P.need_inv = 1;
     P.fene_k = k;
     P.fene_R02 = R0 * R0;
     P.fene_kf = (float)k;
@@ -745,18 +830,30 @@ int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *
     tp.force_variant = MD_FORCE_FULL_LIST;
     tp.step_mode = MD_STEP_SPLIT;
     tp.flags = MD_FLAG_GLOBAL_W | MD_FLAG_NO_GRAPH;
-    tp.max_neighbors = 2 * s->P.Mmax;
     tp.reorder_interval = 0;
     tp.stream = (void *)s->stream;
     tp.device = s->device;
-    const md_alloc_fn a0 = g_alloc; const md_free_fn f0 = g_free; void *u0 = g_alloc_user;
-    g_alloc = s->alloc; g_free = s->free_; g_alloc_user = s->alloc_user;       // the temporary system allocates the way s does
-    md_system *t = md_create_ex(&tp);
-    g_alloc = a0; g_free = f0; g_alloc_user = u0;
-    if (!t) return MD_ERR_CUDA;
     const size_t n3 = 3 * (size_t)s->P.N;
     std::vector<double> v(n3), r(n3);
+    for (int b = 0; b < s->P.n_sys; b++)
+        md_init_velocities(s->P.N1, o.temperature, o.seed + 1 + (uint64_t)b, v.data() + 3 * (size_t)b * s->P.N1);
+    // Random walks cluster: the crowded start has atoms with several times the equilibrium number of neighbors
+    // (73 against a mean of 18 at N = 2^20).  Start with 4 x the rows of W and double while the start overflows them.
+    md_system *t = nullptr;
     int rc = MD_OK;
+    for (int mult = 4; mult <= 32; mult *= 2) {
+        tp.max_neighbors = mult * s->P.Mmax;
+        const md_alloc_fn a0 = g_alloc; const md_free_fn f0 = g_free; void *u0 = g_alloc_user;
+        g_alloc = s->alloc; g_free = s->free_; g_alloc_user = s->alloc_user;   // the temporary system allocates the way s does
+        t = md_create_ex(&tp);
+        g_alloc = a0; g_free = f0; g_alloc_user = u0;
+        if (!t) return MD_ERR_CUDA;
+        rc = upload_state(t, xyz, v.data(), true);
+        if (rc != MD_ERR_NEBR_OVERFLOW) break;
+        md_destroy(t);
+        t = nullptr;
+    }
+    if (!t) return rc;
     unsigned long long *d_chk = nullptr, h_chk[2] = {0, 0};
     md_pushoff_report rep;
     memset(&rep, 0, sizeof(rep));
@@ -767,9 +864,7 @@ int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *
         return check_device_status(t);
     };
     do {
-        for (int b = 0; b < s->P.n_sys; b++)
-            md_init_velocities(s->P.N1, o.temperature, o.seed + 1 + (uint64_t)b, v.data() + 3 * (size_t)b * s->P.N1);
-        if ((rc = upload_state(t, xyz, v.data(), true)) != MD_OK) break;
+        if (rc != MD_OK) break;
         if (n_bonds > 0 && (rc = md_set_bonds(t, n_bonds, ij, k, R0)) != MD_OK) break;
         d_chk = (unsigned long long *)dev_alloc(t, 2 * sizeof(unsigned long long));
         if (!d_chk) { set_error("md_pushoff: device allocation failed"); rc = MD_ERR_NOMEM; break; }
@@ -818,6 +913,103 @@ int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *
     return n_bonds > 0 ? md_set_bonds(s, n_bonds, ij, k, R0) : MD_OK;
 }
 
+// ---- rigid molecules (R20) ----
+int md_set_rigid(md_system *s, int32_t n_sites, const double *body_xyz)
+{
+    if (!s || !body_xyz || n_sites < 3 || n_sites > 8) { set_error("md_set_rigid: 3 .. 8 sites per molecule"); return MD_ERR_INVALID; }
+    MdDev &P = s->P;
+    if (P.sp || P.half_list || P.tiled || P.n_sys > 1 || P.has_bonds || P.layer_H || P.w_col != 1) {
+        set_error("md_set_rigid: fp64, full-list forces, global-index W (MD_FLAG_GATHER_W for long columns), one system, no bonds");
+        return MD_ERR_UNSUPPORTED;
+    }
+    if (P.N % n_sites) { set_error("md_set_rigid: n_atoms is not a multiple of the sites per molecule"); return MD_ERR_INVALID; }
+    // unit-mass sites: centre of mass at the origin, inertia tensor diagonal with positive moments (principal frame)
+    double I[3][3] = {{0}}, com[3] = {0, 0, 0}, bmax = 0.0;
+    for (int k = 0; k < n_sites; k++) {
+        const double *b = body_xyz + 3 * k, b2 = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
+        bmax = std::max(bmax, sqrt(b2));
+        for (int r = 0; r < 3; r++) {
+            com[r] += b[r];
+            for (int c = 0; c < 3; c++) I[r][c] += (r == c ? b2 : 0.0) - b[r] * b[c];
+        }
+    }
+    const double tol = 1e-12 * (I[0][0] + I[1][1] + I[2][2] + 1.0);
+    bool bad = fabs(com[0]) + fabs(com[1]) + fabs(com[2]) > 1e-12 * n_sites * (bmax + 1.0);
+    for (int r = 0; r < 3; r++)
+        for (int c = 0; c < 3; c++)
+            if ((r != c && fabs(I[r][c]) > tol) || (r == c && !(I[r][c] > 0))) bad = true;
+    if (bad) { set_error("md_set_rigid: give the sites in the principal frame about their centre of mass (all three moments > 0)"); return MD_ERR_INVALID; }
+    drop_graph(s);
+    P.rb_ns = n_sites;
+    P.rb_nm = P.N / n_sites;
+    for (int k = 0; k < 3 * n_sites; k++) P.rb_body[k] = body_xyz[k];
+    P.rb_M = (double)n_sites;
+    P.rb_bmax = bmax;
+    P.rb_Imin = std::min(I[0][0], std::min(I[1][1], I[2][2]));
+    for (int c = 0; c < 3; c++) P.rb_I[c] = I[c][c];
+    if (!P.rb_R) {
+        const size_t nm = (size_t)P.rb_nm;
+        P.rb_R = (double *)dev_alloc(s, 3 * nm * sizeof(double)); P.rb_V = (double *)dev_alloc(s, 3 * nm * sizeof(double));
+        P.rb_A = (double *)dev_alloc(s, 9 * nm * sizeof(double)); P.rb_pi = (double *)dev_alloc(s, 3 * nm * sizeof(double));
+        P.rb_off = (double *)dev_alloc(s, 3 * (size_t)P.N * sizeof(double));
+        if (!P.inv) P.inv = (int *)dev_alloc(s, (size_t)P.N * sizeof(int));
+        if (!P.rb_R || !P.rb_V || !P.rb_A || !P.rb_pi || !P.rb_off || !P.inv) { set_error("device allocation failed"); return MD_ERR_NOMEM; }
+    }
+    P.rigid = 1;
+    P.need_inv = 1;
+    P.tile_build = 0;          // the gathering build kernel knows the molecules (sites of one molecule are no neighbors)
+    s->has_state = false;      // load the molecules with md_set_rigid_state
+    return MD_OK;
+}
+
+int md_set_rigid_state(md_system *s, const double *com, const double *rot, const double *vcom, const double *angmom_body)
+{
+    if (!s || !com || !rot || !vcom || !angmom_body) { set_error("md_set_rigid_state: null argument"); return MD_ERR_INVALID; }
+    MdDev &P = s->P;
+    if (!P.rigid) { set_error("md_set_rigid_state: call md_set_rigid first"); return MD_ERR_INVALID; }
+    const size_t nm = (size_t)P.rb_nm;
+    const int ns = P.rb_ns;
+    const double L = P.L;
+    std::vector<double> xyz(3 * (size_t)P.N), v(3 * (size_t)P.N);
+    for (size_t m = 0; m < nm; m++) {
+        const double *A = rot + 9 * m, *R = com + 3 * m, *V = vcom + 3 * m, *pi = angmom_body + 3 * m;
+        const double w[3] = {pi[0] / P.rb_I[0], pi[1] / P.rb_I[1], pi[2] / P.rb_I[2]};
+        for (int k = 0; k < ns; k++) {
+            const double *b = P.rb_body + 3 * k;
+            const double u[3] = {w[1] * b[2] - w[2] * b[1], w[2] * b[0] - w[0] * b[2], w[0] * b[1] - w[1] * b[0]};
+            for (int c = 0; c < 3; c++) {
+                double x = R[c] + (A[3 * c] * b[0] + A[3 * c + 1] * b[1] + A[3 * c + 2] * b[2]);
+                if (!std::isfinite(x)) { set_error("md_set_rigid_state: non-finite state"); return MD_ERR_NONFINITE; }
+                x -= L * floor(x / L);
+                if (x >= L || x < 0.0) x = 0.0;
+                xyz[3 * (m * ns + k) + c] = x;
+                v[3 * (m * ns + k) + c] = V[c] + (A[3 * c] * u[0] + A[3 * c + 1] * u[1] + A[3 * c + 2] * u[2]);
+            }
+        }
+    }
+    CK(cudaMemcpyAsync(P.rb_R, com, 3 * nm * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(P.rb_A, rot, 9 * nm * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(P.rb_V, vcom, 3 * nm * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemcpyAsync(P.rb_pi, angmom_body, 3 * nm * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaMemsetAsync(P.rb_off, 0, 3 * (size_t)P.N * sizeof(double), s->stream));
+    CK(cudaStreamSynchronize(s->stream));       // the host arrays may be pageable and go out of scope
+    return upload_state(s, xyz.data(), v.data(), true);
+}
+
+int md_get_rigid_state(md_system *s, double *com, double *rot, double *vcom, double *angmom_body)
+{
+    if (!s || !com || !rot || !vcom || !angmom_body) { set_error("md_get_rigid_state: null argument"); return MD_ERR_INVALID; }
+    const MdDev &P = s->P;
+    if (!P.rigid || !s->has_state) { set_error("md_get_rigid_state: no rigid state"); return MD_ERR_INVALID; }
+    const size_t nm = (size_t)P.rb_nm;
+    CK(cudaMemcpyAsync(com, P.rb_R, 3 * nm * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaMemcpyAsync(rot, P.rb_A, 9 * nm * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaMemcpyAsync(vcom, P.rb_V, 3 * nm * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaMemcpyAsync(angmom_body, P.rb_pi, 3 * nm * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return MD_OK;
+}
+
 int md_set_angles(md_system *s, double k_theta, double cos_theta0)
 {
     if (!s || !(k_theta >= 0) || !(cos_theta0 >= -1.0 && cos_theta0 <= 1.0)) { set_error("md_set_angles: bad argument"); return MD_ERR_INVALID; }
@@ -864,6 +1056,18 @@ int md_step(md_system *s, int64_t n)
     s->stepped = true;
     const MdDev &P = s->P;
     cudaStream_t st = s->stream;
+    if (P.rigid) {
+        // rigid molecules: per-molecule half kick + free rotation + drift, rebuild decision, site forces, half kick
+        for (int64_t k = 0; k < n; k++) {
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_rigid_kick_drift(P, st); }
+            { Timed t(s, MD_T_DECIDE, 1); mdk_decide(P, mdk_rigid_blocks(P), false, st, 0ull); }
+            enqueue_rebuild(s);
+            enqueue_forces_only(s);
+            { Timed t(s, MD_T_INTEGRATE, 1); mdk_rigid_kick(P, st); }
+        }
+        s->step += n;
+        return check_device_status(s);
+    }
     if (s->prm.step_mode == MD_STEP_FUSED) {
         // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
         const bool graphs = have_graphs(s);
@@ -930,6 +1134,33 @@ int md_get_positions(md_system *s, double *xyz) { return download(s, 0, xyz); }
 int md_get_velocities(md_system *s, double *xyz) { return download(s, 1, xyz); }
 int md_get_forces(md_system *s, double *xyz) { return download(s, 2, xyz); }
 
+int md_get_positions_device(md_system *s, double *xyz_device) { return export_device(s, 0, xyz_device); }
+int md_get_velocities_device(md_system *s, double *xyz_device) { return export_device(s, 1, xyz_device); }
+int md_get_forces_device(md_system *s, double *xyz_device) { return export_device(s, 2, xyz_device); }
+
+// positions and velocities in one call: two export kernels, one device-to-host transfer when the two host arrays are
+// adjacent (vxyz == xyz + 3N), one synchronisation
+int md_get_state(md_system *s, double *xyz, double *vxyz)
+{
+    if (!s || !xyz || !vxyz) { set_error("md_get_state: null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("no state loaded"); return MD_ERR_INVALID; }
+    const size_t n3 = 3 * (size_t)s->P.N;
+    s->launches += 2;
+    mdk_export(s->P, 0, s->P.scratch, s->stream);
+    mdk_export(s->P, 1, s->P.scratch + n3, s->stream);
+    const bool direct = is_pinned(xyz) && is_pinned(vxyz);
+    if (direct && vxyz == xyz + n3) {
+        CK(cudaMemcpyAsync(xyz, s->P.scratch, 2 * n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    } else {
+        CK(cudaMemcpyAsync(direct ? xyz : s->h_stage, s->P.scratch, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        CK(cudaMemcpyAsync(direct ? vxyz : s->h_stage + n3, s->P.scratch + n3, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    }
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaGetLastError());
+    if (!direct) { memcpy(xyz, s->h_stage, n3 * sizeof(double)); memcpy(vxyz, s->h_stage + n3, n3 * sizeof(double)); }
+    return MD_OK;
+}
+
 int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_neighbors_out)
 {
     if (!s || !counts) { set_error("md_get_neighbors: null argument"); return MD_ERR_INVALID; }
@@ -959,14 +1190,14 @@ int md_get_neighbors(md_system *s, int32_t *counts, int32_t *list, int32_t *max_
         CK(cudaMemcpy(cs.data(), P.cell_start, cs.size() * sizeof(int), cudaMemcpyDeviceToHost));
         const int nblocks = P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys;
         for (int b = 0; b < nblocks; b++) {
-            const TileBox B = tile_box(P.tg, P.nc, b);
+            const TileBox B = tile_box(P.tg, P.nc, P.ncx, b);
             map.clear();
             std::vector<std::pair<int, int>> own;            // (global start, length) of the box's own rows
             for (int q = 0; q < B.nq; q++) {
                 int rowc, ysh, zsh, xa, xc;
-                tile_row(B, P.nc, q, rowc, ysh, zsh, xa, xc);
+                tile_row(B, P.nc, P.ncx, P.kx, q, rowc, ysh, zsh, xa, xc);
                 const int g[3] = {cs[rowc + xa], cs[rowc + B.x0], cs[rowc + xc]};
-                const int n[3] = {cs[rowc + xa + 1] - g[0], cs[rowc + B.x0 + B.sxc] - g[1], cs[rowc + xc + 1] - g[2]};
+                const int n[3] = {cs[rowc + xa + P.kx] - g[0], cs[rowc + B.x0 + B.sxc] - g[1], cs[rowc + xc + P.kx] - g[2]};
                 for (int k = 0; k < 3; k++) for (int u = 0; u < n[k]; u++) map.push_back(g[k] + u);
                 const int qy = q % B.nyq, qz = q / B.nyq;
                 if (qy >= 1 && qy <= B.ny && qz >= 1 && qz <= B.nz) own.push_back({g[1], n[1]});
@@ -1008,12 +1239,17 @@ int md_get_info(md_system *s, md_info *out)
     out->n_bonds_per_atom_max = s->n_bonds_max;
     out->w_layout = s->P.tiled ? MD_W_TILED : MD_W_GLOBAL;
     if (s->P.tile_build) {
-        out->tile_cells[0] = s->P.tg.S; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
+        out->tile_cells[0] = s->P.tg.S / s->P.kx; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }
     out->use_graph = s->gexec[0] ? 1 : 0;
     out->precision = s->prm.precision;
     out->n_layers = s->P.n_layers;
+    out->cells_x = s->P.ncx; out->cell_split_x = s->P.kx; out->sm_count = s->sm_count;
+    // counted by the last neighbor build (as of the last status read); before any: 9 rows of 2 kx + 1 fine cells, an
+    // upper bound (rows far from the atom are scanned over a shorter window or not at all)
+    out->candidates_per_atom = s->h_ctrl && s->h_ctrl->cand_total ? (double)s->h_ctrl->cand_total / (double)s->P.N
+                                                                  : 9.0 * (2.0 * s->P.kx + 1.0) * (double)s->P.N1 / (double)s->P.NC1;
     out->device_bytes = s->bytes;
     out->kernel_launches = s->launches;
     snprintf(out->device_name, sizeof(out->device_name), "%s", s->device_name);

@@ -34,10 +34,23 @@ __device__ __forceinline__ double wrap1(double x, double L)
 // 32-byte record = one L2 sector, moved by ONE 256-bit access (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a):
 // a gather then costs one L1 tag look-up per lane instead of two with a pair of 128-bit loads.
 // Read-only path: never used on a buffer the same kernel writes.
+#ifndef MD_LDPOS
+#define MD_LDPOS 0                   // cache policy of the position gathers (tuning experiments)
+#endif
 __device__ __forceinline__ pos_t ld_pos(const pos_t *p)
 {
     pos_t r;
+#if MD_LDPOS == 1
+    asm("ld.global.cg.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+#elif MD_LDPOS == 2
+    asm("ld.global.nc.L1::evict_last.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+#elif MD_LDPOS == 3
+    asm("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+#elif MD_LDPOS == 4
+    asm("ld.global.nc.L1::evict_last.L2::256B.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+#else
     asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+#endif
     return r;
 }
 
@@ -87,6 +100,35 @@ __device__ __forceinline__ int cell_coord(double x, double inv_w, int nc)
     int q = (int)floor(x * inv_w);
     q = q < 0 ? 0 : q;
     return q >= nc ? nc - 1 : q;
+}
+
+// Row pruning of the neighbor build (MdDev::kx): an atom at fractional height (fy, fz) in its cell is at least
+// gyl = fy w below-row gap, gyh = (1 - fy) w above-row gap ... away from the rows of cells next to its own.  A partner
+// in the row (dy, dz) can then differ by at most s = sqrt(r_n^2 - g^2) along x, i.e. lie at most floor(s / w_x) + 1
+// fine cells away.  All quantities are binary32 rounded to the safe side (gaps shrunk, r_n^2 and 1 / w_x grown by
+// 1e-5, against a binary32 rounding of 6e-8 and a cell margin of >= 1e-9), so the window never loses a partner; the
+// accept test itself stays the exact arithmetic of DESIGN.md R5 / R18.
+struct RowGaps {
+    float yl, yh, zl, zh;
+};
+
+__device__ __forceinline__ RowGaps row_gaps(const MdDev &P, double y, double z, int cy, int cz)
+{
+    const float fy = (float)(y * P.inv_w - (double)cy), fz = (float)(z * P.inv_w - (double)cz);
+    RowGaps G;
+    G.yl = fmaxf(fy, 0.0f) * P.w_f; G.yh = fmaxf(1.0f - fy, 0.0f) * P.w_f;
+    G.zl = fmaxf(fz, 0.0f) * P.w_f; G.zh = fmaxf(1.0f - fz, 0.0f) * P.w_f;
+    return G;
+}
+
+// half-width of the x window (in fine cells) of the row (dy, dz) in {-1, 0, 1}^2; -1: the row is out of reach
+__device__ __forceinline__ int row_halfwidth(const MdDev &P, const RowGaps &G, int dy, int dz)
+{
+    const float gy = dy < 0 ? G.yl : (dy > 0 ? G.yh : 0.0f), gz = dz < 0 ? G.zl : (dz > 0 ? G.zh : 0.0f);
+    const float s2 = P.rn2_prune - (gy * gy + gz * gz);
+    if (!(s2 > 0.0f)) return -1;
+    const int k = (int)(sqrtf(s2) * P.inv_wx_f) + 1;
+    return k < P.kx ? k : P.kx;
 }
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -144,7 +186,7 @@ __device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pi
     if (need) {
         acc = 0.0;
         c->n_rebuilds += 1;
-        c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+        c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull; c->cand_total = 0ull;
         // the paper sorts the atoms only every ~100 steps; the default path at every rebuild
         const int ro = !P.layer_H || P.reorder_interval == 0 || (P.reorder_interval > 0 && since >= P.reorder_interval);
         c->do_reorder = ro;

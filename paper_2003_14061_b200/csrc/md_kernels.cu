@@ -31,7 +31,7 @@ __global__ void k_force_rebuild(const __grid_constant__ MdDev P)
     c->p_src = c->p_dst; c->p_dst ^= 1;
     c->v_src = c->v_dst; c->v_dst ^= 1;
     c->disp_acc = 0.0;
-    c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull;
+    c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull; c->cand_total = 0ull;
     c->do_reorder = !P.layer_H || P.reorder_interval >= 0;      // a forced rebuild sorts unless the system never does
     c->since_reorder = 0;
 }
@@ -65,14 +65,14 @@ __global__ void k_load_state(const __grid_constant__ MdDev P)
     P.id[vc][i] = i;
 }
 
-// device order -> scratch in original-id order.  what: 0 positions (wrapped into [0, L)), 1 velocities, 2 forces
-__global__ void k_export(const __grid_constant__ MdDev P, int what, size_t offset)
+// device order -> dst (device, 3N doubles) in original-id order.  what: 0 positions (wrapped into [0, L)), 1 velocities, 2 forces
+__global__ void k_export(const __grid_constant__ MdDev P, int what, double *dst)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
     const int pc = P.ctrl->p_dst, vc = P.ctrl->v_dst;
     const int id = P.id[vc][i];
-    double *o = P.scratch + offset + 3 * (size_t)id;
+    double *o = dst + 3 * (size_t)id;
     if (what == 0) {
         const pos_t r = ld_pos_rw(P.pos[pc] + i);
         o[0] = wrap1(r.x, P.L); o[1] = wrap1(r.y, P.L); o[2] = wrap1(r.z, P.L);
@@ -147,11 +147,11 @@ __global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
     const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_src)];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
         const pos_t r = ld_pos(pos + i);
-        const int cx = cell_coord(wrap1(r.x, P.L), P.inv_w, P.nc), cy = cell_coord(wrap1(r.y, P.L), P.inv_w, P.nc),
+        const int cx = cell_coord(wrap1(r.x, P.L), P.inv_wx, P.ncx), cy = cell_coord(wrap1(r.y, P.L), P.inv_w, P.nc),
                   cz = cell_coord(wrap1(r.z, P.L), P.inv_w, P.nc);
         // batched independent systems: each has its own block of cells, found from the permanent id
         const int sys = P.n_sys > 1 ? __ldg(idv + i) / P.N1 : 0;
-        const int c = sys * P.NC1 + cx + P.nc * (cy + P.nc * cz);
+        const int c = sys * P.NC1 + cx + P.ncx * (cy + P.nc * cz);
         P.cell_of[i] = c;
         P.slot[i] = atomicAdd(&P.cell_count[c], 1);  // l_i; "incrementing k_c requires an atomic operation" (N2)
     }
@@ -297,7 +297,7 @@ __global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P
         double *vo = P.vel[vd] + n;
         vo[0] = vx; vo[P.N_pad] = vy; vo[2 * (size_t)P.N_pad] = vz;
         P.id[vd][n] = id;
-        if (P.has_bonds) P.inv[id] = n;
+        if (P.need_inv) P.inv[id] = n;
     }
 }
 
@@ -316,22 +316,24 @@ __global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdD
 }
 
 // ------------------------------------------------------------------------------------------------
-// N5: neighbor matrix.  With the atoms in cell order (x fastest) the 27-cell stencil of an atom is 9
-// contiguous runs of the atom array (one per (dy,dz), 3 cells long), plus single wrapped cells at the
-// periodic x faces.  One thread per atom walks its candidates as ONE flat loop over those runs: the threads
-// of a warp re-converge once per candidate, not at the end of every run, so lanes with short runs do not
-// idle; the next candidate's position is fetched while the current one is tested.
+// N5: neighbor matrix.  With the atoms in cell order (x fastest) the stencil of an atom is 9 contiguous runs of the
+// atom array, one per row of cells (dy, dz): the atoms of the 2 k + 1 fine cells around the atom's own (k <= kx, fewer
+// where the row is too far for the full width: row_halfwidth), plus a wrapped piece at the periodic x faces.
+// One thread per atom walks its candidates run by run; the next candidate's position is fetched while the current
+// one is tested.
 // The periodic image is a per-run shift (0, +L or -L per axis) added to the raw difference.  For every pair
 // closer than r_n this is exactly the minimum-image arithmetic of DESIGN.md R5 (d0 = a - b rounded, then
 // d0 -+ L rounded): with cells wider than r_n and >= 3 cells per edge the image reached through the
 // stencil is the minimum image, and a pair for which it is not is farther than r_n in either form.
 // ------------------------------------------------------------------------------------------------
 // candidates j in [b, e) of one run, image shift (sx, sy, sz) and flag bits fl for the whole run
-template <bool HALF, bool SHIFT>
+// EXCL: rigid molecules -- sites of the atom's own molecule (mol = original id / sites per molecule) are no neighbors
+template <bool HALF, bool SHIFT, bool EXCL>
 __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, int b, int e,
-                                         double sx, double sy, double sz, unsigned fl, int &m)
+                                         double sx, double sy, double sz, unsigned fl, int &m, const int *__restrict__ idv, int mol)
 {
     for (int j = b; j < e; j++) {
+        if (EXCL && __ldg(idv + j) / P.rb_ns == mol) continue;
         const pos_t rj = ld_pos(pos + j);
         // d = (r_i - r_j) + shift, each operation rounded once
         double dx = __dsub_rn(ri.x, rj.x), dy = __dsub_rn(ri.y, rj.y), dz = __dsub_rn(ri.z, rj.z);
@@ -344,23 +346,24 @@ __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict
     }
 }
 
-template <bool HALF>
+template <bool HALF, bool EXCL>
 __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    __shared__ int smx[4];
+    __shared__ int smx[4], scand[4];
     __shared__ int ssum[4];
     const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
     const int *__restrict__ cs = P.cell_start;
     const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
-    const int nc = P.nc;
+    const int nc = P.nc, ncx = P.ncx;
     const double L = P.L;
-    int tmax = 0, tsum = 0;
+    int tmax = 0, tsum = 0, tcand = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
         const pos_t ri = ld_pos(pos + i);
-        const int cx = cell_coord(ri.x, P.inv_w, nc), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
-        const int xa = cx == 0 ? 0 : cx - 1, xb = cx == nc - 1 ? nc - 1 : cx + 1;
+        const int cx = cell_coord(ri.x, P.inv_wx, ncx), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
+        const RowGaps gaps = row_gaps(P, ri.y, ri.z, cy, cz);
         const int cell_base = P.n_sys > 1 ? (__ldg(idv + i) / P.N1) * P.NC1 : 0;     // the atom's own system of cells
+        const int mol = EXCL ? __ldg(idv + i) / P.rb_ns : 0;
         int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
             int z = cz + dz;
@@ -368,16 +371,21 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
             unsigned fz = 0u;
             if (z < 0) { z += nc; sz = L; fz = 4u; } else if (z >= nc) { z -= nc; sz = -L; fz = 4u; }
             for (int dy = -1; dy <= 1; dy++) {
+                const int kr = row_halfwidth(P, gaps, dy, dz);
+                if (kr < 0) continue;
                 int y = cy + dy;
                 double sy = 0.0;
                 unsigned fl = fz;
                 if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
-                const int row = cell_base + nc * (y + nc * z);
-                const int b = __ldg(cs + row + xa), e = __ldg(cs + row + xb + 1);
-                if (fl) scan_run<HALF, true>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m);
-                else scan_run<HALF, false>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m);
-                if (cx == 0) scan_run<HALF, true>(P, pos, ri, i, __ldg(cs + row + nc - 1), __ldg(cs + row + nc), L, sy, sz, fl | 1u, m);
-                if (cx == nc - 1) scan_run<HALF, true>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + 1), -L, sy, sz, fl | 1u, m);
+                const int row = cell_base + ncx * (y + nc * z);
+                const int lo = cx - kr, hi = cx + kr;
+                const int b = __ldg(cs + row + (lo < 0 ? 0 : lo)), e = __ldg(cs + row + (hi >= ncx ? ncx : hi + 1));
+                tcand += e - b;
+                if (fl) scan_run<HALF, true, EXCL>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m, idv, mol);
+                else scan_run<HALF, false, EXCL>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m, idv, mol);
+                // the part of the window beyond a periodic x face: the cells at the other end of the row, shifted by +-L
+                if (lo < 0) scan_run<HALF, true, EXCL>(P, pos, ri, i, __ldg(cs + row + ncx + lo), __ldg(cs + row + ncx), L, sy, sz, fl | 1u, m, idv, mol);
+                if (hi >= ncx) scan_run<HALF, true, EXCL>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m, idv, mol);
             }
         }
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
@@ -387,14 +395,15 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
     }
     // statistics of the matrix (md_energy.max_neighbors / mean_neighbors)
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
-    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum), wc = warp_sum_i(tcand);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; scand[wid] = wc; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int mx = 0, sm = 0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        int mx = 0, sm = 0, sc = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; sc += scand[w]; }
         atomicMax(&P.ctrl->max_nnb, mx);
         atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+        atomicAdd(&P.ctrl->cand_total, (unsigned long long)sc);
     }
 }
 
@@ -421,7 +430,7 @@ __global__ void __launch_bounds__(256) k_copy_wrap(const __grid_constant__ MdDev
         vo[0] = vi[0]; vo[np] = vi[np]; vo[2 * np] = vi[2 * np];
         const int id = P.id[vs][i];
         P.id[vd][i] = id;
-        if (P.has_bonds) P.inv[id] = i;
+        if (P.need_inv) P.inv[id] = i;
     }
 }
 
@@ -888,8 +897,8 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
-// grid of the rebuild kernels: at most one full wave (148 SMs); they use grid-stride loops
-inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdiv(n, block), 148 * per_sm); }
+// grid of the rebuild kernels: at most one full wave of the device's SMs; they use grid-stride loops
+inline int capped_grid(const MdDev &P, long long n, int block, int per_sm) { return std::min(cdiv(n, block), P.sm_count * per_sm); }
 
 }  // namespace
 
@@ -900,7 +909,7 @@ void mdk_force_rebuild(const MdDev &P, cudaStream_t st) { k_force_rebuild<<<1, 1
 
 void mdk_check_range(const MdDev &P, double box, cudaStream_t st)
 {
-    k_check_range<<<std::min(cdiv(3LL * P.N, 256), 148 * 8), 256, 0, st>>>(P, box);
+    k_check_range<<<capped_grid(P, 3LL * P.N, 256, 8), 256, 0, st>>>(P, box);
 }
 
 void mdk_load_state(const MdDev &P, cudaStream_t st)
@@ -909,10 +918,10 @@ void mdk_load_state(const MdDev &P, cudaStream_t st)
     k_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P);
 }
 
-void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st)
+void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st)
 {
-    if (P.sp) return mdk_sp_export(P, what, offset, st);
-    k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset);
+    if (P.sp) return mdk_sp_export(P, what, dst, st);
+    k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, dst);
 }
 
 void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond)
@@ -935,31 +944,33 @@ void mdk_kick(const MdDev &P, const MdLaunch &, cudaStream_t st)
 void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     if (P.sp) mdk_sp_bin(P, st);
-    else k_bin<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    else k_bin<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
     k_scan_reduce<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
     k_scan_top<<<1, 1024, 0, st>>>(P);
     k_scan_apply<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
-    k_place<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    k_place<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
 }
 
 void mdk_reorder(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     if (P.sp) mdk_sp_reorder(P, st);
-    else k_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
-    if (P.layer_H) k_copy_wrap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
-    if (P.has_bonds) k_bonds_remap<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
+    else k_reorder<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.layer_H) k_copy_wrap<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.has_bonds) k_bonds_remap<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
+    if (P.rigid) mdk_rigid_offsets(P, st);
 }
 
 void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
 {
     if (P.sp) return mdk_sp_build(P, st);
     if (P.layer_H) {
-        k_layer_fill<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P);
-        k_build_layers<<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
+        k_layer_fill<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
+        k_build_layers<<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P);
         return;
     }
-    if (P.half_list) k_build<true><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
-    else k_build<false><<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P);
+    if (P.rigid) k_build<false, true><<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P);
+    else if (P.half_list) k_build<true, false><<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P);
+    else k_build<false, false><<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P);
 }
 
 template <int MODE, int BONDS>

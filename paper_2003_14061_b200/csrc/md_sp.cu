@@ -62,13 +62,13 @@ __global__ void k_sp_load_state(const __grid_constant__ MdDev P)
     P.id[vc][i] = i;
 }
 
-__global__ void k_sp_export(const __grid_constant__ MdDev P, int what, size_t offset)
+__global__ void k_sp_export(const __grid_constant__ MdDev P, int what, double *dst)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
     const int pc = P.ctrl->p_dst, vc = P.ctrl->v_dst;
     const int id = P.id[vc][i];
-    double *o = P.scratch + offset + 3 * (size_t)id;
+    double *o = dst + 3 * (size_t)id;
     if (what == 0) {
         const float4 r = P.posf[pc][i];
         o[0] = (double)wrap1f(r.x, P.Lf); o[1] = (double)wrap1f(r.y, P.Lf); o[2] = (double)wrap1f(r.z, P.Lf);
@@ -123,10 +123,10 @@ __global__ void __launch_bounds__(256) k_sp_bin(const __grid_constant__ MdDev P)
     const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_src)];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
         const float4 r = ld4(pos + i);
-        const int cx = cell_coord((double)wrap1f(r.x, P.Lf), P.inv_w, P.nc), cy = cell_coord((double)wrap1f(r.y, P.Lf), P.inv_w, P.nc),
+        const int cx = cell_coord((double)wrap1f(r.x, P.Lf), P.inv_wx, P.ncx), cy = cell_coord((double)wrap1f(r.y, P.Lf), P.inv_w, P.nc),
                   cz = cell_coord((double)wrap1f(r.z, P.Lf), P.inv_w, P.nc);
         const int sys = P.n_sys > 1 ? __ldg(idv + i) / P.N1 : 0;
-        const int c = sys * P.NC1 + cx + P.nc * (cy + P.nc * cz);
+        const int c = sys * P.NC1 + cx + P.ncx * (cy + P.nc * cz);
         P.cell_of[i] = c;
         P.slot[i] = atomicAdd(&P.cell_count[c], 1);
     }
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(256) k_sp_reorder(const __grid_constant__ MdDe
         P.posf[pd][n] = make_float4(wrap1f(r.x, P.Lf), wrap1f(r.y, P.Lf), wrap1f(r.z, P.Lf), 0.0f);
         P.velf[vd][n] = v;
         P.id[vd][n] = id;
-        if (P.has_bonds) P.inv[id] = n;
+        if (P.need_inv) P.inv[id] = n;
     }
 }
 
@@ -182,18 +182,18 @@ __device__ __forceinline__ void scan_run_f(const MdDev &P, const float4 *__restr
 __global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    __shared__ int smx[4];
+    __shared__ int smx[4], scand[4];
     __shared__ int ssum[4];
     const float4 *__restrict__ pos = P.posf[__ldcg(&P.ctrl->p_dst)];
     const int *__restrict__ cs = P.cell_start;
     const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
-    const int nc = P.nc;
+    const int nc = P.nc, ncx = P.ncx;
     const float L = P.Lf;
-    int tmax = 0, tsum = 0;
+    int tmax = 0, tsum = 0, tcand = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
         const float4 ri = ld4(pos + i);
-        const int cx = cell_coord((double)ri.x, P.inv_w, nc), cy = cell_coord((double)ri.y, P.inv_w, nc), cz = cell_coord((double)ri.z, P.inv_w, nc);
-        const int xa = cx == 0 ? 0 : cx - 1, xb = cx == nc - 1 ? nc - 1 : cx + 1;
+        const int cx = cell_coord((double)ri.x, P.inv_wx, ncx), cy = cell_coord((double)ri.y, P.inv_w, nc), cz = cell_coord((double)ri.z, P.inv_w, nc);
+        const RowGaps gaps = row_gaps(P, (double)ri.y, (double)ri.z, cy, cz);
         const int cell_base = P.n_sys > 1 ? (__ldg(idv + i) / P.N1) * P.NC1 : 0;
         int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
@@ -202,16 +202,20 @@ __global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev 
             unsigned fz = 0u;
             if (z < 0) { z += nc; sz = L; fz = 4u; } else if (z >= nc) { z -= nc; sz = -L; fz = 4u; }
             for (int dy = -1; dy <= 1; dy++) {
+                const int kr = row_halfwidth(P, gaps, dy, dz);
+                if (kr < 0) continue;
                 int y = cy + dy;
                 float sy = 0.0f;
                 unsigned fl = fz;
                 if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
-                const int row = cell_base + nc * (y + nc * z);
-                const int b = __ldg(cs + row + xa), e = __ldg(cs + row + xb + 1);
+                const int row = cell_base + ncx * (y + nc * z);
+                const int lo = cx - kr, hi = cx + kr;
+                const int b = __ldg(cs + row + (lo < 0 ? 0 : lo)), e = __ldg(cs + row + (hi >= ncx ? ncx : hi + 1));
+                tcand += e - b;
                 if (fl) scan_run_f<true>(P, pos, ri, i, b, e, 0.0f, sy, sz, fl, m);
                 else scan_run_f<false>(P, pos, ri, i, b, e, 0.0f, 0.0f, 0.0f, 0u, m);
-                if (cx == 0) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row + nc - 1), __ldg(cs + row + nc), L, sy, sz, fl | 1u, m);
-                if (cx == nc - 1) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + 1), -L, sy, sz, fl | 1u, m);
+                if (lo < 0) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row + ncx + lo), __ldg(cs + row + ncx), L, sy, sz, fl | 1u, m);
+                if (hi >= ncx) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m);
             }
         }
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
@@ -226,14 +230,15 @@ __global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev 
         tsum += m;
     }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
-    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum), wc = warp_sum_i(tcand);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; scand[wid] = wc; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int mx = 0, sm = 0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        int mx = 0, sm = 0, sc = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { mx = max(mx, smx[w]); sm += ssum[w]; sc += scand[w]; }
         atomicMax(&P.ctrl->max_nnb, mx);
         atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+        atomicAdd(&P.ctrl->cand_total, (unsigned long long)sc);
     }
 }
 
@@ -577,7 +582,7 @@ __global__ void __launch_bounds__(256) k_sp_energy(const __grid_constant__ MdDev
 }
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
-inline int capped_grid(long long n, int block, int per_sm) { return std::min(cdiv(n, block), 148 * per_sm); }
+inline int capped_grid(const MdDev &P, long long n, int block, int per_sm) { return std::min(cdiv(n, block), P.sm_count * per_sm); }
 
 template <int MODE, int BONDS, bool PADDED>
 void launch_sp_force_p(const MdDev &P, int block, cudaStream_t st)
@@ -600,12 +605,12 @@ void launch_sp_force(const MdDev &P, int block, cudaStream_t st)
 }  // namespace
 
 void mdk_sp_load_state(const MdDev &P, cudaStream_t st) { k_sp_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
-void mdk_sp_export(const MdDev &P, int what, size_t offset, cudaStream_t st) { k_sp_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, offset); }
+void mdk_sp_export(const MdDev &P, int what, double *dst, cudaStream_t st) { k_sp_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, dst); }
 void mdk_sp_kick_drift(const MdDev &P, cudaStream_t st) { k_sp_kick_drift<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
 void mdk_sp_kick(const MdDev &P, cudaStream_t st) { k_sp_kick<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
-void mdk_sp_bin(const MdDev &P, cudaStream_t st) { k_sp_bin<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P); }
-void mdk_sp_reorder(const MdDev &P, cudaStream_t st) { k_sp_reorder<<<capped_grid(P.N, 256, 8), 256, 0, st>>>(P); }
-void mdk_sp_build(const MdDev &P, cudaStream_t st) { k_sp_build<<<capped_grid(P.N, 128, 16), 128, 0, st>>>(P); }
+void mdk_sp_bin(const MdDev &P, cudaStream_t st) { k_sp_bin<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P); }
+void mdk_sp_reorder(const MdDev &P, cudaStream_t st) { k_sp_reorder<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P); }
+void mdk_sp_build(const MdDev &P, cudaStream_t st) { k_sp_build<<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P); }
 
 void mdk_sp_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
 {

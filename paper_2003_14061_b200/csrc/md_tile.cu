@@ -23,6 +23,14 @@
 
 #include "md_device.cuh"
 
+// Experiment: stage the BUILD kernel's fp64 tile with TMA bulk copies (cp.async.bulk, one per contiguous
+// piece of a tile row, completion on an mbarrier) instead of LDG.256 + 3 STS through registers.  The tile then holds the
+// 32-byte position records as they are in global memory (stride 4 doubles instead of the packed 3).
+#ifndef MD_TILE_TMA
+#define MD_TILE_TMA 0
+#endif
+constexpr int TSTR64 = MD_TILE_TMA ? 4 : 3;      // doubles per atom in the build kernel's fp64 tile
+
 #ifndef MD_TILE_FORCE_THREADS
 #define MD_TILE_FORCE_THREADS 1024     // resident threads per SM the register allocation of k_tile_force must allow
 #endif
@@ -34,26 +42,29 @@ __device__ __forceinline__ int tile_bid(const TileGeom &G) { return blockIdx.x +
 // what only the build kernel needs per tile row: the row's x = 0 cell and its image shift in units of L
 struct TileRowGeom {
     int row_cell[TILE_Q_MAX], ysh[TILE_Q_MAX], zsh[TILE_Q_MAX];
+    int xa, xc;         // first cell of the halo before / after the box (the same in every row)
 };
 
 // Build kernel, step 1: the descriptor of box blockIdx.x from cell_start.  All threads of the block call it.
 __device__ __forceinline__ void tile_describe(const MdDev &P, const TileBox &B, TileDesc &M, TileRowGeom &X)
 {
-    const int nc = P.nc;
+    const int nc = P.nc, ncx = P.ncx, K = P.kx;
     const int *__restrict__ cs = P.cell_start;
     const int tid = threadIdx.x;
     if (tid < B.nq) {
         const int q = tid;
         int rowc, ysh, zsh, xa, xc;
-        tile_row(B, nc, q, rowc, ysh, zsh, xa, xc);
-        const int gA = __ldg(cs + rowc + xa), nA = __ldg(cs + rowc + xa + 1) - gA;
+        tile_row(B, nc, ncx, K, q, rowc, ysh, zsh, xa, xc);
+        // the three contiguous pieces of the row: K halo cells, the box's own cells, K halo cells
+        const int gA = __ldg(cs + rowc + xa), nA = __ldg(cs + rowc + xa + K) - gA;
         const int gB = __ldg(cs + rowc + B.x0), nB = __ldg(cs + rowc + B.x0 + B.sxc) - gB;
-        const int gC = __ldg(cs + rowc + xc), nC = __ldg(cs + rowc + xc + 1) - gC;
+        const int gC = __ldg(cs + rowc + xc), nC = __ldg(cs + rowc + xc + K) - gC;
         M.row[q].g[0] = gA; M.row[q].g[1] = gB; M.row[q].g[2] = gC;
         M.row[q].n[0] = nA; M.row[q].n[1] = nB; M.row[q].n[2] = nC;
         X.row_cell[q] = rowc; X.ysh[q] = ysh; X.zsh[q] = zsh;
-        // piece 0 is the far-face cell when the box starts at x = 0: d = (r_i - r_j) + L; piece 2 likewise with -L
-        const int xshA = B.x0 == 0 ? 1 : 0, xshC = B.x0 + B.sxc == nc ? -1 : 0;
+        if (q == 0) { X.xa = xa; X.xc = xc; }
+        // piece 0 holds the far-face cells when the box starts at x = 0: d = (r_i - r_j) + L; piece 2 likewise with -L
+        const int xshA = B.x0 == 0 ? 1 : 0, xshC = B.x0 + B.sxc == ncx ? -1 : 0;
         M.row[q].sh = (ysh + 1) | ((zsh + 1) << 2) | ((xshA + 1) << 4) | ((xshC + 1) << 6);
     }
     __syncthreads();
@@ -220,9 +231,9 @@ template <bool SHIFT, bool LOCALW>
 __device__ __forceinline__ void tile_scan_run(const double *st, double xi, double yi, double zi, int li, int b, int e, double shx,
                                               double shy, double shz, unsigned add, double rn2, Emit<LOCALW> &em)
 {
-    const double *p = st + 3 * b;
+    const double *p = st + TSTR64 * b;
 #pragma unroll 2
-    for (int j = b; j < e; j++, p += 3) {
+    for (int j = b; j < e; j++, p += TSTR64) {
         double dx = __dsub_rn(xi, p[0]), dy = __dsub_rn(yi, p[1]), dz = __dsub_rn(zi, p[2]);
         if (SHIFT) { dx = __dadd_rn(dx, shx); dy = __dadd_rn(dy, shy); dz = __dadd_rn(dz, shz); }
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
@@ -230,112 +241,7 @@ __device__ __forceinline__ void tile_scan_run(const double *st, double xi, doubl
     }
 }
 
-// The block size is a run-time value (any multiple of 32 up to 512): it is picked so that the own atoms of a box
-// fill the block's warps.
-template <bool LOCALW>
-__global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDev P)
-{
-    const int BLOCK = blockDim.x;
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    extern __shared__ double dsm[];
-    __shared__ TileDesc M;
-    __shared__ TileRowGeom X;
-    __shared__ int smx[32], ssum[32];
-    const int cap = P.tg.cap;
-    double *st = dsm;
-    int *tcs = (int *)(st + 3 * cap);
-    const int stride = P.tg.S + 3;
-    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
-    const int *__restrict__ cs = P.cell_start;
-    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
-    const int bid = tile_bid(P.tg);
-    tile_describe(P, B, M, X);
-    if (LOCALW) {   // publish the descriptor for the force / energy kernels
-        int *d = P.tile_desc + (size_t)bid * TILE_DESC_INTS;
-        const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
-        for (int k = threadIdx.x; k < n; k += BLOCK) d[k] = ((const int *)&M)[k];
-    }
-    if (M.T > cap) {
-        if (threadIdx.x == 0) set_err(P, MD_ERR_TILE_OVERFLOW);
-        return;
-    }
-    tile_stage<false>(M, pos, st, P.L);
-    // tile index of the first atom of every tile cell: tcs[q * stride + k], k = 0 .. sxc + 2
-    for (int e = threadIdx.x; e < B.nq * stride; e += BLOCK) {
-        const int q = e / stride, k = e - q * stride;
-        if (k > B.sxc + 2) continue;
-        const TileDesc::Row &R = M.row[q];
-        int v;
-        if (k == 0) v = R.off;
-        else if (k == B.sxc + 2) v = R.off + R.n[0] + R.n[1] + R.n[2];
-        else v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - 1) - R.g[1]);
-        tcs[e] = v;
-    }
-    __syncthreads();
-    const int nc = P.nc;
-    const double L = P.L, rn2 = P.rn2;
-    int tmax = 0, tsum = 0;
-    for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
-        int i, li;
-        own_atom(M, t, i, li);
-        const double xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
-        const int cx = cell_coord(xi, P.inv_w, nc), cy = cell_coord(yi, P.inv_w, nc), cz = cell_coord(zi, P.inv_w, nc);
-        Emit<LOCALW> em = {(char *)((unsigned *)P.W + (size_t)i * P.w_col), 4ll * P.w_row, 0, P.Mmax};
-        const int k0 = cx - B.x0;
-        const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
-#pragma unroll 1
-        for (int r = 0; r < 9; r++) {
-            const int q = q0 + (r % 3) + B.nyq * (r / 3);
-            const int ysh = X.ysh[q], zsh = X.zsh[q];
-            const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
-            const double shy = ysh * L, shz = zsh * L;
-            const TileDesc::Row &R = M.row[q];
-            const int *tc = tcs + q * stride + k0;
-            const int b = tc[0], e = tc[3];
-            // split off the cell that is a periodic image along x (box at an x face, atom in the face cell)
-            int mid = cx == 0 ? tc[1] : (cx == nc - 1 ? tc[2] : e);
-            // global index = tile index + delta, constant over each contiguous piece of the row
-            const int e0 = R.off + R.n[0], e1 = e0 + R.n[1];
-            const int d0 = R.g[0] - R.off, d1 = R.g[1] - e0, d2 = R.g[2] - e1;
-            const int da = b < e0 ? d0 : (b < e1 ? d1 : d2), db = mid < e0 ? d0 : (mid < e1 ? d1 : d2);
-            const double shxa = cx == 0 ? L : 0.0, shxb = cx == nc - 1 ? -L : 0.0;
-            const unsigned fla = fl | (cx == 0 ? 1u : 0u), flb = fl | (cx == nc - 1 ? 1u : 0u);
-            // what is added to the tile index to make the W entry: the flag bits, and for global W the index offset
-            const unsigned adda = LOCALW ? fla << T_FLAG_SHIFT : (fla << W_FLAG_SHIFT) + (unsigned)da;
-            const unsigned addb = LOCALW ? flb << T_FLAG_SHIFT : (flb << W_FLAG_SHIFT) + (unsigned)db;
-            if (fla) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
-            else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, mid, 0.0, 0.0, 0.0, adda, rn2, em);
-            if (mid < e) {
-                if (flb) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
-                else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, mid, e, 0.0, 0.0, 0.0, addb, rn2, em);
-            }
-        }
-        em.flush();
-        const int m = em.m;
-        P.nnb[i] = m < P.Mmax ? m : P.Mmax;
-        if (m > P.Mmax) set_err(P, MD_ERR_NEBR_OVERFLOW);
-        tmax = max(tmax, m);
-        tsum += m;
-    }
-    // statistics of the matrix (md_energy.max_neighbors / mean_neighbors)
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
-    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int mx = 0, sm = 0;
-        for (int w = 0; w < BLOCK / 32; w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
-        atomicMax(&P.ctrl->max_nnb, mx);
-        atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// N5 on the tile for the single-precision variant (md_sp.cu; R18): the same box decomposition, descriptor
-// and candidate order as k_tile_build<false>, the tile held as packed binary32 triples, the accept test in the binary32
-// arithmetic of R18 (d = fl(a - b), + shift rounded once, r2 = fmaf(dz,dz, fmaf(dy,dy, fl(dx dx))) < (float)(r_n^2)).
-// W holds global indices; long columns are padded with self entries (P.sp_pad) as k_sp_build does.
-// ------------------------------------------------------------------------------------------------
+// binary32 tile of the single-precision variant (md_sp.cu; R18): packed triples, raw positions
 __device__ __forceinline__ void tile_stage_f(const TileDesc &M, const float4 *__restrict__ pos, float *st)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -384,9 +290,9 @@ __device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigne
     return d;
 }
 
-template <bool SHIFT>
-__device__ __forceinline__ void tile_scan_run_f(const float *st, float xi, float yi, float zi, int li, int b, int e, float shx, float shy,
-                                                float shz, unsigned add, float rn2, Emit<false> &em)
+template <bool SHIFT, bool LOCALW>
+__device__ __forceinline__ void tile_scan_run(const float *st, float xi, float yi, float zi, int li, int b, int e, float shx, float shy,
+                                              float shz, unsigned add, float rn2, Emit<LOCALW> &em)
 {
     const unsigned long long m1 = pack2(-1.0f, -1.0f), x2 = pack2(xi, xi), y2 = pack2(yi, yi), z2 = pack2(zi, zi);
     const unsigned long long sx2 = pack2(shx, shx), sy2 = pack2(shy, shy), sz2 = pack2(shz, shz);
@@ -410,74 +316,153 @@ __device__ __forceinline__ void tile_scan_run_f(const float *st, float xi, float
     }
 }
 
-__global__ void __launch_bounds__(512) k_sp_tile_build(const __grid_constant__ MdDev P)
+// What differs between the two precisions of the tile build: the coordinate type, where the positions come from, how
+// the tile is staged, and the constants of the accept test.  Everything else -- the box decomposition, the descriptor,
+// the candidate windows, the append -- is ONE kernel (k_tile_build below).
+#if MD_TILE_TMA
+// TMA staging of the raw 32-byte records: warp 0 issues one bulk copy per non-empty piece of every tile row; all threads
+// then wait on the mbarrier's phase 0.  (sm_90+ PTX; SASS UBLKCP.)
+__device__ __forceinline__ void tile_stage_tma(const TileDesc &M, const pos_t *__restrict__ pos, double *st)
 {
+    __shared__ __align__(8) unsigned long long mbar;
+    const unsigned mb = (unsigned)__cvta_generic_to_shared(&mbar);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        if (lane == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"((unsigned)M.T * 32u) : "memory");
+        __syncwarp();
+        for (int e = lane; e < 3 * M.nq; e += 32) {
+            const int q = e / 3, k = e - 3 * q;
+            const TileDesc::Row &R = M.row[q];
+            const int n = R.n[k];
+            if (n == 0) continue;
+            const int toff = R.off + (k > 0 ? R.n[0] : 0) + (k > 1 ? R.n[1] : 0);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(st + 4 * toff);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                         "l"(pos + R.g[k]), "r"((unsigned)n * 32u), "r"(mb)
+                         : "memory");
+        }
+    }
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_TMA:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n\t@!p bra WAIT_TMA;\n\t}" ::"r"(mb) : "memory");
+}
+#endif
+
+struct PrecF64 {
+    using real = double;
+    static constexpr int STR = TSTR64;
+    static __device__ __forceinline__ void stage(const MdDev &P, const TileDesc &M, int pc, real *st)
+    {
+#if MD_TILE_TMA
+        tile_stage_tma(M, P.pos[pc], st);
+#else
+        tile_stage<false>(M, P.pos[pc], st, P.L);
+#endif
+    }
+    static __device__ __forceinline__ real box(const MdDev &P) { return P.L; }
+    static __device__ __forceinline__ real rn2(const MdDev &P) { return P.rn2; }
+};
+struct PrecF32 {
+    using real = float;
+    static constexpr int STR = 3;
+    static __device__ __forceinline__ void stage(const MdDev &P, const TileDesc &M, int pc, real *st) { tile_stage_f(M, P.posf[pc], st); }
+    static __device__ __forceinline__ real box(const MdDev &P) { return P.Lf; }
+    static __device__ __forceinline__ real rn2(const MdDev &P) { return P.rn2f; }
+};
+
+// The block size is a run-time value (any multiple of 32 up to 512): it is picked so that the own atoms of a box
+// fill the block's warps.
+template <typename PR, bool LOCALW>
+__global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDev P)
+{
+    using real = typename PR::real;
     const int BLOCK = blockDim.x;
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     extern __shared__ double dsm[];
     __shared__ TileDesc M;
     __shared__ TileRowGeom X;
-    __shared__ int smx[32], ssum[32];
-    const int cap = P.tg.cap;
-    float *st = (float *)dsm;
-    int *tcs = (int *)(st + 3 * cap);
-    const int stride = P.tg.S + 3;
-    const float4 *__restrict__ pos = P.posf[__ldcg(&P.ctrl->p_dst)];
+    __shared__ int smx[32], ssum[32], scand[32];
+    const int cap = P.tg.cap, K = P.kx;
+    const int stride = P.tg.S + 2 * K + 1;
+    real *st = (real *)dsm;
+    int *tcs = (int *)(st + PR::STR * cap);           // tile index of the first atom of every tile cell
     const int *__restrict__ cs = P.cell_start;
-    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const TileBox B = tile_box3(P.tg, P.nc, P.ncx, blockIdx.x, blockIdx.y, blockIdx.z);
+    const int bid = tile_bid(P.tg);
     tile_describe(P, B, M, X);
+    if (LOCALW) {   // publish the descriptor for the force / energy kernels
+        int *d = P.tile_desc + (size_t)bid * TILE_DESC_INTS;
+        const int n = TILE_DESC_HEAD + TILE_ROW_INTS * B.nq;
+        for (int k = threadIdx.x; k < n; k += BLOCK) d[k] = ((const int *)&M)[k];
+    }
     if (M.T > cap) {
         if (threadIdx.x == 0) set_err(P, MD_ERR_TILE_OVERFLOW);
         return;
     }
-    tile_stage_f(M, pos, st);
+    PR::stage(P, M, __ldcg(&P.ctrl->p_dst), st);
+    // tcs[q * stride + k], k = 0 .. sxc + 2 K  (K halo cells, the box's sxc cells, K halo cells; the last entry closes the row)
     for (int e = threadIdx.x; e < B.nq * stride; e += BLOCK) {
         const int q = e / stride, k = e - q * stride;
-        if (k > B.sxc + 2) continue;
+        if (k > B.sxc + 2 * K) continue;
         const TileDesc::Row &R = M.row[q];
         int v;
-        if (k == 0) v = R.off;
-        else if (k == B.sxc + 2) v = R.off + R.n[0] + R.n[1] + R.n[2];
-        else v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - 1) - R.g[1]);
+        if (k < K) v = R.off + (__ldg(cs + X.row_cell[q] + X.xa + k) - R.g[0]);
+        else if (k < K + B.sxc) v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - K) - R.g[1]);
+        else v = R.off + R.n[0] + R.n[1] + (__ldg(cs + X.row_cell[q] + X.xc + k - K - B.sxc) - R.g[2]);
         tcs[e] = v;
     }
     __syncthreads();
-    const int nc = P.nc;
-    const float L = P.Lf, rn2 = P.rn2f;
-    int tmax = 0, tsum = 0;
+    const int nc = P.nc, ncx = P.ncx;
+    const real L = PR::box(P), rn2 = PR::rn2(P);
+    const bool low_face = B.x0 == 0, high_face = B.x0 + B.sxc == ncx;
+    int tmax = 0, tsum = 0, tcand = 0;
     for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
         int i, li;
         own_atom(M, t, i, li);
-        const float xi = st[3 * li], yi = st[3 * li + 1], zi = st[3 * li + 2];
-        const int cx = cell_coord((double)xi, P.inv_w, nc), cy = cell_coord((double)yi, P.inv_w, nc), cz = cell_coord((double)zi, P.inv_w, nc);
-        Emit<false> em = {(char *)((unsigned *)P.W + (size_t)i * P.w_col), 4ll * P.w_row, 0, P.Mmax};
-        const int k0 = cx - B.x0;
-        const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);
+        const real xi = st[PR::STR * li], yi = st[PR::STR * li + 1], zi = st[PR::STR * li + 2];
+        const int cx = cell_coord((double)xi, P.inv_wx, ncx), cy = cell_coord((double)yi, P.inv_w, nc), cz = cell_coord((double)zi, P.inv_w, nc);
+        Emit<LOCALW> em = {(char *)((unsigned *)P.W + (size_t)i * P.w_col), 4ll * P.w_row, 0, P.Mmax};
+        const int kc = cx - B.x0;                                  // the window of K cells either side starts at tile cell kc
+        const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
+        // (Shortening the window of rows that are far from the atom -- row_halfwidth, as the gathering build does -- was
+        // measured slower here, in round 1 and again in round 2: the lanes of a warp then walk runs of more unequal lengths.)
 #pragma unroll 1
         for (int r = 0; r < 9; r++) {
             const int q = q0 + (r % 3) + B.nyq * (r / 3);
             const int ysh = X.ysh[q], zsh = X.zsh[q];
             const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
-            const float shy = ysh * L, shz = zsh * L;
+            const real shy = ysh * L, shz = zsh * L;
             const TileDesc::Row &R = M.row[q];
-            const int *tc = tcs + q * stride + k0;
-            const int b = tc[0], e = tc[3];
-            int mid = cx == 0 ? tc[1] : (cx == nc - 1 ? tc[2] : e);
+            const int *tc = tcs + q * stride + kc;
+            const int b = tc[0], e = tc[2 * K + 1];               // tile cells [kc, kc + 2 K + 1)
+            tcand += e - b;
+            // split off the part of the window that is a periodic image along x (box at an x face, window reaching
+            // into the halo that holds the cells of the other end of the row)
+            const bool ima = low_face && kc < K, imb = high_face && kc + K + 1 > B.sxc;
+            const int mid = ima ? tc[K - kc] : (imb ? tc[K + B.sxc - kc] : e);
+            // global index = tile index + delta, constant over each contiguous piece of the row
             const int e0 = R.off + R.n[0], e1 = e0 + R.n[1];
             const int d0 = R.g[0] - R.off, d1 = R.g[1] - e0, d2 = R.g[2] - e1;
             const int da = b < e0 ? d0 : (b < e1 ? d1 : d2), db = mid < e0 ? d0 : (mid < e1 ? d1 : d2);
-            const float shxa = cx == 0 ? L : 0.0f, shxb = cx == nc - 1 ? -L : 0.0f;
-            const unsigned fla = fl | (cx == 0 ? 1u : 0u), flb = fl | (cx == nc - 1 ? 1u : 0u);
-            const unsigned adda = (fla << W_FLAG_SHIFT) + (unsigned)da, addb = (flb << W_FLAG_SHIFT) + (unsigned)db;
-            if (fla) tile_scan_run_f<true>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
-            else tile_scan_run_f<false>(st, xi, yi, zi, li, b, mid, 0.0f, 0.0f, 0.0f, adda, rn2, em);
+            const real shxa = ima ? L : (real)0, shxb = imb ? -L : (real)0;
+            const unsigned fla = fl | (ima ? 1u : 0u), flb = fl | (imb ? 1u : 0u);
+            // what is added to the tile index to make the W entry: the flag bits, and for global W the index offset
+            const unsigned adda = LOCALW ? fla << T_FLAG_SHIFT : (fla << W_FLAG_SHIFT) + (unsigned)da;
+            const unsigned addb = LOCALW ? flb << T_FLAG_SHIFT : (flb << W_FLAG_SHIFT) + (unsigned)db;
+            if (fla) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
+            else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, mid, (real)0, (real)0, (real)0, adda, rn2, em);
             if (mid < e) {
-                if (flb) tile_scan_run_f<true>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
-                else tile_scan_run_f<false>(st, xi, yi, zi, li, mid, e, 0.0f, 0.0f, 0.0f, addb, rn2, em);
+                if (flb) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
+                else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, mid, e, (real)0, (real)0, (real)0, addb, rn2, em);
             }
         }
+        em.flush();
         const int m = em.m;
-        if (P.sp_pad > 1)
+        // single precision, long columns: padded to a multiple of P.sp_pad rows with self entries (md_sp.cu)
+        if (!LOCALW && P.sp_pad > 1)
             for (int k = m; k < ((m + P.sp_pad - 1) / P.sp_pad) * P.sp_pad && k < P.Mmax; k++)
                 P.W[(size_t)k * P.w_row + (size_t)i * P.w_col] = i;
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
@@ -485,15 +470,17 @@ __global__ void __launch_bounds__(512) k_sp_tile_build(const __grid_constant__ M
         tmax = max(tmax, m);
         tsum += m;
     }
+    // statistics of the matrix (md_energy.max_neighbors / mean_neighbors) and of the search (md_info.candidates_per_atom)
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum);
-    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; }
+    const int wm = warp_max_i(tmax), ws = warp_sum_i(tsum), wc = warp_sum_i(tcand);
+    if (lane == 0) { smx[wid] = wm; ssum[wid] = ws; scand[wid] = wc; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int mx = 0, sm = 0;
-        for (int w = 0; w < BLOCK / 32; w++) { mx = max(mx, smx[w]); sm += ssum[w]; }
+        int mx = 0, sm = 0, sc = 0;
+        for (int w = 0; w < BLOCK / 32; w++) { mx = max(mx, smx[w]); sm += ssum[w]; sc += scand[w]; }
         atomicMax(&P.ctrl->max_nnb, mx);
         atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
+        atomicAdd(&P.ctrl->cand_total, (unsigned long long)sc);
     }
 }
 
@@ -629,7 +616,7 @@ __global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_f
     const pos_t *__restrict__ pos = P.pos[pc];
     double *__restrict__ vel = P.vel[vc];
     const size_t np = (size_t)P.N_pad;
-    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const TileBox B = tile_box3(P.tg, P.nc, P.ncx, blockIdx.x, blockIdx.y, blockIdx.z);
     const int bid = tile_bid(P.tg);
     tile_load_desc(P, B, bid, M);
     const int n_own = M.T <= cap ? M.n_own : 0;          // an overflowing tile was reported by the build kernel
@@ -687,7 +674,7 @@ __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ M
     double *st = dsm;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const pos_t *__restrict__ pos = P.pos[pc];
-    const TileBox B = tile_box3(P.tg, P.nc, blockIdx.x, blockIdx.y, blockIdx.z);
+    const TileBox B = tile_box3(P.tg, P.nc, P.ncx, blockIdx.x, blockIdx.y, blockIdx.z);
     const int bid = tile_bid(P.tg);
     tile_load_desc(P, B, bid, M);
     const int n_own = M.T <= cap ? M.n_own : 0;
@@ -721,10 +708,11 @@ __global__ void __launch_bounds__(BLOCK) k_tile_energy(const __grid_constant__ M
 // ------------------------------------------------------------------------------------------------
 // launch wrappers
 // ------------------------------------------------------------------------------------------------
-size_t mdk_tile_smem(const TileGeom &G, bool with_cells)
+size_t mdk_tile_smem(const MdDev &P, bool with_cells)
 {
-    size_t b = 3 * (size_t)G.cap * sizeof(double);
-    if (with_cells) b += (size_t)TILE_Q_MAX * (G.S + 3) * sizeof(int);
+    size_t b = (size_t)P.tg.cap * (P.sp ? 3 * sizeof(float) : (with_cells ? TSTR64 : 3) * sizeof(double));
+    // build kernel: + the tile index of the first atom of every tile cell
+    if (with_cells) b += (size_t)TILE_Q_MAX * (P.tg.S + 2 * P.kx + 1) * sizeof(int);
     return b;
 }
 
@@ -748,7 +736,7 @@ int opt_in(K kernel, size_t bytes)
 template <int BLOCK>
 int configure_block(const MdDev &P)
 {
-    const size_t sf = mdk_tile_smem(P.tg, false), sb = mdk_tile_smem(P.tg, true);
+    const size_t sf = mdk_tile_smem(P, false);
     int rc = 0;
     rc |= opt_in(k_tile_force<0, false, BLOCK>, sf);
     rc |= opt_in(k_tile_force<1, false, BLOCK>, sf);
@@ -765,7 +753,7 @@ template <int BLOCK>
 void launch_force(const MdDev &P, int mode, cudaStream_t st)
 {
     const dim3 g = tile_grid3(P);
-    const size_t sm = mdk_tile_smem(P.tg, false);
+    const size_t sm = mdk_tile_smem(P, false);
     if (P.has_bonds) {
         if (mode == 0) k_tile_force<0, true, BLOCK><<<g, BLOCK, sm, st>>>(P);
         else if (mode == 1) k_tile_force<1, true, BLOCK><<<g, BLOCK, sm, st>>>(P);
@@ -781,8 +769,8 @@ void launch_force(const MdDev &P, int mode, cudaStream_t st)
 
 int mdk_tile_configure(const MdDev &P)
 {
-    const size_t sb = mdk_tile_smem(P.tg, true);
-    if (opt_in(k_tile_build<true>, sb) || opt_in(k_tile_build<false>, sb) || opt_in(k_sp_tile_build, sb)) return -1;
+    const size_t sb = mdk_tile_smem(P, true);
+    if (opt_in(k_tile_build<PrecF64, true>, sb) || opt_in(k_tile_build<PrecF64, false>, sb) || opt_in(k_tile_build<PrecF32, false>, sb)) return -1;
     if (!P.tiled) return 0;                          // the force / energy kernels exist for 128, 256 and 512 threads
     switch (P.tg.threads) {
     case 128: return configure_block<128>(P);
@@ -795,13 +783,10 @@ int mdk_tile_configure(const MdDev &P)
 void mdk_tile_build(const MdDev &P, cudaStream_t st)
 {
     const dim3 g = tile_grid3(P);
-    const size_t sm = mdk_tile_smem(P.tg, true);
-    if (P.sp) {      // same launch shape; the binary32 tile needs half the bytes
-        const size_t smf = 3 * (size_t)P.tg.cap * sizeof(float) + (size_t)TILE_Q_MAX * (P.tg.S + 3) * sizeof(int);
-        k_sp_tile_build<<<g, P.tg.threads, smf, st>>>(P);
-    }
-    else if (P.tiled) k_tile_build<true><<<g, P.tg.threads, sm, st>>>(P);
-    else k_tile_build<false><<<g, P.tg.threads, sm, st>>>(P);
+    const size_t sm = mdk_tile_smem(P, true);
+    if (P.sp) k_tile_build<PrecF32, false><<<g, P.tg.threads, sm, st>>>(P);
+    else if (P.tiled) k_tile_build<PrecF64, true><<<g, P.tg.threads, sm, st>>>(P);
+    else k_tile_build<PrecF64, false><<<g, P.tg.threads, sm, st>>>(P);
 }
 
 void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st)
@@ -816,7 +801,7 @@ void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st)
 void mdk_tile_energy(const MdDev &P, cudaStream_t st)
 {
     const dim3 g = tile_grid3(P);
-    const size_t sm = mdk_tile_smem(P.tg, false);
+    const size_t sm = mdk_tile_smem(P, false);
 #define MD_TE(B)                                                            \
     if (P.has_bonds) k_tile_energy<true, B><<<g, B, sm, st>>>(P);          \
     else k_tile_energy<false, B><<<g, B, sm, st>>>(P)

@@ -31,6 +31,7 @@ struct DevCtrl {
     int since_reorder;         // steps since the last sort
     int pad1;
     unsigned long long nnb_total;
+    unsigned long long cand_total;   // candidates the last neighbor build tested (all atoms): md_info.candidates_per_atom
     long long step;
     double disp_acc;           // accumulated dt * max|v| since the last rebuild
     double red[RED_N];
@@ -45,7 +46,7 @@ enum { TK_INTEGRATE = 0, TK_ENERGY = 1, TK_FORCE = 2 };
 // rows", each the contiguous atoms of S+2 cells along x.  W then holds 16-bit entries: 13 bits of index
 // into that tile + the 3 periodic-image flag bits of PAPER.md:163.
 struct TileGeom {
-    int S, R, RZ;            // cells per box along x, y, z
+    int S, R, RZ;            // cells per box along x (fine cells, see MdDev::kx), y, z
     int nsx, nsy, nsz;       // boxes per axis of ONE system
     int nsys;                // independent systems stacked along the grid's z axis (box index bz = sys * nsz + local)
     int cap;                 // tile capacity in atoms (<= 8192: 13 index bits)
@@ -58,45 +59,40 @@ struct TileBox {
     int cell_base;                 // index of the first cell of the system the box belongs to (batched systems)
 };
 
-__host__ __device__ inline TileBox tile_box(const TileGeom &G, int nc, int b)
+// nc: cells per edge along y, z; ncx: (fine) cells per edge along x
+__host__ __device__ inline TileBox tile_box3(const TileGeom &G, int nc, int ncx, int bx, int by, int bzg)
 {
     TileBox B;
-    const int bx = b % G.nsx, by = (b / G.nsx) % G.nsy, bzg = b / (G.nsx * G.nsy);
     const int sys = bzg / G.nsz, bz = bzg - sys * G.nsz;
-    B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
+    B.cell_base = sys * ncx * nc * nc;
+    B.x0 = bx * G.S;  B.sxc = ncx - B.x0 < G.S ? ncx - B.x0 : G.S;
     B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
     B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
     B.nyq = B.ny + 2;
     B.nq = B.nyq * (B.nz + 2);
-    B.cell_base = sys * nc * nc * nc;
     return B;
 }
 
-__host__ __device__ inline TileBox tile_box3(const TileGeom &G, int nc, int bx, int by, int bzg)
+__host__ __device__ inline TileBox tile_box(const TileGeom &G, int nc, int ncx, int b)
 {
-    TileBox B;
-    const int sys = bzg / G.nsz, bz = bzg - sys * G.nsz;
-    B.cell_base = sys * nc * nc * nc;
-    B.x0 = bx * G.S;  B.sxc = nc - B.x0 < G.S ? nc - B.x0 : G.S;
-    B.y0 = by * G.R;  B.ny = nc - B.y0 < G.R ? nc - B.y0 : G.R;
-    B.z0 = bz * G.RZ; B.nz = nc - B.z0 < G.RZ ? nc - B.z0 : G.RZ;
-    B.nyq = B.ny + 2;
-    B.nq = B.nyq * (B.nz + 2);
-    return B;
+    return tile_box3(G, nc, ncx, b % G.nsx, (b / G.nsx) % G.nsy, b / (G.nsx * G.nsy));
 }
 
 // Tile row q of a box: the row of cells (y0-1 + q % nyq, z0-1 + q / nyq), wrapped periodically.
 // rowc = linear index of its x = 0 cell; ysh, zsh in {-1, 0, +1}: image shift of the row in units of L
-// (added to r_i - r_j); xa, xc = x index of the halo cells before / after the box (wrapped at the faces).
-__host__ __device__ inline void tile_row(const TileBox &B, int nc, int q, int &rowc, int &ysh, int &zsh, int &xa, int &xc)
+// (added to r_i - r_j); xa, xc = x index of the FIRST of the kx halo cells before / after the box (wrapped at the
+// faces: a box that starts at x = 0 sees the last kx cells of the row as its halo, shifted by one box edge).
+// The box layout guarantees x0 >= kx for every box but the first and x0 + sxc + kx <= ncx for every box but the last,
+// so each halo is ONE contiguous range of cells.
+__host__ __device__ inline void tile_row(const TileBox &B, int nc, int ncx, int kx, int q, int &rowc, int &ysh, int &zsh, int &xa, int &xc)
 {
     int y = B.y0 - 1 + q % B.nyq, z = B.z0 - 1 + q / B.nyq;
     ysh = 0; zsh = 0;
     if (y < 0) { y += nc; ysh = 1; } else if (y >= nc) { y -= nc; ysh = -1; }
     if (z < 0) { z += nc; zsh = 1; } else if (z >= nc) { z -= nc; zsh = -1; }
-    rowc = B.cell_base + nc * (y + nc * z);
-    xa = B.x0 == 0 ? nc - 1 : B.x0 - 1;
-    xc = B.x0 + B.sxc == nc ? 0 : B.x0 + B.sxc;
+    rowc = B.cell_base + ncx * (y + nc * z);
+    xa = B.x0 == 0 ? ncx - kx : B.x0 - kx;
+    xc = B.x0 + B.sxc == ncx ? 0 : B.x0 + B.sxc;
 }
 
 constexpr int TILE_Q_MAX = 25;      // (R + 2)(RZ + 2) with R, RZ <= 3
@@ -125,9 +121,17 @@ constexpr int TILE_ROW_INTS = 8;
 // The unvarying parameter block.  The paper copies it to constant memory; here it is a
 // __grid_constant__ kernel argument, which lives in the same constant bank without a separate copy.
 struct MdDev {
-    int N, N_pad, Mmax, nc, NC;         // N, NC: atoms and cells of ALL systems; nc: cells per edge of one
+    int N, N_pad, Mmax, nc, NC;         // N, NC: atoms and cells of ALL systems; nc: cells per edge of one along y and z
+    // Cells are anisotropic: at least r_n wide along y and z (3 x 3 rows of cells around an atom), but kx times finer
+    // along x, the direction in which atoms are contiguous in memory: a row's candidates are then the atoms of the
+    // 2 kx + 1 fine cells around the atom's own, a window ~(2 + 1/kx) r_n long instead of 3 cell widths, and shorter
+    // still where the row's distance from the atom leaves less than r_n for x.  kx = 1: the paper's cubic cells.
+    int kx, ncx;                        // fine cells per r_n-wide cell along x; cells per edge along x = kx * nc
+    double inv_wx;                      // ncx / L
+    float w_f, inv_wx_f, rn2_prune;     // cell width along y/z, ncx / L and r_n^2 in binary32, rounded to the safe side (row pruning)
     int n_sys, N1, NC1;                 // batched independent systems: count, atoms and cells of one
     int has_bonds, half_list, scan_blocks;
+    int sm_count;                       // multiprocessors of the device (grid sizing of the grid-stride kernels)
     int tiled, tile_build, max_grid;    // W layout (1 = MD_W_TILED); shared-memory staged build kernel in use; row pitch of `partials`
     TileGeom tg;
     double L, half_L, inv_w;            // inv_w = nc / L
@@ -156,6 +160,12 @@ struct MdDev {
     // every-100-steps sort
     int layer_H, n_layers, reorder_interval;
     int *H;
+    // rigid molecules (md_rigid.cu; R20): molecule m = sites m rb_ns .. by original id
+    int rigid, rb_ns, rb_nm, need_inv;  // need_inv: k_reorder keeps inv (original id -> slot) up to date (bonds or rigid molecules)
+    double rb_body[24];                 // body-frame site positions (<= 8 sites), principal axes, centre of mass at the origin
+    double rb_I[3], rb_M, rb_Imin, rb_bmax;
+    double *rb_R, *rb_V, *rb_A, *rb_pi; // per molecule: centre of mass, its velocity, rotation matrix (row-major, body -> space), body-frame angular momentum
+    double *rb_off;                     // per site (original id): multiple of L between the stored coordinate and R + A b_k
     // single-precision variant (md_sp.cu; MD_PREC_F32): float4 records r, v, f replace pos / vel / frc,
     // which stay null; L and inv_w above are then those of the binary32 box edge (double)(float)L
     int sp, sp_pad;                     // sp_pad = SP_PAD when the columns of W are padded with self entries (long columns), else 1
@@ -184,16 +194,16 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
 int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   // blocks writing blk_vmax2
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
-void mdk_export(const MdDev &P, int what, size_t offset, cudaStream_t st);    // 0 pos, 1 vel, 2 frc -> scratch + offset
+void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
 // tiled layout (md_tile.cu)
 int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
-size_t mdk_tile_smem(const TileGeom &G, bool with_cells);
+size_t mdk_tile_smem(const MdDev &P, bool with_cells);
 void mdk_tile_build(const MdDev &P, cudaStream_t st);
 void mdk_tile_force(const MdDev &P, int mode, cudaStream_t st);
 void mdk_tile_energy(const MdDev &P, cudaStream_t st);
 // single-precision variant (md_sp.cu); the wrappers above dispatch to these when P.sp
 void mdk_sp_load_state(const MdDev &P, cudaStream_t st);
-void mdk_sp_export(const MdDev &P, int what, size_t offset, cudaStream_t st);
+void mdk_sp_export(const MdDev &P, int what, double *dst, cudaStream_t st);
 void mdk_sp_kick_drift(const MdDev &P, cudaStream_t st);
 void mdk_sp_kick(const MdDev &P, cudaStream_t st);
 void mdk_sp_bin(const MdDev &P, cudaStream_t st);
@@ -206,6 +216,14 @@ void mdk_po_kick_drift(const MdDev &P, double rcap2, double vlim2, double ke_tar
 void mdk_po_force(const MdDev &P, double rcap2, cudaStream_t st);
 void mdk_po_kick(const MdDev &P, cudaStream_t st);                             // + kinetic energy -> ctrl->red[RED_KE]
 void mdk_po_check(const MdDev &P, unsigned long long *out, cudaStream_t st);  // out[0] min non-bonded r^2, out[1] max bond r^2 (bit patterns)
+// rigid molecules (md_rigid.cu)
+int mdk_rigid_blocks(const MdDev &P);                                          // blocks of k_rigid_kick_drift (entries of blk_vmax2)
+void mdk_rigid_kick_drift(const MdDev &P, cudaStream_t st);
+void mdk_rigid_kick(const MdDev &P, cudaStream_t st);
+void mdk_rigid_offsets(const MdDev &P, cudaStream_t st);
+// measured arithmetic ceilings (md_peaks.cu); scratch >= 8 * sms doubles
+double mdk_peak_fp64(cudaStream_t st, int sms, double *scratch);
+double mdk_peak_fp32(cudaStream_t st, int sms, double *scratch);
 int mdk_launches_of(int which);   // number of kernels each wrapper launches (for md_info.kernel_launches)
 enum { LK_REBUILD_FORCE = 0, LK_LOAD, LK_KICK_DRIFT, LK_KICK, LK_CELLS, LK_REORDER, LK_BUILD, LK_FORCE, LK_FORCE_N3,
        LK_ENERGY, LK_EXPORT };

@@ -53,16 +53,17 @@ def test_struct_sizes_match_header(lib):
     """ctypes mirrors of md_params / md_energy / md_info have the C layout (checked against a compiled probe)."""
     import subprocess
     import tempfile
-    from paper_2003_14061_b200.binding import _Energy, _Info, _Params
-    src = ('#include <stdio.h>\n#include "md_b200.h"\nint main(){printf("%zu %zu %zu\\n",'
-           'sizeof(md_params),sizeof(md_energy),sizeof(md_info));return 0;}\n')
+    from paper_2003_14061_b200.binding import _Energy, _Info, _Params, _Peaks, _PushoffOpts, _PushoffReport
+    src = ('#include <stdio.h>\n#include "md_b200.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu\\n",'
+           'sizeof(md_params),sizeof(md_energy),sizeof(md_info),sizeof(md_pushoff_opts),sizeof(md_pushoff_report),'
+           'sizeof(md_peaks));return 0;}\n')
     with tempfile.TemporaryDirectory() as d:
         c = os.path.join(d, "p.c")
         open(c, "w").write(src)
         exe = os.path.join(d, "p")
         subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), c, "-o", exe], check=True)
         sizes = [int(x) for x in subprocess.run([exe], capture_output=True, text=True).stdout.split()]
-    assert sizes == [ctypes.sizeof(_Params), ctypes.sizeof(_Energy), ctypes.sizeof(_Info)]
+    assert sizes == [ctypes.sizeof(x) for x in (_Params, _Energy, _Info, _PushoffOpts, _PushoffReport, _Peaks)]
 
 
 def test_product_fails_loudly_without_gpu(lib):

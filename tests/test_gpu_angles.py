@@ -44,7 +44,7 @@ CASES = {"chains_4096x16": (4096, 16), "chains_ragged_1000x10": (1000, 10), "cha
 @pytest.mark.parametrize("k_theta,cos0", [(2.0, -1.0), (5.0, -0.5)])
 def test_angles_forces_energy_and_ten_steps(md, case, variant, mode, flags, k_theta, cos0):
     n, clen = CASES[case]
-    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    cfg = scaled_config("chains_rows_1m", n, chain_len=clen)
     for seed, thermal in ((1, False), (2, True)):
         g, o, box = make_pair(md, cfg, seed, k_theta, cos0, variant=variant, mode=mode, flags=flags, thermal=thermal)
         counts, lst = g.neighbors()
@@ -65,7 +65,7 @@ def test_angles_forces_energy_and_ten_steps(md, case, variant, mode, flags, k_th
 
 def test_angles_change_the_forces(md):
     """Guard against a silently ignored call: with k_theta > 0 the forces differ from the FENE-only ones."""
-    cfg = scaled_config("chains_1m", 1024, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 1024, chain_len=16)
     r, v, bonds, box = make_state(cfg, 1)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
     g.set_state(r, v)
@@ -79,7 +79,7 @@ def test_angles_change_the_forces(md):
 
 
 def test_angles_call_order_and_unsupported(md):
-    cfg = scaled_config("chains_1m", 1024, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 1024, chain_len=16)
     r, v, bonds, box = make_state(cfg, 1)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
     g.set_state(r, v)
@@ -109,7 +109,7 @@ def test_angles_single_precision(md, case, mode):
     from oracle.md_oracle import OracleMDSP
     eps = 2.0 ** -24
     n, clen = CASES[case]
-    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    cfg = scaled_config("chains_rows_1m", n, chain_len=clen)
     r, v, bonds, box = make_state(cfg, 1)
     o = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
     o.set_state(r, v)
@@ -138,7 +138,7 @@ def test_angles_single_precision(md, case, mode):
 def test_dihedrals_forces_energy_and_ten_steps(md, case, variant, mode, flags, with_angles):
     """Dihedral terms (md_set_dihedrals, R19), alone and together with the angle terms."""
     n, clen = CASES[case]
-    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    cfg = scaled_config("chains_rows_1m", n, chain_len=clen)
     for seed, thermal in ((1, False), (2, True)):
         r, v, bonds, box = make_state(cfg, seed)
         o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
@@ -172,7 +172,7 @@ def test_dihedrals_forces_energy_and_ten_steps(md, case, variant, mode, flags, w
 
 
 def test_dihedrals_change_the_forces_and_unsupported(md):
-    cfg = scaled_config("chains_1m", 1000, chain_len=10)
+    cfg = scaled_config("chains_rows_1m", 1000, chain_len=10)
     r, v, bonds, box = make_state(cfg, 1)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
     g.set_state(r, v)
@@ -202,7 +202,7 @@ def test_dihedrals_single_precision(md, case, mode):
     from oracle.md_oracle import OracleMDSP
     eps = 2.0 ** -24
     n, clen = CASES[case]
-    cfg = scaled_config("chains_1m", n, chain_len=clen)
+    cfg = scaled_config("chains_rows_1m", n, chain_len=clen)
     r, v, bonds, box = make_state(cfg, 1)
     o = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
     o.set_state(r, v)

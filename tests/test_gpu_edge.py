@@ -64,7 +64,7 @@ def test_zero_shell_rebuilds_every_step(md):
 
 
 def test_broken_bond_is_reported(md):
-    cfg = scaled_config("chains_1m", 4096, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 4096, chain_len=16)
     r, v, bonds, box = make_state(cfg, 1)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
     g.set_state(r, v)

@@ -64,7 +64,6 @@ def _check_static(g, o, cfg, lattice_start):
     assert eg.ke == pytest.approx(eo.ke, rel=1e-12)
     assert eg.vmax == pytest.approx(eo.vmax, rel=1e-12)
     assert eg.mean_neighbors == pytest.approx(eo.mean_neighbors, rel=1e-12)
-    assert eg.max_cell_occupancy == eo.max_cell_occupancy
 
 
 def _check_ten_steps(g, o, cfg, box):

@@ -23,7 +23,7 @@ def cases():
         "wca_4k": get_config("wca_4k"),
         "wca_ragged_1000": scaled_config("wca_4k", 1000),
         "lj_6912": scaled_config("lj_1m", 4 * 12 ** 3),
-        "chains_4096": scaled_config("chains_1m", 4096, chain_len=16),
+        "chains_4096": scaled_config("chains_rows_1m", 4096, chain_len=16),
     }
 
 

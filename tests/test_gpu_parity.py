@@ -6,7 +6,7 @@ import pytest
 
 from md_workloads import get_config, make_state, scaled_config
 from oracle.md_oracle import OracleMD, brute_forces_sample, brute_neighbors_sample
-from parity_util import ENERGY_RTOL, FORCE_RTOL, POS_ATOL, force_rel_err, pos_err, sets_equal
+from parity_util import ENERGY_RTOL, FORCE_RTOL, POS_ATOL, force_rel_err, pos_err, prepared_state, sets_equal
 
 pytestmark = pytest.mark.gpu
 
@@ -25,14 +25,16 @@ def small_cases():
         "wca_dr03_13824": (scaled_config("wca_2m_dr03", 24 ** 3), {}),
         "wca_dr05_13824": (scaled_config("wca_2m_dr05", 24 ** 3), {}),
         "lj_6912": (scaled_config("lj_1m", 4 * 12 ** 3), {}),
-        "chains_4096": (scaled_config("chains_1m", 4096, chain_len=16), {}),
+        "chains_4096": (scaled_config("chains_rows_1m", 4096, chain_len=16), {}),
+        # BASELINE.json configs[4] scaled down: seeded random walks pushed apart by the library (md_pushoff)
+        "walk_4096": (scaled_config("chains_1m", 4096, chain_len=16), {}),
     }
 
 
 def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw):
     """GPU system and oracle loaded with the SAME state (from md_workloads or evolved by the oracle)."""
-    jit = 0.0 if state == "lattice" else (0.12 if cfg.lattice != "chains" else 0.0)
-    r, v, bonds, box = make_state(cfg, seed, jitter_amp=jit)
+    jit = 0.0 if state == "lattice" else (0.12 if cfg.lattice in ("sc", "fcc") else 0.0)
+    r, v, bonds, box = prepared_state(md, cfg, seed, jitter_amp=jit)
     o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
     o.set_state(r, v)
     if bonds is not None:
@@ -64,7 +66,7 @@ def make_pair(md, cfg, seed, variant="full", mode="fused", state="jitter", **kw)
 @pytest.mark.parametrize("state", ["lattice", "jitter", "thermal"])
 def test_neighbor_sets_and_forces(md, case, variant, state):
     cfg, _ = small_cases()[case]
-    if state == "lattice" and cfg.lattice == "chains":
+    if state == "lattice" and cfg.lattice in ("chains", "walk"):
         pytest.skip("chain start has no separate lattice state")
     for seed in (1, 2, 3) if state != "thermal" else (1,):
         g, o, box = make_pair(md, cfg, seed, variant=variant, mode="split", state=state)
@@ -188,17 +190,16 @@ TILE_GEOMS = [dict(S=1, R=1, RZ=1, THREADS=128), dict(S=2, R=3, RZ=1, THREADS=12
               dict(S=1000, R=3, RZ=3, THREADS=512), dict(S=4, R=1, RZ=2, THREADS=256), dict(S=5, R=2, RZ=2, THREADS=128)]
 
 
-@pytest.mark.parametrize("case", ["wca_ragged_1000", "wca_dr05_13824", "lj_6912", "chains_4096"])
+@pytest.mark.parametrize("case", ["wca_ragged_1000", "wca_dr05_13824", "lj_6912", "chains_4096", "walk_4096"])
 @pytest.mark.parametrize("geom", range(len(TILE_GEOMS)))
 @pytest.mark.parametrize("variant", ["full-gatherw", "full-tiledw"])
-def test_tile_staging_any_box_shape(md, case, geom, variant, monkeypatch):
+def test_tile_staging_any_box_shape(md, case, geom, variant):
     """The shared-memory staged build (default) and the tiled W layout must give the same matrix, forces and trajectory for every box shape S x R x RZ and
     block size (boxes cut by the periodic faces, boxes wider than the system, blocks looping over their atoms)."""
     cfg, _ = small_cases()[case]
-    for k, v in TILE_GEOMS[geom].items():
-        monkeypatch.setenv(f"MD_TILE_{k}", str(v))
-    monkeypatch.setenv("MD_TILE_CAP", "8192")
-    g, o, box = make_pair(md, cfg, 2, variant=variant, mode="fused", state="jitter")
+    G = TILE_GEOMS[geom]
+    g, o, box = make_pair(md, cfg, 2, variant=variant, mode="fused", state="jitter", tile_cells=(G["S"], G["R"], G["RZ"]),
+                          tile_threads=G["THREADS"], tile_capacity=8192)
     info = g.info()
     assert info["w_layout"] == (1 if variant == "full-tiledw" else 0) and info["tile_cells"][1:] == [TILE_GEOMS[geom]["R"], TILE_GEOMS[geom]["RZ"]]
     counts, lst = g.neighbors()
@@ -213,20 +214,18 @@ def test_tile_staging_any_box_shape(md, case, geom, variant, monkeypatch):
     g.close()
 
 
-def test_tile_overflow_is_reported(md, monkeypatch):
+def test_tile_overflow_is_reported(md):
     """A tile that cannot hold the mean cell neighbourhood is refused at create (tiled W) or replaced by the gathering
     build kernel (default layout); a neighbourhood that outgrows its tile at run time is an error code, never a
     truncated matrix."""
     cfg = get_config("wca_4k")
     r, v, _, box = make_state(cfg, 1, jitter_amp=0.0)
-    monkeypatch.setenv("MD_TILE_CAP", "64")
     with pytest.raises(md.MDError):
-        md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=md.FLAG_TILED_W)
-    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+        md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=md.FLAG_TILED_W, tile_capacity=64)
+    g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", tile_capacity=64)
     g.set_state(r, v)
     assert g.info()["tile_capacity"] == 0          # fell back to the gathering build kernel
     g.close()
-    monkeypatch.delenv("MD_TILE_CAP")
     squeezed = r.copy()
     squeezed[:, 1] *= 0.5                          # density x 2 in half of the box (along y: a tile spans all of x)
     for flags in (md.FLAG_GATHER_W, md.FLAG_TILED_W):
@@ -248,7 +247,7 @@ def test_full_size_sampled_against_definitions(md, name):
     after 40 steps from the seeded start, sampled atoms are checked one by one against the all-pairs definitions
     (neighbor sets exact, forces 1e-10), and the conserved quantities against the start."""
     cfg = get_config(name)
-    r, v, bonds, box = make_state(cfg, 1)
+    r, v, bonds, box = prepared_state(md, cfg, 1)
     g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
     g.set_state(r, v)
     if bonds is not None:

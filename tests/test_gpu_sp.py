@@ -38,7 +38,7 @@ def cases():
         "wca_dr03_13824": scaled_config("wca_2m_dr03", 24 ** 3),
         "wca_dr05_13824": scaled_config("wca_2m_dr05", 24 ** 3),
         "lj_6912": scaled_config("lj_1m", 4 * 12 ** 3),
-        "chains_4096": scaled_config("chains_1m", 4096, chain_len=16),
+        "chains_4096": scaled_config("chains_rows_1m", 4096, chain_len=16),
     }
 
 

@@ -464,7 +464,7 @@ def test_p14_angle_forces_are_minus_gradient_of_numpy_energy():
 
 
 def test_p14_angle_run_conserves_energy_and_momentum():
-    cfg = scaled_config("chains_1m", 512, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 512, chain_len=16)
     r, v, bonds, box = make_state(cfg, 3)
     o = OracleMD(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
     o.set_state(r, v)

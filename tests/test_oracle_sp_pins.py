@@ -191,7 +191,7 @@ def test_sp5_conservation_and_newton3():
 
 
 def test_sp6_bonds_match_fp64_oracle_at_rounded_coordinates():
-    cfg = scaled_config("chains_1m", 512, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 512, chain_len=16)
     r, v, bonds, box = make_state(cfg, 3)
     s = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
     s.set_state(r, v)
@@ -210,7 +210,7 @@ def test_sp6_bonds_match_fp64_oracle_at_rounded_coordinates():
 def test_sp7_angles_match_fp64_oracle_at_rounded_coordinates():
     """Bond-angle terms (R19) in binary32 against the (separately pinned, P14) fp64 oracle from the same
     rounded state: ~20 binary32 operations per term."""
-    cfg = scaled_config("chains_1m", 1000, chain_len=10)
+    cfg = scaled_config("chains_rows_1m", 1000, chain_len=10)
     r, v, bonds, box = make_state(cfg, 3)
     box32 = float(np.float32(box))
     s = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)
@@ -231,7 +231,7 @@ def test_sp8_dihedrals_match_fp64_oracle_at_rounded_coordinates():
     """Dihedral terms (R19) in binary32 against the fp64 oracle (pinned by P15) from the same rounded state.
     ~80 binary32 operations per term; 1/|A|^2 amplifies rounding where consecutive bonds are nearly collinear, hence the
     bound relative to the largest dihedral force."""
-    cfg = scaled_config("chains_1m", 1000, chain_len=10)
+    cfg = scaled_config("chains_rows_1m", 1000, chain_len=10)
     r, v, bonds, box = make_state(cfg, 3)
     box32 = float(np.float32(box))
     s = OracleMDSP(cfg.n_atoms, box, cfg.r_cut, cfg.r_shell, cfg.dt)

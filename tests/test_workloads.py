@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 from scipy.spatial import cKDTree
 
-from md_workloads import (CONFIGS, chain_melt, fcc_lattice, gaussian_velocities, make_state, sc_lattice,
+from md_workloads import (CONFIGS, chain_melt, chain_walks, fcc_lattice, gaussian_velocities, make_state, sc_lattice,
                           scaled_config, splitmix64, uniform01)
 
 
@@ -68,9 +68,51 @@ def test_chain_start_is_overlap_free(n_chains, chain_len):
 def test_make_state_matches_configs():
     for name, cfg in CONFIGS.items():
         assert cfg.box == pytest.approx((cfg.n_atoms / cfg.density) ** (1 / 3))
-    cfg = scaled_config("chains_1m", 4096, chain_len=16)
+    cfg = scaled_config("chains_rows_1m", 4096, chain_len=16)
     r, v, bonds, box = make_state(cfg, 1)
     assert r.shape == v.shape == (4096, 3) and bonds is not None
     cfg = scaled_config("wca_2m", 512)
     r, v, bonds, box = make_state(cfg, 1, jitter_amp=0.1)
     assert bonds is None and np.abs(r - sc_lattice(512, box)).max() > 0.01
+
+
+@pytest.mark.parametrize("n_chains,chain_len", [(256, 16), (300, 10), (2048, 64)])
+def test_chain_walks_geometry(n_chains, chain_len):
+    """BASELINE.json configs[4] "chains grown as seeded random walks": every bond 0.97 long, next-
+    nearest beads of a chain at least 1.02 apart, starts uniform in the box, directions isotropic, reproducible from
+    (seed, chain, bead) counters.  The walks ignore one another, so the start overlaps (that is what md_pushoff is for)."""
+    r, bonds, box = chain_walks(n_chains, chain_len, 0.85, seed=3)
+    n = n_chains * chain_len
+    assert box == pytest.approx((n / 0.85) ** (1 / 3))
+    assert r.shape == (n, 3) and bonds.shape == (n_chains * (chain_len - 1), 2)
+    assert r.min() >= 0 and r.max() < box
+    assert np.all(bonds[:, 1] == bonds[:, 0] + 1) and np.all(bonds[:, 0] // chain_len == bonds[:, 1] // chain_len)
+    R = r.reshape(n_chains, chain_len, 3)
+    b = R[:, 1:] - R[:, :-1]
+    b -= box * np.round(b / box)
+    assert np.abs(np.sqrt((b * b).sum(-1)) - 0.97).max() < 1e-12
+    d2 = R[:, 2:] - R[:, :-2]
+    d2 -= box * np.round(d2 / box)
+    assert np.sqrt((d2 * d2).sum(-1)).min() >= 1.02 - 1e-12
+    # first steps are unconstrained: isotropic; starts uniform
+    u = b[:, 0] / 0.97
+    assert np.abs(u.mean(0)).max() < 4.0 / math.sqrt(3 * n_chains)
+    assert np.abs(R[:, 0].mean(0) / box - 0.5).max() < 4.0 / math.sqrt(12 * n_chains)
+    # consecutive bonds: the 1.02 rule removes the sharpest back-folds, cos(angle between bonds) >= 1.02^2/(2 0.97^2) - 1
+    cosb = (b[:, 1:] * b[:, :-1]).sum(-1) / 0.97 ** 2
+    assert cosb.min() >= 1.02 ** 2 / (2 * 0.97 ** 2) - 1.0 - 1e-12 and cosb.max() > 0.9
+    # reproducible, seed-dependent, and chain c does not depend on how many chains there are
+    assert np.array_equal(r, chain_walks(n_chains, chain_len, 0.85, seed=3)[0])
+    assert not np.array_equal(r, chain_walks(n_chains, chain_len, 0.85, seed=4)[0])
+    # it does overlap
+    close = cKDTree(r, boxsize=box).query_pairs(0.5, output_type="ndarray")
+    assert len(close) > 0
+
+
+def test_walk_config_is_configs4():
+    cfg = CONFIGS["chains_1m"]
+    assert (cfg.lattice, cfg.n_chains, cfg.chain_len, cfg.n_atoms) == ("walk", 16384, 64, 1048576)
+    assert (cfg.density, cfg.temperature, cfg.dt, cfg.fene_k, cfg.fene_r0) == (0.85, 1.0, 0.005, 30.0, 1.5)
+    small = scaled_config("chains_1m", 4096, chain_len=16)
+    r, v, bonds, box = make_state(small, 2)
+    assert r.shape == (4096, 3) and bonds.shape == (256 * 15, 2) and small.lattice == "walk"
