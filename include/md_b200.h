@@ -105,7 +105,7 @@ typedef struct md_params {
                                 default path sorts at every rebuild. */
     int32_t  cell_split_x;   /* cells are >= r_n wide along y and z and this many times finer along x, the direction atoms
                                 are contiguous in after the cell-order sort, which shortens the candidate runs of the
-                                neighbor build; 1 = the paper's cubic cells; 0 = auto (4; 1 with
+                                neighbor build; 1 = the paper's cubic cells; 0 = auto (2; 1 with
                                 MD_FLAG_LAYER_H).  1 .. 8. */
     int32_t  tile_cells[3];  /* shared-memory staged kernels: r_n-wide cells per thread block along x, y, z (y, z: 1..3); 0 = auto */
     int32_t  tile_threads;   /* their block size (multiple of 32 in [64, 512]; tiled W: 128, 256 or 512); 0 = auto */

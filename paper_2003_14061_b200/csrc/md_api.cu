@@ -70,11 +70,12 @@ struct md_system {
     bool profiling = false;
     std::vector<EvPair> pending, pool;
     // CUDA graph of one fused step: force+kick+drift -> decide -> IF(need_rebuild){cells, reorder, build}
-    cudaGraph_t graph[2] = {nullptr, nullptr};          // [0] kick+drift step head, [1] fused force+kick+drift step
-    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    cudaGraph_t graph[3] = {nullptr, nullptr, nullptr};    // [0] kick+drift step head, [1] one fused force+kick+drift step, [2] GRAPH_UNROLL of them
+    cudaGraphExec_t gexec[3] = {nullptr, nullptr, nullptr};
     cudaStream_t cap_stream = nullptr;
     bool graph_tried = false;
     int chain_kernels = 0;         // kernels inside the conditional body
+    int step_kernels = 2;          // kernels of one fused step in the graph (1 when the force kernel takes the rebuild decision)
     int rebuilds_seen = 0;
     int64_t graph_steps = 0;       // steps run through the graph since the last status read         // ctrl->n_rebuilds at the last status read (launch accounting)
     double t_ms[MD_T_COUNT] = {0};
@@ -201,7 +202,7 @@ void enqueue_decide(md_system *s, bool fused_force, unsigned long long cond = 0u
 
 void drop_graph(md_system *s)
 {
-    for (int k = 0; k < 2; k++) {
+    for (int k = 0; k < 3; k++) {
         if (s->gexec[k]) cudaGraphExecDestroy(s->gexec[k]);
         if (s->graph[k]) cudaGraphDestroy(s->graph[k]);
         s->gexec[k] = nullptr; s->graph[k] = nullptr;
@@ -215,39 +216,53 @@ void drop_graph(md_system *s)
 // rebuild so launches 2 kernels instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision
 // on the host every step).  Returns false (and leaves no graph) if any step of the construction is refused;
 // md_step then launches the kernels one by one.
+constexpr int GRAPH_UNROLL = 8;     // fused steps per launch of graph[2]: amortises the per-launch cost of a graph (small systems)
+
 bool build_step_graph(md_system *s, int kind)
 {
     cudaStream_t st = s->stream;
     if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+    const int reps = kind == 2 ? GRAPH_UNROLL : 1;
+    const bool fused = kind >= 1;
+    const bool in_kernel_decision = fused && mdk_force_decides(s->P, s->lc);
     cudaGraph_t g = nullptr;
     bool capturing = false, ok = false;
     do {
         if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
         capturing = true;
-        cudaStreamCaptureStatus status;
-        const cudaGraphNode_t *deps = nullptr;
-        size_t ndeps = 0;
-        if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
-        cudaGraphConditionalHandle h;
-        if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-        if (kind == 1) enqueue_force(s, 1);
-        else mdk_kick_drift(s->P, s->lc, st);
-        mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, kind == 1), kind == 1, st, (unsigned long long)h);
-        if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
-        cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
-        cp.conditional.handle = h;
-        cp.conditional.type = cudaGraphCondTypeIf;
-        cp.conditional.size = 1;
-        cudaGraphNode_t cnode;
-        if (cudaGraphAddNode(&cnode, g, deps, ndeps, &cp) != cudaSuccess) break;
-        cudaGraph_t body = cp.conditional.phGraph_out[0];
-        if (cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        mdk_cells(s->P, s->lc, s->cap_stream);
-        mdk_reorder(s->P, s->lc, s->cap_stream);
-        if (s->P.tile_build) mdk_tile_build(s->P, s->cap_stream); else mdk_build(s->P, s->lc, s->cap_stream);
-        cudaGraph_t body_out = nullptr;
-        if (cudaStreamEndCapture(s->cap_stream, &body_out) != cudaSuccess) break;
-        if (cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) break;
+        bool bad = false;
+        for (int rep = 0; rep < reps && !bad; rep++) {
+            bad = true;
+            cudaStreamCaptureStatus status;
+            const cudaGraphNode_t *deps = nullptr;
+            size_t ndeps = 0;
+            if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
+            cudaGraphConditionalHandle h;
+            if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
+            if (in_kernel_decision) mdk_force_fused_decide(s->P, s->lc, st, (unsigned long long)h);
+            else {
+                if (fused) enqueue_force(s, 1);
+                else mdk_kick_drift(s->P, s->lc, st);
+                mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused), fused, st, (unsigned long long)h);
+            }
+            if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
+            cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
+            cp.conditional.handle = h;
+            cp.conditional.type = cudaGraphCondTypeIf;
+            cp.conditional.size = 1;
+            cudaGraphNode_t cnode;
+            if (cudaGraphAddNode(&cnode, g, deps, ndeps, &cp) != cudaSuccess) break;
+            cudaGraph_t body = cp.conditional.phGraph_out[0];
+            if (cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+            mdk_cells(s->P, s->lc, s->cap_stream);
+            mdk_reorder(s->P, s->lc, s->cap_stream);
+            if (s->P.tile_build) mdk_tile_build(s->P, s->cap_stream); else mdk_build(s->P, s->lc, s->cap_stream);
+            cudaGraph_t body_out = nullptr;
+            if (cudaStreamEndCapture(s->cap_stream, &body_out) != cudaSuccess) break;
+            if (cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) break;
+            bad = false;
+        }
+        if (bad) break;
         capturing = false;
         if (cudaStreamEndCapture(st, &g) != cudaSuccess) { g = nullptr; break; }
         s->graph[kind] = g;
@@ -262,6 +277,7 @@ bool build_step_graph(md_system *s, int kind)
         return false;
     }
     s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1 + (s->P.layer_H ? 2 : 0);
+    s->step_kernels = in_kernel_decision ? 1 : 2;
     return true;
 }
 
@@ -272,7 +288,7 @@ bool have_graphs(md_system *s)
     if (!s->graph_tried) {
         s->graph_tried = true;
         const bool fused = s->prm.step_mode == MD_STEP_FUSED;
-        if (!build_step_graph(s, 0) || (fused && !build_step_graph(s, 1))) {
+        if (!build_step_graph(s, 0) || (fused && (!build_step_graph(s, 1) || !build_step_graph(s, 2)))) {
             const bool tried = true;
             drop_graph(s);
             s->graph_tried = tried;
@@ -519,7 +535,7 @@ md_system *md_create_ex(const md_params *pp)
     if (nc >= 1 && box_eff / nc - rn < (sp ? 1e-5 : 1e-9) * rn) nc -= 1;     // keep the cell strictly wider than r_n
     if (nc < 3) { set_error("box too small: %d cells per edge (need >= 3)", nc); return nullptr; }
     if (p.cell_split_x < 0 || p.cell_split_x > 8) { set_error("cell_split_x must be in [0, 8]"); return nullptr; }
-    if (p.cell_split_x == 0) p.cell_split_x = (p.flags & MD_FLAG_LAYER_H) ? 1 : 4;
+    if (p.cell_split_x == 0) p.cell_split_x = (p.flags & MD_FLAG_LAYER_H) ? 1 : 2;      // measured: BASELINE.md sec. 4
     if ((p.flags & MD_FLAG_LAYER_H) && p.cell_split_x != 1) { set_error("MD_FLAG_LAYER_H keeps the paper's cubic cells (cell_split_x = 1)"); return nullptr; }
     if ((int64_t)nc * nc * nc * p.cell_split_x * std::max(1, p.n_systems) > (1ll << 30)) { set_error("too many cells"); return nullptr; }
     if (p.max_neighbors <= 0) {
@@ -1073,9 +1089,11 @@ int md_step(md_system *s, int64_t n)
         const bool graphs = have_graphs(s);
         if (graphs) {
             CK(cudaGraphLaunch(s->gexec[0], st));
-            for (int64_t k = 1; k < n; k++) CK(cudaGraphLaunch(s->gexec[1], st));
+            int64_t k = 1;
+            for (; k + GRAPH_UNROLL <= n; k += GRAPH_UNROLL) CK(cudaGraphLaunch(s->gexec[2], st));
+            for (; k < n; k++) CK(cudaGraphLaunch(s->gexec[1], st));
             s->graph_steps += n;
-            s->launches += 2 * n;                        // + the rebuild chains, added in check_device_status
+            s->launches += 2 + (n - 1) * s->step_kernels;   // + the rebuild chains, added in check_device_status
         } else {
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
             enqueue_decide(s, false);

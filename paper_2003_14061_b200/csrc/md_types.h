@@ -192,6 +192,8 @@ void mdk_build(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          //
 // mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, per-block max v^2; follow with mdk_decide); 2: f and closing half kick
 void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
 int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   // blocks writing blk_vmax2
+bool mdk_force_decides(const MdDev &P, const MdLaunch &lc);                   // small grid: the fused step can take the rebuild decision itself
+void mdk_force_fused_decide(const MdDev &P, const MdLaunch &lc, cudaStream_t st, unsigned long long cond);   // fused step + decision + IF condition
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
