@@ -126,6 +126,11 @@ enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying 
        MD_FLAG_GATHER_W = 8u, /* never pick the tiled layout automatically (the build kernel still stages tiles) */
        MD_FLAG_W_TRANSPOSED = 16u, /* ablation of PAPER.md:165-167: store W atom-index-SLOWEST, W[i * Mmax + m], so that
                                  the threads of a warp no longer read consecutive words (global-index layout only) */
+       MD_FLAG_NO_PERSIST = 64u, /* Small systems (<= 32768 atoms; fp64, fused steps, no flag and no tile setting given) run
+                                 md_step as ONE cooperative launch whose blocks stay resident over all n steps and meet at
+                                 grid-wide barriers (md_info.use_graph = 2), with W built by the gathering
+                                 kernel.  This flag -- like any other flag or tile setting -- keeps the step graph that larger
+                                 systems use. */
        MD_FLAG_LAYER_H = 32u  /* ablation: the paper's own cell structure (steps N1-N5): a dense cell x
                                  layer matrix H[c][l] = atom, filled from the atomic slot l_i, searched by the neighbor
                                  build; atoms are re-sorted into cell order only every md_params.reorder_interval steps
@@ -159,7 +164,8 @@ typedef struct md_info {
     int32_t tile_cells[3];      /* tiled: cells per thread block along x, y, z */
     int32_t tile_capacity;      /* tiled: atoms the shared-memory tile can hold */
     int32_t tile_threads;       /* tiled: threads per block of the build / force kernels */
-    int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node */
+    int32_t use_graph;          /* 1 when md_step replays a CUDA graph with a conditional rebuild node; 2 when it runs all its
+                                   steps in one cooperative launch (small systems) */
     int32_t n_systems;
     int32_t precision;          /* MD_PREC_* */
     int32_t n_layers;           /* MD_FLAG_LAYER_H: N_l, columns of H; else 0 */

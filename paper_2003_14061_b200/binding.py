@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_PKG, "libmd_b200.so")
 
 MD_OK, MD_ERR_INVALID, MD_ERR_NEBR_OVERFLOW, MD_ERR_BOND_BROKEN = 0, -1, -2, -3
 MD_ERR_NONFINITE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED, MD_ERR_NOMEM, MD_ERR_TILE_OVERFLOW, MD_ERR_CELL_OVERFLOW = -4, -5, -6, -7, -8, -9
-FLAG_NO_GRAPH, FLAG_GLOBAL_W, FLAG_TILED_W, FLAG_GATHER_W, FLAG_W_TRANSPOSED, FLAG_LAYER_H = 1, 2, 4, 8, 16, 32
+FLAG_NO_GRAPH, FLAG_GLOBAL_W, FLAG_TILED_W, FLAG_GATHER_W, FLAG_W_TRANSPOSED, FLAG_LAYER_H, FLAG_NO_PERSIST = 1, 2, 4, 8, 16, 32, 64
 LATTICE = {"auto": 0, "sc": 1, "fcc": 2, "none": 3}
 FORCE_VARIANT = {"full": 0, "newton3": 1}
 STEP_MODE = {"fused": 0, "split": 1}

@@ -75,6 +75,7 @@ struct md_system {
     cudaStream_t cap_stream = nullptr;
     bool graph_tried = false;
     int chain_kernels = 0;         // kernels inside the conditional body
+    bool persist = false;          // small system: md_step runs as one cooperative launch
     int step_kernels = 2;          // kernels of one fused step in the graph (1 when the force kernel takes the rebuild decision)
     int rebuilds_seen = 0;
     int64_t graph_steps = 0;       // steps run through the graph since the last status read         // ctrl->n_rebuilds at the last status read (launch accounting)
@@ -651,6 +652,13 @@ md_system *md_create_ex(const md_params *pp)
         if (P.tiled) { set_error("MD_FLAG_W_TRANSPOSED applies to the global-index W layout only"); md_destroy(s); return nullptr; }
         P.w_row = 1; P.w_col = P.Mmax;
     }
+    // small systems run md_step as one cooperative launch (k_persist); it lists neighbors with the gathering build
+    // -- the default for small systems only: any flag or tile setting that selects a path keeps the step graph
+    const bool tile_knobs = pp->tile_cells[0] || pp->tile_cells[1] || pp->tile_cells[2] || pp->tile_threads || pp->tile_capacity;
+    if (p.flags == 0 && !tile_knobs && p.step_mode == MD_STEP_FUSED && mdk_persist_ok(P)) {
+        s->persist = true;
+        P.tile_build = 0;
+    }
     P.max_grid = std::max((P.N + 63) / 64, P.tile_build ? P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys : 0);
 
     const size_t np = (size_t)P.N_pad;
@@ -972,6 +980,7 @@ int md_set_rigid(md_system *s, int32_t n_sites, const double *body_xyz)
         if (!P.rb_R || !P.rb_V || !P.rb_A || !P.rb_pi || !P.rb_off || !P.inv) { set_error("device allocation failed"); return MD_ERR_NOMEM; }
     }
     P.rigid = 1;
+    s->persist = false;
     P.need_inv = 1;
     P.tile_build = 0;          // the gathering build kernel knows the molecules (sites of one molecule are no neighbors)
     s->has_state = false;      // load the molecules with md_set_rigid_state
@@ -1034,6 +1043,7 @@ int md_set_angles(md_system *s, double k_theta, double cos_theta0)
     if (s->P.tiled) { set_error("md_set_angles: global-index W layouts only (use MD_FLAG_GATHER_W)"); return MD_ERR_UNSUPPORTED; }
     drop_graph(s);                 // the captured kernel arguments (MdDev by value) change
     s->P.has_angles = k_theta > 0;
+    s->persist = s->persist && mdk_persist_ok(s->P);
     s->P.ang_k = k_theta;
     s->P.ang_c0 = cos_theta0;
     enqueue_forces_only(s);
@@ -1048,6 +1058,7 @@ int md_set_dihedrals(md_system *s, double k_phi, double cos_phi0)
     if (s->P.tiled) { set_error("md_set_dihedrals: global-index W layouts only (use MD_FLAG_GATHER_W)"); return MD_ERR_UNSUPPORTED; }
     drop_graph(s);
     s->P.has_dihedrals = k_phi > 0;
+    s->persist = s->persist && mdk_persist_ok(s->P);
     s->P.dih_k = k_phi;
     s->P.dih_c0 = cos_phi0;
     enqueue_forces_only(s);
@@ -1083,6 +1094,17 @@ int md_step(md_system *s, int64_t n)
         }
         s->step += n;
         return check_device_status(s);
+    }
+    if (s->persist && !s->profiling) {
+        // small system: one cooperative launch whose blocks stay resident over all n steps (md_kernels.cu: k_persist)
+        if (mdk_persist_steps(P, (long long)n, st) != 0) {
+            cudaGetLastError();
+            s->persist = false;                         // e.g. the device is shared and the grid no longer fits: step graph
+        } else {
+            s->launches += 1;
+            s->step += n;
+            return check_device_status(s);
+        }
     }
     if (s->prm.step_mode == MD_STEP_FUSED) {
         // leapfrog form: opening half kick + drift, (n-1) fused force+kick+drift kernels, closing force + half kick
@@ -1260,7 +1282,7 @@ int md_get_info(md_system *s, md_info *out)
         out->tile_cells[0] = s->P.tg.S / s->P.kx; out->tile_cells[1] = s->P.tg.R; out->tile_cells[2] = s->P.tg.RZ;
         out->tile_capacity = s->P.tg.cap; out->tile_threads = s->P.tg.threads;
     }
-    out->use_graph = s->gexec[0] ? 1 : 0;
+    out->use_graph = s->persist ? 2 : (s->gexec[0] ? 1 : 0);
     out->precision = s->prm.precision;
     out->n_layers = s->P.n_layers;
     out->cells_x = s->P.ncx; out->cell_split_x = s->P.kx; out->sm_count = s->sm_count;

@@ -61,6 +61,20 @@ __device__ __forceinline__ pos_t ld_pos_rw(const pos_t *p)
     return r;
 }
 
+// How the kernels read arrays that the SAME launch never writes (LdNC: the non-coherent read-only path) -- and how the
+// persistent small-system kernel (md_kernels.cu: k_persist), which rewrites those arrays between its grid-wide barriers,
+// must read them instead (LdPlain: ordinary coherent loads).
+struct LdNC {
+    static __device__ __forceinline__ pos_t pos(const pos_t *p) { return ld_pos(p); }
+    static __device__ __forceinline__ int i32(const int *p) { return __ldg(p); }
+    static __device__ __forceinline__ double f64(const double *p) { return __ldg(p); }
+};
+struct LdPlain {
+    static __device__ __forceinline__ pos_t pos(const pos_t *p) { return ld_pos_rw(p); }
+    static __device__ __forceinline__ int i32(const int *p) { return *(const volatile int *)p; }
+    static __device__ __forceinline__ double f64(const double *p) { return *(const volatile double *)p; }
+};
+
 __device__ __forceinline__ void st_pos(pos_t *p, double x, double y, double z)
 {
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x), "d"(y), "d"(z), "d"(0.0) : "memory");
@@ -176,30 +190,58 @@ __device__ __forceinline__ double block_max(double v, double *sm)
 // (A "last block done" ticket inside the drifting kernel, was measured at ~7.5 ns per block on
 // B200 -- two same-address L2 atomics and a fence per block, ~75 us for the 10^4 blocks of N = 2M, more than
 // the rest of the kernel -- so the decision moved to a one-block kernel ordered by the stream.)
-__device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pingpong)
+// the scalars of the decision and the buffer roles it fixes (a copy of the corresponding DevCtrl fields)
+struct DecState {
+    double disp_acc;
+    int p_src, p_dst, v_src, v_dst, need_rebuild, n_rebuilds, do_reorder, since_reorder;
+};
+
+__device__ __forceinline__ DecState dec_load(const MdDev &P)
+{
+    const volatile DevCtrl *c = P.ctrl;
+    DecState d;
+    d.disp_acc = c->disp_acc; d.p_src = c->p_src; d.p_dst = c->p_dst; d.v_src = c->v_src; d.v_dst = c->v_dst;
+    d.need_rebuild = c->need_rebuild; d.n_rebuilds = c->n_rebuilds; d.do_reorder = c->do_reorder; d.since_reorder = c->since_reorder;
+    return d;
+}
+
+__device__ __forceinline__ void dec_store(const MdDev &P, const DecState &d)
 {
     volatile DevCtrl *c = P.ctrl;
-    double acc = c->disp_acc + P.dt * sqrt(vmax2);
+    if (d.need_rebuild) { c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull; c->cand_total = 0ull; }
+    c->disp_acc = d.disp_acc; c->p_src = d.p_src; c->p_dst = d.p_dst; c->v_src = d.v_src; c->v_dst = d.v_dst;
+    c->need_rebuild = d.need_rebuild; c->n_rebuilds = d.n_rebuilds; c->do_reorder = d.do_reorder; c->since_reorder = d.since_reorder;
+}
+
+// pure: the same inputs give the same decision in every thread that evaluates it (k_persist replicates it per block)
+__device__ __forceinline__ void decide_state(const MdDev &P, DecState &c, double vmax2, bool pos_pingpong)
+{
+    double acc = c.disp_acc + P.dt * sqrt(vmax2);
     const int need = acc > P.thresh;
-    const int since = c->since_reorder + 1;
-    c->since_reorder = since;
+    c.since_reorder += 1;
     if (need) {
         acc = 0.0;
-        c->n_rebuilds += 1;
-        c->max_occ = 0; c->max_nnb = 0; c->nnb_total = 0ull; c->cand_total = 0ull;
+        c.n_rebuilds += 1;
         // the paper sorts the atoms only every ~100 steps; the default path at every rebuild
-        const int ro = !P.layer_H || P.reorder_interval == 0 || (P.reorder_interval > 0 && since >= P.reorder_interval);
-        c->do_reorder = ro;
-        if (ro) c->since_reorder = 0;
+        const int ro = !P.layer_H || P.reorder_interval == 0 || (P.reorder_interval > 0 && c.since_reorder >= P.reorder_interval);
+        c.do_reorder = ro;
+        if (ro) c.since_reorder = 0;
     }
-    c->disp_acc = acc;
-    c->need_rebuild = need;
-    const int ps = pos_pingpong ? (c->p_dst ^ 1) : c->p_dst;
-    c->p_src = ps;
-    c->p_dst = need ? (ps ^ 1) : ps;
-    const int vs = c->v_dst;
-    c->v_src = vs;
-    c->v_dst = need ? (vs ^ 1) : vs;
+    c.disp_acc = acc;
+    c.need_rebuild = need;
+    const int ps = pos_pingpong ? (c.p_dst ^ 1) : c.p_dst;
+    c.p_src = ps;
+    c.p_dst = need ? (ps ^ 1) : ps;
+    const int vs = c.v_dst;
+    c.v_src = vs;
+    c.v_dst = need ? (vs ^ 1) : vs;
+}
+
+__device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pingpong)
+{
+    DecState c = dec_load(P);
+    decide_state(P, c, vmax2, pos_pingpong);
+    dec_store(P, c);
 }
 
 __device__ __forceinline__ void set_err(const MdDev &P, int code) { atomicCAS(&P.ctrl->err, 0, code); }

@@ -17,6 +17,8 @@
 // which is the condition the paper's flag-bit scheme needs.
 #include <algorithm>
 
+#include <cooperative_groups.h>
+
 #include "md_device.cuh"
 
 namespace {
@@ -85,24 +87,28 @@ __global__ void k_export(const __grid_constant__ MdDev P, int what, double *dst)
 // ------------------------------------------------------------------------------------------------
 // integration (split mode): first half kick + drift + max velocity + rebuild decision
 // ------------------------------------------------------------------------------------------------
+// opening half kick + drift of atom i; returns |v|^2
+__device__ __forceinline__ double kick_drift_atom(const MdDev &P, int pc, int vc, int i)
+{
+    pos_t *pp = P.pos[pc] + i;
+    double *vx = P.vel[vc] + i, *vy = vx + P.N_pad, *vz = vy + P.N_pad;
+    const double *fx = P.frc + i, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
+    const pos_t r = ld_pos_rw(pp);
+    const double ax = *vx + P.hdt * *fx, ay = *vy + P.hdt * *fy, az = *vz + P.hdt * *fz;
+    *vx = ax; *vy = ay; *vz = az;
+    const double x = r.x + P.dt * ax, y = r.y + P.dt * ay, z = r.z + P.dt * az;
+    st_pos(pp, x, y, z);
+    double v2 = ax * ax + ay * ay + az * az;
+    if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
+    return v2;
+}
+
 __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
-    double v2 = 0.0;
-    if (i < P.N) {
-        pos_t *pp = P.pos[pc] + i;
-        double *vx = P.vel[vc] + i, *vy = vx + P.N_pad, *vz = vy + P.N_pad;
-        const double *fx = P.frc + i, *fy = fx + P.N_pad, *fz = fy + P.N_pad;
-        const pos_t r = ld_pos_rw(pp);
-        const double ax = *vx + P.hdt * *fx, ay = *vy + P.hdt * *fy, az = *vz + P.hdt * *fz;
-        *vx = ax; *vy = ay; *vz = az;
-        const double x = r.x + P.dt * ax, y = r.y + P.dt * ay, z = r.z + P.dt * az;
-        st_pos(pp, x, y, z);
-        v2 = ax * ax + ay * ay + az * az;
-        if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
-    }
+    const double v2 = i < P.N ? kick_drift_atom(P, pc, vc, i) : 0.0;
     const double bm = block_max(v2, sm);
     if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
 }
@@ -140,30 +146,46 @@ __global__ void __launch_bounds__(256) k_kick(const __grid_constant__ MdDev P)
 // cells: N1/N2 binning with atomic occupancy counters, N3/N4 as a prefix scan.  The rebuild kernels use
 // grid-stride loops over a capped grid: a launch that finds need_rebuild == 0 retires in ~2 us.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
+// which of the ping-pong buffers a rebuild reads (ps, vs) and writes (pd, vd): from the control block, or from the
+// persistent kernel's own copy of the decision
+struct Bufs {
+    int ps, pd, vs, vd;
+};
+__device__ __forceinline__ Bufs bufs_from_ctrl(const MdDev &P)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_src)];
-    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_src)];
+    return {__ldcg(&P.ctrl->p_src), __ldcg(&P.ctrl->p_dst), __ldcg(&P.ctrl->v_src), __ldcg(&P.ctrl->v_dst)};
+}
+
+template <class LD>
+__device__ __forceinline__ void bin_body(const MdDev &P, const Bufs B)
+{
+    const pos_t *__restrict__ pos = P.pos[B.ps];
+    const int *__restrict__ idv = P.id[B.vs];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
-        const pos_t r = ld_pos(pos + i);
+        const pos_t r = LD::pos(pos + i);
         const int cx = cell_coord(wrap1(r.x, P.L), P.inv_wx, P.ncx), cy = cell_coord(wrap1(r.y, P.L), P.inv_w, P.nc),
                   cz = cell_coord(wrap1(r.z, P.L), P.inv_w, P.nc);
         // batched independent systems: each has its own block of cells, found from the permanent id
-        const int sys = P.n_sys > 1 ? __ldg(idv + i) / P.N1 : 0;
+        const int sys = P.n_sys > 1 ? LD::i32(idv + i) / P.N1 : 0;
         const int c = sys * P.NC1 + cx + P.ncx * (cy + P.nc * cz);
         P.cell_of[i] = c;
         P.slot[i] = atomicAdd(&P.cell_count[c], 1);  // l_i; "incrementing k_c requires an atomic operation" (N2)
     }
 }
 
-constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
-
-__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    bin_body<LdNC>(P, bufs_from_ctrl(P));
+}
+
+constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
+
+// occupancy sum and maximum of tile `tile` of SCAN_TILE cells; the block has SCAN_T threads
+__device__ __forceinline__ void scan_reduce_tile(const MdDev &P, int tile)
+{
     __shared__ int ssum[SCAN_T / 32], smax[SCAN_T / 32];
-    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_V;
+    const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
     int sum = 0, mx = 0;
 #pragma unroll
     for (int k = 0; k < SCAN_V; k++) {
@@ -180,9 +202,15 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ 
     if (threadIdx.x == 0) {
         int s = 0, m = 0;
         for (int w = 0; w < SCAN_T / 32; w++) { s += ssum[w]; m = max(m, smax[w]); }
-        P.block_sums[blockIdx.x] = s;
+        P.block_sums[tile] = s;
         atomicMax(&P.ctrl->max_occ, m);              // N3: the paper's layer count N_l = max_c k_c
     }
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    scan_reduce_tile(P, blockIdx.x);
 }
 
 // exclusive scan of the per-tile sums, one block
@@ -224,11 +252,10 @@ __global__ void __launch_bounds__(1024) k_scan_top(const __grid_constant__ MdDev
     }
 }
 
-__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ MdDev P)
+__device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
     __shared__ int wsum[SCAN_T / 32];
-    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_V;
+    const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
     int c[SCAN_V], sum = 0;
 #pragma unroll
     for (int k = 0; k < SCAN_V; k++) {
@@ -247,7 +274,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ M
     __syncthreads();
     int woff = 0;
     for (int w = 0; w < wid; w++) woff += wsum[w];
-    int run = P.block_sums[blockIdx.x] + woff + inc - sum;
+    int run = P.block_sums[tile] + woff + inc - sum;
 #pragma unroll
     for (int k = 0; k < SCAN_V; k++) {
         const int idx = base + k;
@@ -260,34 +287,43 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ M
     }
 }
 
+__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    scan_apply_tile(P, blockIdx.x);
+}
+
 // N4 in CSR form: the atom's place in the cell-ordered sequence s
+__device__ __forceinline__ void place_body(const MdDev &P)
+{
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x)
+        P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
+}
+
 __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     if (P.layer_H && !__ldcg(&P.ctrl->do_reorder)) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x)
-        P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
+    place_body(P);
 }
 
 // Cell-order gather of r, v and the permanent serial numbers; coordinates are wrapped into
 // [0, L) here.  The atomics of N2 leave the order inside a cell indeterminate; ranking the
 // cell's members by their previous slot makes the order -- and with it every floating-point sum downstream --
 // reproducible run to run.
-__global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P)
+template <class LD>
+__device__ __forceinline__ void reorder_body(const MdDev &P, const Bufs B)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    if (P.layer_H && !__ldcg(&P.ctrl->do_reorder)) return;
-    const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
-    const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
+    const int ps = B.ps, pd = B.pd, vs = B.vs, vd = B.vd;
     const pos_t *__restrict__ pin = P.pos[ps];
     const double *__restrict__ vin = P.vel[vs];
     const int *__restrict__ idin = P.id[vs];
     for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P.N; p += gridDim.x * blockDim.x) {
         const int a = P.perm[p];
         // issue the payload loads first; the rank search below overlaps with their latency
-        const pos_t r = ld_pos(pin + a);
-        const double vx = __ldg(vin + a), vy = __ldg(vin + P.N_pad + a), vz = __ldg(vin + 2 * (size_t)P.N_pad + a);
-        const int id = __ldg(idin + a);
+        const pos_t r = LD::pos(pin + a);
+        const double vx = LD::f64(vin + a), vy = LD::f64(vin + P.N_pad + a), vz = LD::f64(vin + 2 * (size_t)P.N_pad + a);
+        const int id = LD::i32(idin + a);
         const int c = P.cell_of[a];
         const int s = P.cell_start[c], e = P.cell_start[c + 1];
         int rank = 0;
@@ -301,10 +337,16 @@ __global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P
     }
 }
 
-__global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
+    if (P.layer_H && !__ldcg(&P.ctrl->do_reorder)) return;
+    reorder_body<LdNC>(P, bufs_from_ctrl(P));
+}
+
+__device__ __forceinline__ void bonds_remap_body(const MdDev &P, const Bufs B)
+{
+    const int *idv = P.id[B.vd];
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < P.N; n += gridDim.x * blockDim.x) {
         const int id = idv[n];
 #pragma unroll
@@ -313,6 +355,12 @@ __global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdD
             P.bond_dev[(size_t)k * P.N_pad + n] = partner >= 0 ? P.inv[partner] : -1;
         }
     }
+}
+
+__global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    bonds_remap_body(P, bufs_from_ctrl(P));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -328,13 +376,13 @@ __global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdD
 // ------------------------------------------------------------------------------------------------
 // candidates j in [b, e) of one run, image shift (sx, sy, sz) and flag bits fl for the whole run
 // EXCL: rigid molecules -- sites of the atom's own molecule (mol = original id / sites per molecule) are no neighbors
-template <bool HALF, bool SHIFT, bool EXCL>
+template <bool HALF, bool SHIFT, bool EXCL, class LD>
 __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, int b, int e,
                                          double sx, double sy, double sz, unsigned fl, int &m, const int *__restrict__ idv, int mol)
 {
     for (int j = b; j < e; j++) {
-        if (EXCL && __ldg(idv + j) / P.rb_ns == mol) continue;
-        const pos_t rj = ld_pos(pos + j);
+        if (EXCL && LD::i32(idv + j) / P.rb_ns == mol) continue;
+        const pos_t rj = LD::pos(pos + j);
         // d = (r_i - r_j) + shift, each operation rounded once
         double dx = __dsub_rn(ri.x, rj.x), dy = __dsub_rn(ri.y, rj.y), dz = __dsub_rn(ri.z, rj.z);
         if (SHIFT) { dx = __dadd_rn(dx, sx); dy = __dadd_rn(dy, sy); dz = __dadd_rn(dz, sz); }
@@ -346,24 +394,23 @@ __device__ __forceinline__ void scan_run(const MdDev &P, const pos_t *__restrict
     }
 }
 
-template <bool HALF, bool EXCL>
-__global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
+template <bool HALF, bool EXCL, class LD>
+__device__ __forceinline__ void build_body(const MdDev &P, const Bufs B)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    __shared__ int smx[4], scand[4];
-    __shared__ int ssum[4];
-    const pos_t *__restrict__ pos = P.pos[__ldcg(&P.ctrl->p_dst)];
+    __shared__ int smx[32], scand[32];
+    __shared__ int ssum[32];
+    const pos_t *__restrict__ pos = P.pos[B.pd];
     const int *__restrict__ cs = P.cell_start;
-    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
+    const int *__restrict__ idv = P.id[B.vd];
     const int nc = P.nc, ncx = P.ncx;
     const double L = P.L;
     int tmax = 0, tsum = 0, tcand = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
-        const pos_t ri = ld_pos(pos + i);
+        const pos_t ri = LD::pos(pos + i);
         const int cx = cell_coord(ri.x, P.inv_wx, ncx), cy = cell_coord(ri.y, P.inv_w, nc), cz = cell_coord(ri.z, P.inv_w, nc);
         const RowGaps gaps = row_gaps(P, ri.y, ri.z, cy, cz);
-        const int cell_base = P.n_sys > 1 ? (__ldg(idv + i) / P.N1) * P.NC1 : 0;     // the atom's own system of cells
-        const int mol = EXCL ? __ldg(idv + i) / P.rb_ns : 0;
+        const int cell_base = P.n_sys > 1 ? (LD::i32(idv + i) / P.N1) * P.NC1 : 0;     // the atom's own system of cells
+        const int mol = EXCL ? LD::i32(idv + i) / P.rb_ns : 0;
         int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
             int z = cz + dz;
@@ -379,13 +426,13 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
                 if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
                 const int row = cell_base + ncx * (y + nc * z);
                 const int lo = cx - kr, hi = cx + kr;
-                const int b = __ldg(cs + row + (lo < 0 ? 0 : lo)), e = __ldg(cs + row + (hi >= ncx ? ncx : hi + 1));
+                const int b = LD::i32(cs + row + (lo < 0 ? 0 : lo)), e = LD::i32(cs + row + (hi >= ncx ? ncx : hi + 1));
                 tcand += e - b;
-                if (fl) scan_run<HALF, true, EXCL>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m, idv, mol);
-                else scan_run<HALF, false, EXCL>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m, idv, mol);
+                if (fl) scan_run<HALF, true, EXCL, LD>(P, pos, ri, i, b, e, 0.0, sy, sz, fl, m, idv, mol);
+                else scan_run<HALF, false, EXCL, LD>(P, pos, ri, i, b, e, 0.0, 0.0, 0.0, 0u, m, idv, mol);
                 // the part of the window beyond a periodic x face: the cells at the other end of the row, shifted by +-L
-                if (lo < 0) scan_run<HALF, true, EXCL>(P, pos, ri, i, __ldg(cs + row + ncx + lo), __ldg(cs + row + ncx), L, sy, sz, fl | 1u, m, idv, mol);
-                if (hi >= ncx) scan_run<HALF, true, EXCL>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m, idv, mol);
+                if (lo < 0) scan_run<HALF, true, EXCL, LD>(P, pos, ri, i, LD::i32(cs + row + ncx + lo), LD::i32(cs + row + ncx), L, sy, sz, fl | 1u, m, idv, mol);
+                if (hi >= ncx) scan_run<HALF, true, EXCL, LD>(P, pos, ri, i, LD::i32(cs + row), LD::i32(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m, idv, mol);
             }
         }
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
@@ -405,6 +452,13 @@ __global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
         atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
         atomicAdd(&P.ctrl->cand_total, (unsigned long long)sc);
     }
+}
+
+template <bool HALF, bool EXCL>
+__global__ void __launch_bounds__(128) k_build(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    build_body<HALF, EXCL, LdNC>(P, bufs_from_ctrl(P));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -653,7 +707,7 @@ __device__ __noinline__ void dihedral_force(const MdDev &P, const pos_t *__restr
 }
 
 // EXTRAS: the angle / dihedral code is compiled in (kernels instantiated without it keep the registers of the FENE-only path)
-template <bool CHECK, bool EXTRAS = true>
+template <bool CHECK, bool EXTRAS = true, class LD = LdNC>
 __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i, PairAcc &a)
 {
     if (EXTRAS && P.has_angles) angle_force(P, pos, ri, i, a);
@@ -662,7 +716,7 @@ __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restri
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
         if (j < 0) continue;
-        const pos_t rj = ld_pos(pos + j);
+        const pos_t rj = LD::pos(pos + j);
         const double dx = minimg(ri.x - rj.x, P.L, P.half_L), dy = minimg(ri.y - rj.y, P.L, P.half_L),
                      dz = minimg(ri.z - rj.z, P.L, P.half_L);
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
@@ -681,7 +735,7 @@ __device__ __forceinline__ void bond_force(const MdDev &P, const pos_t *__restri
 #ifndef MD_FORCE_D
 #define MD_FORCE_D 8
 #endif
-template <int U, int D>
+template <int U, int D, class LD = LdNC>
 __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__restrict__ pos, const pos_t &ri, int i)
 {
     static_assert(D % U == 0, "D must be a multiple of U");
@@ -702,7 +756,7 @@ __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__r
                 pos_t rj[U];
 #pragma unroll
                 for (int u = 0; u < U; u++)
-                    if (base + g + u < m) rj[u] = ld_pos(pos + (cur[g + u] & W_INDEX_MASK));
+                    if (base + g + u < m) rj[u] = LD::pos(pos + (cur[g + u] & W_INDEX_MASK));
 #pragma unroll
                 for (int u = 0; u < U; u++)
                     if (base + g + u < m) pair_force(P, ri, rj[u], cur[g + u] >> W_FLAG_SHIFT, a);
@@ -722,39 +776,45 @@ __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__r
 // ticket) and sets the IF condition of the step graph, which saves the one-block k_decide launch -- a third
 // of a time step when the whole system is a few dozen blocks.  (For large grids the ticket itself costs more than that
 // launch: ~7.5 ns per block, md_device.cuh.)
+// forces on atom i over column i of W (+ bonds) and the MODE's part of the integration; returns |v|^2 (MODE 1)
+template <int MODE, int BONDS, class LD, int U = MD_FORCE_U, int D = MD_FORCE_D>
+__device__ __forceinline__ double force_atom(const MdDev &P, int pc, int vc, int i)
+{
+    const pos_t *__restrict__ pos = P.pos[pc];
+    double v2 = 0.0;
+    const pos_t ri = LD::pos(pos + i);
+    const size_t np = (size_t)P.N_pad;
+    double *v = P.vel[vc] + i;
+    double v0 = 0.0, v1 = 0.0, v2i = 0.0;
+    if (MODE != 0) { v0 = v[0]; v1 = v[np]; v2i = v[2 * np]; }     // in flight while the column is walked
+    PairAcc a = column_force<U, D, LD>(P, pos, ri, i);
+    if (BONDS == 1) bond_force<true, false, LD>(P, pos, ri, i, a);
+    if (BONDS == 2) bond_force<true, true, LD>(P, pos, ri, i, a);
+    if (MODE == 0 || MODE == 2) {
+        double *f = P.frc + i;
+        f[0] = a.fx; f[np] = a.fy; f[2 * np] = a.fz;
+    }
+    if (MODE == 2) {
+        v[0] = v0 + P.hdt * a.fx; v[np] = v1 + P.hdt * a.fy; v[2 * np] = v2i + P.hdt * a.fz;
+    }
+    if (MODE == 1) {
+        const double vx = v0 + P.dt * a.fx, vy = v1 + P.dt * a.fy, vz = v2i + P.dt * a.fz;
+        v[0] = vx; v[np] = vy; v[2 * np] = vz;
+        const double x = ri.x + P.dt * vx, y = ri.y + P.dt * vy, z = ri.z + P.dt * vz;
+        st_pos(P.pos[pc ^ 1] + i, x, y, z);
+        v2 = vx * vx + vy * vy + vz * vz;
+        if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
+    }
+    return v2;
+}
+
 template <int MODE, int BONDS, int BLOCK, bool DECIDE = false>
 __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(const __grid_constant__ MdDev P, cudaGraphConditionalHandle cond)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * BLOCK + threadIdx.x;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
-    const pos_t *__restrict__ pos = P.pos[pc];
-    double v2 = 0.0;
-    if (i < P.N) {
-        const pos_t ri = ld_pos(pos + i);
-        const size_t np = (size_t)P.N_pad;
-        double *v = P.vel[vc] + i;
-        double v0 = 0.0, v1 = 0.0, v2i = 0.0;
-        if (MODE != 0) { v0 = v[0]; v1 = v[np]; v2i = v[2 * np]; }     // in flight while the column is walked
-        PairAcc a = column_force<MD_FORCE_U, MD_FORCE_D>(P, pos, ri, i);
-        if (BONDS == 1) bond_force<true, false>(P, pos, ri, i, a);
-        if (BONDS == 2) bond_force<true, true>(P, pos, ri, i, a);
-        if (MODE == 0 || MODE == 2) {
-            double *f = P.frc + i;
-            f[0] = a.fx; f[np] = a.fy; f[2 * np] = a.fz;
-        }
-        if (MODE == 2) {
-            v[0] = v0 + P.hdt * a.fx; v[np] = v1 + P.hdt * a.fy; v[2 * np] = v2i + P.hdt * a.fz;
-        }
-        if (MODE == 1) {
-            const double vx = v0 + P.dt * a.fx, vy = v1 + P.dt * a.fy, vz = v2i + P.dt * a.fz;
-            v[0] = vx; v[np] = vy; v[2 * np] = vz;
-            const double x = ri.x + P.dt * vx, y = ri.y + P.dt * vy, z = ri.z + P.dt * vz;
-            st_pos(P.pos[pc ^ 1] + i, x, y, z);
-            v2 = vx * vx + vy * vy + vz * vz;
-            if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
-        }
-    }
+    const double v2 = i < P.N ? force_atom<MODE, BONDS, LdNC>(P, pc, vc, i) : 0.0;
     if (MODE == 1) {
         const double bm = block_max(v2, sm);
         if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
@@ -917,6 +977,78 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
     reduce_finish(P, q, S, blockIdx.x, gridDim.x);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Small systems: ALL n time steps of md_step in ONE cooperative launch.  A system of a few thousand atoms is a few
+// dozen thread blocks: its step is not limited by memory or arithmetic but by kernel launches and by the conditional
+// node of the step graph (wca_4k: 20 us per step for ~5 us of kernel work).  Here the blocks stay resident and meet at
+// grid-wide barriers instead: per step the fused force + kick + drift of every atom, a barrier, the rebuild decision by
+// block 0 (decide(), as k_decide takes it), a barrier; and, when the decision says so, the rebuild chain -- the bodies of
+// k_bin, k_scan_*, k_place, k_reorder, k_bonds_remap and k_build, a barrier after each.  The arrays those phases rewrite
+// are read with ordinary coherent loads (LdPlain), never through the read-only path.  Same arithmetic, same order of
+// operations per atom as the graph path with MD_FLAG_GLOBAL_W: results are bitwise equal to it.
+// fp64, global-index W (gathering build), variant A, fused steps, at most FENE bonds.
+// ------------------------------------------------------------------------------------------------
+namespace cg = cooperative_groups;
+constexpr int PERSIST_T = SCAN_T;      // 256 threads: the scan tiles need exactly SCAN_T
+
+#ifndef MD_PERSIST_U
+#define MD_PERSIST_U 4             // gathers in flight per thread: the phase is one latency chain per atom, not a bandwidth problem
+#endif
+template <int BONDS>
+__global__ void __launch_bounds__(PERSIST_T) k_persist(const __grid_constant__ MdDev P, long long n_steps)
+{
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double sm[33];
+    const int nblk = gridDim.x, tid = threadIdx.x;
+    const int stride = nblk * PERSIST_T, first = blockIdx.x * PERSIST_T + tid;
+    // Every thread keeps its own copy of the decision scalars and evaluates decide_state() on the same inputs, so no
+    // second barrier is needed to publish the decision; block 0 mirrors it into the control block for the host.
+    DecState c = dec_load(P);
+    for (long long step = 0; step < n_steps; step++) {
+        // ---- drifting phase: opening half kick + drift (first step), else forces + full kick + drift ----
+        double v2 = 0.0;
+        for (int i = first; i < P.N; i += stride)
+            v2 = fmax(v2, step == 0 ? kick_drift_atom(P, c.p_dst, c.v_dst, i)
+                                    : force_atom<1, BONDS, LdPlain, MD_PERSIST_U, 8>(P, c.p_dst, c.v_dst, i));
+        const double bm = block_max(v2, sm);
+        double *vmax_buf = P.blk_vmax2 + (step & 1) * nblk;       // double-buffered: a fast block may already be in the next step
+        if (tid == 0) vmax_buf[blockIdx.x] = bm;
+        grid.sync();
+        // ---- the rebuild decision, replicated in every block ----
+        double m = 0.0;
+        for (int b = tid; b < nblk; b += PERSIST_T) m = fmax(m, __ldcg(vmax_buf + b));
+        __syncthreads();
+        m = block_max(m, sm);
+        if (tid == 0) sm[32] = m;
+        __syncthreads();
+        decide_state(P, c, sm[32], step != 0);
+        if (blockIdx.x == 0 && tid == 0) dec_store(P, c);
+        if (c.need_rebuild) {
+            const Bufs B = {c.p_src, c.p_dst, c.v_src, c.v_dst};
+            bin_body<LdPlain>(P, B);
+            grid.sync();
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_reduce_tile(P, t); __syncthreads(); }
+            grid.sync();
+            if (blockIdx.x == 0 && tid == 0) {          // exclusive scan of the (few) tile sums
+                int run = 0;
+                for (int t = 0; t < P.scan_blocks; t++) { const int v = P.block_sums[t]; P.block_sums[t] = run; run += v; }
+            }
+            grid.sync();
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile(P, t); __syncthreads(); }
+            grid.sync();
+            place_body(P);
+            grid.sync();
+            reorder_body<LdPlain>(P, B);
+            grid.sync();
+            if (BONDS) { bonds_remap_body(P, B); grid.sync(); }
+            build_body<false, false, LdPlain>(P, B);
+            grid.sync();
+        }
+    }
+    // ---- closing: forces at the final positions + half kick ----
+    for (int i = first; i < P.N; i += stride) force_atom<2, BONDS, LdPlain, MD_PERSIST_U, 8>(P, c.p_dst, c.v_dst, i);
+}
+
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
 // grid of the rebuild kernels: at most one full wave of the device's SMs; they use grid-stride loops
@@ -1056,6 +1188,35 @@ void mdk_energy(const MdDev &P, const MdLaunch &, cudaStream_t st)
     const int grid = cdiv(P.N, 256);
     if (P.has_bonds) k_energy<true><<<grid, 256, 0, st>>>(P);
     else k_energy<false><<<grid, 256, 0, st>>>(P);
+}
+
+// ---- the persistent small-system kernel ----
+static int persist_grid(const MdDev &P)
+{
+    int per_sm = 0;
+    const void *k = P.has_bonds ? (const void *)k_persist<1> : (const void *)k_persist<0>;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return 0; }
+    const int want = cdiv(P.N, PERSIST_T);
+    return want <= per_sm * P.sm_count ? want : 0;       // every atom its own thread, all blocks resident at once
+}
+
+bool mdk_persist_ok(const MdDev &P)
+{
+    if (P.sp || P.tiled || P.half_list || P.layer_H || P.rigid || P.has_angles || P.has_dihedrals || P.w_col != 1) return false;
+    if (P.N > 32768) return false;                        // beyond that the graph path's tile-staged build is the faster one
+    int dev = 0, coop = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) { cudaGetLastError(); return false; }
+    return persist_grid(P) > 0;
+}
+
+int mdk_persist_steps(const MdDev &P, long long n, cudaStream_t st)
+{
+    const int grid = persist_grid(P);
+    if (grid <= 0) return -1;
+    MdDev Pc = P;
+    void *args[] = {(void *)&Pc, (void *)&n};
+    const void *k = P.has_bonds ? (const void *)k_persist<1> : (const void *)k_persist<0>;
+    return cudaLaunchCooperativeKernel(k, dim3(grid), dim3(PERSIST_T), args, 0, st) == cudaSuccess ? 0 : -1;
 }
 
 int mdk_launches_of(int which)

@@ -218,6 +218,9 @@ void mdk_po_kick_drift(const MdDev &P, double rcap2, double vlim2, double ke_tar
 void mdk_po_force(const MdDev &P, double rcap2, cudaStream_t st);
 void mdk_po_kick(const MdDev &P, cudaStream_t st);                             // + kinetic energy -> ctrl->red[RED_KE]
 void mdk_po_check(const MdDev &P, unsigned long long *out, cudaStream_t st);  // out[0] min non-bonded r^2, out[1] max bond r^2 (bit patterns)
+// small systems: all n steps of md_step in one cooperative launch (md_kernels.cu: k_persist); 0 = launched
+bool mdk_persist_ok(const MdDev &P);
+int mdk_persist_steps(const MdDev &P, long long n, cudaStream_t st);
 // rigid molecules (md_rigid.cu)
 int mdk_rigid_blocks(const MdDev &P);                                          // blocks of k_rigid_kick_drift (entries of blk_vmax2)
 void mdk_rigid_kick_drift(const MdDev &P, cudaStream_t st);

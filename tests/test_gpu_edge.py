@@ -113,7 +113,7 @@ def test_graph_and_direct_launch_agree_bitwise(md):
     cfg = get_config("wca_4k")
     r, v, _, box = make_state(cfg, 4, jitter_amp=0.05)
     out = []
-    for flags in (0, md.FLAG_NO_GRAPH, md.FLAG_TILED_W, md.FLAG_TILED_W | md.FLAG_NO_GRAPH):
+    for flags in (md.FLAG_NO_PERSIST, md.FLAG_NO_GRAPH, md.FLAG_TILED_W, md.FLAG_TILED_W | md.FLAG_NO_GRAPH):
         g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags)
         g.set_state(r, v)
         g.step(150)
@@ -197,3 +197,41 @@ def test_set_state_rejects_out_of_range_coordinates_and_keeps_the_old_state(md, 
     g.set_state(edge, v)
     assert g.positions()[0, 0] == 0.0
     g.close()
+
+
+@pytest.mark.parametrize("case", ["wca_4k", "ragged_1000", "chains", "batch"])
+def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
+    """Small systems run md_step as ONE cooperative launch (k_persist: blocks resident over all steps, grid-wide barriers,
+    the bodies of the same kernels).  With the same W build (the gathering kernel, MD_FLAG_GLOBAL_W) the step graph must
+    give bit-identical states, energies and rebuild counts -- across many rebuilds, in one call or several."""
+    n_sys = 1
+    if case == "wca_4k":
+        cfg = get_config("wca_4k")
+    elif case == "ragged_1000":
+        cfg = scaled_config("wca_4k", 1000)
+    elif case == "chains":
+        cfg = scaled_config("chains_rows_1m", 4096, chain_len=16)
+    else:
+        cfg, n_sys = scaled_config("wca_4k", 1728), 3
+    states = [make_state(cfg, 4 + b, jitter_amp=0.05 if cfg.lattice == "sc" else 0.0) for b in range(n_sys)]
+    box = states[0][3]
+    r, v = np.concatenate([s[0] for s in states]), np.concatenate([s[1] for s in states])
+    bonds = None if states[0][2] is None else np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)])
+    out = []
+    for flags in (0, md.FLAG_GLOBAL_W):
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags, n_systems=n_sys)
+        g.set_state(r, v)
+        if bonds is not None:
+            g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
+        assert g.info()["use_graph"] == (2 if flags == 0 else 0)     # the graph is built at the first md_step
+        g.step(150)
+        g.step(1)
+        g.step(37)
+        e = g.energies()
+        assert g.info()["use_graph"] == (2 if flags == 0 else 1)
+        out.append((g.positions(), g.velocities(), g.forces(), e.n_rebuilds, e.ke, e.pe, g.info()["kernel_launches"]))
+        g.close()
+    a, b = out
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    assert a[3] == b[3] > 10 and a[4] == b[4] and a[5] == b[5]
+    assert a[6] < b[6] // 10                      # three launches for the three md_step calls, plus set-up and read-out
