@@ -48,12 +48,13 @@ def load_ncu_traffic(kernel_key):
     path = os.path.join(ROOT, "profiles", "roofline_traffic.txt")
     if not os.path.exists(path):
         return None
+    found = None
     with open(path) as fh:
         for line in fh:
             line = line.split("#", 1)[0].strip()
             if line.startswith(kernel_key + " "):
-                return float(line.rsplit(None, 1)[1])
-    return None
+                found = float(line.rsplit(None, 1)[1])       # the last line for a key is the latest pass
+    return found
 
 
 class ClockSampler:
