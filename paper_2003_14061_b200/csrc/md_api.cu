@@ -188,10 +188,11 @@ void enqueue_rebuild(md_system *s)
     { Timed t(s, MD_T_NEBR, s->P.layer_H ? 2 : 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
-void enqueue_force(md_system *s, int mode)
+void enqueue_force(md_system *s, int mode, const MdDev *Pover = nullptr)
 {
-    if (s->P.tiled) mdk_tile_force(s->P, mode, s->stream);
-    else mdk_force(s->P, s->lc, mode, s->stream);
+    const MdDev &P = Pover ? *Pover : s->P;
+    if (P.tiled) mdk_tile_force(P, mode, s->stream);
+    else mdk_force(P, s->lc, mode, s->stream);
 }
 
 // rebuild decision after a drifting kernel; cond: conditional handle of the step graph or 0
@@ -217,6 +218,7 @@ void drop_graph(md_system *s)
 // rebuild so launches 2 kernels instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision
 // on the host every step).  Returns false (and leaves no graph) if any step of the construction is refused;
 // md_step then launches the kernels one by one.
+constexpr int DEC_GROUP_HOST = 128;  // = DEC_GROUP of md_device.cuh
 constexpr int GRAPH_UNROLL = 8;     // fused steps per launch of graph[2]: amortises the per-launch cost of a graph (small systems)
 
 bool build_step_graph(md_system *s, int kind)
@@ -225,7 +227,10 @@ bool build_step_graph(md_system *s, int kind)
     if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
     const int reps = kind == 2 ? GRAPH_UNROLL : 1;
     const bool fused = kind >= 1;
-    const bool in_kernel_decision = fused && mdk_force_decides(s->P, s->lc);
+    // Small grids: the fused step takes the rebuild decision itself (block_decides) and k_decide is not launched.  For large
+    // grids that was measured slower (wca_2m: 0.206 vs 0.194 ms per step, lj_1m 0.326 vs 0.314): the fence + counter at the
+    // tail of each of the 16,384 blocks costs more than the 8 us of the one-block k_decide launch it saves.
+    const bool in_kernel_decision = fused && mdk_drift_blocks(s->P, s->lc, true) <= 4 * DEC_GROUP_HOST;
     cudaGraph_t g = nullptr;
     bool capturing = false, ok = false;
     do {
@@ -240,8 +245,12 @@ bool build_step_graph(md_system *s, int kind)
             if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
             cudaGraphConditionalHandle h;
             if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-            if (in_kernel_decision) mdk_force_fused_decide(s->P, s->lc, st, (unsigned long long)h);
-            else {
+            if (in_kernel_decision) {
+                MdDev Pd = s->P;
+                Pd.decide_in_kernel = 1;
+                Pd.decide_cond = (unsigned long long)h;
+                enqueue_force(s, 1, &Pd);
+            } else {
                 if (fused) enqueue_force(s, 1);
                 else mdk_kick_drift(s->P, s->lc, st);
                 mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused), fused, st, (unsigned long long)h);
@@ -687,6 +696,8 @@ md_system *md_create_ex(const md_params *pp)
     if (P.layer_H) P.H = (int *)A((size_t)P.NC * P.n_layers * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
     P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
+    P.dec_tickets = (unsigned int *)A(((size_t)P.max_grid / DEC_GROUP_HOST + 2) * sizeof(unsigned int));
+    P.grp_vmax2 = (double *)A(((size_t)P.max_grid / DEC_GROUP_HOST + 2) * sizeof(double));
     if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));

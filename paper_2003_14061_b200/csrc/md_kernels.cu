@@ -772,10 +772,6 @@ __device__ __forceinline__ PairAcc column_force(const MdDev &P, const pos_t *__r
 // MODE 0: store f.  MODE 1: fused leapfrog step: v += dt f, r' = r + dt v into the other position
 // buffer, max |v|, rebuild decision.  MODE 2: store f and apply the closing half kick v += dt/2 f.
 // BONDS: 0 none, 1 FENE bonds, 2 FENE + angle / dihedral terms
-// DECIDE (MODE 1, small grids): the last block to finish also takes the rebuild decision (the paper's "last block done"
-// ticket) and sets the IF condition of the step graph, which saves the one-block k_decide launch -- a third
-// of a time step when the whole system is a few dozen blocks.  (For large grids the ticket itself costs more than that
-// launch: ~7.5 ns per block, md_device.cuh.)
 // forces on atom i over column i of W (+ bonds) and the MODE's part of the integration; returns |v|^2 (MODE 1)
 template <int MODE, int BONDS, class LD, int U = MD_FORCE_U, int D = MD_FORCE_D>
 __device__ __forceinline__ double force_atom(const MdDev &P, int pc, int vc, int i)
@@ -808,8 +804,9 @@ __device__ __forceinline__ double force_atom(const MdDev &P, int pc, int vc, int
     return v2;
 }
 
-template <int MODE, int BONDS, int BLOCK, bool DECIDE = false>
-__global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(const __grid_constant__ MdDev P, cudaGraphConditionalHandle cond)
+// In the step graph the kernel also takes the rebuild decision (P.decide_in_kernel; md_device.cuh: block_decides).
+template <int MODE, int BONDS, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * BLOCK + threadIdx.x;
@@ -817,25 +814,8 @@ __global__ void __launch_bounds__(BLOCK, MD_FORCE_MIN_THREADS / BLOCK) k_force(c
     const double v2 = i < P.N ? force_atom<MODE, BONDS, LdNC>(P, pc, vc, i) : 0.0;
     if (MODE == 1) {
         const double bm = block_max(v2, sm);
-        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
-        if (DECIDE) {
-            __shared__ bool last;
-            if (threadIdx.x == 0) {
-                __threadfence();
-                last = atomicInc(&P.ctrl->ticket[TK_FORCE], gridDim.x - 1) == gridDim.x - 1;
-            }
-            __syncthreads();
-            if (last) {
-                __threadfence();
-                double m = 0.0;
-                for (int b = threadIdx.x; b < (int)gridDim.x; b += BLOCK) m = fmax(m, __ldcg(P.blk_vmax2 + b));
-                m = block_max(m, sm);
-                if (threadIdx.x == 0) {
-                    decide(P, m, true);
-                    if (cond) cudaGraphSetConditional(cond, (unsigned)P.ctrl->need_rebuild);
-                }
-            }
-        }
+        if (P.decide_in_kernel) block_decides(P, bm, blockIdx.x, gridDim.x, sm);
+        else if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 
@@ -1127,14 +1107,14 @@ void mdk_build(const MdDev &P, const MdLaunch &, cudaStream_t st)
     else k_build<false, false><<<capped_grid(P, P.N, 128, 16), 128, 0, st>>>(P);
 }
 
-template <int MODE, int BONDS, bool DECIDE = false>
-static void launch_force_block(const MdDev &P, int block, cudaStream_t st, cudaGraphConditionalHandle cond = 0)
+template <int MODE, int BONDS>
+static void launch_force_block(const MdDev &P, int block, cudaStream_t st)
 {
     switch (block) {
-    case 64: k_force<MODE, BONDS, 64, DECIDE><<<cdiv(P.N, 64), 64, 0, st>>>(P, cond); break;
-    case 128: k_force<MODE, BONDS, 128, DECIDE><<<cdiv(P.N, 128), 128, 0, st>>>(P, cond); break;
-    case 512: k_force<MODE, BONDS, 512, DECIDE><<<cdiv(P.N, 512), 512, 0, st>>>(P, cond); break;
-    default: k_force<MODE, BONDS, 256, DECIDE><<<cdiv(P.N, 256), 256, 0, st>>>(P, cond); break;
+    case 64: k_force<MODE, BONDS, 64><<<cdiv(P.N, 64), 64, 0, st>>>(P); break;
+    case 128: k_force<MODE, BONDS, 128><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
+    case 512: k_force<MODE, BONDS, 512><<<cdiv(P.N, 512), 512, 0, st>>>(P); break;
+    default: k_force<MODE, BONDS, 256><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
     }
 }
 
@@ -1154,18 +1134,6 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
         else if (mode == 1) launch_force_block<1, 0>(P, lc.block, st);
         else launch_force_block<2, 0>(P, lc.block, st);
     }
-}
-
-// the fused step with the rebuild decision taken by its last block (small grids, inside the step graph)
-bool mdk_force_decides(const MdDev &P, const MdLaunch &lc)
-{
-    return !P.sp && !P.tiled && !(P.has_angles || P.has_dihedrals) && cdiv(P.N, lc.block) <= 512;
-}
-
-void mdk_force_fused_decide(const MdDev &P, const MdLaunch &lc, cudaStream_t st, unsigned long long cond)
-{
-    if (P.has_bonds) launch_force_block<1, 1, true>(P, lc.block, st, (cudaGraphConditionalHandle)cond);
-    else launch_force_block<1, 0, true>(P, lc.block, st, (cudaGraphConditionalHandle)cond);
 }
 
 // number of blocks (= entries of blk_vmax2) the drifting kernels write: input size of k_decide

@@ -499,7 +499,8 @@ __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(c
     }
     if (MODE == 1) {
         const double bm = block_max((double)v2, sm);
-        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (P.decide_in_kernel) block_decides(P, bm, blockIdx.x, gridDim.x, sm);
+        else if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 

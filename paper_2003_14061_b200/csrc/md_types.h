@@ -153,6 +153,12 @@ struct MdDev {
                                         // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)
     double *blk_vmax2;                  // max_grid per-block maxima of v^2 from the drifting kernel (input of k_decide)
+    // rebuild decision taken by the drifting kernel itself (step graph; md_device.cuh: block_decides): the blocks count
+    // themselves off in groups of DEC_GROUP, the last block of a group reduces the group, the last group reduces all
+    int decide_in_kernel;
+    unsigned long long decide_cond;     // cudaGraphConditionalHandle of the IF node that holds the rebuild chain
+    unsigned int *dec_tickets;          // [0]: groups done; [1 + g]: blocks of group g done
+    double *grp_vmax2;                  // per-group maxima
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
@@ -192,8 +198,6 @@ void mdk_build(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          //
 // mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, per-block max v^2; follow with mdk_decide); 2: f and closing half kick
 void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
 int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   // blocks writing blk_vmax2
-bool mdk_force_decides(const MdDev &P, const MdLaunch &lc);                   // small grid: the fused step can take the rebuild decision itself
-void mdk_force_fused_decide(const MdDev &P, const MdLaunch &lc, cudaStream_t st, unsigned long long cond);   // fused step + decision + IF condition
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
