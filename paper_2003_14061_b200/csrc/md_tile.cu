@@ -719,7 +719,6 @@ size_t mdk_tile_smem(const MdDev &P, bool with_cells)
 
 namespace {
 
-inline int tile_grid(const MdDev &P) { return P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys; }
 inline dim3 tile_grid3(const MdDev &P) { return dim3(P.tg.nsx, P.tg.nsy, P.tg.nsz * P.tg.nsys); }
 
 // The attribute belongs to the kernel, not to one md_system: opt in to the device maximum, so that systems with

@@ -235,3 +235,36 @@ def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
     assert a[3] == b[3] > 10 and a[4] == b[4] and a[5] == b[5]
     assert a[6] < b[6] // 10                      # three launches for the three md_step calls, plus set-up and read-out
+
+
+def test_bond_list_validation_and_allocators_side_by_side(md):
+    """md_set_bonds rejects a bond between two independent systems and a pair listed twice (either order); systems created
+    under different allocator hooks coexist and free their memory the way it was allocated."""
+    cfg = scaled_config("chains_rows_1m", 1024, chain_len=16)
+    r, v, bonds, box = make_state(cfg, 1)
+    n = cfg.n_atoms
+    g = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", n_systems=2)
+    g.set_state(np.concatenate([r, r]), np.concatenate([v, v]))
+    with pytest.raises(md.MDError) as ei:
+        g.set_bonds(np.array([[3, n + 3]], np.int32), cfg.fene_k, cfg.fene_r0)          # atoms of two mutually invisible systems
+    assert ei.value.code == md.binding.MD_ERR_INVALID
+    for dup in ([[0, 1], [0, 1]], [[0, 1], [1, 0]]):
+        with pytest.raises(md.MDError) as ei:
+            g.set_bonds(np.array(dup, np.int32), cfg.fene_k, cfg.fene_r0)
+        assert ei.value.code == md.binding.MD_ERR_INVALID
+    g.set_bonds(np.concatenate([bonds, bonds + n]), cfg.fene_k, cfg.fene_r0)                # the valid list still goes in
+    g.step(5)
+    # one system on cudaMalloc, one on torch's caching allocator, created and destroyed in interleaved order
+    a = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", torch_memory=False)
+    b = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", torch_memory=True)
+    c = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", torch_memory=False)
+    for s in (a, b, c):
+        s.set_state(r, v)
+        s.step(3)
+    a.close()
+    b.step(3)
+    c.step(3)
+    assert np.array_equal(b.positions(), c.positions())
+    b.close()
+    c.close()
+    g.close()
