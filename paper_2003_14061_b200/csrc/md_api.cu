@@ -76,7 +76,6 @@ struct md_system {
     bool graph_tried = false;
     int chain_kernels = 0;         // kernels inside the conditional body
     bool persist = false;          // small system: md_step runs as one cooperative launch
-    int step_kernels = 2;          // kernels of one fused step in the graph (1 when the force kernel takes the rebuild decision)
     int rebuilds_seen = 0;
     int64_t graph_steps = 0;       // steps run through the graph since the last status read         // ctrl->n_rebuilds at the last status read (launch accounting)
     double t_ms[MD_T_COUNT] = {0};
@@ -188,9 +187,9 @@ void enqueue_rebuild(md_system *s)
     { Timed t(s, MD_T_NEBR, s->P.layer_H ? 2 : 1); if (s->P.tile_build) mdk_tile_build(s->P, s->stream); else mdk_build(s->P, s->lc, s->stream); }
 }
 
-void enqueue_force(md_system *s, int mode, const MdDev *Pover = nullptr)
+void enqueue_force(md_system *s, int mode)
 {
-    const MdDev &P = Pover ? *Pover : s->P;
+    const MdDev &P = s->P;
     if (P.tiled) mdk_tile_force(P, mode, s->stream);
     else mdk_force(P, s->lc, mode, s->stream);
 }
@@ -218,7 +217,6 @@ void drop_graph(md_system *s)
 // rebuild so launches 2 kernels instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision
 // on the host every step).  Returns false (and leaves no graph) if any step of the construction is refused;
 // md_step then launches the kernels one by one.
-constexpr int DEC_GROUP_HOST = 128;  // = DEC_GROUP of md_device.cuh
 constexpr int GRAPH_UNROLL = 8;     // fused steps per launch of graph[2]: amortises the per-launch cost of a graph (small systems)
 
 bool build_step_graph(md_system *s, int kind)
@@ -227,10 +225,10 @@ bool build_step_graph(md_system *s, int kind)
     if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
     const int reps = kind == 2 ? GRAPH_UNROLL : 1;
     const bool fused = kind >= 1;
-    // Small grids: the fused step takes the rebuild decision itself (block_decides) and k_decide is not launched.  For large
-    // grids that was measured slower (wca_2m: 0.206 vs 0.194 ms per step, lj_1m 0.326 vs 0.314): the fence + counter at the
-    // tail of each of the 16,384 blocks costs more than the 8 us of the one-block k_decide launch it saves.
-    const bool in_kernel_decision = fused && mdk_drift_blocks(s->P, s->lc, true) <= 4 * DEC_GROUP_HOST;
+    // The rebuild decision is its own one-block kernel (k_decide).  Taking it in the last block of the drifting kernel
+    // (the paper's "last block done"; one or two levels of block counters) was measured slower at every
+    // grid size, 32 to 16,384 blocks (wca_4k 22.1 vs 20.1 us per step, wca_262k 44.6 vs 41.0, wca_2m 206 vs 194): its chain
+    // of fences, atomics and dependent loads at the tail of the kernel is longer than the launch it saves.  DESIGN.md 6f.
     cudaGraph_t g = nullptr;
     bool capturing = false, ok = false;
     do {
@@ -245,16 +243,9 @@ bool build_step_graph(md_system *s, int kind)
             if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess || !g) break;
             cudaGraphConditionalHandle h;
             if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
-            if (in_kernel_decision) {
-                MdDev Pd = s->P;
-                Pd.decide_in_kernel = 1;
-                Pd.decide_cond = (unsigned long long)h;
-                enqueue_force(s, 1, &Pd);
-            } else {
-                if (fused) enqueue_force(s, 1);
-                else mdk_kick_drift(s->P, s->lc, st);
-                mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused), fused, st, (unsigned long long)h);
-            }
+            if (fused) enqueue_force(s, 1);
+            else mdk_kick_drift(s->P, s->lc, st);
+            mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused), fused, st, (unsigned long long)h);
             if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
             cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
             cp.conditional.handle = h;
@@ -287,7 +278,6 @@ bool build_step_graph(md_system *s, int kind)
         return false;
     }
     s->chain_kernels = mdk_launches_of(LK_CELLS) + (s->P.has_bonds ? 2 : 1) + 1 + (s->P.layer_H ? 2 : 0);
-    s->step_kernels = in_kernel_decision ? 1 : 2;
     return true;
 }
 
@@ -696,8 +686,6 @@ md_system *md_create_ex(const md_params *pp)
     if (P.layer_H) P.H = (int *)A((size_t)P.NC * P.n_layers * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
     P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
-    P.dec_tickets = (unsigned int *)A(((size_t)P.max_grid / DEC_GROUP_HOST + 2) * sizeof(unsigned int));
-    P.grp_vmax2 = (double *)A(((size_t)P.max_grid / DEC_GROUP_HOST + 2) * sizeof(double));
     if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
@@ -1126,7 +1114,7 @@ int md_step(md_system *s, int64_t n)
             for (; k + GRAPH_UNROLL <= n; k += GRAPH_UNROLL) CK(cudaGraphLaunch(s->gexec[2], st));
             for (; k < n; k++) CK(cudaGraphLaunch(s->gexec[1], st));
             s->graph_steps += n;
-            s->launches += 2 + (n - 1) * s->step_kernels;   // + the rebuild chains, added in check_device_status
+            s->launches += 2 + (n - 1) * 2;               // + the rebuild chains, added in check_device_status
         } else {
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_kick_drift(P, s->lc, st); }
             enqueue_decide(s, false);

@@ -244,47 +244,6 @@ __device__ __forceinline__ void decide(const MdDev &P, double vmax2, bool pos_pi
     dec_store(P, c);
 }
 
-// The rebuild decision inside the drifting kernel (the paper's "last block done"), in two levels.  One
-// counter for all blocks costs ~7.5 ns per block on B200 (same-address L2 atomics: 120 us for the 16,384 blocks of
-// N = 2M, round 1); with the blocks counted off in groups of DEC_GROUP no counter sees more than DEC_GROUP increments
-// (or the number of groups) and the groups count in parallel.  Used by the step graph for grids of <= 512 blocks, where the
-// one-block k_decide launch it replaces is a third of a step; at N = 2M (16,384 blocks) it was measured SLOWER than that
-// launch (0.206 vs 0.194 ms per step): every block then ends with a fence and an atomic before it can retire.
-// bm: the block's maximum of v^2, valid in thread 0.  All threads of the block call it.  sm: >= 32 doubles.
-constexpr int DEC_GROUP = 128;
-__device__ __forceinline__ void block_decides(const MdDev &P, double bm, int bid, int nblk, double *sm)
-{
-    __shared__ int s_role;
-    const int g = bid / DEC_GROUP, ng = (nblk + DEC_GROUP - 1) / DEC_GROUP;
-    const int gsize = min(DEC_GROUP, nblk - g * DEC_GROUP);
-    if (threadIdx.x == 0) {
-        P.blk_vmax2[bid] = bm;
-        __threadfence();
-        s_role = atomicInc(P.dec_tickets + 1 + g, gsize - 1) == (unsigned)(gsize - 1) ? 1 : 0;
-    }
-    __syncthreads();
-    if (s_role == 0) return;
-    __threadfence();                                    // last block of its group: the group's maximum
-    double m = 0.0;
-    for (int b = threadIdx.x; b < gsize; b += blockDim.x) m = fmax(m, __ldcg(P.blk_vmax2 + g * DEC_GROUP + b));
-    m = block_max(m, sm);
-    if (threadIdx.x == 0) {
-        P.grp_vmax2[g] = m;
-        __threadfence();
-        s_role = atomicInc(P.dec_tickets, ng - 1) == (unsigned)(ng - 1) ? 2 : 1;
-    }
-    __syncthreads();
-    if (s_role != 2) return;
-    __threadfence();                                    // last group: the maximum of all, and the decision
-    m = 0.0;
-    for (int b = threadIdx.x; b < ng; b += blockDim.x) m = fmax(m, __ldcg(P.grp_vmax2 + b));
-    m = block_max(m, sm);
-    if (threadIdx.x == 0) {
-        decide(P, m, true);
-        if (P.decide_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)P.decide_cond, (unsigned)P.ctrl->need_rebuild);
-    }
-}
-
 __device__ __forceinline__ void set_err(const MdDev &P, int code) { atomicCAS(&P.ctrl->err, 0, code); }
 
 // F2 and the other global sums: warp shuffles -> shared memory -> one partial per block

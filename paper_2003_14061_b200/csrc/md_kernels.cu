@@ -809,7 +809,6 @@ __device__ __forceinline__ double force_atom(const MdDev &P, int pc, int vc, int
     return v2;
 }
 
-// In the step graph the kernel also takes the rebuild decision (P.decide_in_kernel; md_device.cuh: block_decides).
 template <int MODE, int BONDS, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, force_min_threads(BONDS) / BLOCK) k_force(const __grid_constant__ MdDev P)
 {
@@ -820,8 +819,7 @@ __global__ void __launch_bounds__(BLOCK, force_min_threads(BONDS) / BLOCK) k_for
     const double v2 = i < P.N ? force_atom<MODE, BONDS, LdNC, MD_FORCE_U, D>(P, pc, vc, i) : 0.0;
     if (MODE == 1) {
         const double bm = block_max(v2, sm);
-        if (P.decide_in_kernel) block_decides(P, bm, blockIdx.x, gridDim.x, sm);
-        else if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 

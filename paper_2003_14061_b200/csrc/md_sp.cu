@@ -467,9 +467,7 @@ __device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 
 #define MD_SP_MIN_THREADS 1280       // resident threads per SM the register allocation must allow
 #endif
 // BONDS: 0 none, 1 FENE bonds, 2 FENE + angle / dihedral terms
-// DECIDE: the kernel also takes the rebuild decision (small grids).  A template parameter, not a run-time branch on
-// P.decide_in_kernel: the mere presence of the decision code cost the 16,384-block launches of wca_2m 7 % (0.0729 -> 0.0783 ms).
-template <int MODE, int BONDS, int BLOCK, bool PADDED, bool DECIDE>
+template <int MODE, int BONDS, int BLOCK, bool PADDED>
 __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
@@ -501,8 +499,7 @@ __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(c
     }
     if (MODE == 1) {
         const double bm = block_max((double)v2, sm);
-        if (DECIDE) block_decides(P, bm, blockIdx.x, gridDim.x, sm);
-        else if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
 }
 
@@ -587,22 +584,15 @@ __global__ void __launch_bounds__(256) k_sp_energy(const __grid_constant__ MdDev
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 inline int capped_grid(const MdDev &P, long long n, int block, int per_sm) { return std::min(cdiv(n, block), P.sm_count * per_sm); }
 
-template <int MODE, int BONDS, bool PADDED, bool DECIDE>
-void launch_sp_force_d(const MdDev &P, int block, cudaStream_t st)
-{
-    switch (block) {
-    case 64: k_sp_force<MODE, BONDS, 64, PADDED, DECIDE><<<cdiv(P.N, 64), 64, 0, st>>>(P); break;
-    case 256: k_sp_force<MODE, BONDS, 256, PADDED, DECIDE><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
-    case 512: k_sp_force<MODE, BONDS, 512, PADDED, DECIDE><<<cdiv(P.N, 512), 512, 0, st>>>(P); break;
-    default: k_sp_force<MODE, BONDS, 128, PADDED, DECIDE><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
-    }
-}
-
 template <int MODE, int BONDS, bool PADDED>
 void launch_sp_force_p(const MdDev &P, int block, cudaStream_t st)
 {
-    if (MODE == 1 && P.decide_in_kernel) launch_sp_force_d<MODE, BONDS, PADDED, MODE == 1>(P, block, st);
-    else launch_sp_force_d<MODE, BONDS, PADDED, false>(P, block, st);
+    switch (block) {
+    case 64: k_sp_force<MODE, BONDS, 64, PADDED><<<cdiv(P.N, 64), 64, 0, st>>>(P); break;
+    case 256: k_sp_force<MODE, BONDS, 256, PADDED><<<cdiv(P.N, 256), 256, 0, st>>>(P); break;
+    case 512: k_sp_force<MODE, BONDS, 512, PADDED><<<cdiv(P.N, 512), 512, 0, st>>>(P); break;
+    default: k_sp_force<MODE, BONDS, 128, PADDED><<<cdiv(P.N, 128), 128, 0, st>>>(P); break;
+    }
 }
 
 template <int MODE, int BONDS>

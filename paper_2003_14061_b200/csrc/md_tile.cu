@@ -660,8 +660,7 @@ __global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_f
     }
     if (MODE == 1) {
         const double bm = block_max(vm2, red);
-        if (P.decide_in_kernel) block_decides(P, bm, bid, (int)(gridDim.x * gridDim.y * gridDim.z), red);
-        else if (threadIdx.x == 0) P.blk_vmax2[bid] = bm;
+        if (threadIdx.x == 0) P.blk_vmax2[bid] = bm;
     }
 }
 

@@ -153,12 +153,6 @@ struct MdDev {
                                         // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)
     double *blk_vmax2;                  // max_grid per-block maxima of v^2 from the drifting kernel (input of k_decide)
-    // rebuild decision taken by the drifting kernel itself (step graph; md_device.cuh: block_decides): the blocks count
-    // themselves off in groups of DEC_GROUP, the last block of a group reduces the group, the last group reduces all
-    int decide_in_kernel;
-    unsigned long long decide_cond;     // cudaGraphConditionalHandle of the IF node that holds the rebuild chain
-    unsigned int *dec_tickets;          // [0]: groups done; [1 + g]: blocks of group g done
-    double *grp_vmax2;                  // per-group maxima
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
