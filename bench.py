@@ -364,6 +364,11 @@ def measure_gpu(args, cfg, ctx, with_e2e):
                  "steps_per_rebuild": prof_steps / max(1, rebuilds_prof)}
 
     # ---- end to end through the C ABI with HOST buffers: H2D state, one step, D2H state + energies ------------------
+    # Every step uploads a full state (positions + velocities, page-locked host arrays), installs it (range check, bin,
+    # W build, forces), advances it one step, reads the energies and downloads the full state.  `value`: the service
+    # loop over three independent host-resident trajectories with the library's pipelined I/O calls (upload of the next
+    # state, step of the current one and download of the previous one overlap; pipeline fill and drain are inside the
+    # timed region).  `serial_value`: one trajectory fed back through the host with the blocking calls, nothing overlaps.
     e2e = None
     if with_e2e:
         def pinned(shape):                # page-locked host buffers: the library copies to / from them directly
@@ -379,12 +384,35 @@ def measure_gpu(args, cfg, ctx, with_e2e):
             g.energies()
             a, b = b, a
         barrier()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, dist, "cuda")
+        dt_serial = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        nt = 3
+        traj = [a, b, pinned((2, n, 3))]
+        traj[2][:] = traj[0]
+        g.stage_state(traj[2][0], traj[2][1]); g.commit_state(); g.state_async(traj[2][0], traj[2][1]); g.wait_io()    # untimed: staging buffers, copy streams
+        ksteps = args.e2e_steps
+        barrier()
+        t0 = time.perf_counter()
+        g.stage_state(traj[0][0], traj[0][1])
+        g.stage_state(traj[1][0], traj[1][1])
+        for it in range(ksteps):
+            k = it % nt
+            g.commit_state()             # the oldest staged state: range check, rebuild, forces
+            g.step(1)
+            g.state_async(traj[k][0], traj[k][1])
+            g.energies()
+            if it + 2 < ksteps:
+                g.wait_io(1)             # the download started one turn ago is complete: that trajectory may go up again
+                g.stage_state(traj[(it + 2) % nt][0], traj[(it + 2) % nt][1])
+        g.wait_io()
+        barrier()
+        dt = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
         # the boundary arrays are binary64 in both precisions
-        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
-               "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": args.e2e_steps,
-               "what": "md_set_state(pinned host r,v) + md_step(1) + md_get_state + md_energies per step"}
+        e2e = {"value": world * n * ksteps / dt, "unit": UNIT, "h2d_bytes_per_step": 2 * 3 * n * 8,
+               "d2h_bytes_per_step": 2 * 3 * n * 8 + 160, "steps": ksteps, "ms_per_step": dt / ksteps * 1e3,
+               "serial_value": world * n * args.e2e_steps / dt_serial, "serial_ms_per_step": dt_serial / args.e2e_steps * 1e3,
+               "what": "per step: md_stage_state(pinned host r,v) + md_commit_state + md_step(1) + md_energies + md_get_state_async, "
+                       "three independent host trajectories in turn, transfers overlapped on the library's copy streams, "
+                       "pipeline fill and drain timed; serial_value: md_set_state + md_step(1) + md_get_state + md_energies, one trajectory"}
     g.close()
     return {"workload": cfg.name, "value": value, "ms": ms, "n": n, "info": info, "info_end": info_end, "launches": int(launches),
             "roofline": roofline, "roofline_neighbor": roofline_neighbor, "e2e": e2e, "clocks": clocks, "wall_s": t_wall,
@@ -427,7 +455,7 @@ def main():
     ap.add_argument("--cell-split", type=int, default=0, help="md_params.cell_split_x: fine cells per r_n along x (0 = auto)")
     ap.add_argument("--tile-threads", type=int, default=0)
     ap.add_argument("--tile-capacity", type=int, default=0)
-    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--e2e-steps", type=int, default=24)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-seconds", type=float, default=75.0, help="--impl reference: budget of one workload's W + K steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")

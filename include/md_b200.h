@@ -285,6 +285,33 @@ MD_API int md_set_state(md_system *s, const double *xyz, const double *vxyz);
 /* The same from DEVICE arrays (e.g. torch tensors on the system's device): no host transfer.  vxyz_device may be NULL. */
 MD_API int md_set_state_device(md_system *s, const double *xyz_device, const double *vxyz_device);
 
+/* Pipelined host I/O (SURVEY.md 8(b) extension): the two directions of the host link run on the
+ * library's own copy streams, concurrently with each other and with the kernels on the system's stream, so that a
+ * service loop over independent host-resident states pays max(upload, download, compute) per state, not their sum.
+ * All host arrays of these calls must be PAGE-LOCKED (cudaHostAlloc / cudaHostRegister / torch pin_memory), 3*N doubles
+ * each, original-id order, and must stay valid and untouched until the transfer is known to be complete;
+ * MD_ERR_INVALID for pageable memory.  Not for rigid-molecule systems.  The first call allocates four staging buffers
+ * of 6*N doubles on the device (through the system's allocator hooks).
+ *   md_stage_state      starts the upload of a NEXT state (positions and velocities) into a device staging buffer and
+ *                       returns at once; the system's current state and its kernels are not affected.  Up to TWO states
+ *                       can be staged (a FIFO; MD_ERR_INVALID for a third), so that the next upload runs while the
+ *                       previous one is being installed.
+ *   md_commit_state     makes the OLDEST staged state the system's state, exactly as md_set_state would (range check on
+ *                       the device before the old state is touched, re-bin, rebuild W, forces, counters reset).  Waits
+ *                       for that upload; after it returns the host arrays of that upload may be reused.  A state that
+ *                       fails the range check is dropped from the FIFO.  MD_ERR_INVALID if nothing is staged.
+ *   md_get_state_async  exports positions and velocities of the CURRENT state (stream-ordered after the kernels enqueued so
+ *                       far) and starts their download; returns at once.  Downloads complete in the order they were
+ *                       started; two can be in flight before a third makes the system's stream wait for the first.
+ *   md_wait_io          max_pending = 0: blocks until every transfer started by the calls above is complete.
+ *                       max_pending = 1 .. 3: blocks until at most that many of the NEWEST downloads are still in flight
+ *                       (1: everything but the download started last is complete).  Returns MD_ERR_CUDA if a transfer
+ *                       failed.  md_destroy waits for everything. */
+MD_API int md_stage_state(md_system *s, const double *xyz, const double *vxyz);
+MD_API int md_commit_state(md_system *s);
+MD_API int md_get_state_async(md_system *s, double *xyz, double *vxyz);
+MD_API int md_wait_io(md_system *s, int32_t max_pending);
+
 /* Test hooks.  md_rebuild_neighbors forces a rebuild now.  md_get_neighbors returns the matrix by ORIGINAL
  * ids: counts[N]; list[N * max_neighbors] with row i = neighbors of atom i (unordered, -1 padded); for the
  * Newton-3 variant the half list is symmetrised so both variants return the full relation.

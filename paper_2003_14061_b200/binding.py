@@ -26,7 +26,7 @@ TIMER_NAMES = ("integrate", "cells", "reorder", "nebr", "force", "energy", "fuse
 
 EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_pushoff", "md_set_rigid", "md_set_rigid_state", "md_get_rigid_state", "md_set_bonds", "md_set_angles", "md_set_dihedrals", "md_step", "md_energies",
            "md_get_positions", "md_get_velocities", "md_get_forces", "md_get_state", "md_get_positions_device",
-           "md_get_velocities_device", "md_get_forces_device", "md_set_state", "md_set_state_device", "md_measure_peaks",
+           "md_get_velocities_device", "md_get_forces_device", "md_set_state", "md_set_state_device", "md_stage_state", "md_commit_state", "md_get_state_async", "md_wait_io", "md_measure_peaks",
            "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
            "md_set_allocator", "md_last_error", "md_version")
@@ -147,6 +147,10 @@ def load_library(path: str = LIB_PATH):
     for n in ("md_get_positions_device", "md_get_velocities_device", "md_get_forces_device"):
         getattr(L, n).argtypes = [C.c_void_p, C.c_void_p]
     L.md_set_state_device.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.md_stage_state.argtypes = [C.c_void_p, _dp, _dp]
+    L.md_commit_state.argtypes = [C.c_void_p]
+    L.md_get_state_async.argtypes = [C.c_void_p, _dp, _dp]
+    L.md_wait_io.argtypes = [C.c_void_p, C.c_int32]
     L.md_measure_peaks.argtypes = [C.c_void_p, C.POINTER(_Peaks)]
     L.md_rebuild_neighbors.argtypes = [C.c_void_p]
     L.md_get_neighbors.argtypes = [C.c_void_p, _ip, C.c_void_p, C.POINTER(C.c_int32)]
@@ -357,6 +361,24 @@ class MDSystem:
             if t is not None and not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == 3 * self.n):
                 raise MDError(MD_ERR_INVALID, "need contiguous float64 CUDA tensors of 3 N elements")
         self._ck(self._L.md_set_state_device(self._h, C.c_void_p(r.data_ptr()), C.c_void_p(v.data_ptr()) if v is not None else None))
+
+    # double-buffered host I/O on the library's copy streams; all arrays page-locked float64 (N, 3), kept alive and
+    # untouched by the caller until wait_io() (or, for a staged state, commit_state()) has returned
+    def stage_state(self, r, v):
+        """md_stage_state: start the upload of a next state; returns at once.  Up to two states can be staged (FIFO)."""
+        self._ck(self._L.md_stage_state(self._h, r, v))
+
+    def commit_state(self):
+        """md_commit_state: install the oldest staged state as md_set_state would."""
+        self._ck(self._L.md_commit_state(self._h))
+
+    def state_async(self, r_out, v_out):
+        """md_get_state_async: start the download of the current state; complete after wait_io()."""
+        self._ck(self._L.md_get_state_async(self._h, r_out, v_out))
+
+    def wait_io(self, max_pending=0):
+        """md_wait_io: 0 = every transfer complete; 1..3 = all but that many of the newest downloads."""
+        self._ck(self._L.md_wait_io(self._h, int(max_pending)))
 
     def measure_peaks(self) -> dict:
         p = _Peaks()

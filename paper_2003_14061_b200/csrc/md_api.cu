@@ -58,8 +58,15 @@ struct md_system {
     md_free_fn free_ = nullptr;
     void *alloc_user = nullptr;
     int64_t bytes = 0;
-    DevCtrl *h_ctrl = nullptr;     // pinned
+    DevCtrl *h_ctrl = nullptr;     // pinned, mapped
+    DevCtrl *d_h_ctrl = nullptr;   // the device's address of h_ctrl
     double *h_stage = nullptr;     // pinned staging, 6 N doubles
+    // double-buffered host I/O (md_stage_state / md_commit_state / md_get_state_async): copy streams and staging buffers
+    cudaStream_t up_stream = nullptr, down_stream = nullptr;
+    cudaEvent_t ev_up[2] = {nullptr, nullptr}, ev_exported = nullptr, ev_down[4] = {nullptr, nullptr, nullptr, nullptr};
+    double *io_in[2] = {nullptr, nullptr}, *io_out[2] = {nullptr, nullptr};    // device, 6 N doubles each (xyz | vxyz, original order), on first use
+    int in_head = 0, n_staged = 0;   // FIFO of staged states: slots in_head, in_head + 1 (mod 2)
+    int64_t n_down = 0;              // downloads started; download d: staging buffer d % 2, event d % 4
     int64_t step = 0;
     int64_t launches = 0;
     bool has_state = false;
@@ -142,7 +149,8 @@ void resolve_timers(md_system *s)
 
 int fetch_ctrl(md_system *s)
 {
-    CK(cudaMemcpyAsync(s->h_ctrl, s->P.ctrl, sizeof(DevCtrl), cudaMemcpyDeviceToHost, s->stream));
+    mdk_publish_ctrl(s->P, s->d_h_ctrl, s->stream);          // a kernel, not a copy: see k_publish_ctrl
+    s->launches += 1;
     CK(cudaStreamSynchronize(s->stream));
     CK(cudaGetLastError());
     return MD_OK;
@@ -473,6 +481,8 @@ void md_destroy(md_system *s)
 {
     if (!s) return;
     if (s->stream) cudaStreamSynchronize(s->stream);
+    for (cudaStream_t t : {s->up_stream, s->down_stream}) if (t) { cudaStreamSynchronize(t); cudaStreamDestroy(t); }
+    for (cudaEvent_t e : {s->ev_up[0], s->ev_up[1], s->ev_exported, s->ev_down[0], s->ev_down[1], s->ev_down[2], s->ev_down[3]}) if (e) cudaEventDestroy(e);
     for (EvPair &e : s->pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (EvPair &e : s->pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     drop_graph(s);
@@ -690,7 +700,8 @@ md_system *md_create_ex(const md_params *pp)
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
     if (!ok) { set_error("device allocation failed (%.1f MB so far)", s->bytes / 1048576.0); md_destroy(s); return nullptr; }
-    if (cudaMallocHost((void **)&s->h_ctrl, sizeof(DevCtrl)) != cudaSuccess) return fail("cudaMallocHost");
+    if (cudaHostAlloc((void **)&s->h_ctrl, sizeof(DevCtrl), cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostGetDevicePointer((void **)&s->d_h_ctrl, s->h_ctrl, 0) != cudaSuccess) return fail("cudaHostAlloc (mapped)");
     if (cudaMallocHost((void **)&s->h_stage, 6 * (size_t)P.N * sizeof(double)) != cudaSuccess) return fail("cudaMallocHost");
     memset(s->h_ctrl, 0, sizeof(DevCtrl));
 
@@ -757,6 +768,105 @@ int md_set_state_device(md_system *s, const double *xyz_device, const double *vx
         return MD_ERR_INVALID;
     }
     return install_state(s);
+}
+
+namespace {
+
+// copy streams, events and the device staging buffers (two per direction) of the asynchronous I/O calls, on first use
+int io_ready(md_system *s)
+{
+    if (s->P.rigid) { set_error("asynchronous state I/O: a rigid-molecule system exchanges its state through md_set/get_rigid_state"); return MD_ERR_INVALID; }
+    if (s->up_stream) return MD_OK;
+    const size_t bytes = 6 * (size_t)s->P.N * sizeof(double);
+    for (int k = 0; k < 2; k++) {
+        s->io_in[k] = (double *)dev_alloc(s, bytes);
+        s->io_out[k] = (double *)dev_alloc(s, bytes);
+        if (!s->io_in[k] || !s->io_out[k]) { set_error("asynchronous state I/O: out of device memory (4 x %zu bytes)", bytes); return MD_ERR_NOMEM; }
+    }
+    CK(cudaStreamSynchronize(s->stream));           // the buffers were cleared on the system's stream
+    CK(cudaStreamCreateWithFlags(&s->up_stream, cudaStreamNonBlocking));
+    CK(cudaStreamCreateWithFlags(&s->down_stream, cudaStreamNonBlocking));
+    for (cudaEvent_t *e : {&s->ev_up[0], &s->ev_up[1], &s->ev_exported, &s->ev_down[0], &s->ev_down[1], &s->ev_down[2], &s->ev_down[3]})
+        CK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    return MD_OK;
+}
+
+}  // namespace
+
+int md_stage_state(md_system *s, const double *xyz, const double *vxyz)
+{
+    if (!s || !xyz || !vxyz) { set_error("md_stage_state: null argument"); return MD_ERR_INVALID; }
+    if (!is_pinned(xyz) || !is_pinned(vxyz)) { set_error("md_stage_state: the host arrays must be page-locked"); return MD_ERR_INVALID; }
+    int rc = io_ready(s);
+    if (rc) return rc;
+    if (s->n_staged == 2) { set_error("md_stage_state: two states are staged already; md_commit_state takes the older one"); return MD_ERR_INVALID; }
+    const size_t n3 = 3 * (size_t)s->P.N;
+    const int slot = (s->in_head + s->n_staged) & 1;
+    // a staging buffer is read on the system's stream only inside md_commit_state, which returns after that read
+    double *dst = s->io_in[slot];
+    if (vxyz == xyz + n3) {
+        CK(cudaMemcpyAsync(dst, xyz, 2 * n3 * sizeof(double), cudaMemcpyHostToDevice, s->up_stream));
+    } else {
+        CK(cudaMemcpyAsync(dst, xyz, n3 * sizeof(double), cudaMemcpyHostToDevice, s->up_stream));
+        CK(cudaMemcpyAsync(dst + n3, vxyz, n3 * sizeof(double), cudaMemcpyHostToDevice, s->up_stream));
+    }
+    CK(cudaEventRecord(s->ev_up[slot], s->up_stream));
+    s->n_staged++;
+    return MD_OK;
+}
+
+int md_commit_state(md_system *s)
+{
+    if (!s) { set_error("md_commit_state: null argument"); return MD_ERR_INVALID; }
+    if (s->n_staged == 0) { set_error("md_commit_state: no staged state (md_stage_state first)"); return MD_ERR_INVALID; }
+    const int slot = s->in_head;
+    CK(cudaStreamWaitEvent(s->stream, s->ev_up[slot], 0));
+    s->in_head ^= 1;
+    s->n_staged--;
+    return md_set_state_device(s, s->io_in[slot], s->io_in[slot] + 3 * (size_t)s->P.N);
+}
+
+int md_get_state_async(md_system *s, double *xyz, double *vxyz)
+{
+    if (!s || !xyz || !vxyz) { set_error("md_get_state_async: null argument"); return MD_ERR_INVALID; }
+    if (!s->has_state) { set_error("no state loaded"); return MD_ERR_INVALID; }
+    if (!is_pinned(xyz) || !is_pinned(vxyz)) { set_error("md_get_state_async: the host arrays must be page-locked"); return MD_ERR_INVALID; }
+    int rc = io_ready(s);
+    if (rc) return rc;
+    const size_t n3 = 3 * (size_t)s->P.N;
+    const int64_t d = s->n_down;
+    double *src = s->io_out[d & 1];
+    if (d >= 2) CK(cudaStreamWaitEvent(s->stream, s->ev_down[(d - 2) & 3], 0));      // the download before last read this buffer
+    s->launches += 2;
+    mdk_export(s->P, 0, src, s->stream);
+    mdk_export(s->P, 1, src + n3, s->stream);
+    CK(cudaEventRecord(s->ev_exported, s->stream));
+    CK(cudaStreamWaitEvent(s->down_stream, s->ev_exported, 0));
+    if (vxyz == xyz + n3) {
+        CK(cudaMemcpyAsync(xyz, src, 2 * n3 * sizeof(double), cudaMemcpyDeviceToHost, s->down_stream));
+    } else {
+        CK(cudaMemcpyAsync(xyz, src, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->down_stream));
+        CK(cudaMemcpyAsync(vxyz, src + n3, n3 * sizeof(double), cudaMemcpyDeviceToHost, s->down_stream));
+    }
+    CK(cudaEventRecord(s->ev_down[d & 3], s->down_stream));
+    s->n_down = d + 1;
+    return MD_OK;
+}
+
+int md_wait_io(md_system *s, int32_t max_pending)
+{
+    if (!s) { set_error("md_wait_io: null argument"); return MD_ERR_INVALID; }
+    if (max_pending < 0 || max_pending > 3) { set_error("md_wait_io: max_pending must be 0 .. 3"); return MD_ERR_INVALID; }
+    if (!s->up_stream) return MD_OK;
+    if (max_pending == 0) {
+        CK(cudaStreamSynchronize(s->up_stream));
+        CK(cudaStreamSynchronize(s->down_stream));
+    } else if (s->n_down > max_pending) {
+        // the copy stream runs the downloads in order: download n_down - max_pending - 1 complete => all before it too
+        CK(cudaEventSynchronize(s->ev_down[(s->n_down - max_pending - 1) & 3]));
+    }
+    CK(cudaGetLastError());
+    return MD_OK;
 }
 
 int md_measure_peaks(md_system *s, md_peaks *out)

@@ -1050,6 +1050,21 @@ void mdk_check_range(const MdDev &P, double box, cudaStream_t st)
     k_check_range<<<capped_grid(P, 3LL * P.N, 256, 8), 256, 0, st>>>(P, box);
 }
 
+// The control block into page-locked host memory, written by a kernel: a device-to-host cudaMemcpy would queue on the
+// copy engine behind a bulk download in flight on another stream (md_get_state_async) and hold the status read -- and
+// with it the next md_step -- for the length of that transfer (measured: 1.8 ms at N = 2M).
+namespace {
+__global__ void k_publish_ctrl(const DevCtrl *__restrict__ src, DevCtrl *dst)
+{
+    static_assert(sizeof(DevCtrl) % sizeof(int) == 0, "DevCtrl is copied word by word");
+    const int *a = reinterpret_cast<const int *>(src);
+    volatile int *b = reinterpret_cast<volatile int *>(dst);
+    for (int k = threadIdx.x; k < (int)(sizeof(DevCtrl) / sizeof(int)); k += blockDim.x) b[k] = __ldcg(a + k);
+    __threadfence_system();
+}
+}  // namespace
+void mdk_publish_ctrl(const MdDev &P, DevCtrl *host_mapped, cudaStream_t st) { k_publish_ctrl<<<1, 64, 0, st>>>(P.ctrl, host_mapped); }
+
 void mdk_load_state(const MdDev &P, cudaStream_t st)
 {
     if (P.sp) return mdk_sp_load_state(P, st);
