@@ -978,8 +978,11 @@ constexpr int PERSIST_T = SCAN_T;      // 256 threads: the scan tiles need exact
 #ifndef MD_PERSIST_U
 #define MD_PERSIST_U 4             // gathers in flight per thread: the phase is one latency chain per atom, not a bandwidth problem
 #endif
-template <int BONDS>
-__global__ void __launch_bounds__(PERSIST_T) k_persist(const __grid_constant__ MdDev P, long long n_steps)
+// MINB: resident blocks per SM the register allocation must allow.  2 (116 registers, 512 threads per SM): every atom its own
+// thread, the lowest latency per step -- systems of up to ~75,000 atoms.  4 (64 registers, 1024 threads per SM): larger
+// systems, several atoms per thread in grid-stride loops.
+template <int BONDS, int MINB>
+__global__ void __launch_bounds__(PERSIST_T, MINB) k_persist(const __grid_constant__ MdDev P, long long n_steps)
 {
     cg::grid_group grid = cg::this_grid();
     __shared__ double sm[33];
@@ -1178,32 +1181,50 @@ void mdk_energy(const MdDev &P, const MdLaunch &, cudaStream_t st)
 }
 
 // ---- the persistent small-system kernel ----
-static int persist_grid(const MdDev &P)
+#ifndef MD_PERSIST_MAX_N
+#define MD_PERSIST_MAX_N 400000     // beyond ~450,000 atoms the graph path (tile-staged build, 1280 threads per SM in the force kernel) is faster
+#endif
+namespace {
+struct PersistChoice {
+    const void *kernel;
+    int grid;
+};
+template <int MINB>
+const void *persist_kernel(const MdDev &P) { return P.has_bonds ? (const void *)k_persist<1, MINB> : (const void *)k_persist<0, MINB>; }
+
+// every atom its own thread if the low-latency instantiation holds them all at once, else the high-occupancy one with
+// as many blocks as are resident together (a cooperative launch needs that) and grid-stride loops
+PersistChoice persist_choice(const MdDev &P)
 {
-    int per_sm = 0;
-    const void *k = P.has_bonds ? (const void *)k_persist<1> : (const void *)k_persist<0>;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return 0; }
     const int want = cdiv(P.N, PERSIST_T);
-    return want <= per_sm * P.sm_count ? want : 0;       // every atom its own thread, all blocks resident at once
+    int per_sm = 0;
+    const void *k = persist_kernel<2>(P);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) == cudaSuccess && per_sm >= 1 && want <= per_sm * P.sm_count)
+        return {k, want};
+    k = persist_kernel<4>(P);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) == cudaSuccess && per_sm >= 1)
+        return {k, std::min(want, per_sm * P.sm_count)};
+    cudaGetLastError();
+    return {nullptr, 0};
 }
+}  // namespace
 
 bool mdk_persist_ok(const MdDev &P)
 {
     if (P.sp || P.tiled || P.half_list || P.layer_H || P.rigid || P.has_angles || P.has_dihedrals || P.w_col != 1) return false;
-    if (P.N > 32768) return false;                        // beyond that the graph path's tile-staged build is the faster one
+    if (P.N > MD_PERSIST_MAX_N) return false;
     int dev = 0, coop = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) { cudaGetLastError(); return false; }
-    return persist_grid(P) > 0;
+    return persist_choice(P).grid > 0;
 }
 
 int mdk_persist_steps(const MdDev &P, long long n, cudaStream_t st)
 {
-    const int grid = persist_grid(P);
-    if (grid <= 0) return -1;
+    const PersistChoice c = persist_choice(P);
+    if (c.grid <= 0) return -1;
     MdDev Pc = P;
     void *args[] = {(void *)&Pc, (void *)&n};
-    const void *k = P.has_bonds ? (const void *)k_persist<1> : (const void *)k_persist<0>;
-    return cudaLaunchCooperativeKernel(k, dim3(grid), dim3(PERSIST_T), args, 0, st) == cudaSuccess ? 0 : -1;
+    return cudaLaunchCooperativeKernel(c.kernel, dim3(c.grid), dim3(PERSIST_T), args, 0, st) == cudaSuccess ? 0 : -1;
 }
 
 int mdk_launches_of(int which)

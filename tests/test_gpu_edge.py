@@ -200,11 +200,13 @@ def test_set_state_rejects_out_of_range_coordinates_and_keeps_the_old_state(md, 
     g.close()
 
 
-@pytest.mark.parametrize("case", ["wca_4k", "ragged_1000", "chains", "batch"])
+@pytest.mark.parametrize("case", ["wca_4k", "ragged_1000", "chains", "batch", "stride_110k", "stride_chains_98k"])
 def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
     """Small systems run md_step as ONE cooperative launch (k_persist: blocks resident over all steps, grid-wide barriers,
     the bodies of the same kernels).  With the same W build (the gathering kernel, MD_FLAG_GLOBAL_W) the step graph must
-    give bit-identical states, energies and rebuild counts -- across many rebuilds, in one call or several."""
+    give bit-identical states, energies and rebuild counts -- across many rebuilds, in one call or several.  The "stride"
+    cases are larger than the resident grid holds one atom per thread (~75,000): the high-occupancy instantiation with
+    grid-stride loops, several atoms per thread."""
     n_sys = 1
     if case == "wca_4k":
         cfg = get_config("wca_4k")
@@ -212,6 +214,10 @@ def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
         cfg = scaled_config("wca_4k", 1000)
     elif case == "chains":
         cfg = scaled_config("chains_rows_1m", 4096, chain_len=16)
+    elif case == "stride_110k":
+        cfg = scaled_config("wca_262k", 110592)
+    elif case == "stride_chains_98k":
+        cfg = scaled_config("chains_rows_1m", 98304, chain_len=64)
     else:
         cfg, n_sys = scaled_config("wca_4k", 1728), 3
     states = [make_state(cfg, 4 + b, jitter_amp=0.05 if cfg.lattice == "sc" else 0.0) for b in range(n_sys)]

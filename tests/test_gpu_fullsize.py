@@ -92,7 +92,8 @@ def test_full_size_all_atoms_and_ten_steps(md, name, start):
     assert g.info()["n_atoms"] == cfg.n_atoms
     _check_static(g, o, cfg, start == "seeded")
     _check_ten_steps(g, o, cfg, box)
-    assert g.info()["use_graph"] == 1
+    # the launch configuration bench.py times: one cooperative launch up to 400,000 atoms, the step graph above
+    assert g.info()["use_graph"] == (2 if cfg.n_atoms <= 400_000 else 1)
     g.close()
 
 
