@@ -421,6 +421,18 @@ bool choose_tile(MdDev &P, const md_params &prm, size_t smem_optin, bool for_til
     // box length along x in r_n-wide cells; in fine cells it is a multiple of kx, so every box starts at least kx cells
     // from the row's ends or exactly at them: the halo of a box is then one contiguous range on either side (md_types.h)
     int S = prm.tile_cells[0];
+    if (S <= 0 && for_tiled_w && prm.tile_threads <= 0) {
+        // Tiled force kernel (long columns): blocks of 256 threads filled to <= 92 % with own atoms -- four resident blocks
+        // per SM overlap one block's staging with the others' columns, and a box that owns more atoms than the block has
+        // threads costs a second pass.  Measured: lj_1m 3 x 2 x 2 cells @ 256 threads 3.54 G against
+        // 5 x 2 x 2 @ 512 (the round-1 rule) 3.32 G; the paper's LJ state point 5 x 2 x 2 @ 256 4.88 G against 9 x 2 x 2 @ 512 4.40 G.
+        const double q = G.R * G.RZ * per_cell;                        // own atoms per cell of box length
+        const int s256 = std::max(1, (int)floor(0.92 * 256 / q)), s512 = std::max(1, (int)floor(0.92 * 512 / q));
+        const double f256 = s256 * q / 256.0, f512 = s512 * q / 512.0;
+        const bool small = f256 <= 1.0 && (f256 >= 0.75 || f256 >= f512 || f512 > 1.0);
+        G.threads = small ? 256 : 512;
+        S = small ? s256 : s512;
+    }
     if (S <= 0) S = (int)lround(0.8 * G.threads / (G.R * G.RZ * per_cell));
     S = std::min(std::max(S, 1), nc);
     G.nsx = (nc + S - 1) / S;
@@ -439,7 +451,7 @@ bool choose_tile(MdDev &P, const md_params &prm, size_t smem_optin, bool for_til
     G.nsys = P.n_sys;
     const double mean = (double)(S + 2) * (G.R + 2) * (G.RZ + 2) * per_cell;
     int cap = prm.tile_capacity;
-    if (cap <= 0) cap = (int)(1.35 * mean + 6.0 * sqrt(mean) + 32.0);
+    if (cap <= 0) cap = (int)((for_tiled_w ? 1.25 : 1.35) * mean + 6.0 * sqrt(mean) + 32.0);     // tiled force: four 54 KB tiles per SM at lj_1m
     cap = (cap + 31) & ~31;
     if (cap > 8192) cap = 8192;
     G.cap = cap;
