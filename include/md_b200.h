@@ -126,7 +126,7 @@ enum { MD_FLAG_NO_GRAPH = 1u, /* launch kernels one by one instead of replaying 
        MD_FLAG_GATHER_W = 8u, /* never pick the tiled layout automatically (the build kernel still stages tiles) */
        MD_FLAG_W_TRANSPOSED = 16u, /* ablation of PAPER.md:165-167: store W atom-index-SLOWEST, W[i * Mmax + m], so that
                                  the threads of a warp no longer read consecutive words (global-index layout only) */
-       MD_FLAG_NO_PERSIST = 64u, /* Systems of <= 400,000 atoms (fp64, fused steps, no flag and no tile setting given) run
+       MD_FLAG_NO_PERSIST = 64u, /* Systems of <= 400,000 atoms (either precision, fused steps, no flag and no tile setting given) run
                                  md_step as ONE cooperative launch whose blocks stay resident over all n steps and meet at
                                  grid-wide barriers (md_info.use_graph = 2), with W built by the gathering
                                  kernel (one atom per thread up to ~75,000 atoms, several beyond).  This flag -- like any other

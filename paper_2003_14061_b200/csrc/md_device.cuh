@@ -64,12 +64,20 @@ __device__ __forceinline__ pos_t ld_pos_rw(const pos_t *p)
 // How the kernels read arrays that the SAME launch never writes (LdNC: the non-coherent read-only path) -- and how the
 // persistent small-system kernel (md_kernels.cu: k_persist), which rewrites those arrays between its grid-wide barriers,
 // must read them instead (LdPlain: ordinary coherent loads).
+__device__ __forceinline__ float4 ld_f4_rw(const float4 *p)
+{
+    float4 r;
+    asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
 struct LdNC {
+    static __device__ __forceinline__ float4 f4(const float4 *p) { return __ldg(p); }
     static __device__ __forceinline__ pos_t pos(const pos_t *p) { return ld_pos(p); }
     static __device__ __forceinline__ int i32(const int *p) { return __ldg(p); }
     static __device__ __forceinline__ double f64(const double *p) { return __ldg(p); }
 };
 struct LdPlain {
+    static __device__ __forceinline__ float4 f4(const float4 *p) { return ld_f4_rw(p); }
     static __device__ __forceinline__ pos_t pos(const pos_t *p) { return ld_pos_rw(p); }
     static __device__ __forceinline__ int i32(const int *p) { return *(const volatile int *)p; }
     static __device__ __forceinline__ double f64(const double *p) { return *(const volatile double *)p; }

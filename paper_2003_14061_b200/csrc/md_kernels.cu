@@ -20,6 +20,7 @@
 #include <cooperative_groups.h>
 
 #include "md_device.cuh"
+#include "md_rebuild.cuh"
 
 namespace {
 
@@ -146,16 +147,6 @@ __global__ void __launch_bounds__(256) k_kick(const __grid_constant__ MdDev P)
 // cells: N1/N2 binning with atomic occupancy counters, N3/N4 as a prefix scan.  The rebuild kernels use
 // grid-stride loops over a capped grid: a launch that finds need_rebuild == 0 retires in ~2 us.
 // ------------------------------------------------------------------------------------------------
-// which of the ping-pong buffers a rebuild reads (ps, vs) and writes (pd, vd): from the control block, or from the
-// persistent kernel's own copy of the decision
-struct Bufs {
-    int ps, pd, vs, vd;
-};
-__device__ __forceinline__ Bufs bufs_from_ctrl(const MdDev &P)
-{
-    return {__ldcg(&P.ctrl->p_src), __ldcg(&P.ctrl->p_dst), __ldcg(&P.ctrl->v_src), __ldcg(&P.ctrl->v_dst)};
-}
-
 template <class LD>
 __device__ __forceinline__ void bin_body(const MdDev &P, const Bufs B)
 {
@@ -177,34 +168,6 @@ __global__ void __launch_bounds__(256) k_bin(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     bin_body<LdNC>(P, bufs_from_ctrl(P));
-}
-
-constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
-
-// occupancy sum and maximum of tile `tile` of SCAN_TILE cells; the block has SCAN_T threads
-__device__ __forceinline__ void scan_reduce_tile(const MdDev &P, int tile)
-{
-    __shared__ int ssum[SCAN_T / 32], smax[SCAN_T / 32];
-    const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
-    int sum = 0, mx = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_V; k++) {
-        const int idx = base + k;
-        const int c = idx < P.NC ? P.cell_count[idx] : 0;
-        sum += c;
-        mx = max(mx, c);
-    }
-    sum = warp_sum_i(sum);
-    mx = warp_max_i(mx);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (lane == 0) { ssum[wid] = sum; smax[wid] = mx; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int s = 0, m = 0;
-        for (int w = 0; w < SCAN_T / 32; w++) { s += ssum[w]; m = max(m, smax[w]); }
-        P.block_sums[tile] = s;
-        atomicMax(&P.ctrl->max_occ, m);              // N3: the paper's layer count N_l = max_c k_c
-    }
 }
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ MdDev P)
@@ -252,52 +215,10 @@ __global__ void __launch_bounds__(1024) k_scan_top(const __grid_constant__ MdDev
     }
 }
 
-__device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
-{
-    __shared__ int wsum[SCAN_T / 32];
-    const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
-    int c[SCAN_V], sum = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_V; k++) {
-        const int idx = base + k;
-        c[k] = idx < P.NC ? P.cell_count[idx] : 0;
-        sum += c[k];
-    }
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    int inc = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(FULL_MASK, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) wsum[wid] = inc;
-    __syncthreads();
-    int woff = 0;
-    for (int w = 0; w < wid; w++) woff += wsum[w];
-    int run = P.block_sums[tile] + woff + inc - sum;
-#pragma unroll
-    for (int k = 0; k < SCAN_V; k++) {
-        const int idx = base + k;
-        if (idx < P.NC) {
-            P.cell_start[idx] = run;
-            P.cell_count[idx] = 0;                   // ready for the next binning
-            run += c[k];
-            if (idx == P.NC - 1) P.cell_start[P.NC] = run;
-        }
-    }
-}
-
 __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
     scan_apply_tile(P, blockIdx.x);
-}
-
-// N4 in CSR form: the atom's place in the cell-ordered sequence s
-__device__ __forceinline__ void place_body(const MdDev &P)
-{
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x)
-        P.perm[P.cell_start[P.cell_of[i]] + P.slot[i]] = i;
 }
 
 __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
@@ -344,18 +265,6 @@ __global__ void __launch_bounds__(256) k_reorder(const __grid_constant__ MdDev P
     reorder_body<LdNC>(P, bufs_from_ctrl(P));
 }
 
-__device__ __forceinline__ void bonds_remap_body(const MdDev &P, const Bufs B)
-{
-    const int *idv = P.id[B.vd];
-    for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < P.N; n += gridDim.x * blockDim.x) {
-        const int id = idv[n];
-#pragma unroll
-        for (int k = 0; k < 2; k++) {
-            const int partner = P.bond_orig[(size_t)k * P.N + id];
-            P.bond_dev[(size_t)k * P.N_pad + n] = partner >= 0 ? P.inv[partner] : -1;
-        }
-    }
-}
 
 __global__ void __launch_bounds__(256) k_bonds_remap(const __grid_constant__ MdDev P)
 {
@@ -973,7 +882,6 @@ __global__ void __launch_bounds__(256) k_energy(const __grid_constant__ MdDev P)
 // fp64, global-index W (gathering build), variant A, fused steps, at most FENE bonds.
 // ------------------------------------------------------------------------------------------------
 namespace cg = cooperative_groups;
-constexpr int PERSIST_T = SCAN_T;      // 256 threads: the scan tiles need exactly SCAN_T
 
 #ifndef MD_PERSIST_U
 #define MD_PERSIST_U 4             // gathers in flight per thread: the phase is one latency chain per atom, not a bandwidth problem
@@ -1196,6 +1104,11 @@ const void *persist_kernel(const MdDev &P) { return P.has_bonds ? (const void *)
 // as many blocks as are resident together (a cooperative launch needs that) and grid-stride loops
 PersistChoice persist_choice(const MdDev &P)
 {
+    if (P.sp) {
+        const void *k = nullptr;
+        const int grid = mdk_sp_persist_choice(P, &k);
+        return {k, grid};
+    }
     const int want = cdiv(P.N, PERSIST_T);
     int per_sm = 0;
     const void *k = persist_kernel<2>(P);
@@ -1211,7 +1124,8 @@ PersistChoice persist_choice(const MdDev &P)
 
 bool mdk_persist_ok(const MdDev &P)
 {
-    if (P.sp || P.tiled || P.half_list || P.layer_H || P.rigid || P.has_angles || P.has_dihedrals || P.w_col != 1) return false;
+    if (P.tiled || P.half_list || P.layer_H || P.rigid || P.has_angles || P.has_dihedrals || P.w_col != 1) return false;
+    if (P.sp && P.sp_pad > 1) return false;               // padded columns (long binary32 columns): step graph
     if (P.N > MD_PERSIST_MAX_N) return false;
     int dev = 0, coop = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) { cudaGetLastError(); return false; }

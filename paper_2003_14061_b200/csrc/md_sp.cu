@@ -11,7 +11,10 @@
 // No code is shared with oracle/.
 #include <algorithm>
 
+#include <cooperative_groups.h>
+
 #include "md_device.cuh"
+#include "md_rebuild.cuh"
 
 namespace {
 
@@ -81,22 +84,26 @@ __global__ void k_sp_export(const __grid_constant__ MdDev P, int what, double *d
 // ------------------------------------------------------------------------------------------------
 // integration (opening half kick + drift; closing half kick of the split mode)
 // ------------------------------------------------------------------------------------------------
+// opening half kick + drift of atom i; returns |v|^2
+__device__ __forceinline__ float sp_kick_drift_atom(const MdDev &P, int pc, int vc, int i)
+{
+    float4 r = P.posf[pc][i], v = P.velf[vc][i];
+    const float4 f = P.frcf[i];
+    v.x = __fadd_rn(v.x, __fmul_rn(P.hdtf, f.x)); v.y = __fadd_rn(v.y, __fmul_rn(P.hdtf, f.y)); v.z = __fadd_rn(v.z, __fmul_rn(P.hdtf, f.z));
+    r.x = __fadd_rn(r.x, __fmul_rn(P.dtf, v.x)); r.y = __fadd_rn(r.y, __fmul_rn(P.dtf, v.y)); r.z = __fadd_rn(r.z, __fmul_rn(P.dtf, v.z));
+    P.velf[vc][i] = v;
+    P.posf[pc][i] = r;
+    float v2 = v.x * v.x + v.y * v.y + v.z * v.z;
+    if (!isfinite(v2 + r.x + r.y + r.z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0f; }
+    return v2;
+}
+
 __global__ void __launch_bounds__(256) k_sp_kick_drift(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
-    float v2 = 0.0f;
-    if (i < P.N) {
-        float4 r = P.posf[pc][i], v = P.velf[vc][i];
-        const float4 f = P.frcf[i];
-        v.x = __fadd_rn(v.x, __fmul_rn(P.hdtf, f.x)); v.y = __fadd_rn(v.y, __fmul_rn(P.hdtf, f.y)); v.z = __fadd_rn(v.z, __fmul_rn(P.hdtf, f.z));
-        r.x = __fadd_rn(r.x, __fmul_rn(P.dtf, v.x)); r.y = __fadd_rn(r.y, __fmul_rn(P.dtf, v.y)); r.z = __fadd_rn(r.z, __fmul_rn(P.dtf, v.z));
-        P.velf[vc][i] = v;
-        P.posf[pc][i] = r;
-        v2 = v.x * v.x + v.y * v.y + v.z * v.z;
-        if (!isfinite(v2 + r.x + r.y + r.z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0f; }
-    }
+    const float v2 = i < P.N ? sp_kick_drift_atom(P, pc, vc, i) : 0.0f;
     const double bm = block_max((double)v2, sm);
     if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
 }
@@ -116,45 +123,55 @@ __global__ void __launch_bounds__(256) k_sp_kick(const __grid_constant__ MdDev P
 // N1/N2: the cell of an atom is found in binary64 from its binary32 coordinate (cells are
 // kept wider than r_n by 1e-5 relative at create time, far more than the rounding error of a binary32 r2)
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_sp_bin(const __grid_constant__ MdDev P)
+template <class LD>
+__device__ __forceinline__ void sp_bin_body(const MdDev &P, const Bufs B)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const float4 *__restrict__ pos = P.posf[__ldcg(&P.ctrl->p_src)];
-    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_src)];
+    const float4 *pos = P.posf[B.ps];
+    const int *idv = P.id[B.vs];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
-        const float4 r = ld4(pos + i);
+        const float4 r = LD::f4(pos + i);
         const int cx = cell_coord((double)wrap1f(r.x, P.Lf), P.inv_wx, P.ncx), cy = cell_coord((double)wrap1f(r.y, P.Lf), P.inv_w, P.nc),
                   cz = cell_coord((double)wrap1f(r.z, P.Lf), P.inv_w, P.nc);
-        const int sys = P.n_sys > 1 ? __ldg(idv + i) / P.N1 : 0;
+        const int sys = P.n_sys > 1 ? LD::i32(idv + i) / P.N1 : 0;
         const int c = sys * P.NC1 + cx + P.ncx * (cy + P.nc * cz);
         P.cell_of[i] = c;
         P.slot[i] = atomicAdd(&P.cell_count[c], 1);
     }
 }
 
-// cell-order gather (PAPER.md:80, 159), coordinates wrapped here; members of a cell ranked by previous slot
-__global__ void __launch_bounds__(256) k_sp_reorder(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(256) k_sp_bin(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    const int ps = __ldcg(&P.ctrl->p_src), pd = __ldcg(&P.ctrl->p_dst);
-    const int vs = __ldcg(&P.ctrl->v_src), vd = __ldcg(&P.ctrl->v_dst);
-    const float4 *__restrict__ pin = P.posf[ps];
-    const float4 *__restrict__ vin = P.velf[vs];
-    const int *__restrict__ idin = P.id[vs];
+    sp_bin_body<LdNC>(P, bufs_from_ctrl(P));
+}
+
+// cell-order gather (PAPER.md:80, 159), coordinates wrapped here; members of a cell ranked by previous slot
+template <class LD>
+__device__ __forceinline__ void sp_reorder_body(const MdDev &P, const Bufs B)
+{
+    const float4 *pin = P.posf[B.ps];
+    const float4 *vin = P.velf[B.vs];
+    const int *idin = P.id[B.vs];
     for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P.N; p += gridDim.x * blockDim.x) {
         const int a = P.perm[p];
-        const float4 r = ld4(pin + a), v = ld4(vin + a);
-        const int id = __ldg(idin + a);
+        const float4 r = LD::f4(pin + a), v = LD::f4(vin + a);
+        const int id = LD::i32(idin + a);
         const int c = P.cell_of[a];
         const int s = P.cell_start[c], e = P.cell_start[c + 1];
         int rank = 0;
         for (int q = s; q < e; q++) rank += (P.perm[q] < a);
         const int n = s + rank;
-        P.posf[pd][n] = make_float4(wrap1f(r.x, P.Lf), wrap1f(r.y, P.Lf), wrap1f(r.z, P.Lf), 0.0f);
-        P.velf[vd][n] = v;
-        P.id[vd][n] = id;
+        P.posf[B.pd][n] = make_float4(wrap1f(r.x, P.Lf), wrap1f(r.y, P.Lf), wrap1f(r.z, P.Lf), 0.0f);
+        P.velf[B.vd][n] = v;
+        P.id[B.vd][n] = id;
         if (P.need_inv) P.inv[id] = n;
     }
+}
+
+__global__ void __launch_bounds__(256) k_sp_reorder(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    sp_reorder_body<LdNC>(P, bufs_from_ctrl(P));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -163,12 +180,12 @@ __global__ void __launch_bounds__(256) k_sp_reorder(const __grid_constant__ MdDe
 // (A single flat loop over all candidates of an atom, its <= 18 segments tabulated in shared memory so that lanes
 // idle only at the end of the whole list, was measured SLOWER -- 534 vs 390 us per build at wca_2m: lanes then sit
 // in different runs, each gather request touches more lines, and the loop no longer unrolls.)
-template <bool SHIFT>
-__device__ __forceinline__ void scan_run_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, int b, int e,
+template <bool SHIFT, class LD>
+__device__ __forceinline__ void scan_run_f(const MdDev &P, const float4 *pos, const float4 &ri, int i, int b, int e,
                                            float sx, float sy, float sz, unsigned fl, int &m)
 {
     for (int j = b; j < e; j++) {
-        const float4 rj = ld4(pos + j);
+        const float4 rj = LD::f4(pos + j);
         float dx = __fsub_rn(ri.x, rj.x), dy = __fsub_rn(ri.y, rj.y), dz = __fsub_rn(ri.z, rj.z);
         if (SHIFT) { dx = __fadd_rn(dx, sx); dy = __fadd_rn(dy, sy); dz = __fadd_rn(dz, sz); }
         const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
@@ -179,22 +196,23 @@ __device__ __forceinline__ void scan_run_f(const MdDev &P, const float4 *__restr
     }
 }
 
-__global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev P)
+// all threads of the block call it (block reduction of the statistics at the end); blocks of <= 256 threads
+template <class LD>
+__device__ __forceinline__ void sp_build_body(const MdDev &P, const Bufs B)
 {
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    __shared__ int smx[4], scand[4];
-    __shared__ int ssum[4];
-    const float4 *__restrict__ pos = P.posf[__ldcg(&P.ctrl->p_dst)];
-    const int *__restrict__ cs = P.cell_start;
-    const int *__restrict__ idv = P.id[__ldcg(&P.ctrl->v_dst)];
+    __shared__ int smx[8], scand[8];
+    __shared__ int ssum[8];
+    const float4 *pos = P.posf[B.pd];
+    const int *cs = P.cell_start;
+    const int *idv = P.id[B.vd];
     const int nc = P.nc, ncx = P.ncx;
     const float L = P.Lf;
     int tmax = 0, tsum = 0, tcand = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
-        const float4 ri = ld4(pos + i);
+        const float4 ri = LD::f4(pos + i);
         const int cx = cell_coord((double)ri.x, P.inv_wx, ncx), cy = cell_coord((double)ri.y, P.inv_w, nc), cz = cell_coord((double)ri.z, P.inv_w, nc);
         const RowGaps gaps = row_gaps(P, (double)ri.y, (double)ri.z, cy, cz);
-        const int cell_base = P.n_sys > 1 ? (__ldg(idv + i) / P.N1) * P.NC1 : 0;
+        const int cell_base = P.n_sys > 1 ? (LD::i32(idv + i) / P.N1) * P.NC1 : 0;
         int m = 0;
         for (int dz = -1; dz <= 1; dz++) {
             int z = cz + dz;
@@ -210,12 +228,12 @@ __global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev 
                 if (y < 0) { y += nc; sy = L; fl |= 2u; } else if (y >= nc) { y -= nc; sy = -L; fl |= 2u; }
                 const int row = cell_base + ncx * (y + nc * z);
                 const int lo = cx - kr, hi = cx + kr;
-                const int b = __ldg(cs + row + (lo < 0 ? 0 : lo)), e = __ldg(cs + row + (hi >= ncx ? ncx : hi + 1));
+                const int b = LD::i32(cs + row + (lo < 0 ? 0 : lo)), e = LD::i32(cs + row + (hi >= ncx ? ncx : hi + 1));
                 tcand += e - b;
-                if (fl) scan_run_f<true>(P, pos, ri, i, b, e, 0.0f, sy, sz, fl, m);
-                else scan_run_f<false>(P, pos, ri, i, b, e, 0.0f, 0.0f, 0.0f, 0u, m);
-                if (lo < 0) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row + ncx + lo), __ldg(cs + row + ncx), L, sy, sz, fl | 1u, m);
-                if (hi >= ncx) scan_run_f<true>(P, pos, ri, i, __ldg(cs + row), __ldg(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m);
+                if (fl) scan_run_f<true, LD>(P, pos, ri, i, b, e, 0.0f, sy, sz, fl, m);
+                else scan_run_f<false, LD>(P, pos, ri, i, b, e, 0.0f, 0.0f, 0.0f, 0u, m);
+                if (lo < 0) scan_run_f<true, LD>(P, pos, ri, i, LD::i32(cs + row + ncx + lo), LD::i32(cs + row + ncx), L, sy, sz, fl | 1u, m);
+                if (hi >= ncx) scan_run_f<true, LD>(P, pos, ri, i, LD::i32(cs + row), LD::i32(cs + row + hi - ncx + 1), -L, sy, sz, fl | 1u, m);
             }
         }
         P.nnb[i] = m < P.Mmax ? m : P.Mmax;
@@ -240,6 +258,12 @@ __global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev 
         atomicAdd(&P.ctrl->nnb_total, (unsigned long long)sm);
         atomicAdd(&P.ctrl->cand_total, (unsigned long long)sc);
     }
+}
+
+__global__ void __launch_bounds__(128) k_sp_build(const __grid_constant__ MdDev P)
+{
+    if (!__ldcg(&P.ctrl->need_rebuild)) return;
+    sp_build_body<LdNC>(P, bufs_from_ctrl(P));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -379,8 +403,8 @@ __device__ __noinline__ void dihedral_force_f(const MdDev &P, const float4 *__re
 }
 
 // EXTRAS: angle / dihedral code compiled in (the FENE-only instantiation keeps its registers)
-template <bool CHECK, bool EXTRAS = true>
-__device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i, PairAccF &a)
+template <bool CHECK, bool EXTRAS = true, class LD = LdNC>
+__device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *pos, const float4 &ri, int i, PairAccF &a)
 {
     if (EXTRAS && P.has_angles) angle_force_f(P, pos, ri, i, a);
     if (EXTRAS && P.has_dihedrals) dihedral_force_f(P, pos, ri, i, a);
@@ -388,7 +412,7 @@ __device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *__res
     for (int k = 0; k < 2; k++) {
         const int j = P.bond_dev[(size_t)k * P.N_pad + i];
         if (j < 0) continue;
-        const float4 rj = ld4(pos + j);
+        const float4 rj = LD::f4(pos + j);
         const float dx = minimgf(__fsub_rn(ri.x, rj.x), P.Lf, P.half_Lf), dy = minimgf(__fsub_rn(ri.y, rj.y), P.Lf, P.half_Lf),
                     dz = minimgf(__fsub_rn(ri.z, rj.z), P.Lf, P.half_Lf);
         const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
@@ -411,8 +435,8 @@ __device__ __forceinline__ void bond_force_f(const MdDev &P, const float4 *__res
 // 197 -> 169 us per fused step at lj_1m.  For the short WCA columns the ~1.5 extra gather rows per warp cost more
 // than the predicates save (94 -> 99 us at wca_2m: the kernel's time goes with its number of gather instructions),
 // so there the rows past the column end are predicated off instead; such a lane carries r_j = r_i (r2 = 0).
-template <int D, bool PADDED>
-__device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 *__restrict__ pos, const float4 &ri, int i)
+template <int D, bool PADDED, class LD = LdNC>
+__device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 *pos, const float4 &ri, int i)
 {
     constexpr int U = PADDED ? SP_PAD : MD_SP_FORCE_U;       // gathers in flight per thread
     static_assert(D % U == 0, "D must be a multiple of the gather group");
@@ -444,10 +468,10 @@ __device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 
                 float4 rj[U];
 #pragma unroll
                 for (int u = 0; u < U; u++) {
-                    if (PADDED) rj[u] = ld4(pos + (cur[g + u] & W_INDEX_MASK));
+                    if (PADDED) rj[u] = LD::f4(pos + (cur[g + u] & W_INDEX_MASK));
                     else {
                         rj[u] = ri;
-                        if (g + u < rem) rj[u] = ld4(pos + (cur[g + u] & W_INDEX_MASK));
+                        if (g + u < rem) rj[u] = LD::f4(pos + (cur[g + u] & W_INDEX_MASK));
                     }
                 }
 #pragma unroll
@@ -467,40 +491,98 @@ __device__ __forceinline__ PairAccF column_force_f(const MdDev &P, const float4 
 #define MD_SP_MIN_THREADS 1280       // resident threads per SM the register allocation must allow
 #endif
 // BONDS: 0 none, 1 FENE bonds, 2 FENE + angle / dihedral terms
+// forces on atom i over column i of W (+ bonds) and the MODE's part of the integration; returns |v|^2 (MODE 1)
+template <int MODE, int BONDS, bool PADDED, class LD>
+__device__ __forceinline__ float sp_force_atom(const MdDev &P, int pc, int vc, int i)
+{
+    const float4 *pos = P.posf[pc];
+    float v2 = 0.0f;
+    const float4 ri = LD::f4(pos + i);
+    float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (MODE != 0) v = P.velf[vc][i];               // in flight while the column is walked
+    PairAccF a = column_force_f<MD_SP_FORCE_D, PADDED, LD>(P, pos, ri, i);
+    if (BONDS == 1) bond_force_f<true, false, LD>(P, pos, ri, i, a);
+    if (BONDS == 2) bond_force_f<true, true, LD>(P, pos, ri, i, a);
+    if (MODE == 0 || MODE == 2) P.frcf[i] = make_float4(a.fx, a.fy, a.fz, 0.0f);
+    if (MODE == 2) {
+        v.x = __fadd_rn(v.x, __fmul_rn(P.hdtf, a.fx)); v.y = __fadd_rn(v.y, __fmul_rn(P.hdtf, a.fy)); v.z = __fadd_rn(v.z, __fmul_rn(P.hdtf, a.fz));
+        P.velf[vc][i] = v;
+    }
+    if (MODE == 1) {
+        // two half kicks of the oracle's step merged into one full kick (leapfrog form)
+        v.x = __fadd_rn(v.x, __fmul_rn(P.dtf, a.fx)); v.y = __fadd_rn(v.y, __fmul_rn(P.dtf, a.fy)); v.z = __fadd_rn(v.z, __fmul_rn(P.dtf, a.fz));
+        P.velf[vc][i] = v;
+        const float x = __fadd_rn(ri.x, __fmul_rn(P.dtf, v.x)), y = __fadd_rn(ri.y, __fmul_rn(P.dtf, v.y)), z = __fadd_rn(ri.z, __fmul_rn(P.dtf, v.z));
+        P.posf[pc ^ 1][i] = make_float4(x, y, z, 0.0f);
+        v2 = v.x * v.x + v.y * v.y + v.z * v.z;
+        if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0f; }
+    }
+    return v2;
+}
+
 template <int MODE, int BONDS, int BLOCK, bool PADDED>
 __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(const __grid_constant__ MdDev P)
 {
     __shared__ double sm[32];
     const int i = blockIdx.x * BLOCK + threadIdx.x;
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
-    const float4 *__restrict__ pos = P.posf[pc];
-    float v2 = 0.0f;
-    if (i < P.N) {
-        const float4 ri = ld4(pos + i);
-        float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        if (MODE != 0) v = P.velf[vc][i];               // in flight while the column is walked
-        PairAccF a = column_force_f<MD_SP_FORCE_D, PADDED>(P, pos, ri, i);
-        if (BONDS == 1) bond_force_f<true, false>(P, pos, ri, i, a);
-        if (BONDS == 2) bond_force_f<true, true>(P, pos, ri, i, a);
-        if (MODE == 0 || MODE == 2) P.frcf[i] = make_float4(a.fx, a.fy, a.fz, 0.0f);
-        if (MODE == 2) {
-            v.x = __fadd_rn(v.x, __fmul_rn(P.hdtf, a.fx)); v.y = __fadd_rn(v.y, __fmul_rn(P.hdtf, a.fy)); v.z = __fadd_rn(v.z, __fmul_rn(P.hdtf, a.fz));
-            P.velf[vc][i] = v;
-        }
-        if (MODE == 1) {
-            // two half kicks of the oracle's step merged into one full kick (leapfrog form)
-            v.x = __fadd_rn(v.x, __fmul_rn(P.dtf, a.fx)); v.y = __fadd_rn(v.y, __fmul_rn(P.dtf, a.fy)); v.z = __fadd_rn(v.z, __fmul_rn(P.dtf, a.fz));
-            P.velf[vc][i] = v;
-            const float x = __fadd_rn(ri.x, __fmul_rn(P.dtf, v.x)), y = __fadd_rn(ri.y, __fmul_rn(P.dtf, v.y)), z = __fadd_rn(ri.z, __fmul_rn(P.dtf, v.z));
-            P.posf[pc ^ 1][i] = make_float4(x, y, z, 0.0f);
-            v2 = v.x * v.x + v.y * v.y + v.z * v.z;
-            if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0f; }
-        }
-    }
+    const float v2 = i < P.N ? sp_force_atom<MODE, BONDS, PADDED, LdNC>(P, pc, vc, i) : 0.0f;
     if (MODE == 1) {
         const double bm = block_max((double)v2, sm);
         if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
     }
+}
+
+// ---- the persistent kernel in binary32: md_kernels.cu:k_persist with the bodies above (see there for the structure) ----
+namespace cg = cooperative_groups;
+
+template <int BONDS, int MINB>
+__global__ void __launch_bounds__(PERSIST_T, MINB) k_sp_persist(const __grid_constant__ MdDev P, long long n_steps)
+{
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double sm[33];
+    const int nblk = gridDim.x, tid = threadIdx.x;
+    const int stride = nblk * PERSIST_T, first = blockIdx.x * PERSIST_T + tid;
+    DecState c = dec_load(P);
+    for (long long step = 0; step < n_steps; step++) {
+        float v2 = 0.0f;
+        for (int i = first; i < P.N; i += stride)
+            v2 = fmaxf(v2, step == 0 ? sp_kick_drift_atom(P, c.p_dst, c.v_dst, i) : sp_force_atom<1, BONDS, false, LdPlain>(P, c.p_dst, c.v_dst, i));
+        const double bm = block_max((double)v2, sm);
+        double *vmax_buf = P.blk_vmax2 + (step & 1) * nblk;
+        if (tid == 0) vmax_buf[blockIdx.x] = bm;
+        grid.sync();
+        double m = 0.0;
+        for (int b = tid; b < nblk; b += PERSIST_T) m = fmax(m, __ldcg(vmax_buf + b));
+        __syncthreads();
+        m = block_max(m, sm);
+        if (tid == 0) sm[32] = m;
+        __syncthreads();
+        decide_state(P, c, sm[32], step != 0);
+        if (blockIdx.x == 0 && tid == 0) dec_store(P, c);
+        if (c.need_rebuild) {
+            const Bufs B = {c.p_src, c.p_dst, c.v_src, c.v_dst};
+            sp_bin_body<LdPlain>(P, B);
+            grid.sync();
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_reduce_tile(P, t); __syncthreads(); }
+            grid.sync();
+            if (blockIdx.x == 0 && tid == 0) {
+                int run = 0;
+                for (int t = 0; t < P.scan_blocks; t++) { const int v = P.block_sums[t]; P.block_sums[t] = run; run += v; }
+            }
+            grid.sync();
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile(P, t); __syncthreads(); }
+            grid.sync();
+            place_body(P);
+            grid.sync();
+            sp_reorder_body<LdPlain>(P, B);
+            grid.sync();
+            if (BONDS) { bonds_remap_body(P, B); grid.sync(); }
+            sp_build_body<LdPlain>(P, B);
+            grid.sync();
+        }
+    }
+    for (int i = first; i < P.N; i += stride) sp_force_atom<2, BONDS, false, LdPlain>(P, c.p_dst, c.v_dst, i);
 }
 
 // F2 and the other sums: binary32 pair terms, binary64 accumulation
@@ -603,6 +685,31 @@ void launch_sp_force(const MdDev &P, int block, cudaStream_t st)
 }
 
 }  // namespace
+
+// the persistent launch of md_kernels.cu (mdk_persist_ok / mdk_persist_steps) in binary32: kernel and grid
+namespace {
+template <int MINB>
+const void *sp_persist_kernel(const MdDev &P) { return P.has_bonds ? (const void *)k_sp_persist<1, MINB> : (const void *)k_sp_persist<0, MINB>; }
+}  // namespace
+
+int mdk_sp_persist_choice(const MdDev &P, const void **kernel)
+{
+    const int want = cdiv(P.N, PERSIST_T);
+    int per_sm = 0;
+    const void *k = sp_persist_kernel<2>(P);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) == cudaSuccess && per_sm >= 1 && want <= per_sm * P.sm_count) {
+        *kernel = k;
+        return want;
+    }
+    k = sp_persist_kernel<4>(P);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PERSIST_T, 0) == cudaSuccess && per_sm >= 1) {
+        *kernel = k;
+        return std::min(want, per_sm * P.sm_count);
+    }
+    cudaGetLastError();
+    *kernel = nullptr;
+    return 0;
+}
 
 void mdk_sp_load_state(const MdDev &P, cudaStream_t st) { k_sp_load_state<<<cdiv(P.N, 256), 256, 0, st>>>(P); }
 void mdk_sp_export(const MdDev &P, int what, double *dst, cudaStream_t st) { k_sp_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, dst); }

@@ -195,7 +195,8 @@ int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   //
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);
-void mdk_publish_ctrl(const MdDev &P, DevCtrl *host_mapped, cudaStream_t st);       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
+void mdk_publish_ctrl(const MdDev &P, DevCtrl *host_mapped, cudaStream_t st);
+int mdk_sp_persist_choice(const MdDev &P, const void **kernel);     // grid of the binary32 persistent kernel (0: not possible)       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
 // tiled layout (md_tile.cu)
 int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
 size_t mdk_tile_smem(const MdDev &P, bool with_cells);

@@ -200,8 +200,9 @@ def test_set_state_rejects_out_of_range_coordinates_and_keeps_the_old_state(md, 
     g.close()
 
 
+@pytest.mark.parametrize("precision", ["f64", "f32"])
 @pytest.mark.parametrize("case", ["wca_4k", "ragged_1000", "chains", "batch", "stride_110k", "stride_chains_98k"])
-def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
+def test_persistent_launch_equals_the_step_graph_bitwise(md, case, precision):
     """Small systems run md_step as ONE cooperative launch (k_persist: blocks resident over all steps, grid-wide barriers,
     the bodies of the same kernels).  With the same W build (the gathering kernel, MD_FLAG_GLOBAL_W) the step graph must
     give bit-identical states, energies and rebuild counts -- across many rebuilds, in one call or several.  The "stride"
@@ -226,7 +227,7 @@ def test_persistent_launch_equals_the_step_graph_bitwise(md, case):
     bonds = None if states[0][2] is None else np.concatenate([s[2] + b * cfg.n_atoms for b, s in enumerate(states)])
     out = []
     for flags in (0, md.FLAG_GLOBAL_W):
-        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags, n_systems=n_sys)
+        g = md.MDSystem(cfg.n_atoms, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", flags=flags, n_systems=n_sys, precision=precision)
         g.set_state(r, v)
         if bonds is not None:
             g.set_bonds(bonds, cfg.fene_k, cfg.fene_r0)
