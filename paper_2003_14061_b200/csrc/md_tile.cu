@@ -385,6 +385,8 @@ __global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDe
     __shared__ TileDesc M;
     __shared__ TileRowGeom X;
     __shared__ int smx[32], ssum[32], scand[32];
+    struct RowC { real shy, shz; unsigned fl, add0; int e0, e1, d0, d1, d2, pad; };
+    __shared__ RowC rc[TILE_Q_MAX];
     const int cap = P.tg.cap, K = P.kx;
     const int stride = P.tg.S + 2 * K + 1;
     real *st = (real *)dsm;
@@ -414,10 +416,25 @@ __global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDe
         else v = R.off + R.n[0] + R.n[1] + (__ldg(cs + X.row_cell[q] + X.xc + k - K - B.sxc) - R.g[2]);
         tcs[e] = v;
     }
+    // per tile row: periodic shifts along y, z, their flag bits, the index offsets of the row's (up to) three contiguous
+    // pieces (global index = tile index + delta) -- everything of a run's set-up that does not depend on the atom
+    for (int q = threadIdx.x; q < B.nq; q += BLOCK) {
+        const int ysh = X.ysh[q], zsh = X.zsh[q];
+        const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
+        const TileDesc::Row &R = M.row[q];
+        RowC c;
+        c.shy = ysh * PR::box(P); c.shz = zsh * PR::box(P);
+        c.fl = fl;
+        c.e0 = R.off + R.n[0]; c.e1 = c.e0 + R.n[1];
+        c.d0 = R.g[0] - R.off; c.d1 = R.g[1] - c.e0; c.d2 = R.g[2] - c.e1; c.pad = 0;
+        c.add0 = LOCALW ? fl << T_FLAG_SHIFT : (fl << W_FLAG_SHIFT) + (unsigned)c.d0;
+        rc[q] = c;
+    }
     __syncthreads();
     const int nc = P.nc, ncx = P.ncx;
     const real L = PR::box(P), rn2 = PR::rn2(P);
     const bool low_face = B.x0 == 0, high_face = B.x0 + B.sxc == ncx;
+    const bool interior = !low_face && !high_face;           // block-uniform: every tile row is ONE global range, no image along x
     int tmax = 0, tsum = 0, tcand = 0;
     for (int t = threadIdx.x; t < M.n_own; t += BLOCK) {
         int i, li;
@@ -429,34 +446,47 @@ __global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDe
         const int q0 = (cy - B.y0) + B.nyq * (cz - B.z0);          // tile row (cy - 1, cz - 1)
         // (Shortening the window of rows that are far from the atom -- row_halfwidth, as the gathering build does -- was
         // measured slower here, in round 1 and again in round 2: the lanes of a warp then walk runs of more unequal lengths.)
+        if (interior) {
+            // the per-run set-up is one 16-byte and two 4-byte shared-memory reads (measured: build 0.385 -> 0.362 ms at wca_2m_dr03)
 #pragma unroll 1
-        for (int r = 0; r < 9; r++) {
-            const int q = q0 + (r % 3) + B.nyq * (r / 3);
-            const int ysh = X.ysh[q], zsh = X.zsh[q];
-            const unsigned fl = (ysh ? 2u : 0u) | (zsh ? 4u : 0u);
-            const real shy = ysh * L, shz = zsh * L;
-            const TileDesc::Row &R = M.row[q];
-            const int *tc = tcs + q * stride + kc;
-            const int b = tc[0], e = tc[2 * K + 1];               // tile cells [kc, kc + 2 K + 1)
-            tcand += e - b;
-            // split off the part of the window that is a periodic image along x (box at an x face, window reaching
-            // into the halo that holds the cells of the other end of the row)
-            const bool ima = low_face && kc < K, imb = high_face && kc + K + 1 > B.sxc;
-            const int mid = ima ? tc[K - kc] : (imb ? tc[K + B.sxc - kc] : e);
-            // global index = tile index + delta, constant over each contiguous piece of the row
-            const int e0 = R.off + R.n[0], e1 = e0 + R.n[1];
-            const int d0 = R.g[0] - R.off, d1 = R.g[1] - e0, d2 = R.g[2] - e1;
-            const int da = b < e0 ? d0 : (b < e1 ? d1 : d2), db = mid < e0 ? d0 : (mid < e1 ? d1 : d2);
-            const real shxa = ima ? L : (real)0, shxb = imb ? -L : (real)0;
-            const unsigned fla = fl | (ima ? 1u : 0u), flb = fl | (imb ? 1u : 0u);
-            // what is added to the tile index to make the W entry: the flag bits, and for global W the index offset
-            const unsigned adda = LOCALW ? fla << T_FLAG_SHIFT : (fla << W_FLAG_SHIFT) + (unsigned)da;
-            const unsigned addb = LOCALW ? flb << T_FLAG_SHIFT : (flb << W_FLAG_SHIFT) + (unsigned)db;
-            if (fla) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
-            else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, mid, (real)0, (real)0, (real)0, adda, rn2, em);
-            if (mid < e) {
-                if (flb) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
-                else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, mid, e, (real)0, (real)0, (real)0, addb, rn2, em);
+            for (int rz = 0; rz < 3; rz++) {
+#pragma unroll 1
+                for (int ry = 0; ry < 3; ry++) {
+                    const int q = q0 + ry + B.nyq * rz;
+                    const RowC c = rc[q];
+                    const int *tc = tcs + q * stride + kc;
+                    const int b = tc[0], e = tc[2 * K + 1];       // tile cells [kc, kc + 2 K + 1)
+                    tcand += e - b;
+                    if (c.fl) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, e, (real)0, c.shy, c.shz, c.add0, rn2, em);
+                    else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, e, (real)0, (real)0, (real)0, c.add0, rn2, em);
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int r = 0; r < 9; r++) {
+                const int q = q0 + (r % 3) + B.nyq * (r / 3);
+                const RowC c = rc[q];
+                const unsigned fl = c.fl;
+                const real shy = c.shy, shz = c.shz;
+                const int *tc = tcs + q * stride + kc;
+                const int b = tc[0], e = tc[2 * K + 1];
+                tcand += e - b;
+                // split off the part of the window that is a periodic image along x (box at an x face, window reaching
+                // into the halo that holds the cells of the other end of the row)
+                const bool ima = low_face && kc < K, imb = high_face && kc + K + 1 > B.sxc;
+                const int mid = ima ? tc[K - kc] : (imb ? tc[K + B.sxc - kc] : e);
+                const int da = b < c.e0 ? c.d0 : (b < c.e1 ? c.d1 : c.d2), db = mid < c.e0 ? c.d0 : (mid < c.e1 ? c.d1 : c.d2);
+                const real shxa = ima ? L : (real)0, shxb = imb ? -L : (real)0;
+                const unsigned fla = fl | (ima ? 1u : 0u), flb = fl | (imb ? 1u : 0u);
+                // what is added to the tile index to make the W entry: the flag bits, and for global W the index offset
+                const unsigned adda = LOCALW ? fla << T_FLAG_SHIFT : (fla << W_FLAG_SHIFT) + (unsigned)da;
+                const unsigned addb = LOCALW ? flb << T_FLAG_SHIFT : (flb << W_FLAG_SHIFT) + (unsigned)db;
+                if (fla) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, b, mid, shxa, shy, shz, adda, rn2, em);
+                else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, b, mid, (real)0, (real)0, (real)0, adda, rn2, em);
+                if (mid < e) {
+                    if (flb) tile_scan_run<true, LOCALW>(st, xi, yi, zi, li, mid, e, shxb, shy, shz, addb, rn2, em);
+                    else tile_scan_run<false, LOCALW>(st, xi, yi, zi, li, mid, e, (real)0, (real)0, (real)0, addb, rn2, em);
+                }
             }
         }
         em.flush();
