@@ -345,6 +345,20 @@ typedef void *(*md_alloc_fn)(size_t bytes, void *stream, void *user);
 typedef void (*md_free_fn)(void *ptr, void *user);
 MD_API void md_set_allocator(md_alloc_fn alloc, md_free_fn free_, void *user);
 
+/* Allocation-free reduction for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): the velocity part of the sums of md_energies -- kinetic energy, total
+ * momentum and the largest speed, the input of the rebuild rule -- of ANY device array of velocities, without an
+ * md_system.  vxyz_device: 3*n_atoms doubles, v[3*i + k] (what md_get_velocities_device writes).  out5_device: 5 doubles
+ * on the device: ke = sum 1/2 |v|^2, px, py, pz, vmax.  stream: cudaStream_t (NULL = the default stream).  Both arrays must
+ * be device memory of the CURRENT device.  The call enqueues one 256-byte memset and one kernel on the stream and returns;
+ * it does not synchronise and calls no cudaMalloc / cudaFree or allocating routine: the block partials and the "last block
+ * done" ticket live in a static device array inside the library (0.64 MB, held by every GPU that loads the library until
+ * the process exits), which is why n_atoms is limited: MD_ERR_INVALID above MD_NOALLOC_MAX_ATOMS (or for a host pointer,
+ * n_atoms < 1).  ALL calls share that array: calls that overlap on the GPU (two streams, two host threads) race -- serialise
+ * them.  Results are reproducible (fixed summation order) and agree with md_energies to summation rounding. */
+#define MD_NOALLOC_MAX_ATOMS 16777216
+MD_API int md_velocity_sums_noalloc(const double *vxyz_device, int64_t n_atoms, double *out5_device, void *stream);
+
 MD_API const char *md_last_error(void);
 MD_API const char *md_version(void);
 

@@ -29,7 +29,7 @@ EXPORTS = ("md_params_default", "md_create", "md_create_ex", "md_destroy", "md_p
            "md_get_velocities_device", "md_get_forces_device", "md_set_state", "md_set_state_device", "md_stage_state", "md_commit_state", "md_get_state_async", "md_wait_io", "md_measure_peaks",
            "md_rebuild_neighbors",
            "md_get_neighbors", "md_get_info", "md_set_profiling", "md_get_timers", "md_reset_timers",
-           "md_set_allocator", "md_last_error", "md_version")
+           "md_set_allocator", "md_velocity_sums_noalloc", "md_last_error", "md_version")
 
 
 class MDError(RuntimeError):
@@ -152,6 +152,7 @@ def load_library(path: str = LIB_PATH):
     L.md_get_state_async.argtypes = [C.c_void_p, _dp, _dp]
     L.md_wait_io.argtypes = [C.c_void_p, C.c_int32]
     L.md_measure_peaks.argtypes = [C.c_void_p, C.POINTER(_Peaks)]
+    L.md_velocity_sums_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     L.md_rebuild_neighbors.argtypes = [C.c_void_p]
     L.md_get_neighbors.argtypes = [C.c_void_p, _ip, C.c_void_p, C.POINTER(C.c_int32)]
     L.md_get_info.argtypes = [C.c_void_p, C.POINTER(_Info)]
@@ -194,6 +195,25 @@ def use_cuda_allocator():
 
 def _err(L):
     return (L.md_last_error() or b"").decode()
+
+
+NOALLOC_MAX_ATOMS = 16777216       # MD_NOALLOC_MAX_ATOMS
+
+
+def velocity_sums_noalloc(v, out=None, stream=None):
+    """md_velocity_sums_noalloc: ke, px, py, pz, vmax of a float64 CUDA tensor of velocities (N, 3) into a float64 CUDA
+    tensor of 5 elements, on torch's current stream (or `stream`, a cudaStream_t value).  The library allocates nothing;
+    pass `out` to make the whole call allocation-free.  Not synchronised.  Calls that overlap on the GPU race."""
+    import torch
+    L = load_library()
+    if out is None:
+        out = torch.empty(5, dtype=torch.float64, device=v.device)
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = L.md_velocity_sums_noalloc(C.c_void_p(v.data_ptr()), v.numel() // 3, C.c_void_p(out.data_ptr()), C.c_void_p(stream))
+    if rc != MD_OK:
+        raise MDError(rc, _err(L))
+    return out
 
 
 class MDSystem:

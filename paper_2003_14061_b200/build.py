@@ -9,7 +9,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libmd_b200.so")
-SOURCES = ["md_api.cu", "md_kernels.cu", "md_tile.cu", "md_sp.cu", "md_pushoff.cu", "md_peaks.cu", "md_rigid.cu", "md_init.cpp"]
+SOURCES = ["md_api.cu", "md_kernels.cu", "md_tile.cu", "md_sp.cu", "md_pushoff.cu", "md_peaks.cu", "md_rigid.cu", "md_noalloc.cu", "md_init.cpp"]
 HEADERS = [os.path.join(CSRC, "md_types.h"), os.path.join(CSRC, "md_device.cuh"), os.path.join(CSRC, "md_rebuild.cuh"), os.path.join(CSRC, "md_init.h"), os.path.join(ROOT, "include", "md_b200.h")]
 
 

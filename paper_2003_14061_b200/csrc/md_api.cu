@@ -466,6 +466,8 @@ bool choose_tile(MdDev &P, const md_params &prm, size_t smem_optin, bool for_til
 
 }  // namespace
 
+void mdk_set_error(const char *msg) { set_error("%s", msg); }
+
 extern "C" {
 
 const char *md_last_error(void) { return g_err; }

@@ -196,6 +196,7 @@ void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  //
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);
 void mdk_publish_ctrl(const MdDev &P, DevCtrl *host_mapped, cudaStream_t st);
+void mdk_set_error(const char *msg);     // md_last_error() text, for the translation units beside md_api.cu
 int mdk_sp_persist_choice(const MdDev &P, const void **kernel);     // grid of the binary32 persistent kernel (0: not possible)       // 0 pos, 1 vel, 2 frc -> dst (device, 3N doubles, original-id order)
 // tiled layout (md_tile.cu)
 int mdk_tile_configure(const MdDev &P);                                       // opt in to the dynamic shared memory; 0 = ok
