@@ -18,18 +18,31 @@ __device__ __forceinline__ Bufs bufs_from_ctrl(const MdDev &P)
 
 constexpr int SCAN_T = 256, SCAN_V = 8, SCAN_TILE = SCAN_T * SCAN_V;
 
+// the SCAN_V = 8 occupancies of a thread: two 128-bit loads where all 8 cells exist (the arrays are 256-byte aligned, base is
+// a multiple of 8), else one by one with zeros past the last cell.  Plain loads: the persistent kernels rewrite cell_count.
+__device__ __forceinline__ void scan_load8(const MdDev &P, int base, int (&c)[SCAN_V])
+{
+    static_assert(SCAN_V == 8, "two int4 per thread");
+    if (base + SCAN_V <= P.NC) {
+        const int4 a = *reinterpret_cast<const int4 *>(P.cell_count + base), b = *reinterpret_cast<const int4 *>(P.cell_count + base + 4);
+        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < SCAN_V; k++) c[k] = base + k < P.NC ? P.cell_count[base + k] : 0;
+    }
+}
+
 // occupancy sum and maximum of tile `tile` of SCAN_TILE cells; the block has SCAN_T threads
 __device__ __forceinline__ void scan_reduce_tile(const MdDev &P, int tile)
 {
     __shared__ int ssum[SCAN_T / 32], smax[SCAN_T / 32];
     const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
-    int sum = 0, mx = 0;
+    int c[SCAN_V], sum = 0, mx = 0;
+    scan_load8(P, base, c);
 #pragma unroll
     for (int k = 0; k < SCAN_V; k++) {
-        const int idx = base + k;
-        const int c = idx < P.NC ? P.cell_count[idx] : 0;
-        sum += c;
-        mx = max(mx, c);
+        sum += c[k];
+        mx = max(mx, c[k]);
     }
     sum = warp_sum_i(sum);
     mx = warp_max_i(mx);
@@ -49,12 +62,9 @@ __device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
     __shared__ int wsum[SCAN_T / 32];
     const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
     int c[SCAN_V], sum = 0;
+    scan_load8(P, base, c);
 #pragma unroll
-    for (int k = 0; k < SCAN_V; k++) {
-        const int idx = base + k;
-        c[k] = idx < P.NC ? P.cell_count[idx] : 0;
-        sum += c[k];
-    }
+    for (int k = 0; k < SCAN_V; k++) sum += c[k];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int inc = sum;
 #pragma unroll
@@ -67,6 +77,17 @@ __device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
     int woff = 0;
     for (int w = 0; w < wid; w++) woff += wsum[w];
     int run = P.block_sums[tile] + woff + inc - sum;
+    if (base + SCAN_V < P.NC) {      // all 8 cells exist and none is the last: 128-bit stores
+        int st[SCAN_V];
+#pragma unroll
+        for (int k = 0; k < SCAN_V; k++) { st[k] = run; run += c[k]; }
+        int4 *cs = reinterpret_cast<int4 *>(P.cell_start + base), *cc = reinterpret_cast<int4 *>(P.cell_count + base);
+        cs[0] = make_int4(st[0], st[1], st[2], st[3]);
+        cs[1] = make_int4(st[4], st[5], st[6], st[7]);
+        cc[0] = make_int4(0, 0, 0, 0);               // ready for the next binning
+        cc[1] = make_int4(0, 0, 0, 0);
+        return;
+    }
 #pragma unroll
     for (int k = 0; k < SCAN_V; k++) {
         const int idx = base + k;
