@@ -123,9 +123,10 @@ def test_full_size_variants(md, name, kw):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["wca_2m", "lj_1m", "chains_1m"])
+@pytest.mark.parametrize("name", ["wca_262k", "wca_2m", "lj_1m", "chains_1m"])
 def test_full_size_single_precision(md, name):
-    """The single-precision twin against the single-precision oracle at full size (bounds of tests/test_gpu_sp.py)."""
+    """The single-precision twin against the single-precision oracle at full size (bounds of tests/test_gpu_sp.py).
+    wca_262k runs as the persistent launch (k_sp_persist, grid-stride instantiation), the others as the step graph."""
     eps32 = 2.0 ** -24
     cfg = get_config(name)
     g, o, box = _pair(md, cfg, 1, 100, oracle_cls=OracleMDSP, precision="f32")
@@ -144,4 +145,5 @@ def test_full_size_single_precision(md, name):
     assert abs(eg.ke - eo.ke) <= 64 * eps32 * escale
     assert abs(eg.pe - eo.pe) <= 64 * eps32 * escale * 4
     assert eg.n_rebuilds == eo.n_rebuilds
+    assert g.info()["use_graph"] == (2 if cfg.n_atoms <= 400_000 else 1)
     g.close()
