@@ -108,15 +108,17 @@ def test_async_io_equals_the_synchronous_calls(md, precision):
     gb.close()
 
 
-def test_async_io_pipeline_over_independent_host_states(md):
+@pytest.mark.parametrize("name,precision", [("wca_4k", "f64"), ("wca_262k", "f64"), ("wca_262k", "f32")])
+def test_async_io_pipeline_over_independent_host_states(md, name, precision):
     """The service loop bench.py's e2e leg times: three independent host-resident trajectories advanced in turn by one
     system, two uploads queued ahead, downloads two deep; a trajectory's buffer goes up again only after its download is
-    known complete (wait_io(1): everything but the newest download).  Same results as the serial loop, bit for bit."""
-    cfg = get_config("wca_4k")
+    known complete (wait_io(1): everything but the newest download).  Same results as the serial loop, bit for bit.
+    At 262,144 atoms a transfer (12.6 MB each way) outlasts the step it overlaps."""
+    cfg = get_config(name)
     n, nt, turns = cfg.n_atoms, 3, 11
     states = [make_state(cfg, seed, jitter_amp=0.1) for seed in (11, 12, 13)]
     box = states[0][3]
-    g = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none")
+    g = md.MDSystem(n, cfg.r_cut, cfg.r_shell, cfg.dt, box=box, lattice="none", precision=precision)
     ser = [np.stack([s[0], s[1]]) for s in states]
     for it in range(turns):
         k = it % nt
