@@ -375,8 +375,11 @@ struct PrecF32 {
 
 // The block size is a run-time value (any multiple of 32 up to 512): it is picked so that the own atoms of a box
 // fill the block's warps.
+// Register cap (measured): binary64 keeps the 62-64 registers ptxas picks (a cap of 56 -- a fifth resident block
+// per SM -- gains 1 % at wca_2m but loses 2-3 % at lj_1m / chains_1m; 48 spills: +9 %); the binary32 build, whose tile is half
+// the size, gains 6 % at wca_2m with 56 (0.355 -> 0.334 ms).
 template <typename PR, bool LOCALW>
-__global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDev P)
+__global__ void __maxnreg__(sizeof(typename PR::real) == 4 ? 56 : 64) k_tile_build(const __grid_constant__ MdDev P)
 {
     using real = typename PR::real;
     const int BLOCK = blockDim.x;
