@@ -206,7 +206,7 @@ void enqueue_force(md_system *s, int mode)
 void enqueue_decide(md_system *s, bool fused_force, unsigned long long cond = 0ull)
 {
     Timed t(s, MD_T_DECIDE, 1);
-    mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused_force), fused_force, s->stream, cond);
+    mdk_decide(s->P, fused_force, s->stream, cond);
 }
 
 void drop_graph(md_system *s)
@@ -253,7 +253,7 @@ bool build_step_graph(md_system *s, int kind)
             if (cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) != cudaSuccess) break;
             if (fused) enqueue_force(s, 1);
             else mdk_kick_drift(s->P, s->lc, st);
-            mdk_decide(s->P, mdk_drift_blocks(s->P, s->lc, fused), fused, st, (unsigned long long)h);
+            mdk_decide(s->P, fused, st, (unsigned long long)h);
             if (cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps) != cudaSuccess) break;
             cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
             cp.conditional.handle = h;
@@ -709,7 +709,7 @@ md_system *md_create_ex(const md_params *pp)
     P.W = (int *)A((size_t)(P.tiled ? P.Mmax / 2 : P.Mmax) * np * sizeof(int));
     if (P.layer_H) P.H = (int *)A((size_t)P.NC * P.n_layers * sizeof(int));
     P.partials = (double *)A((size_t)RED_N * P.max_grid * sizeof(double));
-    P.blk_vmax2 = (double *)A((size_t)P.max_grid * sizeof(double));
+    P.blk_vmax2 = (double *)A(((size_t)P.max_grid + 64 + 2) * sizeof(double));     // 64 = DEC_SLOTS (md_device.cuh), then the persistent kernels' 2 x grid <= max_grid + 2
     if (P.tiled) P.tile_desc = (int *)A((size_t)P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys * sizeof(TileDesc));
     P.scratch = (double *)A(6 * (size_t)P.N * sizeof(double));
     P.ctrl = (DevCtrl *)A(sizeof(DevCtrl));
@@ -1029,7 +1029,7 @@ int md_pushoff(md_system *s, const double *xyz, int64_t n_bonds, const int32_t *
                 const double x = std::min(1.0, (double)step / o.ramp_steps);
                 rcap = o.r_cap_start + x * (o.r_cap_end - o.r_cap_start);
                 mdk_po_kick_drift(P, rcap * rcap, vlim * vlim, ke_target, step == 0, t->stream);
-                mdk_decide(P, mdk_drift_blocks(P, t->lc, false), false, t->stream, 0ull);
+                mdk_decide(P, false, t->stream, 0ull);
                 enqueue_rebuild(t);
                 mdk_po_force(P, rcap * rcap, t->stream);
                 mdk_po_kick(P, t->stream);
@@ -1210,7 +1210,7 @@ int md_step(md_system *s, int64_t n)
         // rigid molecules: per-molecule half kick + free rotation + drift, rebuild decision, site forces, half kick
         for (int64_t k = 0; k < n; k++) {
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_rigid_kick_drift(P, st); }
-            { Timed t(s, MD_T_DECIDE, 1); mdk_decide(P, mdk_rigid_blocks(P), false, st, 0ull); }
+            { Timed t(s, MD_T_DECIDE, 1); mdk_decide(P, false, st, 0ull); }
             enqueue_rebuild(s);
             enqueue_forces_only(s);
             { Timed t(s, MD_T_INTEGRATE, 1); mdk_rigid_kick(P, st); }

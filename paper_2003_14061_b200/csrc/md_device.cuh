@@ -192,6 +192,16 @@ __device__ __forceinline__ double block_max(double v, double *sm)
     return v;
 }
 
+// A drifting kernel leaves its blocks' maxima of v^2 for k_decide in DEC_SLOTS words (block b in slot b mod DEC_SLOTS) with a
+// fire-and-forget atomic maximum: v^2 is finite and >= +0, and the bit patterns of such doubles order as unsigned integers.
+// k_decide then reads -- and clears -- 64 words instead of one entry per block (16,384 at N = 2M): 6.7 -> 5.1 us per step on top
+// of the fused kernel.  A maximum does not depend on the order of the atomics: results stay bitwise reproducible.
+constexpr int DEC_SLOTS = 64;
+__device__ __forceinline__ void publish_vmax2(const MdDev &P, int bid, double bm)
+{
+    atomicMax(reinterpret_cast<unsigned long long *>(P.blk_vmax2) + (bid & (DEC_SLOTS - 1)), (unsigned long long)__double_as_longlong(bm));
+}
+
 // The rebuild decision (R8), taken on the device by k_decide from the per-block maxima of
 // v^2 that the drifting kernel left in blk_vmax2.  It also fixes which buffers the rebuild kernels read and
 // write, so the host never needs to know whether a rebuild happened.

@@ -111,19 +111,16 @@ __global__ void __launch_bounds__(256) k_kick_drift(const __grid_constant__ MdDe
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const double v2 = i < P.N ? kick_drift_atom(P, pc, vc, i) : 0.0;
     const double bm = block_max(v2, sm);
-    if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+    if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
 }
 
 // max over the per-block maxima of v^2, then the rebuild decision: one block, ordered after the drifting kernel
 // by the stream.  Inside md_step's CUDA graph it also sets the condition of the IF node that holds the rebuild chain.
-__global__ void __launch_bounds__(1024) k_decide(const __grid_constant__ MdDev P, int nblk, int pos_pingpong,
-                                                 cudaGraphConditionalHandle cond)
+__global__ void __launch_bounds__(DEC_SLOTS) k_decide(const __grid_constant__ MdDev P, int pos_pingpong, cudaGraphConditionalHandle cond)
 {
     __shared__ double sm[32];
-    double m = 0.0;
-    const double *__restrict__ v = P.blk_vmax2;
-#pragma unroll 8
-    for (int b = threadIdx.x; b < nblk; b += 1024) m = fmax(m, __ldcg(v + b));
+    // read and clear this thread's slot (publish_vmax2): the next drifting kernel starts from zeros
+    double m = __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(P.blk_vmax2) + threadIdx.x, 0ull));
     m = block_max(m, sm);
     if (threadIdx.x == 0) {
         decide(P, m, pos_pingpong != 0);
@@ -728,7 +725,7 @@ __global__ void __launch_bounds__(BLOCK, force_min_threads(BONDS) / BLOCK) k_for
     const double v2 = i < P.N ? force_atom<MODE, BONDS, LdNC, MD_FORCE_U, D>(P, pc, vc, i) : 0.0;
     if (MODE == 1) {
         const double bm = block_max(v2, sm);
-        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
     }
 }
 
@@ -906,7 +903,7 @@ __global__ void __launch_bounds__(PERSIST_T, MINB) k_persist(const __grid_consta
             v2 = fmax(v2, step == 0 ? kick_drift_atom(P, c.p_dst, c.v_dst, i)
                                     : force_atom<1, BONDS, LdPlain, MD_PERSIST_U, 8>(P, c.p_dst, c.v_dst, i));
         const double bm = block_max(v2, sm);
-        double *vmax_buf = P.blk_vmax2 + (step & 1) * nblk;       // double-buffered: a fast block may already be in the next step
+        double *vmax_buf = P.blk_vmax2 + DEC_SLOTS + (step & 1) * nblk;       // (past k_decide's slots) double-buffered: a fast block may already be in the next step
         if (tid == 0) vmax_buf[blockIdx.x] = bm;
         grid.sync();
         // ---- the rebuild decision, replicated in every block ----
@@ -988,9 +985,9 @@ void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st)
     k_export<<<cdiv(P.N, 256), 256, 0, st>>>(P, what, dst);
 }
 
-void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond)
+void mdk_decide(const MdDev &P, bool pos_pingpong, cudaStream_t st, unsigned long long cond)
 {
-    k_decide<<<1, 1024, 0, st>>>(P, nblk, pos_pingpong ? 1 : 0, (cudaGraphConditionalHandle)cond);
+    k_decide<<<1, DEC_SLOTS, 0, st>>>(P, pos_pingpong ? 1 : 0, (cudaGraphConditionalHandle)cond);
 }
 
 void mdk_kick_drift(const MdDev &P, const MdLaunch &, cudaStream_t st)
@@ -1064,13 +1061,6 @@ void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st)
         else if (mode == 1) launch_force_block<1, 0>(P, lc.block, st);
         else launch_force_block<2, 0>(P, lc.block, st);
     }
-}
-
-// number of blocks (= entries of blk_vmax2) the drifting kernels write: input size of k_decide
-int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force)
-{
-    if (!fused_force) return cdiv(P.N, 256);
-    return P.tiled ? P.tg.nsx * P.tg.nsy * P.tg.nsz * P.tg.nsys : cdiv(P.N, lc.block);   // every box of every system writes its maximum
 }
 
 void mdk_force_newton3(const MdDev &P, const MdLaunch &, cudaStream_t st)

@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) k_po_kick_drift(const __grid_constant__ M
         if (!isfinite(v2 + x + y + z)) { set_err(P, MD_ERR_NONFINITE); v2 = 0.0; }
     }
     const double bm = block_max(v2, sm);
-    if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+    if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
 }
 
 // capped pair force over column i of W + clamped FENE bonds -> f

@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(128) k_rigid_kick_drift(const __grid_constant_
         }
     }
     const double bm = block_max(s2, sm);
-    if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+    if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
 }
 
 __global__ void __launch_bounds__(128) k_rigid_kick(const __grid_constant__ MdDev P)
@@ -157,7 +157,6 @@ inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
 }  // namespace
 
-int mdk_rigid_blocks(const MdDev &P) { return cdiv(P.rb_nm, 128); }
 void mdk_rigid_kick_drift(const MdDev &P, cudaStream_t st) { k_rigid_kick_drift<<<cdiv(P.rb_nm, 128), 128, 0, st>>>(P); }
 void mdk_rigid_kick(const MdDev &P, cudaStream_t st) { k_rigid_kick<<<cdiv(P.rb_nm, 128), 128, 0, st>>>(P); }
 void mdk_rigid_offsets(const MdDev &P, cudaStream_t st) { k_rigid_offsets<<<std::min(cdiv(P.N, 256), P.sm_count * 8), 256, 0, st>>>(P); }

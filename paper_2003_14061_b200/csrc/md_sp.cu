@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(256) k_sp_kick_drift(const __grid_constant__ M
     const int pc = __ldcg(&P.ctrl->p_dst), vc = __ldcg(&P.ctrl->v_dst);
     const float v2 = i < P.N ? sp_kick_drift_atom(P, pc, vc, i) : 0.0f;
     const double bm = block_max((double)v2, sm);
-    if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+    if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
 }
 
 __global__ void __launch_bounds__(256) k_sp_kick(const __grid_constant__ MdDev P)
@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(BLOCK, MD_SP_MIN_THREADS / BLOCK) k_sp_force(c
     const float v2 = i < P.N ? sp_force_atom<MODE, BONDS, PADDED, LdNC>(P, pc, vc, i) : 0.0f;
     if (MODE == 1) {
         const double bm = block_max((double)v2, sm);
-        if (threadIdx.x == 0) P.blk_vmax2[blockIdx.x] = bm;
+        if (threadIdx.x == 0) publish_vmax2(P, blockIdx.x, bm);
     }
 }
 
@@ -549,7 +549,7 @@ __global__ void __launch_bounds__(PERSIST_T, MINB) k_sp_persist(const __grid_con
         for (int i = first; i < P.N; i += stride)
             v2 = fmaxf(v2, step == 0 ? sp_kick_drift_atom(P, c.p_dst, c.v_dst, i) : sp_force_atom<1, BONDS, false, LdPlain>(P, c.p_dst, c.v_dst, i));
         const double bm = block_max((double)v2, sm);
-        double *vmax_buf = P.blk_vmax2 + (step & 1) * nblk;
+        double *vmax_buf = P.blk_vmax2 + DEC_SLOTS + (step & 1) * nblk;
         if (tid == 0) vmax_buf[blockIdx.x] = bm;
         grid.sync();
         double m = 0.0;

@@ -693,7 +693,7 @@ __global__ void __launch_bounds__(BLOCK, MD_TILE_FORCE_THREADS / BLOCK) k_tile_f
     }
     if (MODE == 1) {
         const double bm = block_max(vm2, red);
-        if (threadIdx.x == 0) P.blk_vmax2[bid] = bm;
+        if (threadIdx.x == 0) publish_vmax2(P, bid, bm);
     }
 }
 

@@ -152,7 +152,8 @@ struct MdDev {
     int *W, *nnb;                       // neighbor matrix W[m * N_pad + i], counts m_i
                                         // (tiled layout: 32-bit words of two 16-bit entries, W[(m/2) * N_pad + i])
     int *inv, *bond_orig, *bond_dev;    // original id -> slot; bond partners by original id / by slot (2 x N_pad)
-    double *blk_vmax2;                  // max_grid per-block maxima of v^2 from the drifting kernel (input of k_decide)
+    double *blk_vmax2;                  // DEC_SLOTS maxima of v^2 from the drifting kernel (md_device.cuh: publish_vmax2; input of k_decide), then the
+                                        // persistent kernels' 2 x grid per-block maxima
     double *partials;                   // RED_N x max_grid block partials
     double *scratch;                    // 6 N doubles, original-id order (get/set staging: xyz | vxyz)
     DevCtrl *ctrl;
@@ -183,7 +184,7 @@ void mdk_force_rebuild(const MdDev &P, cudaStream_t st);
 void mdk_check_range(const MdDev &P, double box, cudaStream_t st);           // scratch xyz in [0, box] else ctrl->err = MD_ERR_INVALID
 void mdk_load_state(const MdDev &P, cudaStream_t st);                        // scratch(xyz | vxyz) -> pos/vel/id
 // rebuild decision from blk_vmax2[0..nblk); cond != 0: also set that CUDA-graph conditional handle to need_rebuild
-void mdk_decide(const MdDev &P, int nblk, bool pos_pingpong, cudaStream_t st, unsigned long long cond);
+void mdk_decide(const MdDev &P, bool pos_pingpong, cudaStream_t st, unsigned long long cond);
 void mdk_kick_drift(const MdDev &P, const MdLaunch &lc, cudaStream_t st);     // v += dt/2 f; r += dt v; per-block max v^2
 void mdk_kick(const MdDev &P, const MdLaunch &lc, cudaStream_t st);           // v += dt/2 f
 void mdk_cells(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // bin + scan + place       (N1-N4)
@@ -191,7 +192,6 @@ void mdk_reorder(const MdDev &P, const MdLaunch &lc, cudaStream_t st);        //
 void mdk_build(const MdDev &P, const MdLaunch &lc, cudaStream_t st);          // neighbor matrix         (N5)
 // mode 0: f only; 1: fused leapfrog step (f, kick dt, drift, per-block max v^2; follow with mdk_decide); 2: f and closing half kick
 void mdk_force(const MdDev &P, const MdLaunch &lc, int mode, cudaStream_t st);
-int mdk_drift_blocks(const MdDev &P, const MdLaunch &lc, bool fused_force);   // blocks writing blk_vmax2
 void mdk_force_newton3(const MdDev &P, const MdLaunch &lc, cudaStream_t st);  // zero f + half-list atomics
 void mdk_energy(const MdDev &P, const MdLaunch &lc, cudaStream_t st);         // all reductions -> ctrl->red
 void mdk_export(const MdDev &P, int what, double *dst, cudaStream_t st);
@@ -223,7 +223,6 @@ void mdk_po_check(const MdDev &P, unsigned long long *out, cudaStream_t st);  //
 bool mdk_persist_ok(const MdDev &P);
 int mdk_persist_steps(const MdDev &P, long long n, cudaStream_t st);
 // rigid molecules (md_rigid.cu)
-int mdk_rigid_blocks(const MdDev &P);                                          // blocks of k_rigid_kick_drift (entries of blk_vmax2)
 void mdk_rigid_kick_drift(const MdDev &P, cudaStream_t st);
 void mdk_rigid_kick(const MdDev &P, cudaStream_t st);
 void mdk_rigid_offsets(const MdDev &P, cudaStream_t st);
