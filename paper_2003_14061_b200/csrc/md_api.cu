@@ -225,7 +225,11 @@ void drop_graph(md_system *s)
 // rebuild so launches 2 kernels instead of 2 + 7 that find need_rebuild == 0 (PAPER.md:64 takes this decision
 // on the host every step).  Returns false (and leaves no graph) if any step of the construction is refused;
 // md_step then launches the kernels one by one.
-constexpr int GRAPH_UNROLL = 8;     // fused steps per launch of graph[2]: amortises the per-launch cost of a graph (small systems)
+#ifndef MD_GRAPH_UNROLL
+#define MD_GRAPH_UNROLL 8
+#endif
+constexpr int GRAPH_UNROLL = MD_GRAPH_UNROLL;     // fused steps per launch of graph[2]: amortises the per-launch cost of a graph (small systems);
+                                                  // 16 and 32 measured: no further gain (per-step overhead 4.7 / 5.5 / 5.7 us at N = 2M)
 
 bool build_step_graph(md_system *s, int kind)
 {
