@@ -407,17 +407,39 @@ __global__ void __maxnreg__(sizeof(typename PR::real) == 4 ? 56 : 64) k_tile_bui
         if (threadIdx.x == 0) set_err(P, MD_ERR_TILE_OVERFLOW);
         return;
     }
-    PR::stage(P, M, __ldcg(&P.ctrl->p_dst), st);
-    // tcs[q * stride + k], k = 0 .. sxc + 2 K  (K halo cells, the box's sxc cells, K halo cells; the last entry closes the row)
-    for (int e = threadIdx.x; e < B.nq * stride; e += BLOCK) {
+    // tcs[q * stride + k], k = 0 .. sxc + 2 K  (K halo cells, the box's sxc cells, K halo cells; the last entry closes the row):
+    // tile index of the first atom of tile cell k of row q = (start of the cell in the global order) + (tile offset - global
+    // start of the row's piece).  The cell starts of the first TCS_PRE entries of every thread are requested BEFORE the position
+    // tile is staged and added up after it, so that the two rounds of global-memory latency overlap (measured: DESIGN.md 6f).
+    // Binary64: no gain (0.357 -> 0.355 / 0.384 -> 0.392 / 0.198 -> 0.202 ms at dr03 / dr05 / chains_1m: the 8 registers it holds
+    // across the staging cost more), so there the fetches follow the staging; binary32 0.334 -> 0.324 ms.
+    constexpr int TCS_PRE = sizeof(real) == 4 ? 4 : 0;
+    const int n_tcs = B.nq * stride;
+    auto tcs_fetch = [&](int e, int &add) -> int {      // the global load of entry e; add: what turns it into the tile index
         const int q = e / stride, k = e - q * stride;
-        if (k > B.sxc + 2 * K) continue;
         const TileDesc::Row &R = M.row[q];
-        int v;
-        if (k < K) v = R.off + (__ldg(cs + X.row_cell[q] + X.xa + k) - R.g[0]);
-        else if (k < K + B.sxc) v = R.off + R.n[0] + (__ldg(cs + X.row_cell[q] + B.x0 + k - K) - R.g[1]);
-        else v = R.off + R.n[0] + R.n[1] + (__ldg(cs + X.row_cell[q] + X.xc + k - K - B.sxc) - R.g[2]);
-        tcs[e] = v;
+        if (k < K) { add = R.off - R.g[0]; return __ldg(cs + X.row_cell[q] + X.xa + k); }
+        if (k < K + B.sxc) { add = R.off + R.n[0] - R.g[1]; return __ldg(cs + X.row_cell[q] + B.x0 + k - K); }
+        add = R.off + R.n[0] + R.n[1] - R.g[2];
+        return k <= B.sxc + 2 * K ? __ldg(cs + X.row_cell[q] + X.xc + k - K - B.sxc) : 0;       // past the closing entry: never read
+    };
+    int tv[TCS_PRE + 1], ta[TCS_PRE + 1];
+#pragma unroll
+    for (int k = 0; k < TCS_PRE; k++) {
+        const int e = threadIdx.x + k * BLOCK;
+        tv[k] = 0; ta[k] = 0;
+        if (e < n_tcs) tv[k] = tcs_fetch(e, ta[k]);
+    }
+    PR::stage(P, M, __ldcg(&P.ctrl->p_dst), st);
+#pragma unroll
+    for (int k = 0; k < TCS_PRE; k++) {
+        const int e = threadIdx.x + k * BLOCK;
+        if (e < n_tcs) tcs[e] = tv[k] + ta[k];
+    }
+    for (int e = threadIdx.x + TCS_PRE * BLOCK; e < n_tcs; e += BLOCK) {
+        int add;
+        const int v = tcs_fetch(e, add);
+        tcs[e] = v + add;
     }
     // per tile row: periodic shifts along y, z, their flag bits, the index offsets of the row's (up to) three contiguous
     // pieces (global index = tile index + delta) -- everything of a run's set-up that does not depend on the atom
