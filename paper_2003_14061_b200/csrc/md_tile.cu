@@ -375,11 +375,11 @@ struct PrecF32 {
 
 // The block size is a run-time value (any multiple of 32 up to 512): it is picked so that the own atoms of a box
 // fill the block's warps.
-// Register cap (measured): binary64 keeps the 62-64 registers ptxas picks (a cap of 56 -- a fifth resident block
-// per SM -- gains 1 % at wca_2m but loses 2-3 % at lj_1m / chains_1m; 48 spills: +9 %); the binary32 build, whose tile is half
-// the size, gains 6 % at wca_2m with 56 (0.355 -> 0.334 ms).
+// Registers (measured): ptxas picks 56-64 under this bound; caps of 56 / 48 (a fifth resident block of the former
+// 224-thread blocks) gained only in binary32 and nothing once the boxes were made for 256-thread blocks (4 blocks of 256 = 1024
+// threads per SM need <= 64 registers anyway).
 template <typename PR, bool LOCALW>
-__global__ void __maxnreg__(sizeof(typename PR::real) == 4 ? 56 : 64) k_tile_build(const __grid_constant__ MdDev P)
+__global__ void __launch_bounds__(512) k_tile_build(const __grid_constant__ MdDev P)
 {
     using real = typename PR::real;
     const int BLOCK = blockDim.x;
@@ -409,11 +409,7 @@ __global__ void __maxnreg__(sizeof(typename PR::real) == 4 ? 56 : 64) k_tile_bui
     }
     // tcs[q * stride + k], k = 0 .. sxc + 2 K  (K halo cells, the box's sxc cells, K halo cells; the last entry closes the row):
     // tile index of the first atom of tile cell k of row q = (start of the cell in the global order) + (tile offset - global
-    // start of the row's piece).  The cell starts of the first TCS_PRE entries of every thread are requested BEFORE the position
-    // tile is staged and added up after it, so that the two rounds of global-memory latency overlap (measured: DESIGN.md 6f).
-    // Binary64: no gain (0.357 -> 0.355 / 0.384 -> 0.392 / 0.198 -> 0.202 ms at dr03 / dr05 / chains_1m: the 8 registers it holds
-    // across the staging cost more), so there the fetches follow the staging; binary32 0.334 -> 0.324 ms.
-    constexpr int TCS_PRE = sizeof(real) == 4 ? 4 : 0;
+    // start of the row's piece)
     const int n_tcs = B.nq * stride;
     auto tcs_fetch = [&](int e, int &add) -> int {      // the global load of entry e; add: what turns it into the tile index
         const int q = e / stride, k = e - q * stride;
@@ -423,23 +419,12 @@ __global__ void __maxnreg__(sizeof(typename PR::real) == 4 ? 56 : 64) k_tile_bui
         add = R.off + R.n[0] + R.n[1] - R.g[2];
         return k <= B.sxc + 2 * K ? __ldg(cs + X.row_cell[q] + X.xc + k - K - B.sxc) : 0;       // past the closing entry: never read
     };
-    int tv[TCS_PRE + 1], ta[TCS_PRE + 1];
-#pragma unroll
-    for (int k = 0; k < TCS_PRE; k++) {
-        const int e = threadIdx.x + k * BLOCK;
-        tv[k] = 0; ta[k] = 0;
-        if (e < n_tcs) tv[k] = tcs_fetch(e, ta[k]);
-    }
     PR::stage(P, M, __ldcg(&P.ctrl->p_dst), st);
-#pragma unroll
-    for (int k = 0; k < TCS_PRE; k++) {
-        const int e = threadIdx.x + k * BLOCK;
-        if (e < n_tcs) tcs[e] = tv[k] + ta[k];
-    }
-    // the rest (binary64: all) in batches of four loads before their four stores: a shared-memory store that waits for its
-    // global load would otherwise hold back the next entry's load (one round of latency per entry): build 0.357 -> 0.342 ms
-    // at wca_2m_dr03
-    for (int e0 = threadIdx.x + TCS_PRE * BLOCK; e0 < n_tcs; e0 += 4 * BLOCK) {
+    // in batches of four loads before their four stores: a shared-memory store that waits for its global load would otherwise
+    // hold back the next entry's load (one round of latency per entry): build 0.357 -> 0.342 ms at wca_2m_dr03.  (Requesting them
+    // BEFORE the tile is staged, 8 registers held across the staging, gained 3 % in binary32 with the former 224-thread boxes and
+    // nothing with the present ones.)
+    for (int e0 = threadIdx.x; e0 < n_tcs; e0 += 4 * BLOCK) {
         int v[4], add[4];
 #pragma unroll
         for (int k = 0; k < 4; k++) {
