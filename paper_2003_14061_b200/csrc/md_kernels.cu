@@ -173,49 +173,10 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const __grid_constant__ 
     scan_reduce_tile(P, blockIdx.x);
 }
 
-// exclusive scan of the per-tile sums, one block
-__global__ void __launch_bounds__(1024) k_scan_top(const __grid_constant__ MdDev P)
-{
-    if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    __shared__ int wsum[32];
-    __shared__ int carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int start = 0; start < P.scan_blocks; start += 1024) {
-        const int idx = start + threadIdx.x;
-        const int v = idx < P.scan_blocks ? P.block_sums[idx] : 0;
-        int inc = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(FULL_MASK, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) wsum[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            int w = wsum[lane], winc = w;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(FULL_MASK, winc, o);
-                if (lane >= o) winc += t;
-            }
-            wsum[lane] = winc - w;                   // exclusive prefix of warp totals
-        }
-        __syncthreads();
-        const int carry = carry_s;
-        const int excl = carry + wsum[wid] + inc - v;
-        if (idx < P.scan_blocks) P.block_sums[idx] = excl;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = excl + v;
-        __syncthreads();
-    }
-}
-
 __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const __grid_constant__ MdDev P)
 {
     if (!__ldcg(&P.ctrl->need_rebuild)) return;
-    scan_apply_tile(P, blockIdx.x);
+    scan_apply_tile<true>(P, blockIdx.x);
 }
 
 __global__ void __launch_bounds__(256) k_place(const __grid_constant__ MdDev P)
@@ -928,7 +889,7 @@ __global__ void __launch_bounds__(PERSIST_T, MINB) k_persist(const __grid_consta
                 for (int t = 0; t < P.scan_blocks; t++) { const int v = P.block_sums[t]; P.block_sums[t] = run; run += v; }
             }
             grid.sync();
-            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile(P, t); __syncthreads(); }
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile<false>(P, t); __syncthreads(); }
             grid.sync();
             place_body(P);
             grid.sync();
@@ -1009,7 +970,6 @@ void mdk_cells(const MdDev &P, const MdLaunch &, cudaStream_t st)
     if (P.sp) mdk_sp_bin(P, st);
     else k_bin<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
     k_scan_reduce<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
-    k_scan_top<<<1, 1024, 0, st>>>(P);
     k_scan_apply<<<P.scan_blocks, SCAN_T, 0, st>>>(P);
     k_place<<<capped_grid(P, P.N, 256, 8), 256, 0, st>>>(P);
 }
@@ -1136,7 +1096,7 @@ int mdk_persist_steps(const MdDev &P, long long n, cudaStream_t st)
 int mdk_launches_of(int which)
 {
     switch (which) {
-    case LK_CELLS: return 5;
+    case LK_CELLS: return 4;
     case LK_FORCE_N3: return 2;
     default: return 1;
     }

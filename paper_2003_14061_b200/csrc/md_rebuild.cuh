@@ -57,9 +57,18 @@ __device__ __forceinline__ void scan_reduce_tile(const MdDev &P, int tile)
     }
 }
 
+// RAW: block_sums holds the tiles' own sums and the block adds up the tiles before its own (the kernel chain: one launch less
+// than with a separate scan of the tile sums); else block_sums holds the exclusive prefix already (persistent kernels).
+template <bool RAW>
 __device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
 {
-    __shared__ int wsum[SCAN_T / 32];
+    __shared__ int wsum[SCAN_T / 32], psum[SCAN_T / 32];
+    int before = 0;
+    if (RAW) {
+        for (int t = threadIdx.x; t < tile; t += SCAN_T) before += P.block_sums[t];
+        before = warp_sum_i(before);
+        if ((threadIdx.x & 31) == 0) psum[threadIdx.x >> 5] = before;
+    }
     const int base = tile * SCAN_TILE + threadIdx.x * SCAN_V;
     int c[SCAN_V], sum = 0;
     scan_load8(P, base, c);
@@ -76,7 +85,13 @@ __device__ __forceinline__ void scan_apply_tile(const MdDev &P, int tile)
     __syncthreads();
     int woff = 0;
     for (int w = 0; w < wid; w++) woff += wsum[w];
-    int run = P.block_sums[tile] + woff + inc - sum;
+    if (RAW) {
+        before = 0;
+        for (int w = 0; w < SCAN_T / 32; w++) before += psum[w];
+    } else {
+        before = P.block_sums[tile];
+    }
+    int run = before + woff + inc - sum;
     if (base + SCAN_V < P.NC) {      // all 8 cells exist and none is the last: 128-bit stores
         int st[SCAN_V];
 #pragma unroll

@@ -571,7 +571,7 @@ __global__ void __launch_bounds__(PERSIST_T, MINB) k_sp_persist(const __grid_con
                 for (int t = 0; t < P.scan_blocks; t++) { const int v = P.block_sums[t]; P.block_sums[t] = run; run += v; }
             }
             grid.sync();
-            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile(P, t); __syncthreads(); }
+            for (int t = blockIdx.x; t < P.scan_blocks; t += nblk) { scan_apply_tile<false>(P, t); __syncthreads(); }
             grid.sync();
             place_body(P);
             grid.sync();
